@@ -1,0 +1,204 @@
+"""ctypes binding of include/cx_bwt.h: same names, argument marshalling only.
+
+PyTorch supplies device memory and streams; every step of the path runs in libcxbwt.so.  There is no
+fallback: if the library is missing and cannot be built, or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+from . import build as _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+CX_OK, CX_ERR_ARG, CX_ERR_BAD_BASE, CX_ERR_WORKSPACE, CX_ERR_BUCKET_TOO_LARGE, CX_ERR_CUDA, CX_ERR_NOMEM = 0, -1, -2, -3, -4, -5, -6
+KERNEL_CLASSES = ["pack", "prep", "hist", "list", "sort_hist", "sort_scan", "sort_pass", "flag", "refine_local",
+                  "refine_scan", "refine_key", "refine_write", "emit"]
+
+
+class CxError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"cx error {code}: {text}")
+        self.code = code
+
+
+class cx_bwt_opts_t(ctypes.Structure):
+    _fields_ = [("prefix_len", ctypes.c_uint32), ("key_bases", ctypes.c_uint32), ("max_batch_suffixes", ctypes.c_uint64),
+                ("max_read_len", ctypes.c_uint32), ("out_is_host_pinned", ctypes.c_int32), ("small_group_max", ctypes.c_uint32),
+                ("profile", ctypes.c_uint32)]
+
+
+class cx_bwt_stats_t(ctypes.Structure):
+    _fields_ = [("n_suffixes", ctypes.c_uint64), ("max_batch", ctypes.c_uint64), ("largest_bucket", ctypes.c_uint64),
+                ("refine_elements", ctypes.c_uint64), ("small_group_elems", ctypes.c_uint64), ("kernel_launches", ctypes.c_uint64),
+                ("n_batches", ctypes.c_uint32), ("id_bytes", ctypes.c_uint32), ("sort_passes", ctypes.c_uint32),
+                ("refine_rounds", ctypes.c_uint32), ("max_read_len", ctypes.c_uint32), ("uniform_len", ctypes.c_uint32)]
+
+    def as_dict(self) -> dict:
+        return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load (building first if stale) libcxbwt.so.  Fails loudly; never substitutes another path."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = ctypes.CDLL(path)
+        vp, u64, u32, i32 = ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_int
+        L.cx_bwt_workspace_bytes.argtypes = [u64, u64, ctypes.POINTER(cx_bwt_opts_t), ctypes.POINTER(u64)]
+        L.cx_bwt_plan.argtypes = [ctypes.POINTER(vp), u64, u64, ctypes.POINTER(cx_bwt_opts_t), vp, u64]
+        L.cx_pack_reads.argtypes = [vp, u64, vp, vp, vp]
+        L.cx_bwt_build.argtypes = [vp, vp, vp, u64, vp, vp]
+        L.cx_bwt_free.argtypes = [vp]
+        L.cx_bwt_get_stats.argtypes = [vp, ctypes.POINTER(cx_bwt_stats_t)]
+        L.cx_bwt_get_histogram.argtypes = [vp, vp, u64, ctypes.POINTER(u64)]
+        L.cx_bwt_kernel_time.argtypes = [vp, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64), ctypes.POINTER(u64)]
+        L.cx_sort_pairs_workspace_bytes.argtypes = [u64, ctypes.POINTER(u64)]
+        L.cx_sort_pairs.argtypes = [vp, vp, vp, vp, u64, u32, u32, u32, vp, u64, ctypes.POINTER(i32), vp]
+        L.cx_strerror.argtypes = [i32]
+        L.cx_strerror.restype = ctypes.c_char_p
+        for name in ("cx_bwt_workspace_bytes", "cx_bwt_plan", "cx_pack_reads", "cx_bwt_build", "cx_bwt_free", "cx_bwt_get_stats",
+                     "cx_bwt_get_histogram", "cx_bwt_kernel_time", "cx_sort_pairs_workspace_bytes", "cx_sort_pairs"):
+            getattr(L, name).restype = i32
+        _lib = L
+    return _lib
+
+
+def cx_strerror(code: int) -> str:
+    return lib().cx_strerror(code).decode()
+
+
+def _check(rc: int) -> None:
+    if rc != CX_OK:
+        raise CxError(rc, cx_strerror(rc))
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream
+
+
+def _opts(**kw) -> cx_bwt_opts_t:
+    o = cx_bwt_opts_t()
+    for k, v in kw.items():
+        if v is not None:
+            setattr(o, k, int(v))
+    return o
+
+
+def cx_bwt_workspace_bytes(n_reads: int, total_bases: int, **opts) -> int:
+    out = ctypes.c_uint64(0)
+    o = _opts(**opts)
+    _check(lib().cx_bwt_workspace_bytes(n_reads, total_bases, ctypes.byref(o), ctypes.byref(out)))
+    return int(out.value)
+
+
+def cx_pack_reads(ascii_dev: torch.Tensor, packed_out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """ASCII bases (uint8, cuda) -> packed words (int64 tensor holding uint64 bit patterns)."""
+    assert ascii_dev.is_cuda and ascii_dev.dtype == torch.uint8 and ascii_dev.is_contiguous()
+    n = ascii_dev.numel()
+    if packed_out is None:
+        packed_out = torch.empty(max(1, (n + 31) // 32), dtype=torch.int64, device=ascii_dev.device)
+    status = torch.zeros(1, dtype=torch.int32, device=ascii_dev.device)
+    _check(lib().cx_pack_reads(ascii_dev.data_ptr(), n, packed_out.data_ptr(), status.data_ptr(), _stream_ptr(stream)))
+    if int(status.item()) != 0:
+        raise CxError(CX_ERR_BAD_BASE, cx_strerror(CX_ERR_BAD_BASE))
+    return packed_out
+
+
+class Plan:
+    """cx_bwt_plan / cx_bwt_build / cx_bwt_free with a torch-owned workspace."""
+
+    def __init__(self, max_reads: int, max_total_bases: int, workspace_bytes: int | None = None, device=None, **opts):
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        self.opts = _opts(**opts)
+        if workspace_bytes is None:
+            workspace_bytes = cx_bwt_workspace_bytes(max_reads, max_total_bases, **opts)
+        self.workspace = torch.empty(int(workspace_bytes) + 256, dtype=torch.uint8, device=self.device)
+        base = self.workspace.data_ptr()
+        self._ws_ptr = (base + 255) // 256 * 256
+        self._h = ctypes.c_void_p(None)
+        with torch.cuda.device(self.device):
+            _check(lib().cx_bwt_plan(ctypes.byref(self._h), max_reads, max_total_bases, ctypes.byref(self.opts), self._ws_ptr,
+                                     int(workspace_bytes)))
+
+    def build(self, packed: torch.Tensor, offsets: torch.Tensor, n_reads: int, out: torch.Tensor, stream=None) -> torch.Tensor:
+        """cx_bwt_build: out receives N = total_bases + n_reads bytes over b"$ACGT"."""
+        assert offsets.dtype == torch.int64 and offsets.is_cuda and offsets.is_contiguous()
+        assert out.dtype == torch.uint8 and out.is_contiguous()
+        with torch.cuda.device(self.device):
+            _check(lib().cx_bwt_build(self._h, packed.data_ptr(), offsets.data_ptr(), n_reads, out.data_ptr(), _stream_ptr(stream)))
+        return out
+
+    def stats(self) -> dict:
+        s = cx_bwt_stats_t()
+        _check(lib().cx_bwt_get_stats(self._h, ctypes.byref(s)))
+        return s.as_dict()
+
+    def histogram(self):
+        import numpy as np
+        n = ctypes.c_uint64(0)
+        lib().cx_bwt_get_histogram(self._h, None, 0, ctypes.byref(n))
+        h = np.zeros(int(n.value), dtype=np.uint64)
+        _check(lib().cx_bwt_get_histogram(self._h, h.ctypes.data, h.shape[0], ctypes.byref(n)))
+        return h
+
+    def kernel_times(self) -> dict:
+        out = {}
+        for i, name in enumerate(KERNEL_CLASSES):
+            ms, ln, by = ctypes.c_double(0), ctypes.c_uint64(0), ctypes.c_uint64(0)
+            _check(lib().cx_bwt_kernel_time(self._h, i, ctypes.byref(ms), ctypes.byref(ln), ctypes.byref(by)))
+            out[name] = {"ms": ms.value, "launches": int(ln.value), "bytes": int(by.value)}
+        return out
+
+    def free(self) -> None:
+        if self._h:
+            lib().cx_bwt_free(self._h)
+            self._h = ctypes.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+def cx_sort_pairs(keys: torch.Tensor, vals: torch.Tensor, begin_bit: int = 0, end_bit: int = 64, stream=None):
+    """Stable LSD radix sort of (uint64 key as int64 bits, 4- or 8-byte value) pairs; returns new tensors."""
+    assert keys.is_cuda and keys.dtype == torch.int64 and vals.dtype in (torch.int32, torch.int64)
+    n = keys.numel()
+    k0, v0 = keys.clone(), vals.clone()
+    k1, v1 = torch.empty_like(k0), torch.empty_like(v0)
+    wsb = ctypes.c_uint64(0)
+    _check(lib().cx_sort_pairs_workspace_bytes(n, ctypes.byref(wsb)))
+    ws = torch.empty(int(wsb.value), dtype=torch.uint8, device=keys.device)
+    alt = ctypes.c_int(0)
+    _check(lib().cx_sort_pairs(k0.data_ptr(), v0.data_ptr(), k1.data_ptr(), v1.data_ptr(), n, vals.element_size(), begin_bit,
+                               end_bit, ws.data_ptr(), int(wsb.value), ctypes.byref(alt), _stream_ptr(stream)))
+    return (k1, v1) if alt.value else (k0, v0)
+
+
+def bwt_of_collection(ascii_host, offsets_host, device="cuda", **opts):
+    """The call a user makes: host ASCII reads + offsets -> host BWT bytes (numpy), through pack + build."""
+    import numpy as np
+    n_reads = int(offsets_host.shape[0] - 1)
+    total = int(offsets_host[-1]) if n_reads > 0 else 0
+    N = total + n_reads
+    if n_reads <= 0:
+        return np.zeros(0, dtype=np.uint8)
+    a = torch.from_numpy(np.ascontiguousarray(ascii_host)).to(device) if total else torch.zeros(0, dtype=torch.uint8, device=device)
+    off = torch.from_numpy(np.ascontiguousarray(offsets_host).astype(np.int64)).to(device)
+    packed = cx_pack_reads(a) if total else torch.zeros(1, dtype=torch.int64, device=device)
+    plan = Plan(n_reads, total, **opts)
+    out = torch.empty(N, dtype=torch.uint8, device=device)
+    plan.build(packed, off, n_reads, out)
+    res = out.cpu().numpy()
+    plan.free()
+    return res

@@ -1,0 +1,164 @@
+// cx_internal.cuh -- shared declarations of libcxbwt (sm_100a only).  Not part of the C ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "cx_bwt.h"
+
+namespace cx {
+
+// ---------------------------------------------------------------------------------------------
+// geometry shared by host and device
+// ---------------------------------------------------------------------------------------------
+constexpr int kListThreads = 256;
+constexpr int kListItems = 8;
+constexpr int kListTile = kListThreads * kListItems;   // suffix slots per listing / histogram tile
+
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;
+
+// onesweep tile shapes (threads x items); one per value width so that registers/smem stay balanced
+constexpr int kSortThreads = 256;
+constexpr int kSortItems32 = 16;   // 64-bit key + 32-bit id
+constexpr int kSortItems64 = 12;   // 64-bit key + 64-bit id
+template <typename ValT> struct SortShape { static constexpr int items = sizeof(ValT) == 4 ? kSortItems32 : kSortItems64; };
+constexpr int kSortTileMin = kSortThreads * kSortItems64;   // smallest tile: sizes the tile-state array
+
+// tile-state word of the decoupled look-back: [epoch:8][flag:2][count:54]
+constexpr uint64_t kStatusValueMask = (1ull << 54) - 1;
+constexpr uint32_t kFlagAggregate = 1, kFlagInclusive = 2;
+
+// in-block refinement
+constexpr int kLocalThreads = 256;
+constexpr int kLocalTile = 2048;         // sorted positions owned by one block
+constexpr int kLocalGroupCap = 256;      // largest tie group the in-block path accepts
+
+// Facts about one build, produced by the prep kernel and read by later kernels and by the host.
+struct BuildInfo {
+    uint64_t total_bases;
+    uint64_t n_suffixes;
+    uint64_t max_len;
+    uint64_t first_len;
+    uint32_t bad_offsets;   // offsets[0] != 0 or a decreasing pair
+    uint32_t nonuniform;    // some read differs in length from read 0
+};
+
+// The read collection as kernels see it.
+struct Reads {
+    const uint64_t* packed;    // 2 bit/base, MSB-first in each word
+    const uint64_t* offsets;   // n_reads + 1
+    uint64_t n_reads;
+    uint64_t n_words;          // valid words of `packed`; loads at or past it read as zero
+    uint64_t uniform_len;      // length of every read when `uniform`
+    uint32_t pos_bits;         // id = (read << pos_bits) | pos
+    uint32_t uniform;          // 1: all reads have the same length, offsets need not be gathered
+};
+
+// ---------------------------------------------------------------------------------------------
+// device helpers
+// ---------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+
+__device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31; }
+__device__ __forceinline__ uint32_t lanemask_lt() {
+    uint32_t m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+__device__ __forceinline__ uint64_t ld_relaxed_u64(const uint64_t* p) {
+    uint64_t v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed_u64(uint64_t* p, uint64_t v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+// 32 bases starting at base position b, first base in the two most significant bits.
+// Words at or past n_words read as zero (A-padding; callers mask by the true remaining length).
+__device__ __forceinline__ uint64_t load_window(const uint64_t* __restrict__ packed, uint64_t n_words, uint64_t b) {
+    uint64_t wi = b >> 5;
+    uint32_t sh = (uint32_t)(b & 31) * 2;
+    uint64_t w0 = wi < n_words ? __ldg(packed + wi) : 0ull;
+    if (sh == 0) return w0;
+    uint64_t w1 = wi + 1 < n_words ? __ldg(packed + wi + 1) : 0ull;
+    return (w0 << sh) | (w1 >> (64 - sh));
+}
+
+// Order-preserving key of a window (reading A3 of PAPER.md:99):
+// the first min(rem, w) bases, A-padded to w bases, then min(rem, w) in the low 5 bits.
+// A value < w in the length field means the end-marker falls inside this window.
+__device__ __forceinline__ uint64_t make_key(uint64_t window, uint64_t rem, uint32_t w) {
+    uint32_t r = rem < (uint64_t)w ? (uint32_t)rem : w;
+    uint64_t bases = r ? ((window >> (64 - 2 * r)) << (2 * (w - r))) : 0ull;
+    return (bases << 5) | r;
+}
+
+template <typename IdT>
+__device__ __forceinline__ IdT make_id(uint64_t read, uint64_t pos, uint32_t pos_bits) {
+    return (IdT)((read << pos_bits) | pos);
+}
+
+#endif  // __CUDACC__
+
+// ---------------------------------------------------------------------------------------------
+// host-side launchers (one translation unit per group of kernels)
+// ---------------------------------------------------------------------------------------------
+struct Launch;   // profiling hook, defined in cx_api.cu
+
+// cx_pack.cu
+cudaError_t launch_pack(const uint8_t* ascii, uint64_t total_bases, uint64_t* packed, uint32_t* status, cudaStream_t s);
+uint32_t* pack_fallback_status();
+
+// cx_scan_reads.cu
+cudaError_t launch_prep(const uint64_t* offsets, uint64_t n_reads, BuildInfo* info, cudaStream_t s);
+cudaError_t launch_tile_table(const uint64_t* offsets, uint64_t n_reads, const BuildInfo* info, uint32_t* tile_first_read,
+                              uint64_t max_tiles, cudaStream_t s);
+cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
+                               uint64_t* hist, uint64_t max_tiles, int n_sms, cudaStream_t s);
+// count suffixes of each tile whose bucket lies in [bucket_lo, bucket_hi]
+cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
+                              uint32_t bucket_lo, uint32_t bucket_hi, uint64_t* tile_count, uint64_t n_tiles, cudaStream_t s);
+// write (key, id) of those suffixes in (read, pos) order; tile_base == nullptr means "every suffix, index = slot"
+template <typename IdT>
+cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
+                              uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, uint64_t* keys, IdT* ids,
+                              uint64_t n_tiles, cudaStream_t s);
+
+// cx_onesweep.cu
+struct SortWorkspace {
+    uint64_t* hist = nullptr;     // [8][256] digit counts, then exclusive bin bases in place
+    uint64_t* status = nullptr;   // [max_tiles][256] tile state
+    uint32_t* ticket = nullptr;   // dynamic tile counter (monotone across launches)
+    uint64_t max_tiles = 0;
+    uint32_t epoch = 0;           // host-side: last epoch used (1..255)
+    uint32_t ticket_base = 0;     // host-side: tickets handed out so far
+};
+size_t sort_workspace_bytes(uint64_t n);
+// carve a zeroed region of sort_workspace_bytes(n) bytes
+void sort_workspace_carve(SortWorkspace& ws, void* mem, uint64_t n);
+// Sorts by key bits [begin_bit, end_bit).  *result_in_alt = 1 if the result is in the alt buffers.
+template <typename ValT>
+cudaError_t sort_pairs(uint64_t* keys, ValT* vals, uint64_t* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
+                       uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s);
+
+// cx_refine.cu
+cudaError_t launch_flag_heads(const uint64_t* keys, uint64_t n, uint32_t w, uint32_t* heads, cudaStream_t s);
+// word-level counts of active elements / active heads, packed (heads << 32 | elements)
+cudaError_t launch_active_count(const uint32_t* heads, uint64_t n, uint64_t* word_counts, cudaStream_t s);
+// exclusive scan in place; total written to *total; block_sums needs scan_block_count(n) entries
+uint64_t scan_block_count(uint64_t n);
+cudaError_t launch_scan_u64(uint64_t* data, uint64_t n, uint64_t* block_sums, uint64_t* total, cudaStream_t s);
+template <typename IdT>
+cudaError_t launch_refine_rekey(const Reads& R, const uint32_t* heads, const uint64_t* word_base, const IdT* ids, uint64_t n,
+                                uint32_t depth, uint32_t w, uint64_t* keys_c, IdT* ids_c, uint32_t* pos_c, cudaStream_t s);
+template <typename IdT>
+cudaError_t launch_refine_writeback(const uint64_t* keys_c, const IdT* ids_c, const uint32_t* pos_c, uint64_t n_c, uint32_t w,
+                                    IdT* ids, uint32_t* heads, cudaStream_t s);
+template <typename IdT>
+cudaError_t launch_refine_local(const Reads& R, const uint32_t* heads_in, uint32_t* heads_out, IdT* ids, uint64_t n, uint32_t depth,
+                                uint32_t group_cap, unsigned long long* elems_done, cudaStream_t s);
+template <typename IdT>
+cudaError_t launch_emit(const Reads& R, const IdT* ids, uint64_t n, uint8_t* out, cudaStream_t s);
+
+}  // namespace cx

@@ -1,0 +1,316 @@
+// cx_onesweep.cu -- step a6: stable LSD radix sort of (64-bit key, suffix id) pairs
+// (PAPER.md:91 LSD radix sort over several characters per iteration; "sorting by
+// index"; PAPER.md:99 the sort must be stable).
+//
+// "Onesweep" structure: one upfront kernel builds the digit histograms of every pass; then each
+// pass reads every pair once and scatter-writes it once.  A tile learns how many equal-digit pairs
+// precede it from the tile-state words of earlier tiles (decoupled look-back), so there is no
+// separate scan between passes.  Within a tile, ranks come from warp match + popc (multi-split),
+// pairs are staged in shared memory in digit order and leave as runs of consecutive addresses.
+//
+// Algorithmic traffic per pass: 2 * (8 + sizeof(id)) bytes per pair; histogram kernel: 8 bytes per pair.
+#include "cx_internal.cuh"
+#include "cx_launch.h"
+
+namespace cx {
+namespace {
+
+constexpr uint32_t kFull = 0xffffffffu;
+
+__device__ __forceinline__ uint64_t pack_status(uint32_t epoch, uint32_t flag, uint64_t value) {
+    return ((uint64_t)epoch << 56) | ((uint64_t)flag << 54) | value;
+}
+
+// ---------------------------------------------------------------------------------------------
+// upfront histograms: hist[p][d] = number of keys whose p-th digit is d
+// ---------------------------------------------------------------------------------------------
+constexpr int kHistThreads = 512;
+constexpr int kHistItems = 8;
+
+__global__ void __launch_bounds__(kHistThreads) digit_hist_kernel(const uint64_t* __restrict__ keys, uint64_t n, uint32_t begin_bit,
+                                                                 uint32_t end_bit, uint32_t n_passes,
+                                                                 unsigned long long* __restrict__ hist) {
+    __shared__ uint32_t s_hist[8][kRadix];
+    for (uint32_t i = threadIdx.x; i < 8 * kRadix; i += kHistThreads) (&s_hist[0][0])[i] = 0;
+    __syncthreads();
+    const uint64_t chunk = (uint64_t)kHistThreads * kHistItems;
+    for (uint64_t base = (uint64_t)blockIdx.x * chunk; base < n; base += (uint64_t)gridDim.x * chunk) {
+        uint64_t k[kHistItems];
+#pragma unroll
+        for (int i = 0; i < kHistItems; ++i) {
+            uint64_t idx = base + (uint64_t)i * kHistThreads + threadIdx.x;
+            k[i] = idx < n ? __ldcs(keys + idx) : 0ull;
+        }
+#pragma unroll
+        for (int i = 0; i < kHistItems; ++i) {
+            uint64_t idx = base + (uint64_t)i * kHistThreads + threadIdx.x;
+            if (idx < n) {
+                for (uint32_t p = 0; p < n_passes; ++p) {
+                    uint32_t lo = begin_bit + p * kRadixBits;
+                    uint32_t bits = min((uint32_t)kRadixBits, end_bit - lo);
+                    uint32_t d = (uint32_t)(k[i] >> lo) & ((1u << bits) - 1);
+                    atomicAdd(&s_hist[p][d], 1u);
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kHistThreads) {
+        uint32_t v = (&s_hist[0][0])[i];
+        if (v) atomicAdd(hist + i, (unsigned long long)v);
+    }
+}
+
+// exclusive scan of each pass's 256 counts, in place: hist[p][d] becomes the first output index of digit d
+__global__ void __launch_bounds__(kRadix) bin_scan_kernel(unsigned long long* __restrict__ hist) {
+    __shared__ unsigned long long s_warp[kRadix / 32];
+    unsigned long long* h = hist + (uint64_t)blockIdx.x * kRadix;
+    unsigned long long v = h[threadIdx.x];
+    unsigned long long incl = v;
+    for (int o = 1; o < 32; o <<= 1) {
+        unsigned long long up = __shfl_up_sync(kFull, incl, o);
+        if ((int)lane_id() >= o) incl += up;
+    }
+    if (lane_id() == 31) s_warp[threadIdx.x >> 5] = incl;
+    __syncthreads();
+    unsigned long long carry = 0;
+    for (uint32_t wq = 0; wq < (threadIdx.x >> 5); ++wq) carry += s_warp[wq];
+    h[threadIdx.x] = carry + incl - v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// one onesweep pass
+// ---------------------------------------------------------------------------------------------
+template <typename ValT, int THREADS, int ITEMS>
+struct PassSmem {
+    static constexpr int kTile = THREADS * ITEMS;
+    static constexpr int kWarps = THREADS / 32;
+    uint64_t keys[kTile];
+    ValT vals[kTile];
+    uint64_t gofs[kRadix];               // global index of staged slot e with digit d = gofs[d] + e
+    uint32_t warp_count[kWarps][kRadix];  // per-warp digit counts, then the warp's offset inside the digit
+    uint32_t bin_start[kRadix];           // first staged slot of each digit
+    uint32_t warp_total[kRadix / 32];
+    uint32_t tile;
+};
+
+template <typename ValT, int THREADS, int ITEMS, int MIN_BLOCKS>
+__global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
+onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const ValT* __restrict__ vals_in, uint64_t* __restrict__ keys_out,
+                     ValT* __restrict__ vals_out, uint64_t n, uint32_t shift, uint32_t digit_mask,
+                     const uint64_t* __restrict__ bin_base, uint64_t* __restrict__ status, uint32_t* __restrict__ ticket,
+                     uint32_t ticket_base, uint32_t epoch) {
+    using Smem = PassSmem<ValT, THREADS, ITEMS>;
+    constexpr int kTile = Smem::kTile;
+    constexpr int kWarps = Smem::kWarps;
+    static_assert(THREADS >= kRadix && THREADS % 32 == 0, "one thread per digit is required");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
+
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    // Tiles are claimed in launch order of the blocks, so every earlier tile is owned by a block that
+    // is already running: the look-back below can never wait on a block that has not started.
+    if (tid == 0) sm.tile = atomicAdd(ticket, 1u) - ticket_base;
+    for (uint32_t i = tid; i < kWarps * kRadix; i += THREADS) (&sm.warp_count[0][0])[i] = 0;
+    __syncthreads();
+    const uint32_t tile = sm.tile;
+    const uint64_t tile_off = (uint64_t)tile * kTile;
+    const uint32_t tile_n = (uint32_t)min((uint64_t)kTile, n - tile_off);
+    const uint32_t warp_base = warp * (32 * ITEMS);
+
+    // warp-striped loads: element order inside the tile = (warp, item, lane); fully coalesced
+    uint64_t key[ITEMS];
+    ValT val[ITEMS];
+#pragma unroll
+    for (int k = 0; k < ITEMS; ++k) {
+        uint32_t e = warp_base + k * 32 + lane;
+        key[k] = e < tile_n ? __ldcs(keys_in + tile_off + e) : ~0ull;
+    }
+#pragma unroll
+    for (int k = 0; k < ITEMS; ++k) {
+        uint32_t e = warp_base + k * 32 + lane;
+        val[k] = e < tile_n ? __ldcs(vals_in + tile_off + e) : (ValT)0;
+    }
+
+    // rank inside the warp, item by item (keeps element order, hence stability)
+    uint32_t rank[ITEMS];
+#pragma unroll
+    for (int k = 0; k < ITEMS; ++k) {
+        bool valid = warp_base + k * 32 + lane < tile_n;
+        uint32_t d = (uint32_t)(key[k] >> shift) & digit_mask;
+        uint32_t peers = __match_any_sync(kFull, valid ? d : (uint32_t)kRadix);
+        uint32_t below = __popc(peers & lanemask_lt());
+        uint32_t old = 0;
+        if (valid && below == 0) {
+            old = sm.warp_count[warp][d];
+            sm.warp_count[warp][d] = old + __popc(peers);
+        }
+        old = __shfl_sync(kFull, old, __ffs(peers) - 1);
+        rank[k] = old + below;
+        __syncwarp();
+    }
+    __syncthreads();
+
+    // per digit: tile count, warp offsets, tile-state publication, look-back
+    uint32_t count = 0;
+    if (tid < kRadix) {
+#pragma unroll
+        for (int wq = 0; wq < kWarps; ++wq) {
+            uint32_t c = sm.warp_count[wq][tid];
+            sm.warp_count[wq][tid] = count;
+            count += c;
+        }
+        uint64_t* my_status = status + (uint64_t)tile * kRadix + tid;
+        st_relaxed_u64(my_status, pack_status(epoch, tile == 0 ? kFlagInclusive : kFlagAggregate, count));
+        // exclusive scan of the 256 counts -> first staged slot of each digit
+        uint32_t incl = count;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t up = __shfl_up_sync(kFull, incl, o);
+            if ((int)lane >= o) incl += up;
+        }
+        if (lane == 31) sm.warp_total[warp] = incl;
+        asm volatile("bar.sync 1, %0;" ::"n"(kRadix));   // only the 256 digit threads
+        uint32_t carry = 0;
+        for (uint32_t wq = 0; wq < warp; ++wq) carry += sm.warp_total[wq];
+        uint32_t excl = carry + incl - count;
+        sm.bin_start[tid] = excl;
+
+        uint64_t before = 0;   // equal-digit pairs in earlier tiles
+        if (tile > 0) {
+            int64_t t = (int64_t)tile - 1;
+            while (true) {
+                uint64_t st = ld_relaxed_u64(status + (uint64_t)t * kRadix + tid);
+                uint32_t flag = (uint32_t)(st >> 54) & 3u;
+                if ((uint32_t)(st >> 56) != epoch || flag == 0) continue;   // not published yet
+                before += st & kStatusValueMask;
+                if (flag == kFlagInclusive) break;
+                --t;
+            }
+            st_relaxed_u64(my_status, pack_status(epoch, kFlagInclusive, before + count));
+        }
+        sm.gofs[tid] = bin_base[tid] + before - excl;
+    }
+    __syncthreads();
+
+    // stage pairs in digit order
+#pragma unroll
+    for (int k = 0; k < ITEMS; ++k) {
+        if (warp_base + k * 32 + lane < tile_n) {
+            uint32_t d = (uint32_t)(key[k] >> shift) & digit_mask;
+            uint32_t slot = sm.bin_start[d] + sm.warp_count[warp][d] + rank[k];
+            sm.keys[slot] = key[k];
+            sm.vals[slot] = val[k];
+        }
+    }
+    __syncthreads();
+
+    // runs of equal digit leave as consecutive addresses
+#pragma unroll
+    for (int k = 0; k < ITEMS; ++k) {
+        uint32_t e = k * THREADS + tid;
+        if (e < tile_n) {
+            uint64_t kk = sm.keys[e];
+            uint32_t d = (uint32_t)(kk >> shift) & digit_mask;
+            uint64_t dst = sm.gofs[d] + e;
+            keys_out[dst] = kk;
+            vals_out[dst] = sm.vals[e];
+        }
+    }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// host driver
+// ---------------------------------------------------------------------------------------------
+size_t sort_workspace_bytes(uint64_t n) {
+    uint64_t tiles = (n + kSortTileMin - 1) / kSortTileMin + 1;
+    return 8 * kRadix * sizeof(uint64_t) + tiles * kRadix * sizeof(uint64_t) + 256;
+}
+
+void sort_workspace_carve(SortWorkspace& ws, void* mem, uint64_t n) {
+    unsigned char* p = static_cast<unsigned char*>(mem);
+    ws.hist = reinterpret_cast<uint64_t*>(p);
+    p += 8 * kRadix * sizeof(uint64_t);
+    ws.max_tiles = (n + kSortTileMin - 1) / kSortTileMin + 1;
+    ws.status = reinterpret_cast<uint64_t*>(p);
+    p += ws.max_tiles * kRadix * sizeof(uint64_t);
+    ws.ticket = reinterpret_cast<uint32_t*>(p);
+    ws.epoch = 0;
+    ws.ticket_base = 0;
+}
+
+template <typename ValT>
+cudaError_t sort_pairs(uint64_t* keys, ValT* vals, uint64_t* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
+                       uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s) {
+    *result_in_alt = 0;
+    if (n <= 1 || end_bit <= begin_bit) return cudaSuccess;
+    constexpr int ITEMS = SortShape<ValT>::items;
+    constexpr int kTile = kSortThreads * ITEMS;
+    using Smem = PassSmem<ValT, kSortThreads, ITEMS>;
+    constexpr int kMinBlocks = 2;
+    auto kernel = onesweep_pass_kernel<ValT, kSortThreads, ITEMS, kMinBlocks>;
+    static bool attr_set = false;
+    cudaError_t e;
+    if (!attr_set) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const uint32_t n_passes = (end_bit - begin_bit + kRadixBits - 1) / kRadixBits;
+    const uint64_t n_tiles = (n + kTile - 1) / kTile;
+    if (n_tiles > ws.max_tiles || n_passes > 8) return cudaErrorInvalidValue;
+
+    e = cudaMemsetAsync(ws.hist, 0, (size_t)n_passes * kRadix * sizeof(uint64_t), s);
+    if (e != cudaSuccess) return e;
+    {
+        uint64_t chunk = (uint64_t)kHistThreads * kHistItems;
+        uint64_t blocks = (n + chunk - 1) / chunk;
+        unsigned grid = (unsigned)(blocks < 148ull * 4 ? blocks : 148ull * 4);
+        ScopedLaunch sl(prof, CX_K_SORT_HIST, n * 8, s);
+        digit_hist_kernel<<<grid, kHistThreads, 0, s>>>(keys, n, begin_bit, end_bit, n_passes, (unsigned long long*)ws.hist);
+    }
+    {
+        ScopedLaunch sl(prof, CX_K_SORT_SCAN, (uint64_t)n_passes * kRadix * 16, s);
+        bin_scan_kernel<<<n_passes, kRadix, 0, s>>>((unsigned long long*)ws.hist);
+    }
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+
+    uint64_t* kin = keys;
+    ValT* vin = vals;
+    uint64_t* kout = keys_alt;
+    ValT* vout = vals_alt;
+    for (uint32_t p = 0; p < n_passes; ++p) {
+        uint32_t lo = begin_bit + p * kRadixBits;
+        uint32_t bits = end_bit - lo < (uint32_t)kRadixBits ? end_bit - lo : (uint32_t)kRadixBits;
+        if (ws.epoch == 255) {   // epoch wrap: forget every old tile state
+            e = cudaMemsetAsync(ws.status, 0, ws.max_tiles * kRadix * sizeof(uint64_t), s);
+            if (e != cudaSuccess) return e;
+            ws.epoch = 0;
+        }
+        ws.epoch += 1;
+        {
+            ScopedLaunch sl(prof, CX_K_SORT_PASS, n * 2 * (8 + sizeof(ValT)), s);
+            kernel<<<(unsigned)n_tiles, kSortThreads, sizeof(Smem), s>>>(kin, vin, kout, vout, n, lo, (1u << bits) - 1,
+                                                                        ws.hist + (uint64_t)p * kRadix, ws.status, ws.ticket,
+                                                                        ws.ticket_base, ws.epoch);
+        }
+        ws.ticket_base += (uint32_t)n_tiles;
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        uint64_t* tk = kin; kin = kout; kout = tk;
+        ValT* tv = vin; vin = vout; vout = tv;
+    }
+    *result_in_alt = (int)(n_passes & 1);
+    return cudaSuccess;
+}
+
+template cudaError_t sort_pairs<uint32_t>(uint64_t*, uint32_t*, uint64_t*, uint32_t*, uint64_t, uint32_t, uint32_t, SortWorkspace&,
+                                          int*, Launch*, cudaStream_t);
+template cudaError_t sort_pairs<uint64_t>(uint64_t*, uint64_t*, uint64_t*, uint64_t*, uint64_t, uint32_t, uint32_t, SortWorkspace&,
+                                          int*, Launch*, cudaStream_t);
+
+}  // namespace cx

@@ -1,0 +1,497 @@
+// cx_refine.cu -- step a7: segmented tie refinement, and step a8: the BWT emit gather.
+//
+// After a sort by the first d symbols, suffixes with equal keys form a tie group.  A group whose key
+// carries a length field < w saw its end-marker: its members are identical strings, already in
+// read-index order because ids were listed in (read, pos) order and every reordering is stable
+// -- it is final.  Every other group of two or more must be ordered by what follows
+// (the first differing symbol decides).  The paper always runs all ceil(2(m+1)/32)
+// iterations over all suffixes; here only the groups still tied are re-keyed:
+//
+//   local path : groups of at most kLocalGroupCap suffixes are finished inside one thread block --
+//                ids in shared memory, one window gather per member per round, stable rank by
+//                counting, looping over depth until every member is placed;
+//   global path: larger groups are compacted, re-keyed as (group ordinal | next w' bases | length)
+//                in one 64-bit key, sorted by the onesweep sorter, and written back in place.
+//
+// Group heads live in a bitmask: bit j = 1 iff sorted position j starts a group.
+#include "cx_internal.cuh"
+
+namespace cx {
+namespace {
+
+constexpr uint32_t kFull = 0xffffffffu;
+
+// (start, length) of read i
+__device__ __forceinline__ void read_span(const Reads& R, uint64_t i, uint64_t& start, uint64_t& len) {
+    if (R.uniform) {
+        start = i * R.uniform_len;
+        len = R.uniform_len;
+    } else {
+        start = __ldg(R.offsets + i);
+        len = __ldg(R.offsets + i + 1) - start;
+    }
+}
+
+// key of suffix `id` at depth d: the next w bases after the first d symbols (the next
+// "stringword" permuted by the index already on the GPU -- here gathered from the resident reads)
+template <typename IdT>
+__device__ __forceinline__ uint64_t key_at_depth(const Reads& R, IdT id, uint32_t depth, uint32_t w) {
+    uint64_t read = (uint64_t)id >> R.pos_bits;
+    uint64_t pos = (uint64_t)id & ((1ull << R.pos_bits) - 1);
+    uint64_t start, len;
+    read_span(R, read, start, len);
+    uint64_t at = pos + depth;
+    uint64_t rem = at < len ? len - at : 0;
+    uint64_t window = rem ? load_window(R.packed, R.n_words, start + at) : 0ull;
+    return make_key(window, rem, w);
+}
+
+// ---------------------------------------------------------------------------------------------
+// head flags of a freshly sorted key array
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) flag_heads_kernel(const uint64_t* __restrict__ keys, uint64_t n, uint32_t w,
+                                                         uint32_t* __restrict__ heads) {
+    uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint64_t n_words = (n + 31) >> 5;
+    bool head = true;   // positions past n count as heads
+    if (j < n) {
+        uint64_t k = __ldcs(keys + j);
+        head = j == 0 || k != __ldg(keys + j - 1) || (uint32_t)(k & 31) < w;
+    }
+    uint32_t word = __ballot_sync(kFull, head);
+    if (lane_id() == 0 && (j >> 5) < n_words) heads[j >> 5] = word;
+    if (j == 0) heads[n_words] = kFull;   // padding word: "the next position is a head"
+}
+
+// per 32 positions: active elements (members of groups of >= 2) and active heads, packed hi|lo
+__device__ __forceinline__ void active_masks(uint32_t H, uint32_t next_word, uint32_t& act, uint32_t& act_heads) {
+    uint32_t Hn = (H >> 1) | (next_word << 31);   // bit j = head(j + 1)
+    act = ~(H & Hn);
+    act_heads = H & ~Hn;
+}
+
+__global__ void __launch_bounds__(256) active_count_kernel(const uint32_t* __restrict__ heads, uint64_t n_words,
+                                                           uint64_t* __restrict__ word_counts) {
+    uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (wi >= n_words) return;
+    uint32_t act, ah;
+    active_masks(heads[wi], heads[wi + 1], act, ah);
+    word_counts[wi] = ((uint64_t)__popc(ah) << 32) | (uint64_t)__popc(act);
+}
+
+// ---------------------------------------------------------------------------------------------
+// exclusive scan of uint64 (reduce, scan of block sums, down-sweep)
+// ---------------------------------------------------------------------------------------------
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 8;
+constexpr int kScanChunk = kScanThreads * kScanItems;
+
+__device__ __forceinline__ uint64_t block_exclusive_scan(uint64_t v, uint64_t* s_warp, uint64_t& total) {
+    uint64_t incl = v;
+    for (int o = 1; o < 32; o <<= 1) {
+        uint64_t up = __shfl_up_sync(kFull, incl, o);
+        if ((int)lane_id() >= o) incl += up;
+    }
+    uint32_t warp = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane_id() == 31) s_warp[warp] = incl;
+    __syncthreads();
+    uint64_t carry = 0, all = 0;
+    for (uint32_t q = 0; q < kScanThreads / 32; ++q) {
+        uint64_t t = s_warp[q];
+        if (q < warp) carry += t;
+        all += t;
+    }
+    total = all;
+    return carry + incl - v;
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_reduce_kernel(const uint64_t* __restrict__ data, uint64_t n,
+                                                                   uint64_t* __restrict__ block_sums) {
+    __shared__ uint64_t s_warp[kScanThreads / 32];
+    uint64_t base = (uint64_t)blockIdx.x * kScanChunk;
+    uint64_t sum = 0;
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) {
+        uint64_t idx = base + (uint64_t)i * kScanThreads + threadIdx.x;
+        if (idx < n) sum += data[idx];
+    }
+    uint64_t total;
+    block_exclusive_scan(sum, s_warp, total);
+    if (threadIdx.x == 0) block_sums[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_sums_kernel(uint64_t* __restrict__ block_sums, uint64_t n_blocks,
+                                                                 uint64_t* __restrict__ total_out) {
+    __shared__ uint64_t s_warp[kScanThreads / 32];
+    uint64_t carry = 0;
+    for (uint64_t base = 0; base < n_blocks; base += kScanThreads) {
+        uint64_t idx = base + threadIdx.x;
+        uint64_t v = idx < n_blocks ? block_sums[idx] : 0;
+        uint64_t total;
+        uint64_t excl = block_exclusive_scan(v, s_warp, total);
+        if (idx < n_blocks) block_sums[idx] = carry + excl;
+        carry += total;
+    }
+    if (threadIdx.x == 0) *total_out = carry;
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_down_kernel(uint64_t* __restrict__ data, uint64_t n,
+                                                                 const uint64_t* __restrict__ block_sums) {
+    __shared__ uint64_t s_warp[kScanThreads / 32];
+    // blocked arrangement: thread t owns kScanItems consecutive entries
+    uint64_t base = (uint64_t)blockIdx.x * kScanChunk + (uint64_t)threadIdx.x * kScanItems;
+    uint64_t v[kScanItems];
+    uint64_t sum = 0;
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) {
+        v[i] = base + i < n ? data[base + i] : 0;
+        sum += v[i];
+    }
+    uint64_t total;
+    uint64_t run = block_exclusive_scan(sum, s_warp, total) + block_sums[blockIdx.x];
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) {
+        if (base + i < n) data[base + i] = run;
+        run += v[i];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// global path: compact + re-key, write back
+// ---------------------------------------------------------------------------------------------
+template <typename IdT>
+__global__ void __launch_bounds__(256) refine_rekey_kernel(Reads R, const uint32_t* __restrict__ heads,
+                                                           const uint64_t* __restrict__ word_base, const IdT* __restrict__ ids,
+                                                           uint64_t n, uint32_t depth, uint32_t w, uint64_t* __restrict__ keys_c,
+                                                           IdT* __restrict__ ids_c, uint32_t* __restrict__ pos_c) {
+    uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    uint64_t wi = j >> 5;
+    uint32_t bit = (uint32_t)(j & 31);
+    uint32_t act, ah;
+    active_masks(heads[wi], heads[wi + 1], act, ah);
+    if (!((act >> bit) & 1u)) return;
+    uint64_t base = word_base[wi];
+    uint32_t below = (1u << bit) - 1;
+    uint64_t c = (base & 0xffffffffull) + __popc(act & below);
+    uint64_t g = (base >> 32) + __popc(ah & (below | (1u << bit))) - 1;   // ordinal of this element's group
+    IdT id = ids[j];
+    uint64_t key = key_at_depth(R, id, depth, w);
+    keys_c[c] = (g << (2 * w + 5)) | key;
+    ids_c[c] = id;
+    pos_c[c] = (uint32_t)j;
+}
+
+template <typename IdT>
+__global__ void __launch_bounds__(256) refine_writeback_kernel(const uint64_t* __restrict__ keys_c, const IdT* __restrict__ ids_c,
+                                                               const uint32_t* __restrict__ pos_c, uint64_t n_c, uint32_t w,
+                                                               IdT* __restrict__ ids, uint32_t* __restrict__ heads) {
+    uint64_t c = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= n_c) return;
+    uint64_t k = keys_c[c];
+    uint32_t pos = pos_c[c];
+    ids[pos] = ids_c[c];
+    bool head = c == 0 || k != keys_c[c - 1] || (uint32_t)(k & 31) < w;
+    if (head) atomicOr(&heads[pos >> 5], 1u << (pos & 31));
+}
+
+// ---------------------------------------------------------------------------------------------
+// local path
+// ---------------------------------------------------------------------------------------------
+constexpr int kLocalElems = kLocalTile + kLocalGroupCap;   // positions a block may touch
+constexpr int kLocalWords = kLocalElems / 32 + 2;
+constexpr int kLocalItems = (kLocalElems + kLocalThreads - 1) / kLocalThreads;
+constexpr uint32_t kLocalW = 29;                            // bases per in-block round
+constexpr uint16_t kNone = 0xffff;
+
+template <typename IdT>
+struct LocalSmem {
+    uint64_t key_a[kLocalElems];
+    uint64_t key_b[kLocalElems];
+    IdT id_a[kLocalElems];
+    IdT id_b[kLocalElems];
+    uint16_t gs[kLocalElems];   // first position of the element's current group (kNone: not ours / placed)
+    uint16_t ge[kLocalElems];   // one past its last position
+    uint32_t hw[kLocalWords];   // head bits of the window, updated as groups split
+    uint32_t hw0[kLocalWords];  // as loaded
+    uint8_t owned[kLocalElems];
+};
+
+// nearest set bit at or below position e, not lower than `lo`; -1 if none
+__device__ __forceinline__ int prev_head(const uint32_t* hw, int e, int lo) {
+    int wi = e >> 5;
+    uint32_t bits = hw[wi] & (0xffffffffu >> (31 - (e & 31)));
+    while (true) {
+        if (bits) {
+            int p = (wi << 5) + 31 - __clz(bits);
+            return p >= lo ? p : -1;
+        }
+        if ((wi << 5) <= lo) return -1;
+        --wi;
+        bits = hw[wi];
+    }
+}
+// nearest set bit above position e, not higher than `hi`; -1 if none
+__device__ __forceinline__ int next_head(const uint32_t* hw, int e, int hi) {
+    int wi = e >> 5;
+    uint32_t bits = (e & 31) == 31 ? 0u : hw[wi] & (0xffffffffu << ((e & 31) + 1));
+    while (true) {
+        if (bits) {
+            int p = (wi << 5) + __ffs(bits) - 1;
+            return p <= hi ? p : -1;
+        }
+        ++wi;
+        if ((wi << 5) > hi) return -1;
+        bits = hw[wi];
+    }
+}
+
+template <typename IdT>
+__global__ void __launch_bounds__(kLocalThreads) refine_local_kernel(Reads R, const uint32_t* __restrict__ heads_in,
+                                                                     uint32_t* __restrict__ heads_out, IdT* __restrict__ ids, uint64_t n,
+                                                                     uint32_t depth0, uint32_t cap, unsigned long long* elems_done) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    LocalSmem<IdT>& sm = *reinterpret_cast<LocalSmem<IdT>*>(smem_raw);
+    const uint64_t base = (uint64_t)blockIdx.x * kLocalTile;
+    const uint64_t w0 = base >> 5;
+    const uint64_t n_words = ((n + 31) >> 5) + 1;   // including the padding word
+    const int tid = threadIdx.x;
+
+    uint32_t incomplete = 0;
+    for (int i = tid; i < kLocalWords; i += kLocalThreads) {
+        uint32_t v = w0 + i < n_words ? heads_in[w0 + i] : kFull;
+        sm.hw[i] = v;
+        sm.hw0[i] = v;
+        // positions 1 .. kLocalTile decide whether a group of >= 2 starts in this tile
+        if (i <= kLocalTile / 32) {
+            uint32_t care = i == 0 ? ~1u : (i == kLocalTile / 32 ? 1u : kFull);
+            incomplete |= (~v) & care;
+        }
+    }
+    if (!__syncthreads_or(incomplete)) return;
+
+    // classify: which positions belong to a group that starts in this tile and has 2..cap members
+    uint32_t mine = 0;
+#pragma unroll
+    for (int k = 0; k < kLocalItems; ++k) {
+        int e = k * kLocalThreads + tid;
+        if (e >= kLocalElems) break;
+        uint16_t s = kNone, t = kNone;
+        uint8_t own = 0;
+        if (base + e < n) {
+            int lo = e - (int)cap + 1;
+            int ps = prev_head(sm.hw, e, lo < 0 ? 0 : lo);
+            if (ps >= 0 && ps < kLocalTile) {
+                int ne = next_head(sm.hw, e, ps + (int)cap);
+                if (ne > 0 && ne - ps >= 2) {
+                    s = (uint16_t)ps;
+                    t = (uint16_t)ne;
+                    own = 1;
+                    sm.id_a[e] = ids[base + e];
+                    ++mine;
+                }
+            }
+        }
+        sm.gs[e] = s;
+        sm.ge[e] = t;
+        sm.owned[e] = own;
+    }
+    __syncthreads();
+
+    for (uint32_t depth = depth0;; depth += kLocalW) {
+        // one window gather per member still tied
+        uint32_t any = 0;
+#pragma unroll
+        for (int k = 0; k < kLocalItems; ++k) {
+            int e = k * kLocalThreads + tid;
+            if (e >= kLocalElems) break;
+            if (sm.gs[e] != kNone) {
+                sm.key_a[e] = key_at_depth(R, sm.id_a[e], depth, kLocalW);
+                any = 1;
+            }
+        }
+        if (!__syncthreads_or(any)) break;
+        // stable rank inside the group by counting smaller members
+#pragma unroll
+        for (int k = 0; k < kLocalItems; ++k) {
+            int e = k * kLocalThreads + tid;
+            if (e >= kLocalElems) break;
+            int s = sm.gs[e];
+            if (s != kNone) {
+                int t = sm.ge[e];
+                uint64_t mykey = sm.key_a[e];
+                int cnt = 0;
+                for (int q = s; q < t; ++q) {
+                    uint64_t kq = sm.key_a[q];
+                    cnt += (kq < mykey) || (kq == mykey && q < e);
+                }
+                sm.key_b[s + cnt] = mykey;
+                sm.id_b[s + cnt] = sm.id_a[e];
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < kLocalItems; ++k) {
+            int e = k * kLocalThreads + tid;
+            if (e >= kLocalElems) break;
+            if (sm.gs[e] != kNone) {
+                uint64_t kk = sm.key_b[e];
+                sm.key_a[e] = kk;
+                sm.id_a[e] = sm.id_b[e];
+                bool head = e == sm.gs[e] || kk != sm.key_b[e - 1] || (uint32_t)(kk & 31) < kLocalW;
+                if (head) atomicOr(&sm.hw[e >> 5], 1u << (e & 31));
+            }
+        }
+        __syncthreads();
+        // new group bounds; singletons are placed for good
+#pragma unroll
+        for (int k = 0; k < kLocalItems; ++k) {
+            int e = k * kLocalThreads + tid;
+            if (e >= kLocalElems) break;
+            int s = sm.gs[e];
+            if (s != kNone) {
+                int t = sm.ge[e];
+                int ps = prev_head(sm.hw, e, s);
+                int ne = next_head(sm.hw, e, t);
+                if (ne - ps >= 2) {
+                    sm.gs[e] = (uint16_t)ps;
+                    sm.ge[e] = (uint16_t)ne;
+                } else {
+                    sm.gs[e] = kNone;
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    // publish: ids of our groups, and their positions as heads (every member is placed)
+#pragma unroll
+    for (int k = 0; k < kLocalItems; ++k) {
+        int e = k * kLocalThreads + tid;
+        if (e >= kLocalElems) break;
+        if (sm.owned[e]) ids[base + e] = sm.id_a[e];
+    }
+    for (int i = tid; i < kLocalWords; i += kLocalThreads) {
+        uint32_t add = sm.hw[i] & ~sm.hw0[i];
+        if (add) atomicOr(&heads_out[w0 + i], add);
+    }
+    for (int o = 16; o; o >>= 1) mine += __shfl_xor_sync(kFull, mine, o);
+    if (lane_id() == 0 && mine) atomicAdd(elems_done, (unsigned long long)mine);
+}
+
+// ---------------------------------------------------------------------------------------------
+// a8: emit.  B[k] = '$' if the k-th suffix starts its read, else the base before it
+// ---------------------------------------------------------------------------------------------
+template <typename IdT>
+__device__ __forceinline__ uint8_t preceding_symbol(const Reads& R, IdT id) {
+    uint64_t read = (uint64_t)id >> R.pos_bits;
+    uint64_t pos = (uint64_t)id & ((1ull << R.pos_bits) - 1);
+    if (pos == 0) return (uint8_t)'$';
+    uint64_t b = (R.uniform ? read * R.uniform_len : __ldg(R.offsets + read)) + pos - 1;
+    uint32_t code = (uint32_t)(__ldg(R.packed + (b >> 5)) >> (62 - 2 * (b & 31))) & 3u;
+    return (uint8_t)((0x54474341u >> (8 * code)) & 0xFFu);
+}
+
+template <typename IdT>
+__global__ void __launch_bounds__(256) emit_kernel(Reads R, const IdT* __restrict__ ids, uint64_t n, uint8_t* __restrict__ out) {
+    // four consecutive outputs per thread where the address allows a 32-bit store
+    uint64_t lead = (4 - (reinterpret_cast<uintptr_t>(out) & 3)) & 3;   // bytes before the first aligned word
+    if (lead > n) lead = n;
+    uint64_t q = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint64_t n_quads = (n - lead) >> 2;
+    if (q < n_quads) {
+        uint64_t j = lead + (q << 2);
+        uint32_t v = 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) v |= (uint32_t)preceding_symbol(R, __ldcs(ids + j + i)) << (8 * i);
+        *reinterpret_cast<uint32_t*>(out + j) = v;
+    } else if (q == n_quads) {
+        for (uint64_t j = 0; j < lead; ++j) out[j] = preceding_symbol(R, ids[j]);
+        for (uint64_t j = lead + (n_quads << 2); j < n; ++j) out[j] = preceding_symbol(R, ids[j]);
+    }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// launchers
+// ---------------------------------------------------------------------------------------------
+cudaError_t launch_flag_heads(const uint64_t* keys, uint64_t n, uint32_t w, uint32_t* heads, cudaStream_t s) {
+    if (n == 0) return cudaSuccess;
+    uint64_t padded = ((n + 31) >> 5) << 5;
+    flag_heads_kernel<<<(unsigned)((padded + 255) / 256), 256, 0, s>>>(keys, n, w, heads);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_active_count(const uint32_t* heads, uint64_t n, uint64_t* word_counts, cudaStream_t s) {
+    uint64_t n_words = (n + 31) >> 5;
+    if (n_words == 0) return cudaSuccess;
+    active_count_kernel<<<(unsigned)((n_words + 255) / 256), 256, 0, s>>>(heads, n_words, word_counts);
+    return cudaGetLastError();
+}
+
+uint64_t scan_block_count(uint64_t n) { return (n + kScanChunk - 1) / kScanChunk; }
+
+cudaError_t launch_scan_u64(uint64_t* data, uint64_t n, uint64_t* block_sums, uint64_t* total, cudaStream_t s) {
+    if (n == 0) return cudaMemsetAsync(total, 0, sizeof(uint64_t), s);
+    uint64_t blocks = scan_block_count(n);
+    scan_reduce_kernel<<<(unsigned)blocks, kScanThreads, 0, s>>>(data, n, block_sums);
+    scan_sums_kernel<<<1, kScanThreads, 0, s>>>(block_sums, blocks, total);
+    scan_down_kernel<<<(unsigned)blocks, kScanThreads, 0, s>>>(data, n, block_sums);
+    return cudaGetLastError();
+}
+
+template <typename IdT>
+cudaError_t launch_refine_rekey(const Reads& R, const uint32_t* heads, const uint64_t* word_base, const IdT* ids, uint64_t n,
+                                uint32_t depth, uint32_t w, uint64_t* keys_c, IdT* ids_c, uint32_t* pos_c, cudaStream_t s) {
+    if (n == 0) return cudaSuccess;
+    refine_rekey_kernel<IdT><<<(unsigned)((n + 255) / 256), 256, 0, s>>>(R, heads, word_base, ids, n, depth, w, keys_c, ids_c, pos_c);
+    return cudaGetLastError();
+}
+
+template <typename IdT>
+cudaError_t launch_refine_writeback(const uint64_t* keys_c, const IdT* ids_c, const uint32_t* pos_c, uint64_t n_c, uint32_t w,
+                                    IdT* ids, uint32_t* heads, cudaStream_t s) {
+    if (n_c == 0) return cudaSuccess;
+    refine_writeback_kernel<IdT><<<(unsigned)((n_c + 255) / 256), 256, 0, s>>>(keys_c, ids_c, pos_c, n_c, w, ids, heads);
+    return cudaGetLastError();
+}
+
+template <typename IdT>
+cudaError_t launch_refine_local(const Reads& R, const uint32_t* heads_in, uint32_t* heads_out, IdT* ids, uint64_t n, uint32_t depth,
+                                uint32_t group_cap, unsigned long long* elems_done, cudaStream_t s) {
+    if (n == 0) return cudaSuccess;
+    auto kernel = refine_local_kernel<IdT>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem<IdT>));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
+    uint64_t blocks = (n + kLocalTile - 1) / kLocalTile;
+    kernel<<<(unsigned)blocks, kLocalThreads, sizeof(LocalSmem<IdT>), s>>>(R, heads_in, heads_out, ids, n, depth, group_cap, elems_done);
+    return cudaGetLastError();
+}
+
+template <typename IdT>
+cudaError_t launch_emit(const Reads& R, const IdT* ids, uint64_t n, uint8_t* out, cudaStream_t s) {
+    if (n == 0) return cudaSuccess;
+    uint64_t threads = (n >> 2) + 1;
+    emit_kernel<IdT><<<(unsigned)((threads + 255) / 256), 256, 0, s>>>(R, ids, n, out);
+    return cudaGetLastError();
+}
+
+#define CX_INSTANTIATE(IdT)                                                                                                          \
+    template cudaError_t launch_refine_rekey<IdT>(const Reads&, const uint32_t*, const uint64_t*, const IdT*, uint64_t, uint32_t,   \
+                                                  uint32_t, uint64_t*, IdT*, uint32_t*, cudaStream_t);                               \
+    template cudaError_t launch_refine_writeback<IdT>(const uint64_t*, const IdT*, const uint32_t*, uint64_t, uint32_t, IdT*,       \
+                                                      uint32_t*, cudaStream_t);                                                      \
+    template cudaError_t launch_refine_local<IdT>(const Reads&, const uint32_t*, uint32_t*, IdT*, uint64_t, uint32_t, uint32_t,     \
+                                                  unsigned long long*, cudaStream_t);                                                \
+    template cudaError_t launch_emit<IdT>(const Reads&, const IdT*, uint64_t, uint8_t*, cudaStream_t);
+CX_INSTANTIATE(uint32_t)
+CX_INSTANTIATE(uint64_t)
+
+}  // namespace cx

@@ -1,0 +1,367 @@
+// cx_scan_reads.cu -- the kernels that walk every suffix of R in (read, position) order:
+//   prep        offsets sanity, longest read, uniform-length test
+//   tile table  first read of every tile of kListTile consecutive suffix slots
+//   a2 bucket histogram   (Fig. 2 step 1: "Scan all suffixes ... Store the size of each partition")
+//   a4+a5 list + key build (Fig. 2 steps 3(a), 3(c)i; key = the paper's "stringword")
+//
+// A suffix slot g in [0, N) is suffix (i, p) with g = offsets[i] + i + p: reads laid end to end, each
+// followed by one slot for its end-marker.  Slots ascend in (read, position) order, which is the
+// listing order PAPER.md:99 requires for the stable sort to realise $_i < $_j.
+#include "cx_internal.cuh"
+
+namespace cx {
+namespace {
+
+// ---------------------------------------------------------------------------------------------
+// prep
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) prep_kernel(const uint64_t* __restrict__ offsets, uint64_t n_reads, BuildInfo* info) {
+    uint64_t first_len = offsets[1] - offsets[0];
+    uint64_t local_max = 0;
+    uint32_t bad = 0, nonuni = 0;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_reads; i += (uint64_t)gridDim.x * blockDim.x) {
+        uint64_t a = offsets[i], b = offsets[i + 1];
+        if (b < a) {
+            bad = 1;
+        } else {
+            uint64_t len = b - a;
+            local_max = len > local_max ? len : local_max;
+            nonuni |= len != first_len;
+        }
+    }
+    for (int o = 16; o; o >>= 1) {
+        uint64_t other = __shfl_xor_sync(0xffffffffu, local_max, o);
+        local_max = other > local_max ? other : local_max;
+    }
+    bad = __any_sync(0xffffffffu, bad);
+    nonuni = __any_sync(0xffffffffu, nonuni);
+    if (lane_id() == 0) {
+        if (local_max) atomicMax((unsigned long long*)&info->max_len, (unsigned long long)local_max);
+        if (bad) atomicOr(&info->bad_offsets, 1u);
+        if (nonuni) atomicOr(&info->nonuniform, 1u);
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        if (offsets[0] != 0) atomicOr(&info->bad_offsets, 1u);
+        info->total_bases = offsets[n_reads];
+        info->n_suffixes = offsets[n_reads] + n_reads;
+        info->first_len = first_len;
+    }
+}
+
+// tile_first_read[t] = the read that owns slot t * kListTile (largest i with offsets[i] + i <= slot)
+__global__ void __launch_bounds__(256) tile_table_kernel(const uint64_t* __restrict__ offsets, uint64_t n_reads,
+                                                         const BuildInfo* __restrict__ info, uint32_t* __restrict__ tile_first_read,
+                                                         uint64_t max_tiles) {
+    uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint64_t N = info->n_suffixes;
+    uint64_t n_tiles = (N + kListTile - 1) / kListTile;
+    if (t >= n_tiles || t >= max_tiles) return;
+    uint64_t g = t * kListTile;
+    uint64_t lo = 0, hi = n_reads - 1;   // invariant: offsets[lo] + lo <= g
+    while (lo < hi) {
+        uint64_t mid = (lo + hi + 1) >> 1;
+        if (offsets[mid] + mid <= g) lo = mid; else hi = mid - 1;
+    }
+    tile_first_read[t] = (uint32_t)lo;
+}
+
+// ---------------------------------------------------------------------------------------------
+// tile decode: the reads and packed bases that the slots [g0, g0 + kListTile) touch
+// ---------------------------------------------------------------------------------------------
+struct TileSmem {
+    uint64_t off[kListTile + 2];           // offsets of the reads that intersect the tile
+    uint64_t packed[kListTile / 32 + 4];   // the bases of the tile plus one window of look-ahead
+    uint32_t scan[kListItems * (kListThreads / 32) + 1];
+};
+
+struct TileCtx {
+    uint64_t g0;        // first slot
+    uint32_t n_slots;   // slots in this tile
+    uint64_t r0;        // first read
+    uint32_t n_tile_reads;
+    uint64_t word0;     // first packed word staged
+};
+
+__device__ __forceinline__ TileCtx load_tile(const Reads& R, const uint32_t* __restrict__ tile_first_read, uint64_t t,
+                                             uint64_t n_tiles, uint64_t N, TileSmem& sm) {
+    TileCtx c;
+    c.g0 = t * kListTile;
+    c.n_slots = (uint32_t)min((uint64_t)kListTile, N - c.g0);
+    c.r0 = tile_first_read[t];
+    uint64_t r_last = (t + 1 < n_tiles) ? (uint64_t)tile_first_read[t + 1] : R.n_reads - 1;
+    c.n_tile_reads = (uint32_t)(r_last - c.r0 + 1);                       // <= kListTile + 1
+    for (uint32_t j = threadIdx.x; j <= c.n_tile_reads; j += blockDim.x) sm.off[j] = R.offsets[c.r0 + j];
+    // base position of slot g is g - (its read index); it grows by 0 or 1 per slot
+    uint64_t b0 = c.g0 - c.r0;
+    c.word0 = b0 >> 5;
+    for (uint32_t j = threadIdx.x; j < kListTile / 32 + 4; j += blockDim.x) {
+        uint64_t wi = c.word0 + j;
+        sm.packed[j] = wi < R.n_words ? __ldg(R.packed + wi) : 0ull;
+    }
+    __syncthreads();
+    return c;
+}
+
+struct Slot {
+    uint64_t read, pos, rem;   // suffix (read, pos); rem = bases left = m_i - pos
+    uint64_t window;           // the next 32 bases, MSB-first, junk past rem
+};
+
+__device__ __forceinline__ Slot decode_slot(const TileCtx& c, const TileSmem& sm, uint32_t s) {
+    uint64_t g = c.g0 + s;
+    // largest j with off[j] + r0 + j <= g
+    uint32_t lo = 0, hi = c.n_tile_reads - 1;
+    while (lo < hi) {
+        uint32_t mid = (lo + hi + 1) >> 1;
+        if (sm.off[mid] + c.r0 + mid <= g) lo = mid; else hi = mid - 1;
+    }
+    Slot sl;
+    sl.read = c.r0 + lo;
+    uint64_t start = sm.off[lo];
+    sl.pos = g - (start + sl.read);
+    sl.rem = sm.off[lo + 1] - start - sl.pos;
+    uint64_t b = start + sl.pos;
+    uint32_t wi = (uint32_t)((b >> 5) - c.word0);
+    uint32_t sh = (uint32_t)(b & 31) * 2;
+    uint64_t w0 = sm.packed[wi], w1 = sm.packed[wi + 1];
+    sl.window = sh ? (w0 << sh) | (w1 >> (64 - sh)) : w0;
+    return sl;
+}
+
+// Partition code of a suffix (reading A4 of PAPER.md:79 "suffixes shorter than l require special
+// but easy handling"): (first l bases, A-padded) * (l + 1) + min(rem, l).  Order-preserving.
+__device__ __forceinline__ uint32_t bucket_of(const Slot& sl, uint32_t ell, uint32_t& kmer, uint32_t& r) {
+    r = sl.rem < ell ? (uint32_t)sl.rem : ell;
+    kmer = r ? (uint32_t)((sl.window >> (64 - 2 * r)) << (2 * (ell - r))) : 0u;
+    return kmer * (ell + 1) + r;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2: bucket histogram.  Persistent blocks; full-length partitions (the bulk) are counted in a
+// shared-memory histogram with warp-aggregated updates, the few short ones go straight to global.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kListThreads) bucket_hist_kernel(Reads R, const BuildInfo* __restrict__ info,
+                                                                   const uint32_t* __restrict__ tile_first_read, uint32_t ell,
+                                                                   unsigned long long* __restrict__ hist) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    TileSmem& sm = *reinterpret_cast<TileSmem*>(smem_raw);
+    uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem_raw + sizeof(TileSmem));
+    const uint32_t n_kmers = 1u << (2 * ell);
+    for (uint32_t k = threadIdx.x; k < n_kmers; k += blockDim.x) s_hist[k] = 0;
+    R.n_words = (info->total_bases + 31) >> 5;
+    const uint64_t N = info->n_suffixes;
+    const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        __syncthreads();   // previous tile done with sm (and s_hist zeroed on the first trip)
+        TileCtx c = load_tile(R, tile_first_read, t, n_tiles, N, sm);
+#pragma unroll
+        for (int k = 0; k < kListItems; ++k) {
+            uint32_t s = k * kListThreads + threadIdx.x;
+            bool valid = s < c.n_slots;
+            uint32_t kmer = 0, r = 0, code = 0xffffffffu;
+            if (valid) {
+                Slot sl = decode_slot(c, sm, s);
+                uint32_t b = bucket_of(sl, ell, kmer, r);
+                if (r == ell) code = kmer;
+                else atomicAdd(hist + b, 1ull);
+            }
+            // warp-aggregated update: one shared-memory atomic per distinct k-mer in the warp
+            uint32_t peers = __match_any_sync(0xffffffffu, code);
+            if (code != 0xffffffffu && (peers & lanemask_lt()) == 0) atomicAdd(&s_hist[code], (uint32_t)__popc(peers));
+        }
+    }
+    __syncthreads();
+    for (uint32_t k = threadIdx.x; k < n_kmers; k += blockDim.x) {
+        uint32_t v = s_hist[k];
+        if (v) atomicAdd(hist + (uint64_t)k * (ell + 1) + ell, (unsigned long long)v);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a4 (count half): suffixes per tile whose partition lies in [bucket_lo, bucket_hi]
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const BuildInfo* __restrict__ info,
+                                                                  const uint32_t* __restrict__ tile_first_read, uint32_t ell,
+                                                                  uint32_t bucket_lo, uint32_t bucket_hi, uint64_t* __restrict__ tile_count) {
+    __shared__ TileSmem sm;
+    __shared__ uint32_t s_total;
+    R.n_words = (info->total_bases + 31) >> 5;
+    const uint64_t N = info->n_suffixes;
+    const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
+    uint64_t t = blockIdx.x;
+    if (t >= n_tiles) return;
+    if (threadIdx.x == 0) s_total = 0;
+    TileCtx c = load_tile(R, tile_first_read, t, n_tiles, N, sm);
+    uint32_t mine = 0;
+#pragma unroll
+    for (int k = 0; k < kListItems; ++k) {
+        uint32_t s = k * kListThreads + threadIdx.x;
+        if (s < c.n_slots) {
+            Slot sl = decode_slot(c, sm, s);
+            uint32_t kmer, r;
+            uint32_t b = bucket_of(sl, ell, kmer, r);
+            mine += (b >= bucket_lo && b <= bucket_hi);
+        }
+    }
+    for (int o = 16; o; o >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
+    if (lane_id() == 0 && mine) atomicAdd(&s_total, mine);
+    __syncthreads();
+    if (threadIdx.x == 0) tile_count[t] = s_total;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a4 (write half) + a5: ids of the batch in (read, pos) order, each with its first key.
+// The read is in shared memory already, so the round-1 key costs no gather.
+// ---------------------------------------------------------------------------------------------
+template <typename IdT, bool ALL>
+__global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const BuildInfo* __restrict__ info,
+                                                                  const uint32_t* __restrict__ tile_first_read, uint32_t ell, uint32_t w,
+                                                                  uint32_t bucket_lo, uint32_t bucket_hi,
+                                                                  const uint64_t* __restrict__ tile_base, uint64_t* __restrict__ keys,
+                                                                  IdT* __restrict__ ids) {
+    __shared__ TileSmem sm;
+    R.n_words = (info->total_bases + 31) >> 5;
+    const uint64_t N = info->n_suffixes;
+    const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
+    uint64_t t = blockIdx.x;
+    if (t >= n_tiles) return;
+    TileCtx c = load_tile(R, tile_first_read, t, n_tiles, N, sm);
+    const uint32_t warp = threadIdx.x >> 5;
+    constexpr int kWarps = kListThreads / 32;
+
+    uint64_t key[kListItems];
+    IdT id[kListItems];
+    uint32_t rank[kListItems];
+    bool take[kListItems];
+#pragma unroll
+    for (int k = 0; k < kListItems; ++k) {
+        uint32_t s = k * kListThreads + threadIdx.x;
+        take[k] = false;
+        key[k] = 0;
+        id[k] = 0;
+        rank[k] = 0;
+        if (s < c.n_slots) {
+            Slot sl = decode_slot(c, sm, s);
+            key[k] = make_key(sl.window, sl.rem, w);
+            id[k] = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
+            if (ALL) {
+                take[k] = true;
+            } else {
+                uint32_t kmer, r;
+                uint32_t b = bucket_of(sl, ell, kmer, r);
+                take[k] = b >= bucket_lo && b <= bucket_hi;
+            }
+        }
+        if (!ALL) {
+            uint32_t m = __ballot_sync(0xffffffffu, take[k]);
+            rank[k] = __popc(m & lanemask_lt());
+            if (lane_id() == 0) sm.scan[k * kWarps + warp] = __popc(m);
+        }
+    }
+    if (ALL) {
+#pragma unroll
+        for (int k = 0; k < kListItems; ++k) {
+            uint32_t s = k * kListThreads + threadIdx.x;
+            if (take[k]) {
+                keys[c.g0 + s] = key[k];
+                ids[c.g0 + s] = id[k];
+            }
+        }
+        return;
+    }
+    __syncthreads();
+    // exclusive scan of the kListItems * kWarps row counts (slot order = item-major, then warp)
+    if (threadIdx.x < 32) {
+        uint32_t carry = 0;
+        for (int base = 0; base < kListItems * kWarps; base += 32) {
+            uint32_t idx = base + threadIdx.x;
+            uint32_t v = idx < kListItems * kWarps ? sm.scan[idx] : 0;
+            uint32_t incl = v;
+            for (int o = 1; o < 32; o <<= 1) {
+                uint32_t up = __shfl_up_sync(0xffffffffu, incl, o);
+                if ((int)threadIdx.x >= o) incl += up;
+            }
+            if (idx < kListItems * kWarps) sm.scan[idx] = carry + incl - v;
+            carry += __shfl_sync(0xffffffffu, incl, 31);
+        }
+    }
+    __syncthreads();
+    const uint64_t base = tile_base[t];
+#pragma unroll
+    for (int k = 0; k < kListItems; ++k) {
+        if (take[k]) {
+            uint64_t dst = base + sm.scan[k * kWarps + warp] + rank[k];
+            keys[dst] = key[k];
+            ids[dst] = id[k];
+        }
+    }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// launchers
+// ---------------------------------------------------------------------------------------------
+cudaError_t launch_prep(const uint64_t* offsets, uint64_t n_reads, BuildInfo* info, cudaStream_t s) {
+    cudaError_t e = cudaMemsetAsync(info, 0, sizeof(BuildInfo), s);
+    if (e != cudaSuccess) return e;
+    uint64_t blocks = (n_reads + 255) / 256;
+    unsigned grid = (unsigned)(blocks < 148ull * 8 ? (blocks ? blocks : 1) : 148ull * 8);
+    prep_kernel<<<grid, 256, 0, s>>>(offsets, n_reads, info);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_tile_table(const uint64_t* offsets, uint64_t n_reads, const BuildInfo* info, uint32_t* tile_first_read,
+                              uint64_t max_tiles, cudaStream_t s) {
+    if (max_tiles == 0) return cudaSuccess;
+    unsigned grid = (unsigned)((max_tiles + 255) / 256);
+    tile_table_kernel<<<grid, 256, 0, s>>>(offsets, n_reads, info, tile_first_read, max_tiles);
+    return cudaGetLastError();
+}
+
+size_t bucket_hist_smem(uint32_t ell) { return sizeof(TileSmem) + (sizeof(uint32_t) << (2 * ell)); }
+
+cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
+                               uint64_t* hist, uint64_t max_tiles, int n_sms, cudaStream_t s) {
+    if (max_tiles == 0) return cudaSuccess;
+    size_t smem = bucket_hist_smem(ell);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(bucket_hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bucket_hist_smem(7));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    int per_sm = ell <= 6 ? 4 : 2;
+    uint64_t want = (uint64_t)n_sms * per_sm;
+    unsigned grid = (unsigned)(max_tiles < want ? max_tiles : want);
+    bucket_hist_kernel<<<grid, kListThreads, smem, s>>>(R, info, tile_first_read, ell, (unsigned long long*)hist);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
+                              uint32_t bucket_lo, uint32_t bucket_hi, uint64_t* tile_count, uint64_t n_tiles, cudaStream_t s) {
+    if (n_tiles == 0) return cudaSuccess;
+    list_count_kernel<<<(unsigned)n_tiles, kListThreads, 0, s>>>(R, info, tile_first_read, ell, bucket_lo, bucket_hi, tile_count);
+    return cudaGetLastError();
+}
+
+template <typename IdT>
+cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
+                              uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, uint64_t* keys, IdT* ids,
+                              uint64_t n_tiles, cudaStream_t s) {
+    if (n_tiles == 0) return cudaSuccess;
+    if (tile_base == nullptr)
+        list_write_kernel<IdT, true><<<(unsigned)n_tiles, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
+                                                                               nullptr, keys, ids);
+    else
+        list_write_kernel<IdT, false><<<(unsigned)n_tiles, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
+                                                                                tile_base, keys, ids);
+    return cudaGetLastError();
+}
+
+template cudaError_t launch_list_write<uint32_t>(const Reads&, const BuildInfo*, const uint32_t*, uint32_t, uint32_t, uint32_t,
+                                                 uint32_t, const uint64_t*, uint64_t*, uint32_t*, uint64_t, cudaStream_t);
+template cudaError_t launch_list_write<uint64_t>(const Reads&, const BuildInfo*, const uint32_t*, uint32_t, uint32_t, uint32_t,
+                                                 uint32_t, const uint64_t*, uint64_t*, uint64_t*, uint64_t, cudaStream_t);
+
+}  // namespace cx

@@ -1,0 +1,206 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Integer/byte work: the bar is bit-exact.  Needs a B200: `pytest -m gpu`."""
+import itertools
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from tests import bwt_checks as chk
+from workloads import generate as gen
+
+pytestmark = pytest.mark.gpu
+
+
+def gpu_bwt(coll, **opts):
+    import paper_1401_7457_b200 as cx
+    opts.setdefault("max_read_len", max(coll.max_read_len, 1))
+    return cx.bwt_of_collection(coll.ascii, coll.offsets, **opts)
+
+
+def assert_parity(coll, **opts):
+    want = oracle.bwt(coll.ascii, coll.offsets)
+    got = gpu_bwt(coll, **opts)
+    assert got.shape == want.shape
+    if not np.array_equal(got, want):
+        bad = np.flatnonzero(got != want)
+        raise AssertionError(f"{coll.name} {opts}: {bad.size} of {want.size} symbols differ, first at {bad[:5]}: "
+                             f"got {got[bad[:5]].tobytes()} want {want[bad[:5]].tobytes()}")
+
+
+# ---- the paper's worked example and the closed forms ---------------------------------------------
+
+def test_figure1():
+    got = gpu_bwt(gen.from_strings(["ACGT", "TAGT", "GGAA"]))
+    assert got.tobytes() == b"TTAAG$TAG$CAGG$"          # PAPER.md:59, Figure 1
+
+
+@pytest.mark.parametrize("reads,want", [
+    (["ACGT"] * 3, "TTT$$$AAACCCGGG"),
+    (["A", "AA", "AAA"], "AAA$AA$A$"),
+    (["", "A", ""], "$A$$"),
+    ([""], "$"),
+    (["T"], "T$"),
+])
+def test_closed_forms(reads, want):
+    assert gpu_bwt(gen.from_strings(reads)).tobytes().decode() == want
+
+
+def test_empty_collection():
+    import paper_1401_7457_b200 as cx
+    assert cx.bwt_of_collection(np.zeros(0, np.uint8), np.zeros(1, np.uint64)).size == 0
+
+
+def test_all_small_collections_two_letters():
+    words = [""] + ["".join(w) for L in range(1, 4) for w in itertools.product("AC", repeat=L)]
+    for reads in itertools.product(words, repeat=2):
+        c = gen.from_strings(list(reads))
+        assert gpu_bwt(c).tobytes().decode() == oracle.bwt_of_strings(list(reads)), reads
+
+
+@pytest.mark.parametrize("seed", range(40))
+def test_random_ragged_collections(seed):
+    c = gen.random_collection(seed, n_reads=1 + (seed * 37) % 300, max_len=1 + (seed * 13) % 140,
+                              alphabet=["ACGT", "GT", "A", "CGT", "AC"][seed % 5])
+    assert_parity(c)
+    assert_parity(c, small_group_max=1)                 # global re-key path only
+    assert_parity(c, key_bases=7 + seed % 20, prefix_len=1 + seed % 7)
+
+
+def test_homopolymer_reads_one_giant_group():
+    c = gen.from_strings(["A" * 100] * 700 + ["A" * 37] * 50 + ["C" * 64] * 3)
+    assert_parity(c)
+    assert_parity(c, small_group_max=1)
+    assert_parity(c, small_group_max=16)
+
+
+def test_long_reads_and_tandem_repeats():
+    c = gen.from_strings(["ACGT" * 200, "ACGT" * 150 + "T", "CGTA" * 180, "G" * 900, ""] * 7)
+    assert_parity(c)
+
+
+# ---- config shapes ---------------------------------------------------------------------------------
+
+def test_config1_full():
+    c = gen.config(0)
+    assert_parity(c)                                     # 1,010,000 suffixes, spans many tiles + ragged tail
+
+
+@pytest.mark.parametrize("idx,scale", [(1, 0.02), (2, 0.002), (3, 0.0005), (4, 0.000002)])
+def test_config_shapes_scaled(idx, scale):
+    c = gen.config(idx, scale)
+    assert_parity(c)
+
+
+def test_eight_byte_ids():
+    c = gen.config(1, 0.02)
+    assert_parity(c, max_read_len=0)                     # unknown read length -> 64-bit suffix ids
+    import paper_1401_7457_b200 as cx
+    p = cx.Plan(c.n_reads, c.total_bases)
+    a = torch.from_numpy(c.ascii).cuda()
+    out = torch.empty(c.n_suffixes, dtype=torch.uint8, device="cuda")
+    p.build(cx.cx_pack_reads(a), torch.from_numpy(c.offsets.astype(np.int64)).cuda(), c.n_reads, out)
+    assert p.stats()["id_bytes"] == 8
+
+
+@pytest.mark.parametrize("m1", [5000, 70_000, 400_000])
+def test_multiple_batches(m1):
+    c = gen.config(2, 0.001)                             # ~1.01e6 suffixes
+    assert_parity(c, max_batch_suffixes=m1, prefix_len=5)
+    assert_parity(c, max_batch_suffixes=m1, prefix_len=6, out_is_host_pinned=0, small_group_max=1)
+
+
+def test_pinned_host_output_streams_batches():
+    import paper_1401_7457_b200 as cx
+    c = gen.config(1, 0.01)
+    want = oracle.bwt(c.ascii, c.offsets)
+    a = torch.from_numpy(c.ascii).cuda()
+    off = torch.from_numpy(c.offsets.astype(np.int64)).cuda()
+    p = cx.Plan(c.n_reads, c.total_bases, max_read_len=100, max_batch_suffixes=150_000, out_is_host_pinned=1)
+    out = torch.empty(c.n_suffixes, dtype=torch.uint8).pin_memory()
+    p.build(cx.cx_pack_reads(a), off, c.n_reads, out)
+    assert p.stats()["n_batches"] > 3
+    assert np.array_equal(out.numpy(), want)
+
+
+def test_bucket_too_large_is_reported():
+    import paper_1401_7457_b200 as cx
+    c = gen.from_strings(["A" * 100] * 200)
+    with pytest.raises(cx.CxError) as e:
+        gpu_bwt(c, max_batch_suffixes=1000)
+    assert e.value.code == cx.binding.CX_ERR_BUCKET_TOO_LARGE
+
+
+def test_deterministic():
+    c = gen.config(2, 0.001)
+    assert np.array_equal(gpu_bwt(c), gpu_bwt(c))
+
+
+# ---- single steps ------------------------------------------------------------------------------------
+
+def test_pack_matches_numpy_and_rejects_bad_bases():
+    import paper_1401_7457_b200 as cx
+    for n in (0, 1, 31, 32, 33, 1000, 100_003):
+        codes = np.random.default_rng(n).integers(0, 4, n).astype(np.uint8)
+        ascii_ = np.frombuffer(b"ACGT", np.uint8)[codes]
+        if n == 0:
+            continue
+        padded = np.zeros((n + 31) // 32 * 32, dtype=np.uint64)
+        padded[:n] = codes
+        want = np.zeros(padded.size // 32, dtype=np.uint64)
+        for j in range(32):
+            want |= padded[j::32] << np.uint64(62 - 2 * j)
+        got = cx.cx_pack_reads(torch.from_numpy(ascii_.copy()).cuda()).cpu().numpy().view(np.uint64)
+        assert np.array_equal(got, want), n
+        # unaligned input pointer
+        buf = torch.zeros(n + 3, dtype=torch.uint8, device="cuda")
+        buf[3:] = torch.from_numpy(ascii_.copy()).cuda()
+        assert np.array_equal(cx.cx_pack_reads(buf[3:]).cpu().numpy().view(np.uint64), want)
+    for bad in (b"ACGN", b"acgt", b"AC$T" * 100):
+        with pytest.raises(cx.CxError) as e:
+            cx.cx_pack_reads(torch.from_numpy(np.frombuffer(bad, np.uint8).copy()).cuda())
+        assert e.value.code == cx.binding.CX_ERR_BAD_BASE
+
+
+@pytest.mark.parametrize("n,bits,vb", [(1, 64, 4), (1000, 64, 4), (5000, 13, 8), (300_001, 63, 4), (1_000_003, 40, 8),
+                                       (2_000_000, 8, 4)])
+def test_sort_pairs_against_torch_stable_sort(n, bits, vb):
+    import paper_1401_7457_b200 as cx
+    g = torch.Generator(device="cuda").manual_seed(n)
+    keys = torch.randint(-2**63, 2**63 - 1, (n,), dtype=torch.int64, device="cuda", generator=g)
+    if bits < 64:
+        keys = keys & ((1 << bits) - 1)
+    if n > 1000:
+        keys[::3] = keys[1::3][: keys[::3].numel()]      # plenty of duplicates: stability matters
+    vals = torch.arange(n, device="cuda", dtype=torch.int32 if vb == 4 else torch.int64)
+    ks, vs = cx.cx_sort_pairs(keys, vals, 0, bits)
+    # reference order: unsigned 64-bit compare == signed compare after flipping the sign bit
+    order = torch.sort(keys ^ (-2**63), stable=True).indices
+    assert torch.equal(ks, keys[order])
+    assert torch.equal(vs.long(), order)
+
+
+def test_partition_sizes_match_linear_scan():
+    """P6 / Fig. 2 step 1: the histogram equals a plain count over the reads."""
+    import paper_1401_7457_b200 as cx
+    c = gen.config(3, 0.0001)
+    ell = 4
+    p = cx.Plan(c.n_reads, c.total_bases, max_read_len=c.max_read_len, prefix_len=ell)
+    out = torch.empty(c.n_suffixes, dtype=torch.uint8, device="cuda")
+    p.build(cx.cx_pack_reads(torch.from_numpy(c.ascii).cuda()), torch.from_numpy(c.offsets.astype(np.int64)).cuda(), c.n_reads, out)
+    got = p.histogram()
+    want = np.zeros(4 ** ell * (ell + 1), dtype=np.uint64)
+    code = {65: 0, 67: 1, 71: 2, 84: 3}
+    for i in range(c.n_reads):
+        r = c.ascii[int(c.offsets[i]):int(c.offsets[i + 1])]
+        for q in range(len(r) + 1):
+            s = r[q:q + ell]
+            k = 0
+            for ch in s:
+                k = k * 4 + code[int(ch)]
+            k <<= 2 * (ell - len(s))
+            want[k * (ell + 1) + len(s)] += 1
+    assert np.array_equal(got, want)
+    # partitions are contiguous and ordered in the output: per-partition symbol multiset check
+    chk.check_all(out.cpu().numpy(), c)
