@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for BASELINE.json's metric: suffixes sorted/s (and Gbases/hour) of the
+collection-BWT hot path on B200, with the dominant kernel's HBM roofline and the CPU oracle beside it.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--impl cx|reference]
+
+A "step" is one pass of the whole hot path (rows a1-a8 of DESIGN.md: 2-bit pack, partition sizes,
+batch plan, list + key build, onesweep sort, tie refinement, emit) over one synthetic collection.
+At N=1 the workload is BASELINE.json configs[1] (1,000,000 reads x 100 bp, 100x coverage of a seeded
+1 Mbp genome -> 1.01e8 suffixes), the case the paper's design is hardest on (deep shared substrings).
+For N>1 (torchrun, one rank per GPU) every rank runs an independent replica with its own seed: the
+north_star fixes the path to one GPU with no collectives.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+recipe; nothing else in this file touches oracle/ except the `cpu_baseline` leg.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "suffixes_sorted_per_s"
+UNIT = "suffixes/s"
+WORKLOADS = {
+    0: "configs[0]: 10,000 reads x 100 bp iid (1.01e6 suffixes)",
+    1: "configs[1]: 1,000,000 reads x 100 bp at 100x over a seeded 1 Mbp genome (1.01e8 suffixes)",
+    2: "configs[2]: 10,000,000 reads x 100 bp at 30x over 33 Mbp, both strands, 1% subst. (1.01e9 suffixes)",
+    3: "configs[3]: 40,000,000 reads x 50-250 bp over a 50 Mbp repeat genome (~6.04e9 suffixes)",
+}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture named here (None until one exists for this workload).
+NCU_TRAFFIC = {"file": None, "bytes_per_launch": None}
+FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+CPU_SAMPLE_SCALE = 0.1        # cpu_baseline leg: the workload's recipe at this scale (coverage preserved)
+REF_SAMPLE_SCALE = 0.05       # --impl reference: one step = the oracle on the recipe at this scale
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (0-based)")
+    ap.add_argument("--scale", type=float, default=1.0, help="debug only: scale the workload down")
+    ap.add_argument("--impl", default="cx", choices=["cx", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def hbm_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy read+write)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.proc = None
+        self.gpu = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------------------------------
+# CPU oracle legs (the only code in this file that may touch oracle/)
+# --------------------------------------------------------------------------------------------------
+def oracle_sample(config: int, scale: float):
+    from workloads import generate as gen
+    coll = gen.config(config, scale)
+    desc = (f"configs[{config}] recipe at scale {scale:g} (coverage preserved): {coll.n_reads:,} reads, "
+            f"{coll.n_suffixes:,} suffixes, full plain oracle (materialise, qsort with the definition's comparator, read off)")
+    return coll, desc
+
+
+def time_oracle(coll) -> float:
+    import oracle
+    t0 = time.perf_counter()
+    oracle.bwt(coll.ascii, coll.offsets)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(config: int) -> dict:
+    import oracle
+    oracle.build()
+    coll, desc = oracle_sample(config, CPU_SAMPLE_SCALE if config >= 1 else 1.0)
+    dt = time_oracle(coll)
+    return {"value": coll.n_suffixes / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc, "seconds": round(dt, 3),
+            "host_cpus": os.cpu_count()}
+
+
+def run_reference(args) -> None:
+    """The reference arm of this tier = the oracle, timed as it stands on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    oracle.build()
+    coll, desc = oracle_sample(args.config, (REF_SAMPLE_SCALE if args.config >= 1 else 1.0) * args.scale)
+    for _ in range(args.warmup):
+        time_oracle(coll)
+    times = [time_oracle(coll) for _ in range(args.steps)]
+    ms = 1e3 * sum(times) / len(times)
+    value = coll.n_suffixes / (ms / 1e3)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "u64", "data": "synthetic", "config": {"workload": WORKLOADS[args.config], "sample": desc},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gbases_per_hour": coll.total_bases / (ms / 1e3) * 3600 / 1e9, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------------
+# the CUDA arm
+# --------------------------------------------------------------------------------------------------
+def run_cx(args) -> None:
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    import paper_1401_7457_b200 as cx
+    from workloads import generate as gen
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    cx.lib()
+
+    # ---- synthetic input (seeded; replicas differ only in seed) -------------------------------------
+    coll = gen.config(args.config, args.scale, seed=gen.BASE_SEED + args.config + 1000 * rank)
+    n_reads, total, N = coll.n_reads, coll.total_bases, coll.n_suffixes
+    h_ascii = torch.from_numpy(coll.ascii).pin_memory()
+    h_off = torch.from_numpy(coll.offsets.astype(np.int64)).pin_memory()
+    h_out = torch.empty(N, dtype=torch.uint8).pin_memory()
+    d_ascii = h_ascii.to(dev)
+    d_off = h_off.to(dev)
+    d_packed = torch.empty((total + 31) // 32 + 1, dtype=torch.int64, device=dev)
+    d_out = torch.empty(N, dtype=torch.uint8, device=dev)
+    plan = cx.Plan(n_reads, total, max_read_len=coll.max_read_len, profile=1, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step_device():
+        cx.cx_pack_reads(d_ascii, d_packed, check=False)
+        plan.build(d_packed, d_off, n_reads, d_out)
+
+    def step_e2e():
+        d_ascii.copy_(h_ascii, non_blocking=True)
+        d_off.copy_(h_off, non_blocking=True)
+        cx.cx_pack_reads(d_ascii, d_packed, check=False)
+        plan.build(d_packed, d_off, n_reads, d_out)
+        h_out.copy_(d_out, non_blocking=True)
+        stream.synchronize()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        flush.fill_(1)
+        step_device()
+    torch.cuda.synchronize()
+    stats = plan.stats()
+    # cheap whole-output invariants (the parity proper is tests/ -m gpu): |B| = N, n_reads '$', base counts
+    got = torch.bincount(d_out.to(torch.int64), minlength=128).cpu().numpy()
+    want = np.bincount(coll.ascii, minlength=128)
+    want[ord("$")] += n_reads
+    if not np.array_equal(got[:128], want[:128]):
+        raise SystemExit("bench.py: output symbol counts differ from the input's")
+
+    # ---- device-resident timing -----------------------------------------------------------------------
+    classes = {k: {"ms": 0.0, "launches": 0, "bytes": 0} for k in cx.KERNEL_CLASSES}
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    pack_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    launches = 0
+    for i in range(args.steps):
+        flush.fill_(i)                       # L2 flush between timed iterations (outside the events)
+        ev[i][0].record(stream)
+        pack_ev[i][0].record(stream)
+        cx.cx_pack_reads(d_ascii, d_packed, check=False)
+        pack_ev[i][1].record(stream)
+        plan.build(d_packed, d_off, n_reads, d_out)
+        ev[i][1].record(stream)
+        stream.synchronize()
+        for k, v in plan.kernel_times().items():
+            for f in ("ms", "launches", "bytes"):
+                classes[k][f] += v[f]
+        launches += plan.stats()["kernel_launches"] + 1
+    barrier()
+    clocks = sampler.stop()
+    dev_ms = sum(a.elapsed_time(b) for a, b in ev) / args.steps
+    classes["pack"]["ms"] = sum(a.elapsed_time(b) for a, b in pack_ev)
+    classes["pack"]["launches"] = args.steps
+    classes["pack"]["bytes"] = args.steps * (total + total // 4)
+
+    # ---- end to end: pinned host in, pinned host out ----------------------------------------------------
+    for _ in range(2):
+        step_e2e()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step_e2e()
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
+    barrier()
+    if world > 1:
+        t = torch.tensor([dev_ms, e2e_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dev_ms, e2e_ms = float(t[0]), float(t[1])
+    if rank != 0:
+        dist.destroy_process_group()
+        return
+
+    # ---- report --------------------------------------------------------------------------------------
+    peak, peak_src = hbm_peak()
+    kernels = {}
+    for k, v in classes.items():
+        if v["launches"] == 0:
+            continue
+        gbs = v["bytes"] / (v["ms"] * 1e-3) / 1e9 if v["ms"] > 0 else None
+        kernels[k] = {"ms_per_step": round(v["ms"] / args.steps, 4), "launches_per_step": v["launches"] / args.steps,
+                      "alg_bytes_per_step": v["bytes"] // args.steps, "gb_s": round(gbs, 1) if gbs else None,
+                      "frac_of_peak": round(gbs / peak, 4) if gbs else None}
+    dom = classes["sort_pass"]
+    bytes_per_launch = dom["bytes"] / max(dom["launches"], 1)
+    ms_per_launch = dom["ms"] / max(dom["launches"], 1)
+    achieved = bytes_per_launch / (ms_per_launch * 1e-3) / 1e9 if ms_per_launch > 0 else 0.0
+    total_alg = sum(v["bytes"] for v in classes.values()) / args.steps
+    kern_ms = sum(v["ms"] for v in classes.values()) / args.steps
+    line = {
+        "metric": METRIC, "value": world * N / (dev_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": dev_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u64", "data": "synthetic",
+        "config": {"workload": WORKLOADS.get(args.config, str(args.config)) + (f" x scale {args.scale:g}" if args.scale != 1 else ""),
+                   "n_reads": n_reads, "total_bases": total, "n_suffixes": N, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": "256 MiB L2-flush write between timed steps; working set >> L2", "prefix_len": 6, "key_bases": 29,
+                   "id_bytes": stats["id_bytes"], "n_batches": stats["n_batches"], "sort_passes": stats["sort_passes"],
+                   "refine_rounds": stats["refine_rounds"], "refine_elements": stats["refine_elements"],
+                   "small_group_elems": stats["small_group_elems"]},
+        "gbases_per_hour": world * total / (dev_ms * 1e-3) * 3600 / 1e9,
+        "e2e": {"value": world * N / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": int(h_ascii.numel() + h_off.numel() * 8), "d2h_bytes_per_step": int(h_out.numel())},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": {"kernel": "onesweep_pass_kernel (a6, one radix pass)", "bound": "hbm", "achieved": round(achieved, 1),
+                     "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4), "traffic": NCU_TRAFFIC["bytes_per_launch"],
+                     "traffic_from": NCU_TRAFFIC["file"], "peak_source": peak_src, "nominal_peak": 8000.0,
+                     "alg_bytes_per_launch": int(bytes_per_launch), "us_per_launch": round(ms_per_launch * 1e3, 2),
+                     "launches_per_step": dom["launches"] / args.steps},
+        "pipeline": {"alg_bytes_per_step": int(total_alg), "alg_bytes_per_suffix": round(total_alg / N, 1),
+                     "gb_s": round(total_alg / (dev_ms * 1e-3) / 1e9, 1), "frac_of_peak": round(total_alg / (dev_ms * 1e-3) / 1e9 / peak, 4),
+                     "kernel_ms_per_step": round(kern_ms, 3), "host_gap_ms_per_step": round(dev_ms - kern_ms, 3)},
+        "kernels": kernels,
+        "paper_context": "CX1: 100 Gbases in 6,886 s on i7-3930K + GTX 680 (14.7 M suffixes/s, 52 Gbases/h; PAPER.md:141); BCR 46,899 s "
+                         "(abstract: 'BRC ... 12 hours'); other hardware, context only",
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(args.config)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cx(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -100,17 +100,33 @@ def cx_bwt_workspace_bytes(n_reads: int, total_bases: int, **opts) -> int:
     return int(out.value)
 
 
-def cx_pack_reads(ascii_dev: torch.Tensor, packed_out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
-    """ASCII bases (uint8, cuda) -> packed words (int64 tensor holding uint64 bit patterns)."""
+def cx_pack_reads(ascii_dev: torch.Tensor, packed_out: torch.Tensor | None = None, stream=None, check: bool = True,
+                  status: torch.Tensor | None = None) -> torch.Tensor:
+    """ASCII bases (uint8, cuda) -> packed words (int64 tensor holding uint64 bit patterns).
+
+    check=True reads the status word back (one synchronisation) and raises CX_ERR_BAD_BASE; with check=False the
+    call is fully asynchronous and the caller inspects `status` (count of warps that saw a byte outside ACGT)."""
     assert ascii_dev.is_cuda and ascii_dev.dtype == torch.uint8 and ascii_dev.is_contiguous()
     n = ascii_dev.numel()
     if packed_out is None:
         packed_out = torch.empty(max(1, (n + 31) // 32), dtype=torch.int64, device=ascii_dev.device)
-    status = torch.zeros(1, dtype=torch.int32, device=ascii_dev.device)
-    _check(lib().cx_pack_reads(ascii_dev.data_ptr(), n, packed_out.data_ptr(), status.data_ptr(), _stream_ptr(stream)))
-    if int(status.item()) != 0:
+    if status is None:
+        status = _pack_status(ascii_dev.device)
+    with torch.cuda.device(ascii_dev.device):
+        _check(lib().cx_pack_reads(ascii_dev.data_ptr(), n, packed_out.data_ptr(), status.data_ptr(), _stream_ptr(stream)))
+    if check and int(status.item()) != 0:
         raise CxError(CX_ERR_BAD_BASE, cx_strerror(CX_ERR_BAD_BASE))
     return packed_out
+
+
+_status_words: dict = {}
+
+
+def _pack_status(device) -> torch.Tensor:
+    key = str(device)
+    if key not in _status_words:
+        _status_words[key] = torch.zeros(1, dtype=torch.int32, device=device)
+    return _status_words[key]
 
 
 class Plan:
