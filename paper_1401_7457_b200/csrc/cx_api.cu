@@ -86,9 +86,9 @@ int make_shape(uint64_t max_reads, uint64_t max_bases, const cx_bwt_opts_t* o, S
     memset(&z, 0, sizeof(z));
     if (!o) o = &z;
     sh.ell = o->prefix_len ? o->prefix_len : 6;
-    sh.w = o->key_bases ? o->key_bases : 29;
+    sh.w = o->key_bases;   // 0 = chosen in cx_bwt_plan from m1
     sh.cap = o->small_group_max ? o->small_group_max : (uint32_t)kLocalGroupCap;
-    if (sh.ell < 1 || sh.ell > 7 || sh.w < 1 || sh.w > 29 || sh.w < sh.ell) return CX_ERR_ARG;
+    if (sh.ell < 1 || sh.ell > 7 || sh.w > 29 || (sh.w && sh.w < sh.ell)) return CX_ERR_ARG;
     if (sh.cap > (uint32_t)kLocalGroupCap) sh.cap = kLocalGroupCap;
     if (max_reads >= 0xFFFFFFFFull) return CX_ERR_ARG;   // read indices travel as 32 bits in the tile table
     sh.max_reads = max_reads;
@@ -166,6 +166,11 @@ extern "C" int cx_bwt_plan(cx_bwt_plan_t** plan_out, uint64_t max_reads, uint64_
     CX_CUDA(cudaGetDevice(&dev));
     CX_CUDA(cudaDeviceGetAttribute(&n_sms, cudaDevAttrMultiProcessorCount, dev));
 
+    // First-round window ("stringword"): wide enough that 4^w exceeds the batch, so that random
+    // collisions are rare and tie groups are the genuinely shared substrings; 14 bases + a 4-bit length is
+    // the most a 32-bit key holds, which halves the bytes every radix pass moves and the passes it needs.
+    if (sh.w == 0) sh.w = lo <= (1ull << 28) ? 14 : 29;
+    if (sh.w < sh.ell) sh.w = sh.ell;
     cx_bwt_plan_t* p = new (std::nothrow) cx_bwt_plan_t();
     if (!p) return CX_ERR_NOMEM;
     p->sh = sh;
@@ -315,7 +320,7 @@ int plan_batches(cx_bwt_plan_t* p, uint64_t N) {
     return out == N ? CX_OK : CX_ERR_CUDA;   // a mismatch means the histogram kernel misbehaved
 }
 
-template <typename IdT>
+template <typename KeyT, typename IdT>
 int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets, uint64_t n_reads, uint8_t* out, cudaStream_t s) {
     const Shape& sh = p->sh;
     const Layout& L = p->L;
@@ -380,7 +385,8 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
     const bool single = p->batches.size() == 1;
     const uint32_t w = sh.w;
-    const uint32_t key_bits = 2 * w + 5;
+    const uint32_t key_bits = 2 * w + key_len_bits(w);
+    KeyT* d_keys1[2] = {reinterpret_cast<KeyT*>(d_keys[0]), reinterpret_cast<KeyT*>(d_keys[1])};   // first-round keys
     p->stats.sort_passes = (key_bits + kRadixBits - 1) / kRadixBits;
 
     for (size_t bi = 0; bi < p->batches.size(); ++bi) {
@@ -388,9 +394,9 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         const uint64_t nb = B.count;
         // ---- step 3(a) + 3(c)i: list the batch's suffixes with their first keys ----------------
         if (single) {
-            ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (8 + sizeof(IdT)), s);
-            CX_CUDA(launch_list_write<IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, nullptr, d_keys[0], d_ids[0],
-                                           n_tiles, s));
+            ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (sizeof(KeyT) + sizeof(IdT)), s);
+            CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, nullptr, d_keys1[0],
+                                                  d_ids[0], n_tiles, s)));
         } else {
             {
                 ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + n_tiles * 8, s);
@@ -401,19 +407,19 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
                 CX_CUDA(launch_scan_u64(d_tile_count, n_tiles, d_tile_sums, d_scalars + 2, s));
             }
             prof->launches[CX_K_LIST] += 2;   // the scan is three kernels
-            ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (8 + sizeof(IdT)), s);
-            CX_CUDA(launch_list_write<IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, d_tile_count, d_keys[0],
-                                           d_ids[0], n_tiles, s));
+            ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (sizeof(KeyT) + sizeof(IdT)), s);
+            CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, d_tile_count,
+                                                  d_keys1[0], d_ids[0], n_tiles, s)));
         }
         // ---- step 3(c)ii: sort (first w symbols) ------------------------------------------------
         int in_alt = 0;
-        CX_CUDA(sort_pairs<IdT>(d_keys[0], d_ids[0], d_keys[1], d_ids[1], nb, 0, key_bits, p->sort, &in_alt, prof, s));
+        CX_CUDA((sort_pairs<KeyT, IdT>(d_keys1[0], d_ids[0], d_keys1[1], d_ids[1], nb, 0, key_bits, p->sort, &in_alt, prof, s)));
         const int cur = in_alt;
         IdT* ids = d_ids[cur];
         int hc = 0;
         {
-            ScopedLaunch sl(prof, CX_K_FLAG, nb * 8 + nb / 8, s);
-            CX_CUDA(launch_flag_heads(d_keys[cur], nb, w, d_heads[0], s));
+            ScopedLaunch sl(prof, CX_K_FLAG, nb * sizeof(KeyT) + nb / 8, s);
+            CX_CUDA(launch_flag_heads<KeyT>(d_keys1[cur], nb, w, d_heads[0], s));
         }
         // ---- tie refinement ---------------------------------------------------------------------
         const uint64_t n_words = (nb + 31) >> 5;
@@ -452,7 +458,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
                 CX_CUDA(launch_refine_rekey<IdT>(R, d_heads[hc], d_word_counts, ids, nb, depth, w_r, kc, ic, d_pos, s));
             }
             int alt = 0;
-            CX_CUDA(sort_pairs<IdT>(kc, ic, d_keys[cur], d_ids[2], n_act, 0, 2 * w_r + 5 + gbits, p->sort, &alt, prof, s));
+            CX_CUDA((sort_pairs<uint64_t, IdT>(kc, ic, d_keys[cur], d_ids[2], n_act, 0, 2 * w_r + 5 + gbits, p->sort, &alt, prof, s)));
             {
                 ScopedLaunch sl(prof, CX_K_REFINE_WRITE, n_act * (8 + 2 * sizeof(IdT) + 4), s);
                 CX_CUDA(launch_refine_writeback<IdT>(alt ? d_keys[cur] : kc, alt ? d_ids[2] : ic, d_pos, n_act, w_r, ids, d_heads[hc], s));
@@ -508,8 +514,12 @@ extern "C" int cx_bwt_build(cx_bwt_plan_t* p, const uint64_t* packed_reads, cons
     if (n_reads == 0) return CX_OK;
     if (!read_offsets || !out_bwt || n_reads > p->sh.max_reads) return CX_ERR_ARG;
     if (!packed_reads && p->sh.max_bases) return CX_ERR_ARG;
-    return p->sh.id_bytes == 4 ? build_impl<uint32_t>(p, packed_reads, read_offsets, n_reads, out_bwt, stream)
-                               : build_impl<uint64_t>(p, packed_reads, read_offsets, n_reads, out_bwt, stream);
+    const bool key32 = 2 * p->sh.w + key_len_bits(p->sh.w) <= 32;
+    if (p->sh.id_bytes == 4)
+        return key32 ? build_impl<uint32_t, uint32_t>(p, packed_reads, read_offsets, n_reads, out_bwt, stream)
+                     : build_impl<uint64_t, uint32_t>(p, packed_reads, read_offsets, n_reads, out_bwt, stream);
+    return key32 ? build_impl<uint32_t, uint64_t>(p, packed_reads, read_offsets, n_reads, out_bwt, stream)
+                 : build_impl<uint64_t, uint64_t>(p, packed_reads, read_offsets, n_reads, out_bwt, stream);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -535,10 +545,10 @@ extern "C" int cx_sort_pairs(uint64_t* keys, void* vals, uint64_t* keys_alt, voi
     SortWorkspace ws;
     sort_workspace_carve(ws, workspace_dev, n);
     if (val_bytes == 4)
-        CX_CUDA(sort_pairs<uint32_t>(keys, (uint32_t*)vals, keys_alt, (uint32_t*)vals_alt, n, begin_bit, end_bit, ws, result_in_alt,
-                                     nullptr, stream));
+        CX_CUDA((sort_pairs<uint64_t, uint32_t>(keys, (uint32_t*)vals, keys_alt, (uint32_t*)vals_alt, n, begin_bit, end_bit, ws,
+                                                result_in_alt, nullptr, stream)));
     else
-        CX_CUDA(sort_pairs<uint64_t>(keys, (uint64_t*)vals, keys_alt, (uint64_t*)vals_alt, n, begin_bit, end_bit, ws, result_in_alt,
-                                     nullptr, stream));
+        CX_CUDA((sort_pairs<uint64_t, uint64_t>(keys, (uint64_t*)vals, keys_alt, (uint64_t*)vals_alt, n, begin_bit, end_bit, ws,
+                                                result_in_alt, nullptr, stream)));
     return CX_OK;
 }

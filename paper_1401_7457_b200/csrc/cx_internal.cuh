@@ -19,10 +19,11 @@ constexpr int kRadix = 1 << kRadixBits;
 
 // onesweep tile shapes (threads x items); one per value width so that registers/smem stay balanced
 constexpr int kSortThreads = 256;
-constexpr int kSortItems32 = 16;   // 64-bit key + 32-bit id
-constexpr int kSortItems64 = 12;   // 64-bit key + 64-bit id
-template <typename ValT> struct SortShape { static constexpr int items = sizeof(ValT) == 4 ? kSortItems32 : kSortItems64; };
-constexpr int kSortTileMin = kSortThreads * kSortItems64;   // smallest tile: sizes the tile-state array
+template <typename KeyT, typename ValT> struct SortShape {
+    // 8-byte pairs (32-bit key + 32-bit id): 16 items; 12-byte pairs: 16; 16-byte pairs: 12
+    static constexpr int items = sizeof(KeyT) + sizeof(ValT) >= 16 ? 12 : 16;
+};
+constexpr int kSortTileMin = kSortThreads * 12;   // smallest tile: sizes the tile-state array
 
 // tile-state word of the decoupled look-back: [epoch:8][flag:2][count:54]
 constexpr uint64_t kStatusValueMask = (1ull << 54) - 1;
@@ -86,12 +87,14 @@ __device__ __forceinline__ uint64_t load_window(const uint64_t* __restrict__ pac
 }
 
 // Order-preserving key of a window (reading A3 of PAPER.md:99):
-// the first min(rem, w) bases, A-padded to w bases, then min(rem, w) in the low 5 bits.
-// A value < w in the length field means the end-marker falls inside this window.
-__device__ __forceinline__ uint64_t make_key(uint64_t window, uint64_t rem, uint32_t w) {
+// the first min(rem, w) bases, A-padded to w bases, then min(rem, w) in the low len_bits bits
+// (len_bits = bit width of w: 5 for w = 29, 4 for w = 14).  A value < w in the length field means
+// the end-marker falls inside this window.
+__host__ __device__ __forceinline__ uint32_t key_len_bits(uint32_t w) { return w >= 16 ? 5u : w >= 8 ? 4u : w >= 4 ? 3u : w >= 2 ? 2u : 1u; }
+__device__ __forceinline__ uint64_t make_key(uint64_t window, uint64_t rem, uint32_t w, uint32_t len_bits = 5) {
     uint32_t r = rem < (uint64_t)w ? (uint32_t)rem : w;
     uint64_t bases = r ? ((window >> (64 - 2 * r)) << (2 * (w - r))) : 0ull;
-    return (bases << 5) | r;
+    return (bases << len_bits) | r;
 }
 
 template <typename IdT>
@@ -120,9 +123,9 @@ cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint
 cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
                               uint32_t bucket_lo, uint32_t bucket_hi, uint64_t* tile_count, uint64_t n_tiles, cudaStream_t s);
 // write (key, id) of those suffixes in (read, pos) order; tile_base == nullptr means "every suffix, index = slot"
-template <typename IdT>
+template <typename KeyT, typename IdT>
 cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
-                              uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, uint64_t* keys, IdT* ids,
+                              uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, KeyT* keys, IdT* ids,
                               uint64_t n_tiles, cudaStream_t s);
 
 // cx_onesweep.cu
@@ -138,12 +141,13 @@ size_t sort_workspace_bytes(uint64_t n);
 // carve a zeroed region of sort_workspace_bytes(n) bytes
 void sort_workspace_carve(SortWorkspace& ws, void* mem, uint64_t n);
 // Sorts by key bits [begin_bit, end_bit).  *result_in_alt = 1 if the result is in the alt buffers.
-template <typename ValT>
-cudaError_t sort_pairs(uint64_t* keys, ValT* vals, uint64_t* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
+template <typename KeyT, typename ValT>
+cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
                        uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s);
 
 // cx_refine.cu
-cudaError_t launch_flag_heads(const uint64_t* keys, uint64_t n, uint32_t w, uint32_t* heads, cudaStream_t s);
+template <typename KeyT>
+cudaError_t launch_flag_heads(const KeyT* keys, uint64_t n, uint32_t w, uint32_t* heads, cudaStream_t s);
 // word-level counts of active elements / active heads, packed (heads << 32 | elements)
 cudaError_t launch_active_count(const uint32_t* heads, uint64_t n, uint64_t* word_counts, cudaStream_t s);
 // exclusive scan in place; total written to *total; block_sums needs scan_block_count(n) entries

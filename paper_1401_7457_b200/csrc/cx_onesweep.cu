@@ -16,6 +16,7 @@ namespace cx {
 namespace {
 
 constexpr uint32_t kFull = 0xffffffffu;
+constexpr int kLookWindow = 8;   // tile states fetched per look-back round trip
 
 __device__ __forceinline__ uint64_t pack_status(uint32_t epoch, uint32_t flag, uint64_t value) {
     return ((uint64_t)epoch << 56) | ((uint64_t)flag << 54) | value;
@@ -27,7 +28,8 @@ __device__ __forceinline__ uint64_t pack_status(uint32_t epoch, uint32_t flag, u
 constexpr int kHistThreads = 512;
 constexpr int kHistItems = 8;
 
-__global__ void __launch_bounds__(kHistThreads) digit_hist_kernel(const uint64_t* __restrict__ keys, uint64_t n, uint32_t begin_bit,
+template <typename KeyT>
+__global__ void __launch_bounds__(kHistThreads) digit_hist_kernel(const KeyT* __restrict__ keys, uint64_t n, uint32_t begin_bit,
                                                                  uint32_t end_bit, uint32_t n_passes,
                                                                  unsigned long long* __restrict__ hist) {
     __shared__ uint32_t s_hist[8][kRadix];
@@ -35,11 +37,11 @@ __global__ void __launch_bounds__(kHistThreads) digit_hist_kernel(const uint64_t
     __syncthreads();
     const uint64_t chunk = (uint64_t)kHistThreads * kHistItems;
     for (uint64_t base = (uint64_t)blockIdx.x * chunk; base < n; base += (uint64_t)gridDim.x * chunk) {
-        uint64_t k[kHistItems];
+        KeyT k[kHistItems];
 #pragma unroll
         for (int i = 0; i < kHistItems; ++i) {
             uint64_t idx = base + (uint64_t)i * kHistThreads + threadIdx.x;
-            k[i] = idx < n ? __ldcs(keys + idx) : 0ull;
+            k[i] = idx < n ? __ldcs(keys + idx) : (KeyT)0;
         }
 #pragma unroll
         for (int i = 0; i < kHistItems; ++i) {
@@ -81,11 +83,11 @@ __global__ void __launch_bounds__(kRadix) bin_scan_kernel(unsigned long long* __
 // ---------------------------------------------------------------------------------------------
 // one onesweep pass
 // ---------------------------------------------------------------------------------------------
-template <typename ValT, int THREADS, int ITEMS>
+template <typename KeyT, typename ValT, int THREADS, int ITEMS>
 struct PassSmem {
     static constexpr int kTile = THREADS * ITEMS;
     static constexpr int kWarps = THREADS / 32;
-    uint64_t keys[kTile];
+    KeyT keys[kTile];
     ValT vals[kTile];
     uint64_t gofs[kRadix];               // global index of staged slot e with digit d = gofs[d] + e
     uint32_t warp_count[kWarps][kRadix];  // per-warp digit counts, then the warp's offset inside the digit
@@ -94,13 +96,13 @@ struct PassSmem {
     uint32_t tile;
 };
 
-template <typename ValT, int THREADS, int ITEMS, int MIN_BLOCKS>
+template <typename KeyT, typename ValT, int THREADS, int ITEMS, int MIN_BLOCKS>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
-onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const ValT* __restrict__ vals_in, uint64_t* __restrict__ keys_out,
+onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ vals_in, KeyT* __restrict__ keys_out,
                      ValT* __restrict__ vals_out, uint64_t n, uint32_t shift, uint32_t digit_mask,
                      const uint64_t* __restrict__ bin_base, uint64_t* __restrict__ status, uint32_t* __restrict__ ticket,
                      uint32_t ticket_base, uint32_t epoch) {
-    using Smem = PassSmem<ValT, THREADS, ITEMS>;
+    using Smem = PassSmem<KeyT, ValT, THREADS, ITEMS>;
     constexpr int kTile = Smem::kTile;
     constexpr int kWarps = Smem::kWarps;
     static_assert(THREADS >= kRadix && THREADS % 32 == 0, "one thread per digit is required");
@@ -120,12 +122,12 @@ onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const ValT* __restric
     const uint32_t warp_base = warp * (32 * ITEMS);
 
     // warp-striped loads: element order inside the tile = (warp, item, lane); fully coalesced
-    uint64_t key[ITEMS];
+    KeyT key[ITEMS];
     ValT val[ITEMS];
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
         uint32_t e = warp_base + k * 32 + lane;
-        key[k] = e < tile_n ? __ldcs(keys_in + tile_off + e) : ~0ull;
+        key[k] = e < tile_n ? __ldcs(keys_in + tile_off + e) : (KeyT)~(KeyT)0;
     }
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
@@ -177,24 +179,10 @@ onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const ValT* __restric
         uint32_t excl = carry + incl - count;
         sm.bin_start[tid] = excl;
 
-        uint64_t before = 0;   // equal-digit pairs in earlier tiles
-        if (tile > 0) {
-            int64_t t = (int64_t)tile - 1;
-            while (true) {
-                uint64_t st = ld_relaxed_u64(status + (uint64_t)t * kRadix + tid);
-                uint32_t flag = (uint32_t)(st >> 54) & 3u;
-                if ((uint32_t)(st >> 56) != epoch || flag == 0) continue;   // not published yet
-                before += st & kStatusValueMask;
-                if (flag == kFlagInclusive) break;
-                --t;
-            }
-            st_relaxed_u64(my_status, pack_status(epoch, kFlagInclusive, before + count));
-        }
-        sm.gofs[tid] = bin_base[tid] + before - excl;
     }
     __syncthreads();
 
-    // stage pairs in digit order
+    // stage pairs in digit order (needs only tile-local offsets; overlaps the predecessors' publications)
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
         if (warp_base + k * 32 + lane < tile_n) {
@@ -204,6 +192,35 @@ onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const ValT* __restric
             sm.vals[slot] = val[k];
         }
     }
+
+    // decoupled look-back, kLookWindow predecessors per round trip
+    if (tid < kRadix) {
+        uint64_t before = 0;   // equal-digit pairs in earlier tiles
+        if (tile > 0) {
+            int64_t t = (int64_t)tile - 1;
+            bool done = false;
+            while (!done) {
+                uint64_t st[kLookWindow];
+#pragma unroll
+                for (int j = 0; j < kLookWindow; ++j) {
+                    int64_t tj = t - j;
+                    st[j] = tj >= 0 ? ld_relaxed_u64(status + (uint64_t)tj * kRadix + tid) : 0ull;
+                }
+#pragma unroll
+                for (int j = 0; j < kLookWindow; ++j) {
+                    if (done) break;
+                    uint64_t v = st[j];
+                    while ((uint32_t)(v >> 56) != epoch || ((uint32_t)(v >> 54) & 3u) == 0)   // not published yet
+                        v = ld_relaxed_u64(status + (uint64_t)(t - j) * kRadix + tid);
+                    before += v & kStatusValueMask;
+                    done = ((uint32_t)(v >> 54) & 3u) == kFlagInclusive;
+                }
+                t -= kLookWindow;
+            }
+            st_relaxed_u64(status + (uint64_t)tile * kRadix + tid, pack_status(epoch, kFlagInclusive, before + count));
+        }
+        sm.gofs[tid] = bin_base[tid] + before - sm.bin_start[tid];
+    }
     __syncthreads();
 
     // runs of equal digit leave as consecutive addresses
@@ -211,7 +228,7 @@ onesweep_pass_kernel(const uint64_t* __restrict__ keys_in, const ValT* __restric
     for (int k = 0; k < ITEMS; ++k) {
         uint32_t e = k * THREADS + tid;
         if (e < tile_n) {
-            uint64_t kk = sm.keys[e];
+            KeyT kk = sm.keys[e];
             uint32_t d = (uint32_t)(kk >> shift) & digit_mask;
             uint64_t dst = sm.gofs[d] + e;
             keys_out[dst] = kk;
@@ -242,16 +259,16 @@ void sort_workspace_carve(SortWorkspace& ws, void* mem, uint64_t n) {
     ws.ticket_base = 0;
 }
 
-template <typename ValT>
-cudaError_t sort_pairs(uint64_t* keys, ValT* vals, uint64_t* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
+template <typename KeyT, typename ValT>
+cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
                        uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s) {
     *result_in_alt = 0;
     if (n <= 1 || end_bit <= begin_bit) return cudaSuccess;
-    constexpr int ITEMS = SortShape<ValT>::items;
+    constexpr int ITEMS = SortShape<KeyT, ValT>::items;
     constexpr int kTile = kSortThreads * ITEMS;
-    using Smem = PassSmem<ValT, kSortThreads, ITEMS>;
-    constexpr int kMinBlocks = 2;
-    auto kernel = onesweep_pass_kernel<ValT, kSortThreads, ITEMS, kMinBlocks>;
+    using Smem = PassSmem<KeyT, ValT, kSortThreads, ITEMS>;
+    constexpr int kMinBlocks = sizeof(KeyT) + sizeof(ValT) <= 8 ? 3 : 2;
+    auto kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks>;
     static bool attr_set = false;
     cudaError_t e;
     if (!attr_set) {
@@ -269,8 +286,8 @@ cudaError_t sort_pairs(uint64_t* keys, ValT* vals, uint64_t* keys_alt, ValT* val
         uint64_t chunk = (uint64_t)kHistThreads * kHistItems;
         uint64_t blocks = (n + chunk - 1) / chunk;
         unsigned grid = (unsigned)(blocks < 148ull * 4 ? blocks : 148ull * 4);
-        ScopedLaunch sl(prof, CX_K_SORT_HIST, n * 8, s);
-        digit_hist_kernel<<<grid, kHistThreads, 0, s>>>(keys, n, begin_bit, end_bit, n_passes, (unsigned long long*)ws.hist);
+        ScopedLaunch sl(prof, CX_K_SORT_HIST, n * sizeof(KeyT), s);
+        digit_hist_kernel<KeyT><<<grid, kHistThreads, 0, s>>>(keys, n, begin_bit, end_bit, n_passes, (unsigned long long*)ws.hist);
     }
     {
         ScopedLaunch sl(prof, CX_K_SORT_SCAN, (uint64_t)n_passes * kRadix * 16, s);
@@ -279,9 +296,9 @@ cudaError_t sort_pairs(uint64_t* keys, ValT* vals, uint64_t* keys_alt, ValT* val
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
 
-    uint64_t* kin = keys;
+    KeyT* kin = keys;
     ValT* vin = vals;
-    uint64_t* kout = keys_alt;
+    KeyT* kout = keys_alt;
     ValT* vout = vals_alt;
     for (uint32_t p = 0; p < n_passes; ++p) {
         uint32_t lo = begin_bit + p * kRadixBits;
@@ -293,7 +310,7 @@ cudaError_t sort_pairs(uint64_t* keys, ValT* vals, uint64_t* keys_alt, ValT* val
         }
         ws.epoch += 1;
         {
-            ScopedLaunch sl(prof, CX_K_SORT_PASS, n * 2 * (8 + sizeof(ValT)), s);
+            ScopedLaunch sl(prof, CX_K_SORT_PASS, n * 2 * (sizeof(KeyT) + sizeof(ValT)), s);
             kernel<<<(unsigned)n_tiles, kSortThreads, sizeof(Smem), s>>>(kin, vin, kout, vout, n, lo, (1u << bits) - 1,
                                                                         ws.hist + (uint64_t)p * kRadix, ws.status, ws.ticket,
                                                                         ws.ticket_base, ws.epoch);
@@ -301,16 +318,18 @@ cudaError_t sort_pairs(uint64_t* keys, ValT* vals, uint64_t* keys_alt, ValT* val
         ws.ticket_base += (uint32_t)n_tiles;
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
-        uint64_t* tk = kin; kin = kout; kout = tk;
+        KeyT* tk = kin; kin = kout; kout = tk;
         ValT* tv = vin; vin = vout; vout = tv;
     }
     *result_in_alt = (int)(n_passes & 1);
     return cudaSuccess;
 }
 
-template cudaError_t sort_pairs<uint32_t>(uint64_t*, uint32_t*, uint64_t*, uint32_t*, uint64_t, uint32_t, uint32_t, SortWorkspace&,
-                                          int*, Launch*, cudaStream_t);
-template cudaError_t sort_pairs<uint64_t>(uint64_t*, uint64_t*, uint64_t*, uint64_t*, uint64_t, uint32_t, uint32_t, SortWorkspace&,
-                                          int*, Launch*, cudaStream_t);
+#define CX_SORT_INST(K, V)                                                                                               \
+    template cudaError_t sort_pairs<K, V>(K*, V*, K*, V*, uint64_t, uint32_t, uint32_t, SortWorkspace&, int*, Launch*, cudaStream_t);
+CX_SORT_INST(uint32_t, uint32_t)
+CX_SORT_INST(uint32_t, uint64_t)
+CX_SORT_INST(uint64_t, uint32_t)
+CX_SORT_INST(uint64_t, uint64_t)
 
 }  // namespace cx

@@ -49,14 +49,15 @@ __device__ __forceinline__ uint64_t key_at_depth(const Reads& R, IdT id, uint32_
 // ---------------------------------------------------------------------------------------------
 // head flags of a freshly sorted key array
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) flag_heads_kernel(const uint64_t* __restrict__ keys, uint64_t n, uint32_t w,
+template <typename KeyT>
+__global__ void __launch_bounds__(256) flag_heads_kernel(const KeyT* __restrict__ keys, uint64_t n, uint32_t w, uint32_t len_mask,
                                                          uint32_t* __restrict__ heads) {
     uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     uint64_t n_words = (n + 31) >> 5;
     bool head = true;   // positions past n count as heads
     if (j < n) {
-        uint64_t k = __ldcs(keys + j);
-        head = j == 0 || k != __ldg(keys + j - 1) || (uint32_t)(k & 31) < w;
+        KeyT k = __ldcs(keys + j);
+        head = j == 0 || k != __ldg(keys + j - 1) || ((uint32_t)k & len_mask) < w;
     }
     uint32_t word = __ballot_sync(kFull, head);
     if (lane_id() == 0 && (j >> 5) < n_words) heads[j >> 5] = word;
@@ -417,12 +418,15 @@ __global__ void __launch_bounds__(256) emit_kernel(Reads R, const IdT* __restric
 // ---------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------
-cudaError_t launch_flag_heads(const uint64_t* keys, uint64_t n, uint32_t w, uint32_t* heads, cudaStream_t s) {
+template <typename KeyT>
+cudaError_t launch_flag_heads(const KeyT* keys, uint64_t n, uint32_t w, uint32_t* heads, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
     uint64_t padded = ((n + 31) >> 5) << 5;
-    flag_heads_kernel<<<(unsigned)((padded + 255) / 256), 256, 0, s>>>(keys, n, w, heads);
+    flag_heads_kernel<KeyT><<<(unsigned)((padded + 255) / 256), 256, 0, s>>>(keys, n, w, (1u << key_len_bits(w)) - 1, heads);
     return cudaGetLastError();
 }
+template cudaError_t launch_flag_heads<uint32_t>(const uint32_t*, uint64_t, uint32_t, uint32_t*, cudaStream_t);
+template cudaError_t launch_flag_heads<uint64_t>(const uint64_t*, uint64_t, uint32_t, uint32_t*, cudaStream_t);
 
 cudaError_t launch_active_count(const uint32_t* heads, uint64_t n, uint64_t* word_counts, cudaStream_t s) {
     uint64_t n_words = (n + 31) >> 5;

@@ -213,11 +213,11 @@ __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const
 // a4 (write half) + a5: ids of the batch in (read, pos) order, each with its first key.
 // The read is in shared memory already, so the round-1 key costs no gather.
 // ---------------------------------------------------------------------------------------------
-template <typename IdT, bool ALL>
+template <typename KeyT, typename IdT, bool ALL>
 __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const BuildInfo* __restrict__ info,
                                                                   const uint32_t* __restrict__ tile_first_read, uint32_t ell, uint32_t w,
                                                                   uint32_t bucket_lo, uint32_t bucket_hi,
-                                                                  const uint64_t* __restrict__ tile_base, uint64_t* __restrict__ keys,
+                                                                  const uint64_t* __restrict__ tile_base, KeyT* __restrict__ keys,
                                                                   IdT* __restrict__ ids) {
     __shared__ TileSmem sm;
     R.n_words = (info->total_bases + 31) >> 5;
@@ -229,7 +229,8 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
     const uint32_t warp = threadIdx.x >> 5;
     constexpr int kWarps = kListThreads / 32;
 
-    uint64_t key[kListItems];
+    const uint32_t len_bits = key_len_bits(w);
+    KeyT key[kListItems];
     IdT id[kListItems];
     uint32_t rank[kListItems];
     bool take[kListItems];
@@ -242,7 +243,7 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
         rank[k] = 0;
         if (s < c.n_slots) {
             Slot sl = decode_slot(c, sm, s);
-            key[k] = make_key(sl.window, sl.rem, w);
+            key[k] = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
             id[k] = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
             if (ALL) {
                 take[k] = true;
@@ -345,23 +346,26 @@ cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint3
     return cudaGetLastError();
 }
 
-template <typename IdT>
+template <typename KeyT, typename IdT>
 cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
-                              uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, uint64_t* keys, IdT* ids,
+                              uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, KeyT* keys, IdT* ids,
                               uint64_t n_tiles, cudaStream_t s) {
     if (n_tiles == 0) return cudaSuccess;
     if (tile_base == nullptr)
-        list_write_kernel<IdT, true><<<(unsigned)n_tiles, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
-                                                                               nullptr, keys, ids);
+        list_write_kernel<KeyT, IdT, true><<<(unsigned)n_tiles, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo,
+                                                                                     bucket_hi, nullptr, keys, ids);
     else
-        list_write_kernel<IdT, false><<<(unsigned)n_tiles, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
-                                                                                tile_base, keys, ids);
+        list_write_kernel<KeyT, IdT, false><<<(unsigned)n_tiles, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo,
+                                                                                      bucket_hi, tile_base, keys, ids);
     return cudaGetLastError();
 }
 
-template cudaError_t launch_list_write<uint32_t>(const Reads&, const BuildInfo*, const uint32_t*, uint32_t, uint32_t, uint32_t,
-                                                 uint32_t, const uint64_t*, uint64_t*, uint32_t*, uint64_t, cudaStream_t);
-template cudaError_t launch_list_write<uint64_t>(const Reads&, const BuildInfo*, const uint32_t*, uint32_t, uint32_t, uint32_t,
-                                                 uint32_t, const uint64_t*, uint64_t*, uint64_t*, uint64_t, cudaStream_t);
+#define CX_LIST_INST(K, I)                                                                                                        \
+    template cudaError_t launch_list_write<K, I>(const Reads&, const BuildInfo*, const uint32_t*, uint32_t, uint32_t, uint32_t,  \
+                                                 uint32_t, const uint64_t*, K*, I*, uint64_t, cudaStream_t);
+CX_LIST_INST(uint32_t, uint32_t)
+CX_LIST_INST(uint32_t, uint64_t)
+CX_LIST_INST(uint64_t, uint32_t)
+CX_LIST_INST(uint64_t, uint64_t)
 
 }  // namespace cx
