@@ -20,10 +20,10 @@ constexpr int kRadix = 1 << kRadixBits;
 // onesweep tile shapes (threads x items); one per value width so that registers/smem stay balanced
 constexpr int kSortThreads = 256;
 template <typename KeyT, typename ValT> struct SortShape {
-    // 8-byte pairs (32-bit key + 32-bit id): 16 items; 12-byte pairs: 16; 16-byte pairs: 12
-    static constexpr int items = sizeof(KeyT) + sizeof(ValT) >= 16 ? 12 : 16;
+    // pairs staged per tile: 8-byte pairs 8192 (64 KB), 12-byte pairs 6144 (72 KB), 16-byte pairs 5120 (80 KB); 2 blocks per SM
+    static constexpr int items = sizeof(KeyT) + sizeof(ValT) >= 16 ? 10 : sizeof(KeyT) + sizeof(ValT) >= 12 ? 12 : 16;
 };
-constexpr int kSortTileMin = kSortThreads * 12;   // smallest tile: sizes the tile-state array
+constexpr int kSortTileMin = kSortThreads * 10;   // smallest tile: sizes the tile-state array
 
 // tile-state word of the decoupled look-back: [epoch:8][flag:2][count:54]
 constexpr uint64_t kStatusValueMask = (1ull << 54) - 1;

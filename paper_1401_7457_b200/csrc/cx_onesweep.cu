@@ -11,6 +11,7 @@
 // Algorithmic traffic per pass: 2 * (8 + sizeof(id)) bytes per pair; histogram kernel: 8 bytes per pair.
 #include "cx_internal.cuh"
 #include "cx_launch.h"
+#include <stdlib.h>
 
 namespace cx {
 namespace {
@@ -89,14 +90,46 @@ struct PassSmem {
     static constexpr int kWarps = THREADS / 32;
     KeyT keys[kTile];
     ValT vals[kTile];
-    uint64_t gofs[kRadix];               // global index of staged slot e with digit d = gofs[d] + e
-    uint32_t warp_count[kWarps][kRadix];  // per-warp digit counts, then the warp's offset inside the digit
-    uint32_t bin_start[kRadix];           // first staged slot of each digit
+    uint32_t warp_count[kWarps][kRadix];  // per-warp digit counts, then the staged slot of the warp's first pair of that digit
+    uint32_t gofs[kRadix];                // output index of staged slot e with digit d = gofs[d] + e (mod 2^32; batches are < 2^32)
     uint32_t warp_total[kRadix / 32];
     uint32_t tile;
 };
 
-template <typename KeyT, typename ValT, int THREADS, int ITEMS, int MIN_BLOCKS>
+// Lanes of the warp whose 8-bit digit equals mine.  Eight ballots: constant cost whatever the digit
+// distribution (match.any on sm_100a takes ~25 cycles per DISTINCT value in the warp, ~700 cycles for
+// random digits -- measured).
+// p &= (my bit B set) ? ballot : ~ballot, as LOP3.P, VOTE, SEL, LOP3 (nvcc's own code for the C++ form takes six)
+template <int B>
+__device__ __forceinline__ void ballot_step(uint32_t& p, uint32_t d) {
+    asm("{\n\t.reg .pred q;\n\t.reg .b32 t, v, m;\n\t"
+        "and.b32 t, %1, %2;\n\tsetp.ne.u32 q, t, 0;\n\t"
+        "vote.sync.ballot.b32 v, q, 0xffffffff;\n\t"
+        "selp.b32 m, 0, 0xffffffff, q;\n\t"
+        "lop3.b32 %0, %0, v, m, 0x60;\n\t}"
+        : "+r"(p)
+        : "r"(d), "n"(1u << B));
+}
+template <int B, int END>
+__device__ __forceinline__ void ballot_steps(uint32_t& p, uint32_t d) {
+    if constexpr (B < END) {
+        ballot_step<B>(p, d);
+        ballot_steps<B + 1, END>(p, d);
+    }
+}
+
+template <int MODE>
+__device__ __forceinline__ uint32_t digit_peers(uint32_t d) {
+    // MODE = number of low digit bits resolved by match.any (0, 2, 3, 4, or 22 = two 2-bit matches); the rest by ballots
+    uint32_t p = kFull;
+    constexpr int kMatchBits = MODE == 22 ? 4 : MODE;
+    if (MODE == 22) p = __match_any_sync(kFull, d & 3u) & __match_any_sync(kFull, (d >> 2) & 3u);
+    else if (MODE > 0) p = __match_any_sync(kFull, d & ((1u << MODE) - 1));
+    ballot_steps<kMatchBits, kRadixBits>(p, d);
+    return p;
+}
+
+template <typename KeyT, typename ValT, int THREADS, int ITEMS, int MIN_BLOCKS, int RANK_MODE>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
 onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ vals_in, KeyT* __restrict__ keys_out,
                      ValT* __restrict__ vals_out, uint64_t n, uint32_t shift, uint32_t digit_mask,
@@ -117,54 +150,56 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ 
     for (uint32_t i = tid; i < kWarps * kRadix; i += THREADS) (&sm.warp_count[0][0])[i] = 0;
     __syncthreads();
     const uint32_t tile = sm.tile;
-    const uint64_t tile_off = (uint64_t)tile * kTile;
+    const uint32_t tile_off = tile * (uint32_t)kTile;
     const uint32_t tile_n = (uint32_t)min((uint64_t)kTile, n - tile_off);
+    const bool full = tile_n == (uint32_t)kTile;
     const uint32_t warp_base = warp * (32 * ITEMS);
 
-    // warp-striped loads: element order inside the tile = (warp, item, lane); fully coalesced
+    // warp-striped loads: element order inside the tile = (warp, item, lane); fully coalesced.
+    // Slots past the end of the input get the all-ones key: they rank last in the last digit and are
+    // never written out.
     KeyT key[ITEMS];
     ValT val[ITEMS];
+    {
+        const KeyT* kp = keys_in + tile_off + warp_base + lane;
+        const ValT* vp = vals_in + tile_off + warp_base + lane;
+        if (full) {
 #pragma unroll
-    for (int k = 0; k < ITEMS; ++k) {
-        uint32_t e = warp_base + k * 32 + lane;
-        key[k] = e < tile_n ? __ldcs(keys_in + tile_off + e) : (KeyT)~(KeyT)0;
-    }
+            for (int k = 0; k < ITEMS; ++k) key[k] = __ldcs(kp + k * 32);
 #pragma unroll
-    for (int k = 0; k < ITEMS; ++k) {
-        uint32_t e = warp_base + k * 32 + lane;
-        val[k] = e < tile_n ? __ldcs(vals_in + tile_off + e) : (ValT)0;
+            for (int k = 0; k < ITEMS; ++k) val[k] = __ldcs(vp + k * 32);
+        } else {
+#pragma unroll
+            for (int k = 0; k < ITEMS; ++k) key[k] = warp_base + k * 32 + lane < tile_n ? __ldcs(kp + k * 32) : (KeyT)~(KeyT)0;
+#pragma unroll
+            for (int k = 0; k < ITEMS; ++k) val[k] = warp_base + k * 32 + lane < tile_n ? __ldcs(vp + k * 32) : (ValT)0;
+        }
     }
 
-    // rank inside the warp, item by item (keeps element order, hence stability)
+    // rank inside the warp, row by row (keeps element order, hence stability: PAPER.md:99)
     uint32_t rank[ITEMS];
+    const uint32_t lt = lanemask_lt();
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
-        bool valid = warp_base + k * 32 + lane < tile_n;
-        uint32_t d = (uint32_t)(key[k] >> shift) & digit_mask;
-        uint32_t peers = __match_any_sync(kFull, valid ? d : (uint32_t)kRadix);
-        uint32_t below = __popc(peers & lanemask_lt());
+        const uint32_t d = (uint32_t)(key[k] >> shift) & digit_mask;
+        const uint32_t peers = digit_peers<RANK_MODE>(d);
+        const uint32_t below = __popc(peers & lt);
         uint32_t old = 0;
-        if (valid && below == 0) {
-            old = sm.warp_count[warp][d];
-            sm.warp_count[warp][d] = old + __popc(peers);
-        }
+        if (below == 0) old = atomicAdd(&sm.warp_count[warp][d], (uint32_t)__popc(peers));   // lowest peer lane
         old = __shfl_sync(kFull, old, __ffs(peers) - 1);
         rank[k] = old + below;
         __syncwarp();
     }
     __syncthreads();
 
-    // per digit: tile count, warp offsets, tile-state publication, look-back
-    uint32_t count = 0;
+    // per digit: tile count, tile-state publication, staged slot of every (warp, digit)
+    uint32_t count = 0, excl = 0;
     if (tid < kRadix) {
 #pragma unroll
-        for (int wq = 0; wq < kWarps; ++wq) {
-            uint32_t c = sm.warp_count[wq][tid];
-            sm.warp_count[wq][tid] = count;
-            count += c;
-        }
-        uint64_t* my_status = status + (uint64_t)tile * kRadix + tid;
-        st_relaxed_u64(my_status, pack_status(epoch, tile == 0 ? kFlagInclusive : kFlagAggregate, count));
+        for (int wq = 0; wq < kWarps; ++wq) count += sm.warp_count[wq][tid];
+        // the padding slots of a ragged last tile were counted in the top digit
+        const uint32_t real = count - ((tid == digit_mask) ? (uint32_t)kTile - tile_n : 0u);
+        st_relaxed_u64(status + (uint64_t)tile * kRadix + tid, pack_status(epoch, tile == 0 ? kFlagInclusive : kFlagAggregate, real));
         // exclusive scan of the 256 counts -> first staged slot of each digit
         uint32_t incl = count;
 #pragma unroll
@@ -176,26 +211,30 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ 
         asm volatile("bar.sync 1, %0;" ::"n"(kRadix));   // only the 256 digit threads
         uint32_t carry = 0;
         for (uint32_t wq = 0; wq < warp; ++wq) carry += sm.warp_total[wq];
-        uint32_t excl = carry + incl - count;
-        sm.bin_start[tid] = excl;
-
+        excl = carry + incl - count;
+        uint32_t run = excl;
+#pragma unroll
+        for (int wq = 0; wq < kWarps; ++wq) {
+            uint32_t c = sm.warp_count[wq][tid];
+            sm.warp_count[wq][tid] = run;
+            run += c;
+        }
+        count = real;
     }
     __syncthreads();
 
     // stage pairs in digit order (needs only tile-local offsets; overlaps the predecessors' publications)
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
-        if (warp_base + k * 32 + lane < tile_n) {
-            uint32_t d = (uint32_t)(key[k] >> shift) & digit_mask;
-            uint32_t slot = sm.bin_start[d] + sm.warp_count[warp][d] + rank[k];
-            sm.keys[slot] = key[k];
-            sm.vals[slot] = val[k];
-        }
+        const uint32_t d = (uint32_t)(key[k] >> shift) & digit_mask;
+        const uint32_t slot = sm.warp_count[warp][d] + rank[k];
+        sm.keys[slot] = key[k];
+        sm.vals[slot] = val[k];
     }
 
     // decoupled look-back, kLookWindow predecessors per round trip
     if (tid < kRadix) {
-        uint64_t before = 0;   // equal-digit pairs in earlier tiles
+        uint32_t before = 0;   // equal-digit pairs in earlier tiles
         if (tile > 0) {
             int64_t t = (int64_t)tile - 1;
             bool done = false;
@@ -212,25 +251,24 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ 
                     uint64_t v = st[j];
                     while ((uint32_t)(v >> 56) != epoch || ((uint32_t)(v >> 54) & 3u) == 0)   // not published yet
                         v = ld_relaxed_u64(status + (uint64_t)(t - j) * kRadix + tid);
-                    before += v & kStatusValueMask;
+                    before += (uint32_t)(v & kStatusValueMask);
                     done = ((uint32_t)(v >> 54) & 3u) == kFlagInclusive;
                 }
                 t -= kLookWindow;
             }
-            st_relaxed_u64(status + (uint64_t)tile * kRadix + tid, pack_status(epoch, kFlagInclusive, before + count));
+            st_relaxed_u64(status + (uint64_t)tile * kRadix + tid, pack_status(epoch, kFlagInclusive, (uint64_t)before + count));
         }
-        sm.gofs[tid] = bin_base[tid] + before - sm.bin_start[tid];
+        sm.gofs[tid] = (uint32_t)bin_base[tid] + before - excl;
     }
     __syncthreads();
 
     // runs of equal digit leave as consecutive addresses
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
-        uint32_t e = k * THREADS + tid;
-        if (e < tile_n) {
-            KeyT kk = sm.keys[e];
-            uint32_t d = (uint32_t)(kk >> shift) & digit_mask;
-            uint64_t dst = sm.gofs[d] + e;
+        const uint32_t e = k * THREADS + tid;
+        if (full || e < tile_n) {
+            const KeyT kk = sm.keys[e];
+            const uint32_t dst = sm.gofs[(uint32_t)(kk >> shift) & digit_mask] + e;
             keys_out[dst] = kk;
             vals_out[dst] = sm.vals[e];
         }
@@ -267,18 +305,21 @@ cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, u
     constexpr int ITEMS = SortShape<KeyT, ValT>::items;
     constexpr int kTile = kSortThreads * ITEMS;
     using Smem = PassSmem<KeyT, ValT, kSortThreads, ITEMS>;
-    constexpr int kMinBlocks = sizeof(KeyT) + sizeof(ValT) <= 8 ? 3 : 2;
-    auto kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks>;
-    static bool attr_set = false;
-    cudaError_t e;
-    if (!attr_set) {
-        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
-        if (e != cudaSuccess) return e;
-        attr_set = true;
+    constexpr int kMinBlocks = 4;
+    auto kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks, 0>;
+    {   // EXPERIMENT: rank mode from the environment
+        static int mode = getenv("CX_RANK_MODE") ? atoi(getenv("CX_RANK_MODE")) : 0;
+        if (mode == 2) kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks, 2>;
+        if (mode == 3) kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks, 3>;
+        if (mode == 4) kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks, 4>;
+        if (mode == 22) kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks, 22>;
     }
+    cudaError_t e;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
+    if (e != cudaSuccess) return e;
     const uint32_t n_passes = (end_bit - begin_bit + kRadixBits - 1) / kRadixBits;
     const uint64_t n_tiles = (n + kTile - 1) / kTile;
-    if (n_tiles > ws.max_tiles || n_passes > 8) return cudaErrorInvalidValue;
+    if (n_tiles > ws.max_tiles || n_passes > 8 || n > 0xFFFF0000ull) return cudaErrorInvalidValue;
 
     e = cudaMemsetAsync(ws.hist, 0, (size_t)n_passes * kRadix * sizeof(uint64_t), s);
     if (e != cudaSuccess) return e;
