@@ -301,7 +301,7 @@ def run_cx(args) -> None:
         "dtype": "u64", "data": "synthetic",
         "config": {"workload": WORKLOADS.get(args.config, str(args.config)) + (f" x scale {args.scale:g}" if args.scale != 1 else ""),
                    "n_reads": n_reads, "total_bases": total, "n_suffixes": N, "parallelism": "replicas only" if world > 1 else "1 gpu",
-                   "l2": "256 MiB L2-flush write between timed steps; working set >> L2", "prefix_len": 6, "key_bases": 29,
+                   "l2": "256 MiB L2-flush write between timed steps; working set >> L2", "prefix_len": 6, "key_bases": "auto (14 in a 32-bit key when the batch is under 2^28 suffixes, else 29 in a 64-bit key)",
                    "id_bytes": stats["id_bytes"], "n_batches": stats["n_batches"], "sort_passes": stats["sort_passes"],
                    "refine_rounds": stats["refine_rounds"], "refine_elements": stats["refine_elements"],
                    "small_group_elems": stats["small_group_elems"]},

@@ -84,12 +84,10 @@ enum {
     CX_K_SORT_HIST,       /* a6 upfront digit histograms                      */
     CX_K_SORT_SCAN,       /* a6 bin offsets                                   */
     CX_K_SORT_PASS,       /* a6 onesweep radix pass                           */
-    CX_K_FLAG,            /* a7 group-head flags                              */
-    CX_K_REFINE_LOCAL,    /* a7 in-block refinement of small tie groups       */
+    CX_K_FINISH,          /* a7+a8 head flags, in-block refinement of small tie groups, emit */
     CX_K_REFINE_SCAN,     /* a7 compaction scans of the global path           */
     CX_K_REFINE_KEY,      /* a7 re-key gather of the global path              */
-    CX_K_REFINE_WRITE,    /* a7 write-back + new flags of the global path     */
-    CX_K_EMIT,            /* a8 BWT emit gather                               */
+    CX_K_REFINE_WRITE,    /* a7+a8 write-back, new flags, emit (global path)  */
     CX_K_COUNT
 };
 

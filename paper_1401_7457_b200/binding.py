@@ -15,8 +15,8 @@ from . import build as _build
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
 CX_OK, CX_ERR_ARG, CX_ERR_BAD_BASE, CX_ERR_WORKSPACE, CX_ERR_BUCKET_TOO_LARGE, CX_ERR_CUDA, CX_ERR_NOMEM = 0, -1, -2, -3, -4, -5, -6
-KERNEL_CLASSES = ["pack", "prep", "hist", "list", "sort_hist", "sort_scan", "sort_pass", "flag", "refine_local",
-                  "refine_scan", "refine_key", "refine_write", "emit"]
+KERNEL_CLASSES = ["pack", "prep", "hist", "list", "sort_hist", "sort_scan", "sort_pass", "finish", "refine_scan", "refine_key",
+                  "refine_write"]
 
 
 class CxError(RuntimeError):

@@ -416,23 +416,23 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         CX_CUDA((sort_pairs<KeyT, IdT>(d_keys1[0], d_ids[0], d_keys1[1], d_ids[1], nb, 0, key_bits, p->sort, &in_alt, prof, s)));
         const int cur = in_alt;
         IdT* ids = d_ids[cur];
-        int hc = 0;
-        {
-            ScopedLaunch sl(prof, CX_K_FLAG, nb * sizeof(KeyT) + nb / 8, s);
-            CX_CUDA(launch_flag_heads<KeyT>(d_keys1[cur], nb, w, d_heads[0], s));
-        }
-        // ---- tie refinement ---------------------------------------------------------------------
+        // a9: with pinned-host output the batch is emitted into a staging buffer of the workspace
+        const int st = (int)(bi & 1);
+        uint8_t* dst = sh.host_out ? ws + L.stage[st] : out + B.out_offset;
+        if (sh.host_out && p->stage_busy[st]) CX_CUDA(cudaStreamWaitEvent(s, p->stage_free[st], 0));
+        // ---- steps 3(c)ii-iii fused: head flags, in-block tie refinement, emit ----------------------
         const uint64_t n_words = (nb + 31) >> 5;
+        int hc = 0;
+        unsigned long long* d_done = reinterpret_cast<unsigned long long*>(d_scalars + 1);
+        CX_CUDA(cudaMemsetAsync(d_heads[0], 0, (n_words + 1) * 4, s));
+        {
+            ScopedLaunch sl(prof, CX_K_FINISH, nb * (sizeof(KeyT) + sizeof(IdT) + 1) + nb / 8, s);
+            CX_CUDA((launch_finish_first<KeyT, IdT>(R, d_keys1[cur], w, d_heads[0], ids, nb, sh.cap, dst, d_done, s)));
+        }
+        // ---- what is still tied goes through global rounds: re-key, sort, write back ------------------
         uint32_t depth = w, rounds = 0;
         uint64_t local_before = p->h_scalars[1];
         while (true) {
-            if (sh.cap > 1) {
-                CX_CUDA(cudaMemcpyAsync(d_heads[1 - hc], d_heads[hc], (n_words + 1) * 4, cudaMemcpyDeviceToDevice, s));
-                ScopedLaunch sl(prof, CX_K_REFINE_LOCAL, nb / 4, s);
-                CX_CUDA(launch_refine_local<IdT>(R, d_heads[hc], d_heads[1 - hc], ids, nb, depth, sh.cap,
-                                                 reinterpret_cast<unsigned long long*>(d_scalars + 1), s));
-                hc = 1 - hc;
-            }
             {
                 ScopedLaunch sl(prof, CX_K_REFINE_SCAN, n_words * 12, s);
                 CX_CUDA(launch_active_count(d_heads[hc], nb, d_word_counts, s));
@@ -460,33 +460,29 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             int alt = 0;
             CX_CUDA((sort_pairs<uint64_t, IdT>(kc, ic, d_keys[cur], d_ids[2], n_act, 0, 2 * w_r + 5 + gbits, p->sort, &alt, prof, s)));
             {
-                ScopedLaunch sl(prof, CX_K_REFINE_WRITE, n_act * (8 + 2 * sizeof(IdT) + 4), s);
-                CX_CUDA(launch_refine_writeback<IdT>(alt ? d_keys[cur] : kc, alt ? d_ids[2] : ic, d_pos, n_act, w_r, ids, d_heads[hc], s));
+                ScopedLaunch sl(prof, CX_K_REFINE_WRITE, n_act * (8 + 2 * sizeof(IdT) + 4 + 1), s);
+                CX_CUDA(launch_refine_writeback<IdT>(R, alt ? d_keys[cur] : kc, alt ? d_ids[2] : ic, d_pos, n_act, w_r, ids, d_heads[hc],
+                                                     dst, s));
             }
             p->stats.refine_elements += n_act;
             depth += w_r;
             ++rounds;
+            if (sh.cap > 1) {
+                CX_CUDA(cudaMemcpyAsync(d_heads[1 - hc], d_heads[hc], (n_words + 1) * 4, cudaMemcpyDeviceToDevice, s));
+                ScopedLaunch sl(prof, CX_K_FINISH, nb / 4, s);
+                CX_CUDA(launch_finish_later<IdT>(R, d_heads[hc], d_heads[1 - hc], ids, nb, depth, sh.cap, dst, d_done, s));
+                hc = 1 - hc;
+            }
         }
         p->stats.small_group_elems = p->h_scalars[1];
         p->stats.refine_elements += p->h_scalars[1] - local_before;
         if (rounds > p->stats.refine_rounds) p->stats.refine_rounds = rounds;
 
-        // ---- step 3(c)iii: emit preceding symbols ------------------------------------------------
-        if (!sh.host_out) {
-            ScopedLaunch sl(prof, CX_K_EMIT, nb * (sizeof(IdT) + 2), s);
-            CX_CUDA(launch_emit<IdT>(R, ids, nb, out + B.out_offset, s));
-        } else {
-            // a9: stage in the workspace, copy on the side stream while the next batch computes
-            const int st = (int)(bi & 1);
-            uint8_t* stage = ws + L.stage[st];
-            if (p->stage_busy[st]) CX_CUDA(cudaStreamWaitEvent(s, p->stage_free[st], 0));
-            {
-                ScopedLaunch sl(prof, CX_K_EMIT, nb * (sizeof(IdT) + 2), s);
-                CX_CUDA(launch_emit<IdT>(R, ids, nb, stage, s));
-            }
+        if (sh.host_out) {
+            // a9: copy the staged batch on the side stream while the next batch computes
             CX_CUDA(cudaEventRecord(p->emit_done, s));
             CX_CUDA(cudaStreamWaitEvent(p->copy_stream, p->emit_done, 0));
-            CX_CUDA(cudaMemcpyAsync(out + B.out_offset, stage, nb, cudaMemcpyDeviceToHost, p->copy_stream));
+            CX_CUDA(cudaMemcpyAsync(out + B.out_offset, dst, nb, cudaMemcpyDeviceToHost, p->copy_stream));
             CX_CUDA(cudaEventRecord(p->stage_free[st], p->copy_stream));
             p->stage_busy[st] = true;
         }

@@ -146,8 +146,6 @@ cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, u
                        uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s);
 
 // cx_refine.cu
-template <typename KeyT>
-cudaError_t launch_flag_heads(const KeyT* keys, uint64_t n, uint32_t w, uint32_t* heads, cudaStream_t s);
 // word-level counts of active elements / active heads, packed (heads << 32 | elements)
 cudaError_t launch_active_count(const uint32_t* heads, uint64_t n, uint64_t* word_counts, cudaStream_t s);
 // exclusive scan in place; total written to *total; block_sums needs scan_block_count(n) entries
@@ -156,13 +154,17 @@ cudaError_t launch_scan_u64(uint64_t* data, uint64_t n, uint64_t* block_sums, ui
 template <typename IdT>
 cudaError_t launch_refine_rekey(const Reads& R, const uint32_t* heads, const uint64_t* word_base, const IdT* ids, uint64_t n,
                                 uint32_t depth, uint32_t w, uint64_t* keys_c, IdT* ids_c, uint32_t* pos_c, cudaStream_t s);
+// writes ids back in place, sets new head bits, emits the BWT symbol of every suffix that became final
 template <typename IdT>
-cudaError_t launch_refine_writeback(const uint64_t* keys_c, const IdT* ids_c, const uint32_t* pos_c, uint64_t n_c, uint32_t w,
-                                    IdT* ids, uint32_t* heads, cudaStream_t s);
+cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, const IdT* ids_c, const uint32_t* pos_c, uint64_t n_c,
+                                    uint32_t w, IdT* ids, uint32_t* heads, uint8_t* out, cudaStream_t s);
+// fused head flags + in-block refinement + emit over the freshly sorted first-round keys; heads_out must be zero-filled
+template <typename KeyT, typename IdT>
+cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t* heads_out, const IdT* ids, uint64_t n,
+                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, cudaStream_t s);
+// in-block refinement + emit of the groups a global round has split to at most group_cap members; heads_out = copy of heads_in
 template <typename IdT>
-cudaError_t launch_refine_local(const Reads& R, const uint32_t* heads_in, uint32_t* heads_out, IdT* ids, uint64_t n, uint32_t depth,
-                                uint32_t group_cap, unsigned long long* elems_done, cudaStream_t s);
-template <typename IdT>
-cudaError_t launch_emit(const Reads& R, const IdT* ids, uint64_t n, uint8_t* out, cudaStream_t s);
+cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32_t* heads_out, const IdT* ids, uint64_t n, uint32_t depth,
+                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, cudaStream_t s);
 
 }  // namespace cx

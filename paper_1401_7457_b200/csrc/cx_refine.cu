@@ -46,24 +46,6 @@ __device__ __forceinline__ uint64_t key_at_depth(const Reads& R, IdT id, uint32_
     return make_key(window, rem, w);
 }
 
-// ---------------------------------------------------------------------------------------------
-// head flags of a freshly sorted key array
-// ---------------------------------------------------------------------------------------------
-template <typename KeyT>
-__global__ void __launch_bounds__(256) flag_heads_kernel(const KeyT* __restrict__ keys, uint64_t n, uint32_t w, uint32_t len_mask,
-                                                         uint32_t* __restrict__ heads) {
-    uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    uint64_t n_words = (n + 31) >> 5;
-    bool head = true;   // positions past n count as heads
-    if (j < n) {
-        KeyT k = __ldcs(keys + j);
-        head = j == 0 || k != __ldg(keys + j - 1) || ((uint32_t)k & len_mask) < w;
-    }
-    uint32_t word = __ballot_sync(kFull, head);
-    if (lane_id() == 0 && (j >> 5) < n_words) heads[j >> 5] = word;
-    if (j == 0) heads[n_words] = kFull;   // padding word: "the next position is a head"
-}
-
 // per 32 positions: active elements (members of groups of >= 2) and active heads, packed hi|lo
 __device__ __forceinline__ void active_masks(uint32_t H, uint32_t next_word, uint32_t& act, uint32_t& act_heads) {
     uint32_t Hn = (H >> 1) | (next_word << 31);   // bit j = head(j + 1)
@@ -159,6 +141,19 @@ __global__ void __launch_bounds__(kScanThreads) scan_down_kernel(uint64_t* __res
 }
 
 // ---------------------------------------------------------------------------------------------
+// a8 helper: B[k] = '$' if the k-th suffix starts its read, else the base before it
+// ---------------------------------------------------------------------------------------------
+template <typename IdT>
+__device__ __forceinline__ uint8_t preceding_symbol(const Reads& R, IdT id) {
+    uint64_t read = (uint64_t)id >> R.pos_bits;
+    uint64_t pos = (uint64_t)id & ((1ull << R.pos_bits) - 1);
+    if (pos == 0) return (uint8_t)'$';
+    uint64_t b = (R.uniform ? read * R.uniform_len : __ldg(R.offsets + read)) + pos - 1;
+    uint32_t code = (uint32_t)(__ldg(R.packed + (b >> 5)) >> (62 - 2 * (b & 31))) & 3u;
+    return (uint8_t)((0x54474341u >> (8 * code)) & 0xFFu);
+}
+
+// ---------------------------------------------------------------------------------------------
 // global path: compact + re-key, write back
 // ---------------------------------------------------------------------------------------------
 template <typename IdT>
@@ -185,24 +180,39 @@ __global__ void __launch_bounds__(256) refine_rekey_kernel(Reads R, const uint32
 }
 
 template <typename IdT>
-__global__ void __launch_bounds__(256) refine_writeback_kernel(const uint64_t* __restrict__ keys_c, const IdT* __restrict__ ids_c,
+__global__ void __launch_bounds__(256) refine_writeback_kernel(Reads R, const uint64_t* __restrict__ keys_c, const IdT* __restrict__ ids_c,
                                                                const uint32_t* __restrict__ pos_c, uint64_t n_c, uint32_t w,
-                                                               IdT* __restrict__ ids, uint32_t* __restrict__ heads) {
+                                                               IdT* __restrict__ ids, uint32_t* __restrict__ heads, uint8_t* __restrict__ out) {
     uint64_t c = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= n_c) return;
     uint64_t k = keys_c[c];
     uint32_t pos = pos_c[c];
-    ids[pos] = ids_c[c];
+    IdT id = ids_c[c];
+    ids[pos] = id;
     bool head = c == 0 || k != keys_c[c - 1] || (uint32_t)(k & 31) < w;
     if (head) atomicOr(&heads[pos >> 5], 1u << (pos & 31));
+    // alone in its group now (or its end-marker was inside the window): final, emit its BWT symbol
+    bool next_is_head = true;
+    if (c + 1 < n_c) {
+        uint64_t kn = keys_c[c + 1];
+        next_is_head = kn != k || (uint32_t)(kn & 31) < w;
+    }
+    if (head && next_is_head) out[pos] = preceding_symbol(R, id);
 }
 
 // ---------------------------------------------------------------------------------------------
-// local path
+// a7 + a8 fused, one block per tile of kLocalTile sorted positions ("finish" kernel):
+//   FIRST : head flags from the freshly sorted first-round keys; every suffix that is alone in its
+//           group is final and its BWT symbol is emitted at once; groups of 2..cap suffixes that start
+//           in the tile are refined to the end in shared memory and emitted; larger groups are left
+//           to the global path (their head bits go to `heads`).
+//   !FIRST: after a global round; head flags come from `heads`; only groups of 2..cap are touched.
+// A position is emitted exactly once, by whoever makes it final (here, or the global write-back).
 // ---------------------------------------------------------------------------------------------
 constexpr int kLocalElems = kLocalTile + kLocalGroupCap;   // positions a block may touch
 constexpr int kLocalWords = kLocalElems / 32 + 2;
-constexpr int kLocalItems = (kLocalElems + kLocalThreads - 1) / kLocalThreads;
+constexpr int kLocalItems = kLocalElems / kLocalThreads;
+static_assert(kLocalElems % kLocalThreads == 0 && kLocalThreads % 32 == 0, "tile shape");
 constexpr uint32_t kLocalW = 29;                            // bases per in-block round
 constexpr uint16_t kNone = 0xffff;
 
@@ -216,7 +226,7 @@ struct LocalSmem {
     uint16_t ge[kLocalElems];   // one past its last position
     uint32_t hw[kLocalWords];   // head bits of the window, updated as groups split
     uint32_t hw0[kLocalWords];  // as loaded
-    uint8_t owned[kLocalElems];
+    uint8_t mine[kLocalElems];  // 1: this block emits the position
 };
 
 // nearest set bit at or below position e, not lower than `lo`; -1 if none
@@ -248,113 +258,132 @@ __device__ __forceinline__ int next_head(const uint32_t* hw, int e, int hi) {
     }
 }
 
-template <typename IdT>
-__global__ void __launch_bounds__(kLocalThreads) refine_local_kernel(Reads R, const uint32_t* __restrict__ heads_in,
-                                                                     uint32_t* __restrict__ heads_out, IdT* __restrict__ ids, uint64_t n,
-                                                                     uint32_t depth0, uint32_t cap, unsigned long long* elems_done) {
+template <typename KeyT, typename IdT, bool FIRST>
+__global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, const KeyT* __restrict__ keys1, uint32_t w1, uint32_t len_mask,
+                                                                    const uint32_t* __restrict__ heads_in, uint32_t* __restrict__ heads,
+                                                                    const IdT* __restrict__ ids, uint64_t n,
+                                                                    uint32_t depth0, uint32_t cap, uint8_t* __restrict__ out,
+                                                                    unsigned long long* elems_done) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     LocalSmem<IdT>& sm = *reinterpret_cast<LocalSmem<IdT>*>(smem_raw);
     const uint64_t base = (uint64_t)blockIdx.x * kLocalTile;
     const uint64_t w0 = base >> 5;
-    const uint64_t n_words = ((n + 31) >> 5) + 1;   // including the padding word
+    const uint64_t n_words = (n + 31) >> 5;   // heads[n_words] is the padding word ("the next position is a head")
     const int tid = threadIdx.x;
 
-    uint32_t incomplete = 0;
-    for (int i = tid; i < kLocalWords; i += kLocalThreads) {
-        uint32_t v = w0 + i < n_words ? heads_in[w0 + i] : kFull;
-        sm.hw[i] = v;
-        sm.hw0[i] = v;
-        // positions 1 .. kLocalTile decide whether a group of >= 2 starts in this tile
-        if (i <= kLocalTile / 32) {
-            uint32_t care = i == 0 ? ~1u : (i == kLocalTile / 32 ? 1u : kFull);
-            incomplete |= (~v) & care;
+    // ---- head bits of the window ------------------------------------------------------------------
+    if (FIRST) {
+#pragma unroll
+        for (int k = 0; k < kLocalItems; ++k) {
+            const int e = k * kLocalThreads + tid;
+            const uint64_t j = base + e;
+            bool head = true;   // positions past n count as heads
+            if (j < n) {
+                const KeyT kc = __ldcs(keys1 + j);
+                head = j == 0 || kc != __ldg(keys1 + j - 1) || ((uint32_t)kc & len_mask) < w1;
+                sm.id_a[e] = __ldcs(ids + j);
+            }
+            const uint32_t word = __ballot_sync(kFull, head);
+            if ((tid & 31) == 0) sm.hw[e >> 5] = word;
         }
+        if (tid < kLocalWords - kLocalElems / 32) sm.hw[kLocalElems / 32 + tid] = kFull;
+    } else {
+        uint32_t incomplete = 0;
+        for (int i = tid; i < kLocalWords; i += kLocalThreads) {
+            const uint32_t v = w0 + i <= n_words ? heads_in[w0 + i] : kFull;
+            sm.hw[i] = v;
+            sm.hw0[i] = v;
+            // positions 1 .. kLocalTile decide whether a group of >= 2 starts in this tile
+            if (i <= kLocalTile / 32) {
+                const uint32_t care = i == 0 ? ~1u : (i == kLocalTile / 32 ? 1u : kFull);
+                incomplete |= (~v) & care;
+            }
+        }
+        if (!__syncthreads_or(incomplete)) return;
     }
-    if (!__syncthreads_or(incomplete)) return;
+    __syncthreads();
 
-    // classify: which positions belong to a group that starts in this tile and has 2..cap members
-    uint32_t mine = 0;
+    // ---- classify: groups that start in this tile and have at most cap members are ours -----------
+    uint32_t n_active = 0;
 #pragma unroll
     for (int k = 0; k < kLocalItems; ++k) {
-        int e = k * kLocalThreads + tid;
-        if (e >= kLocalElems) break;
+        const int e = k * kLocalThreads + tid;
         uint16_t s = kNone, t = kNone;
-        uint8_t own = 0;
+        uint8_t mine = 0;
         if (base + e < n) {
-            int lo = e - (int)cap + 1;
-            int ps = prev_head(sm.hw, e, lo < 0 ? 0 : lo);
+            const int lo = e - (int)cap + 1;
+            const int ps = prev_head(sm.hw, e, lo < 0 ? 0 : lo);
             if (ps >= 0 && ps < kLocalTile) {
-                int ne = next_head(sm.hw, e, ps + (int)cap);
-                if (ne > 0 && ne - ps >= 2) {
-                    s = (uint16_t)ps;
-                    t = (uint16_t)ne;
-                    own = 1;
-                    sm.id_a[e] = ids[base + e];
-                    ++mine;
+                const int ne = next_head(sm.hw, e, ps + (int)cap);
+                if (ne > 0) {
+                    if (ne - ps >= 2) {
+                        s = (uint16_t)ps;
+                        t = (uint16_t)ne;
+                        mine = 1;
+                        ++n_active;
+                        if (!FIRST) sm.id_a[e] = ids[base + e];
+                    } else if (FIRST) {
+                        mine = 1;   // alone in its group after the first sort: final
+                    }
                 }
             }
         }
         sm.gs[e] = s;
         sm.ge[e] = t;
-        sm.owned[e] = own;
+        sm.mine[e] = mine;
     }
     __syncthreads();
 
+    // ---- rounds: one window gather per member still tied, stable rank by counting -------------------
     for (uint32_t depth = depth0;; depth += kLocalW) {
-        // one window gather per member still tied
         uint32_t any = 0;
 #pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
-            int e = k * kLocalThreads + tid;
-            if (e >= kLocalElems) break;
+            const int e = k * kLocalThreads + tid;
             if (sm.gs[e] != kNone) {
                 sm.key_a[e] = key_at_depth(R, sm.id_a[e], depth, kLocalW);
                 any = 1;
             }
         }
         if (!__syncthreads_or(any)) break;
-        // stable rank inside the group by counting smaller members
-#pragma unroll
+#pragma unroll 1
         for (int k = 0; k < kLocalItems; ++k) {
-            int e = k * kLocalThreads + tid;
-            if (e >= kLocalElems) break;
-            int s = sm.gs[e];
+            const int e = k * kLocalThreads + tid;
+            const int s = sm.gs[e];
             if (s != kNone) {
-                int t = sm.ge[e];
-                uint64_t mykey = sm.key_a[e];
+                const int t = sm.ge[e];
+                const uint64_t my = sm.key_a[e];
                 int cnt = 0;
-                for (int q = s; q < t; ++q) {
-                    uint64_t kq = sm.key_a[q];
-                    cnt += (kq < mykey) || (kq == mykey && q < e);
-                }
-                sm.key_b[s + cnt] = mykey;
+                // members listed before me rank below me on equal keys (stability: PAPER.md:99)
+#pragma unroll 4
+                for (int q = s; q < e; ++q) cnt += sm.key_a[q] <= my;
+#pragma unroll 4
+                for (int q = e + 1; q < t; ++q) cnt += sm.key_a[q] < my;
+                sm.key_b[s + cnt] = my;
                 sm.id_b[s + cnt] = sm.id_a[e];
             }
         }
         __syncthreads();
 #pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
-            int e = k * kLocalThreads + tid;
-            if (e >= kLocalElems) break;
+            const int e = k * kLocalThreads + tid;
             if (sm.gs[e] != kNone) {
-                uint64_t kk = sm.key_b[e];
-                sm.key_a[e] = kk;
+                const uint64_t kk = sm.key_b[e];
                 sm.id_a[e] = sm.id_b[e];
-                bool head = e == sm.gs[e] || kk != sm.key_b[e - 1] || (uint32_t)(kk & 31) < kLocalW;
+                const bool head = e == sm.gs[e] || kk != sm.key_b[e - 1] || (uint32_t)(kk & 31) < kLocalW;
                 if (head) atomicOr(&sm.hw[e >> 5], 1u << (e & 31));
             }
         }
         __syncthreads();
-        // new group bounds; singletons are placed for good
+        // new group bounds; members alone in their group are placed for good
 #pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
-            int e = k * kLocalThreads + tid;
-            if (e >= kLocalElems) break;
-            int s = sm.gs[e];
+            const int e = k * kLocalThreads + tid;
+            const int s = sm.gs[e];
             if (s != kNone) {
-                int t = sm.ge[e];
-                int ps = prev_head(sm.hw, e, s);
-                int ne = next_head(sm.hw, e, t);
+                const int t = sm.ge[e];
+                const int ps = prev_head(sm.hw, e, s);
+                const int ne = next_head(sm.hw, e, t);
                 if (ne - ps >= 2) {
                     sm.gs[e] = (uint16_t)ps;
                     sm.ge[e] = (uint16_t)ne;
@@ -366,51 +395,19 @@ __global__ void __launch_bounds__(kLocalThreads) refine_local_kernel(Reads R, co
         __syncthreads();
     }
 
-    // publish: ids of our groups, and their positions as heads (every member is placed)
+    // ---- emit what became final here; publish head bits for the global path ----------------------------
 #pragma unroll
     for (int k = 0; k < kLocalItems; ++k) {
-        int e = k * kLocalThreads + tid;
-        if (e >= kLocalElems) break;
-        if (sm.owned[e]) ids[base + e] = sm.id_a[e];
+        const int e = k * kLocalThreads + tid;
+        if (sm.mine[e]) out[base + e] = preceding_symbol(R, sm.id_a[e]);
     }
     for (int i = tid; i < kLocalWords; i += kLocalThreads) {
-        uint32_t add = sm.hw[i] & ~sm.hw0[i];
-        if (add) atomicOr(&heads_out[w0 + i], add);
+        if (w0 + i > n_words) continue;
+        const uint32_t add = FIRST ? (i < kLocalElems / 32 ? sm.hw[i] : 0u) : (sm.hw[i] & ~sm.hw0[i]);
+        if (add) atomicOr(&heads[w0 + i], add);
     }
-    for (int o = 16; o; o >>= 1) mine += __shfl_xor_sync(kFull, mine, o);
-    if (lane_id() == 0 && mine) atomicAdd(elems_done, (unsigned long long)mine);
-}
-
-// ---------------------------------------------------------------------------------------------
-// a8: emit.  B[k] = '$' if the k-th suffix starts its read, else the base before it
-// ---------------------------------------------------------------------------------------------
-template <typename IdT>
-__device__ __forceinline__ uint8_t preceding_symbol(const Reads& R, IdT id) {
-    uint64_t read = (uint64_t)id >> R.pos_bits;
-    uint64_t pos = (uint64_t)id & ((1ull << R.pos_bits) - 1);
-    if (pos == 0) return (uint8_t)'$';
-    uint64_t b = (R.uniform ? read * R.uniform_len : __ldg(R.offsets + read)) + pos - 1;
-    uint32_t code = (uint32_t)(__ldg(R.packed + (b >> 5)) >> (62 - 2 * (b & 31))) & 3u;
-    return (uint8_t)((0x54474341u >> (8 * code)) & 0xFFu);
-}
-
-template <typename IdT>
-__global__ void __launch_bounds__(256) emit_kernel(Reads R, const IdT* __restrict__ ids, uint64_t n, uint8_t* __restrict__ out) {
-    // four consecutive outputs per thread where the address allows a 32-bit store
-    uint64_t lead = (4 - (reinterpret_cast<uintptr_t>(out) & 3)) & 3;   // bytes before the first aligned word
-    if (lead > n) lead = n;
-    uint64_t q = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    uint64_t n_quads = (n - lead) >> 2;
-    if (q < n_quads) {
-        uint64_t j = lead + (q << 2);
-        uint32_t v = 0;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) v |= (uint32_t)preceding_symbol(R, __ldcs(ids + j + i)) << (8 * i);
-        *reinterpret_cast<uint32_t*>(out + j) = v;
-    } else if (q == n_quads) {
-        for (uint64_t j = 0; j < lead; ++j) out[j] = preceding_symbol(R, ids[j]);
-        for (uint64_t j = lead + (n_quads << 2); j < n; ++j) out[j] = preceding_symbol(R, ids[j]);
-    }
+    for (int o = 16; o; o >>= 1) n_active += __shfl_xor_sync(kFull, n_active, o);
+    if (lane_id() == 0 && n_active) atomicAdd(elems_done, (unsigned long long)n_active);
 }
 
 }  // namespace
@@ -418,16 +415,6 @@ __global__ void __launch_bounds__(256) emit_kernel(Reads R, const IdT* __restric
 // ---------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------
-template <typename KeyT>
-cudaError_t launch_flag_heads(const KeyT* keys, uint64_t n, uint32_t w, uint32_t* heads, cudaStream_t s) {
-    if (n == 0) return cudaSuccess;
-    uint64_t padded = ((n + 31) >> 5) << 5;
-    flag_heads_kernel<KeyT><<<(unsigned)((padded + 255) / 256), 256, 0, s>>>(keys, n, w, (1u << key_len_bits(w)) - 1, heads);
-    return cudaGetLastError();
-}
-template cudaError_t launch_flag_heads<uint32_t>(const uint32_t*, uint64_t, uint32_t, uint32_t*, cudaStream_t);
-template cudaError_t launch_flag_heads<uint64_t>(const uint64_t*, uint64_t, uint32_t, uint32_t*, cudaStream_t);
-
 cudaError_t launch_active_count(const uint32_t* heads, uint64_t n, uint64_t* word_counts, cudaStream_t s) {
     uint64_t n_words = (n + 31) >> 5;
     if (n_words == 0) return cudaSuccess;
@@ -455,18 +442,18 @@ cudaError_t launch_refine_rekey(const Reads& R, const uint32_t* heads, const uin
 }
 
 template <typename IdT>
-cudaError_t launch_refine_writeback(const uint64_t* keys_c, const IdT* ids_c, const uint32_t* pos_c, uint64_t n_c, uint32_t w,
-                                    IdT* ids, uint32_t* heads, cudaStream_t s) {
+cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, const IdT* ids_c, const uint32_t* pos_c, uint64_t n_c,
+                                    uint32_t w, IdT* ids, uint32_t* heads, uint8_t* out, cudaStream_t s) {
     if (n_c == 0) return cudaSuccess;
-    refine_writeback_kernel<IdT><<<(unsigned)((n_c + 255) / 256), 256, 0, s>>>(keys_c, ids_c, pos_c, n_c, w, ids, heads);
+    refine_writeback_kernel<IdT><<<(unsigned)((n_c + 255) / 256), 256, 0, s>>>(R, keys_c, ids_c, pos_c, n_c, w, ids, heads, out);
     return cudaGetLastError();
 }
 
-template <typename IdT>
-cudaError_t launch_refine_local(const Reads& R, const uint32_t* heads_in, uint32_t* heads_out, IdT* ids, uint64_t n, uint32_t depth,
-                                uint32_t group_cap, unsigned long long* elems_done, cudaStream_t s) {
+template <typename KeyT, typename IdT>
+cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t* heads_out, const IdT* ids, uint64_t n,
+                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
-    auto kernel = refine_local_kernel<IdT>;
+    auto kernel = finish_tile_kernel<KeyT, IdT, true>;
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem<IdT>));
@@ -475,26 +462,40 @@ cudaError_t launch_refine_local(const Reads& R, const uint32_t* heads_in, uint32
     }
     if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
     uint64_t blocks = (n + kLocalTile - 1) / kLocalTile;
-    kernel<<<(unsigned)blocks, kLocalThreads, sizeof(LocalSmem<IdT>), s>>>(R, heads_in, heads_out, ids, n, depth, group_cap, elems_done);
+    kernel<<<(unsigned)blocks, kLocalThreads, sizeof(LocalSmem<IdT>), s>>>(R, keys1, w1, (1u << key_len_bits(w1)) - 1, nullptr, heads_out, ids, n,
+                                                                          w1, group_cap, out, elems_done);
     return cudaGetLastError();
 }
 
 template <typename IdT>
-cudaError_t launch_emit(const Reads& R, const IdT* ids, uint64_t n, uint8_t* out, cudaStream_t s) {
+cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32_t* heads_out, const IdT* ids, uint64_t n, uint32_t depth,
+                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
-    uint64_t threads = (n >> 2) + 1;
-    emit_kernel<IdT><<<(unsigned)((threads + 255) / 256), 256, 0, s>>>(R, ids, n, out);
+    auto kernel = finish_tile_kernel<uint64_t, IdT, false>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem<IdT>));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
+    uint64_t blocks = (n + kLocalTile - 1) / kLocalTile;
+    kernel<<<(unsigned)blocks, kLocalThreads, sizeof(LocalSmem<IdT>), s>>>(R, nullptr, 0, 0, heads_in, heads_out, ids, n, depth, group_cap, out,
+                                                                          elems_done);
     return cudaGetLastError();
 }
 
 #define CX_INSTANTIATE(IdT)                                                                                                          \
     template cudaError_t launch_refine_rekey<IdT>(const Reads&, const uint32_t*, const uint64_t*, const IdT*, uint64_t, uint32_t,   \
                                                   uint32_t, uint64_t*, IdT*, uint32_t*, cudaStream_t);                               \
-    template cudaError_t launch_refine_writeback<IdT>(const uint64_t*, const IdT*, const uint32_t*, uint64_t, uint32_t, IdT*,       \
-                                                      uint32_t*, cudaStream_t);                                                      \
-    template cudaError_t launch_refine_local<IdT>(const Reads&, const uint32_t*, uint32_t*, IdT*, uint64_t, uint32_t, uint32_t,     \
-                                                  unsigned long long*, cudaStream_t);                                                \
-    template cudaError_t launch_emit<IdT>(const Reads&, const IdT*, uint64_t, uint8_t*, cudaStream_t);
+    template cudaError_t launch_refine_writeback<IdT>(const Reads&, const uint64_t*, const IdT*, const uint32_t*, uint64_t,         \
+                                                      uint32_t, IdT*, uint32_t*, uint8_t*, cudaStream_t);                            \
+    template cudaError_t launch_finish_first<uint32_t, IdT>(const Reads&, const uint32_t*, uint32_t, uint32_t*, const IdT*,         \
+                                                            uint64_t, uint32_t, uint8_t*, unsigned long long*, cudaStream_t);        \
+    template cudaError_t launch_finish_first<uint64_t, IdT>(const Reads&, const uint64_t*, uint32_t, uint32_t*, const IdT*,         \
+                                                            uint64_t, uint32_t, uint8_t*, unsigned long long*, cudaStream_t);        \
+    template cudaError_t launch_finish_later<IdT>(const Reads&, const uint32_t*, uint32_t*, const IdT*, uint64_t, uint32_t,         \
+                                                  uint32_t, uint8_t*, unsigned long long*, cudaStream_t);
 CX_INSTANTIATE(uint32_t)
 CX_INSTANTIATE(uint64_t)
 
