@@ -213,15 +213,15 @@ constexpr int kLocalElems = kLocalTile + kLocalGroupCap;   // positions a block 
 constexpr int kLocalWords = kLocalElems / 32 + 2;
 constexpr int kLocalItems = kLocalElems / kLocalThreads;
 static_assert(kLocalElems % kLocalThreads == 0 && kLocalThreads % 32 == 0, "tile shape");
-constexpr uint32_t kLocalW = 29;                            // bases per in-block round
+constexpr uint32_t kLocalW = 57;                            // bases per in-block round
+typedef unsigned __int128 u128;
 constexpr uint16_t kNone = 0xffff;
 
 template <typename IdT>
 struct LocalSmem {
-    uint64_t key_a[kLocalElems];
-    uint64_t key_b[kLocalElems];
+    u128 key[kLocalElems];      // [57 bases, A-padded : 114][min(remaining, 57) : 6][index inside the group : 8]
     IdT id_a[kLocalElems];
-    IdT id_b[kLocalElems];
+    uint16_t src[kLocalElems];  // src[p] = member that ranks at position p after this round
     uint16_t gs[kLocalElems];   // first position of the element's current group (kNone: not ours / placed)
     uint16_t ge[kLocalElems];   // one past its last position
     uint32_t hw[kLocalWords];   // head bits of the window, updated as groups split
@@ -256,6 +256,46 @@ __device__ __forceinline__ int next_head(const uint32_t* hw, int e, int hi) {
         if ((wi << 5) > hi) return -1;
         bits = hw[wi];
     }
+}
+
+// 128-bit round key of suffix `id` at depth d: the next 57 bases (A-padded), then min(remaining, 57), then the
+// member's index inside its tie group -- so that one unsigned compare orders the group stably
+template <typename IdT>
+__device__ __forceinline__ u128 key128_at_depth(const Reads& R, IdT id, uint32_t depth, uint32_t idx) {
+    const uint64_t read = (uint64_t)id >> R.pos_bits;
+    const uint64_t pos = (uint64_t)id & ((1ull << R.pos_bits) - 1);
+    uint64_t start, len;
+    read_span(R, read, start, len);
+    const uint64_t at = pos + depth;
+    const uint64_t rem = at < len ? len - at : 0;
+    const uint32_t r = rem < kLocalW ? (uint32_t)rem : kLocalW;
+    uint64_t hi = 0, mid = 0;
+    if (r) {
+        const uint64_t b = start + at;
+        const uint64_t wi = b >> 5;
+        const uint32_t sh = (uint32_t)(b & 31) * 2;
+        const uint64_t w0 = __ldg(R.packed + wi);
+        const uint64_t w1 = (sh || r > 32) && wi + 1 < R.n_words ? __ldg(R.packed + wi + 1) : 0ull;
+        hi = sh ? (w0 << sh) | (w1 >> (64 - sh)) : w0;
+        if (r < 32) {
+            hi &= ~0ull << (64 - 2 * r);
+        } else if (r > 32) {
+            const uint64_t w2 = sh && wi + 2 < R.n_words ? __ldg(R.packed + wi + 2) : 0ull;
+            mid = sh ? (w1 << sh) | (w2 >> (64 - sh)) : w1;
+            mid &= ~0ull << (64 - 2 * (r - 32));   // at most 25 bases: the low 14 bits are clear
+        }
+    }
+    const uint64_t lo = mid | ((uint64_t)r << 8) | idx;
+    return ((u128)hi << 64) | lo;
+}
+
+// acc -= (a < b) for 128-bit unsigned a, b (x = least significant word): the borrow of a - b, five instructions
+__device__ __forceinline__ void count_if_less(uint32_t& acc, const uint4& a, const uint4& b) {
+    asm("{\n\t.reg .u32 t;\n\t"
+        "sub.cc.u32 t, %1, %5;\n\tsubc.cc.u32 t, %2, %6;\n\tsubc.cc.u32 t, %3, %7;\n\tsubc.cc.u32 t, %4, %8;\n\t"
+        "subc.u32 %0, %0, 0;\n\t}"
+        : "+r"(acc)
+        : "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w), "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w));
 }
 
 template <typename KeyT, typename IdT, bool FIRST>
@@ -334,14 +374,15 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
     }
     __syncthreads();
 
-    // ---- rounds: one window gather per member still tied, stable rank by counting -------------------
+    // ---- rounds: one 57-base gather per member still tied, stable rank by counting -------------------
     for (uint32_t depth = depth0;; depth += kLocalW) {
         uint32_t any = 0;
 #pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
             const int e = k * kLocalThreads + tid;
-            if (sm.gs[e] != kNone) {
-                sm.key_a[e] = key_at_depth(R, sm.id_a[e], depth, kLocalW);
+            const int s = sm.gs[e];
+            if (s != kNone) {
+                sm.key[e] = key128_at_depth(R, sm.id_a[e], depth, (uint32_t)(e - s));
                 any = 1;
             }
         }
@@ -352,15 +393,25 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
             const int s = sm.gs[e];
             if (s != kNone) {
                 const int t = sm.ge[e];
-                const uint64_t my = sm.key_a[e];
-                int cnt = 0;
-                // members listed before me rank below me on equal keys (stability: PAPER.md:99)
+                const uint4 my = reinterpret_cast<const uint4*>(sm.key)[e];
+                uint32_t neg = 0;   // minus the number of members whose key is below mine
 #pragma unroll 4
-                for (int q = s; q < e; ++q) cnt += sm.key_a[q] <= my;
-#pragma unroll 4
-                for (int q = e + 1; q < t; ++q) cnt += sm.key_a[q] < my;
-                sm.key_b[s + cnt] = my;
-                sm.id_b[s + cnt] = sm.id_a[e];
+                for (int q = s; q < t; ++q) count_if_less(neg, reinterpret_cast<const uint4*>(sm.key)[q], my);
+                sm.src[s - (int)neg] = (uint16_t)e;
+            }
+        }
+        __syncthreads();
+        IdT idn[kLocalItems];
+        uint32_t headbit = 0;
+#pragma unroll
+        for (int k = 0; k < kLocalItems; ++k) {
+            const int e = k * kLocalThreads + tid;
+            if (sm.gs[e] != kNone) {
+                const int se = sm.src[e];
+                const u128 kk = sm.key[se] >> 8;
+                idn[k] = sm.id_a[se];
+                const bool head = e == sm.gs[e] || kk != (sm.key[sm.src[e - 1]] >> 8) || ((uint32_t)kk & 63u) < kLocalW;
+                headbit |= (uint32_t)head << k;
             }
         }
         __syncthreads();
@@ -368,10 +419,8 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
         for (int k = 0; k < kLocalItems; ++k) {
             const int e = k * kLocalThreads + tid;
             if (sm.gs[e] != kNone) {
-                const uint64_t kk = sm.key_b[e];
-                sm.id_a[e] = sm.id_b[e];
-                const bool head = e == sm.gs[e] || kk != sm.key_b[e - 1] || (uint32_t)(kk & 31) < kLocalW;
-                if (head) atomicOr(&sm.hw[e >> 5], 1u << (e & 31));
+                sm.id_a[e] = idn[k];
+                if ((headbit >> k) & 1u) atomicOr(&sm.hw[e >> 5], 1u << (e & 31));
             }
         }
         __syncthreads();
@@ -392,7 +441,6 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
                 }
             }
         }
-        __syncthreads();
     }
 
     // ---- emit what became final here; publish head bits for the global path ----------------------------
