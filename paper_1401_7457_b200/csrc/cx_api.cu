@@ -393,10 +393,12 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         const Batch& B = p->batches[bi];
         const uint64_t nb = B.count;
         // ---- step 3(a) + 3(c)i: list the batch's suffixes with their first keys ----------------
+        const uint32_t n_passes = (key_bits + kRadixBits - 1) / kRadixBits;
+        CX_CUDA(cudaMemsetAsync(p->sort.hist, 0, (size_t)n_passes * kRadix * sizeof(uint64_t), s));
         if (single) {
             ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (sizeof(KeyT) + sizeof(IdT)), s);
             CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, nullptr, d_keys1[0],
-                                                  d_ids[0], n_tiles, s)));
+                                                  d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, s)));
         } else {
             {
                 ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + n_tiles * 8, s);
@@ -409,11 +411,11 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             prof->launches[CX_K_LIST] += 2;   // the scan is three kernels
             ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (sizeof(KeyT) + sizeof(IdT)), s);
             CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, d_tile_count,
-                                                  d_keys1[0], d_ids[0], n_tiles, s)));
+                                                  d_keys1[0], d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, s)));
         }
         // ---- step 3(c)ii: sort (first w symbols) ------------------------------------------------
         int in_alt = 0;
-        CX_CUDA((sort_pairs<KeyT, IdT>(d_keys1[0], d_ids[0], d_keys1[1], d_ids[1], nb, 0, key_bits, p->sort, &in_alt, prof, s)));
+        CX_CUDA((sort_pairs<KeyT, IdT>(d_keys1[0], d_ids[0], d_keys1[1], d_ids[1], nb, 0, key_bits, p->sort, &in_alt, prof, s, true)));
         const int cur = in_alt;
         IdT* ids = d_ids[cur];
         // a9: with pinned-host output the batch is emitted into a staging buffer of the workspace

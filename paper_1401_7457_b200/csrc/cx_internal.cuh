@@ -122,11 +122,13 @@ cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint
 // count suffixes of each tile whose bucket lies in [bucket_lo, bucket_hi]
 cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
                               uint32_t bucket_lo, uint32_t bucket_hi, uint64_t* tile_count, uint64_t n_tiles, cudaStream_t s);
-// write (key, id) of those suffixes in (read, pos) order; tile_base == nullptr means "every suffix, index = slot"
+// write (key, id) of those suffixes in (read, pos) order; tile_base == nullptr means "every suffix, index = slot".
+// Also accumulates the digit counts of the n_passes radix passes over key bits [0, 8 * n_passes) into digit_hist
+// (zeroed by the caller), which is what sort_pairs(..., hist_ready = true) expects.
 template <typename KeyT, typename IdT>
 cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
                               uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, KeyT* keys, IdT* ids,
-                              uint64_t n_tiles, cudaStream_t s);
+                              uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, cudaStream_t s);
 
 // cx_onesweep.cu
 struct SortWorkspace {
@@ -141,9 +143,10 @@ size_t sort_workspace_bytes(uint64_t n);
 // carve a zeroed region of sort_workspace_bytes(n) bytes
 void sort_workspace_carve(SortWorkspace& ws, void* mem, uint64_t n);
 // Sorts by key bits [begin_bit, end_bit).  *result_in_alt = 1 if the result is in the alt buffers.
+// hist_ready: ws.hist already holds the digit counts of every pass (the list kernel built them); begin_bit must be 0.
 template <typename KeyT, typename ValT>
 cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
-                       uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s);
+                       uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s, bool hist_ready = false);
 
 // cx_refine.cu
 // word-level counts of active elements / active heads, packed (heads << 32 | elements)

@@ -299,7 +299,7 @@ void sort_workspace_carve(SortWorkspace& ws, void* mem, uint64_t n) {
 
 template <typename KeyT, typename ValT>
 cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
-                       uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s) {
+                       uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s, bool hist_ready) {
     *result_in_alt = 0;
     if (n <= 1 || end_bit <= begin_bit) return cudaSuccess;
     constexpr int ITEMS = SortShape<KeyT, ValT>::items;
@@ -321,9 +321,9 @@ cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, u
     const uint64_t n_tiles = (n + kTile - 1) / kTile;
     if (n_tiles > ws.max_tiles || n_passes > 8 || n > 0xFFFF0000ull) return cudaErrorInvalidValue;
 
-    e = cudaMemsetAsync(ws.hist, 0, (size_t)n_passes * kRadix * sizeof(uint64_t), s);
-    if (e != cudaSuccess) return e;
-    {
+    if (!hist_ready) {
+        e = cudaMemsetAsync(ws.hist, 0, (size_t)n_passes * kRadix * sizeof(uint64_t), s);
+        if (e != cudaSuccess) return e;
         uint64_t chunk = (uint64_t)kHistThreads * kHistItems;
         uint64_t blocks = (n + chunk - 1) / chunk;
         unsigned grid = (unsigned)(blocks < 148ull * 4 ? blocks : 148ull * 4);
@@ -367,7 +367,7 @@ cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, u
 }
 
 #define CX_SORT_INST(K, V)                                                                                               \
-    template cudaError_t sort_pairs<K, V>(K*, V*, K*, V*, uint64_t, uint32_t, uint32_t, SortWorkspace&, int*, Launch*, cudaStream_t);
+    template cudaError_t sort_pairs<K, V>(K*, V*, K*, V*, uint64_t, uint32_t, uint32_t, SortWorkspace&, int*, Launch*, cudaStream_t, bool);
 CX_SORT_INST(uint32_t, uint32_t)
 CX_SORT_INST(uint32_t, uint64_t)
 CX_SORT_INST(uint64_t, uint32_t)

@@ -454,8 +454,14 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
         const uint32_t add = FIRST ? (i < kLocalElems / 32 ? sm.hw[i] : 0u) : (sm.hw[i] & ~sm.hw0[i]);
         if (add) atomicOr(&heads[w0 + i], add);
     }
+    // one statistics update per block (hundreds of thousands of atomics on one address would serialise in L2)
+    __shared__ uint32_t s_done;
+    if (tid == 0) s_done = 0;
+    __syncthreads();
     for (int o = 16; o; o >>= 1) n_active += __shfl_xor_sync(kFull, n_active, o);
-    if (lane_id() == 0 && n_active) atomicAdd(elems_done, (unsigned long long)n_active);
+    if (lane_id() == 0 && n_active) atomicAdd(&s_done, n_active);
+    __syncthreads();
+    if (tid == 0 && s_done) atomicAdd(elems_done, (unsigned long long)s_done);
 }
 
 }  // namespace

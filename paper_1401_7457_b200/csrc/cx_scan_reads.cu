@@ -80,17 +80,29 @@ struct TileCtx {
     uint64_t r0;        // first read
     uint32_t n_tile_reads;
     uint64_t word0;     // first packed word staged
+    uint32_t uniform;   // every read has length L: slot -> (read, pos) by division, no offsets needed
+    uint32_t L1;        // L + 1
+    uint32_t pos0;      // position of slot g0 inside read r0 (uniform only)
 };
 
-__device__ __forceinline__ TileCtx load_tile(const Reads& R, const uint32_t* __restrict__ tile_first_read, uint64_t t,
-                                             uint64_t n_tiles, uint64_t N, TileSmem& sm) {
+__device__ __forceinline__ TileCtx load_tile(const Reads& R, const BuildInfo* __restrict__ info,
+                                             const uint32_t* __restrict__ tile_first_read, uint64_t t, uint64_t n_tiles, uint64_t N,
+                                             TileSmem& sm) {
     TileCtx c;
     c.g0 = t * kListTile;
     c.n_slots = (uint32_t)min((uint64_t)kListTile, N - c.g0);
+    c.uniform = info->nonuniform ? 0u : 1u;
+    c.L1 = (uint32_t)info->first_len + 1u;
     c.r0 = tile_first_read[t];
-    uint64_t r_last = (t + 1 < n_tiles) ? (uint64_t)tile_first_read[t + 1] : R.n_reads - 1;
-    c.n_tile_reads = (uint32_t)(r_last - c.r0 + 1);                       // <= kListTile + 1
-    for (uint32_t j = threadIdx.x; j <= c.n_tile_reads; j += blockDim.x) sm.off[j] = R.offsets[c.r0 + j];
+    c.pos0 = 0;
+    c.n_tile_reads = 0;
+    if (c.uniform) {
+        c.pos0 = (uint32_t)(c.g0 - c.r0 * c.L1);
+    } else {
+        uint64_t r_last = (t + 1 < n_tiles) ? (uint64_t)tile_first_read[t + 1] : R.n_reads - 1;
+        c.n_tile_reads = (uint32_t)(r_last - c.r0 + 1);                       // <= kListTile + 1
+        for (uint32_t j = threadIdx.x; j <= c.n_tile_reads; j += blockDim.x) sm.off[j] = R.offsets[c.r0 + j];
+    }
     // base position of slot g is g - (its read index); it grows by 0 or 1 per slot
     uint64_t b0 = c.g0 - c.r0;
     c.word0 = b0 >> 5;
@@ -108,19 +120,29 @@ struct Slot {
 };
 
 __device__ __forceinline__ Slot decode_slot(const TileCtx& c, const TileSmem& sm, uint32_t s) {
-    uint64_t g = c.g0 + s;
-    // largest j with off[j] + r0 + j <= g
-    uint32_t lo = 0, hi = c.n_tile_reads - 1;
-    while (lo < hi) {
-        uint32_t mid = (lo + hi + 1) >> 1;
-        if (sm.off[mid] + c.r0 + mid <= g) lo = mid; else hi = mid - 1;
-    }
     Slot sl;
-    sl.read = c.r0 + lo;
-    uint64_t start = sm.off[lo];
-    sl.pos = g - (start + sl.read);
-    sl.rem = sm.off[lo + 1] - start - sl.pos;
-    uint64_t b = start + sl.pos;
+    uint64_t b;
+    if (c.uniform) {
+        const uint32_t x = c.pos0 + s;
+        const uint32_t rr = x / c.L1;
+        sl.read = c.r0 + rr;
+        sl.pos = x - rr * c.L1;
+        sl.rem = (c.L1 - 1) - sl.pos;
+        b = sl.read * (c.L1 - 1) + sl.pos;
+    } else {
+        uint64_t g = c.g0 + s;
+        // largest j with off[j] + r0 + j <= g
+        uint32_t lo = 0, hi = c.n_tile_reads - 1;
+        while (lo < hi) {
+            uint32_t mid = (lo + hi + 1) >> 1;
+            if (sm.off[mid] + c.r0 + mid <= g) lo = mid; else hi = mid - 1;
+        }
+        sl.read = c.r0 + lo;
+        uint64_t start = sm.off[lo];
+        sl.pos = g - (start + sl.read);
+        sl.rem = sm.off[lo + 1] - start - sl.pos;
+        b = start + sl.pos;
+    }
     uint32_t wi = (uint32_t)((b >> 5) - c.word0);
     uint32_t sh = (uint32_t)(b & 31) * 2;
     uint64_t w0 = sm.packed[wi], w1 = sm.packed[wi + 1];
@@ -147,33 +169,43 @@ __global__ void __launch_bounds__(kListThreads) bucket_hist_kernel(Reads R, cons
     TileSmem& sm = *reinterpret_cast<TileSmem*>(smem_raw);
     uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem_raw + sizeof(TileSmem));
     const uint32_t n_kmers = 1u << (2 * ell);
-    for (uint32_t k = threadIdx.x; k < n_kmers; k += blockDim.x) s_hist[k] = 0;
+    // suffixes that end inside the prefix: (4^r - 1) / 3 + (their r bases) indexes the 4^r partitions of length r
+    uint32_t* s_short = s_hist + n_kmers;
+    const uint32_t n_short = (n_kmers - 1) / 3;
+    for (uint32_t k = threadIdx.x; k < n_kmers + n_short; k += blockDim.x) s_hist[k] = 0;
     R.n_words = (info->total_bases + 31) >> 5;
     const uint64_t N = info->n_suffixes;
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
     for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
         __syncthreads();   // previous tile done with sm (and s_hist zeroed on the first trip)
-        TileCtx c = load_tile(R, tile_first_read, t, n_tiles, N, sm);
+        TileCtx c = load_tile(R, info, tile_first_read, t, n_tiles, N, sm);
 #pragma unroll
         for (int k = 0; k < kListItems; ++k) {
             uint32_t s = k * kListThreads + threadIdx.x;
             bool valid = s < c.n_slots;
-            uint32_t kmer = 0, r = 0, code = 0xffffffffu;
             if (valid) {
+                uint32_t kmer = 0, r = 0;
                 Slot sl = decode_slot(c, sm, s);
                 uint32_t b = bucket_of(sl, ell, kmer, r);
-                if (r == ell) code = kmer;
-                else atomicAdd(hist + b, 1ull);
+                // consecutive suffixes rarely share an l-mer, so one shared-memory atomic per suffix beats warp
+                // aggregation here (match.any costs ~25 cycles per distinct value on sm_100a)
+                (void)b;
+                if (r == ell) atomicAdd(&s_hist[kmer], 1u);
+                else atomicAdd(&s_short[(((1u << (2 * r)) - 1) / 3) + (kmer >> (2 * (ell - r)))], 1u);
             }
-            // warp-aggregated update: one shared-memory atomic per distinct k-mer in the warp
-            uint32_t peers = __match_any_sync(0xffffffffu, code);
-            if (code != 0xffffffffu && (peers & lanemask_lt()) == 0) atomicAdd(&s_hist[code], (uint32_t)__popc(peers));
         }
     }
     __syncthreads();
     for (uint32_t k = threadIdx.x; k < n_kmers; k += blockDim.x) {
         uint32_t v = s_hist[k];
         if (v) atomicAdd(hist + (uint64_t)k * (ell + 1) + ell, (unsigned long long)v);
+    }
+    for (uint32_t r = 0; r < ell; ++r) {
+        const uint32_t first = ((1u << (2 * r)) - 1) / 3, count = 1u << (2 * r);
+        for (uint32_t k = threadIdx.x; k < count; k += blockDim.x) {
+            uint32_t v = s_short[first + k];
+            if (v) atomicAdd(hist + ((uint64_t)k << (2 * (ell - r))) * (ell + 1) + r, (unsigned long long)v);
+        }
     }
 }
 
@@ -191,7 +223,7 @@ __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const
     uint64_t t = blockIdx.x;
     if (t >= n_tiles) return;
     if (threadIdx.x == 0) s_total = 0;
-    TileCtx c = load_tile(R, tile_first_read, t, n_tiles, N, sm);
+    TileCtx c = load_tile(R, info, tile_first_read, t, n_tiles, N, sm);
     uint32_t mine = 0;
 #pragma unroll
     for (int k = 0; k < kListItems; ++k) {
@@ -218,83 +250,95 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
                                                                   const uint32_t* __restrict__ tile_first_read, uint32_t ell, uint32_t w,
                                                                   uint32_t bucket_lo, uint32_t bucket_hi,
                                                                   const uint64_t* __restrict__ tile_base, KeyT* __restrict__ keys,
-                                                                  IdT* __restrict__ ids) {
+                                                                  IdT* __restrict__ ids, uint32_t n_passes,
+                                                                  unsigned long long* __restrict__ digit_hist) {
     __shared__ TileSmem sm;
+    __shared__ uint32_t s_dh[8][kRadix];   // digit counts of every radix pass of the sort that follows (a6's upfront histogram)
     R.n_words = (info->total_bases + 31) >> 5;
     const uint64_t N = info->n_suffixes;
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
-    uint64_t t = blockIdx.x;
-    if (t >= n_tiles) return;
-    TileCtx c = load_tile(R, tile_first_read, t, n_tiles, N, sm);
     const uint32_t warp = threadIdx.x >> 5;
     constexpr int kWarps = kListThreads / 32;
-
     const uint32_t len_bits = key_len_bits(w);
-    KeyT key[kListItems];
-    IdT id[kListItems];
-    uint32_t rank[kListItems];
-    bool take[kListItems];
-#pragma unroll
-    for (int k = 0; k < kListItems; ++k) {
-        uint32_t s = k * kListThreads + threadIdx.x;
-        take[k] = false;
-        key[k] = 0;
-        id[k] = 0;
-        rank[k] = 0;
-        if (s < c.n_slots) {
-            Slot sl = decode_slot(c, sm, s);
-            key[k] = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
-            id[k] = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
-            if (ALL) {
-                take[k] = true;
-            } else {
-                uint32_t kmer, r;
-                uint32_t b = bucket_of(sl, ell, kmer, r);
-                take[k] = b >= bucket_lo && b <= bucket_hi;
-            }
-        }
-        if (!ALL) {
-            uint32_t m = __ballot_sync(0xffffffffu, take[k]);
-            rank[k] = __popc(m & lanemask_lt());
-            if (lane_id() == 0) sm.scan[k * kWarps + warp] = __popc(m);
-        }
-    }
-    if (ALL) {
+    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) (&s_dh[0][0])[i] = 0;
+
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        __syncthreads();   // previous tile done with sm
+        TileCtx c = load_tile(R, info, tile_first_read, t, n_tiles, N, sm);
+        KeyT key[kListItems];
+        IdT id[kListItems];
+        uint32_t rank[kListItems];
+        bool take[kListItems];
 #pragma unroll
         for (int k = 0; k < kListItems; ++k) {
             uint32_t s = k * kListThreads + threadIdx.x;
+            take[k] = false;
+            key[k] = 0;
+            id[k] = 0;
+            rank[k] = 0;
+            if (s < c.n_slots) {
+                Slot sl = decode_slot(c, sm, s);
+                key[k] = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
+                id[k] = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
+                if (ALL) {
+                    take[k] = true;
+                } else {
+                    uint32_t kmer, r;
+                    uint32_t b = bucket_of(sl, ell, kmer, r);
+                    take[k] = b >= bucket_lo && b <= bucket_hi;
+                }
+            }
             if (take[k]) {
-                keys[c.g0 + s] = key[k];
-                ids[c.g0 + s] = id[k];
+                for (uint32_t p = 0; p < n_passes; ++p) atomicAdd(&s_dh[p][(uint32_t)(key[k] >> (p * kRadixBits)) & (kRadix - 1)], 1u);
+            }
+            if (!ALL) {
+                uint32_t m = __ballot_sync(0xffffffffu, take[k]);
+                rank[k] = __popc(m & lanemask_lt());
+                if (lane_id() == 0) sm.scan[k * kWarps + warp] = __popc(m);
             }
         }
-        return;
-    }
-    __syncthreads();
-    // exclusive scan of the kListItems * kWarps row counts (slot order = item-major, then warp)
-    if (threadIdx.x < 32) {
-        uint32_t carry = 0;
-        for (int base = 0; base < kListItems * kWarps; base += 32) {
-            uint32_t idx = base + threadIdx.x;
-            uint32_t v = idx < kListItems * kWarps ? sm.scan[idx] : 0;
-            uint32_t incl = v;
-            for (int o = 1; o < 32; o <<= 1) {
-                uint32_t up = __shfl_up_sync(0xffffffffu, incl, o);
-                if ((int)threadIdx.x >= o) incl += up;
-            }
-            if (idx < kListItems * kWarps) sm.scan[idx] = carry + incl - v;
-            carry += __shfl_sync(0xffffffffu, incl, 31);
-        }
-    }
-    __syncthreads();
-    const uint64_t base = tile_base[t];
+        if (ALL) {
 #pragma unroll
-    for (int k = 0; k < kListItems; ++k) {
-        if (take[k]) {
-            uint64_t dst = base + sm.scan[k * kWarps + warp] + rank[k];
-            keys[dst] = key[k];
-            ids[dst] = id[k];
+            for (int k = 0; k < kListItems; ++k) {
+                uint32_t s = k * kListThreads + threadIdx.x;
+                if (take[k]) {
+                    keys[c.g0 + s] = key[k];
+                    ids[c.g0 + s] = id[k];
+                }
+            }
+            continue;
         }
+        __syncthreads();
+        // exclusive scan of the kListItems * kWarps row counts (slot order = item-major, then warp)
+        if (threadIdx.x < 32) {
+            uint32_t carry = 0;
+            for (int base = 0; base < kListItems * kWarps; base += 32) {
+                uint32_t idx = base + threadIdx.x;
+                uint32_t v = idx < kListItems * kWarps ? sm.scan[idx] : 0;
+                uint32_t incl = v;
+                for (int o = 1; o < 32; o <<= 1) {
+                    uint32_t up = __shfl_up_sync(0xffffffffu, incl, o);
+                    if ((int)threadIdx.x >= o) incl += up;
+                }
+                if (idx < kListItems * kWarps) sm.scan[idx] = carry + incl - v;
+                carry += __shfl_sync(0xffffffffu, incl, 31);
+            }
+        }
+        __syncthreads();
+        const uint64_t base = tile_base[t];
+#pragma unroll
+        for (int k = 0; k < kListItems; ++k) {
+            if (take[k]) {
+                uint64_t dst = base + sm.scan[k * kWarps + warp] + rank[k];
+                keys[dst] = key[k];
+                ids[dst] = id[k];
+            }
+        }
+    }
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) {
+        uint32_t v = (&s_dh[0][0])[i];
+        if (v) atomicAdd(digit_hist + i, (unsigned long long)v);
     }
 }
 
@@ -320,7 +364,7 @@ cudaError_t launch_tile_table(const uint64_t* offsets, uint64_t n_reads, const B
     return cudaGetLastError();
 }
 
-size_t bucket_hist_smem(uint32_t ell) { return sizeof(TileSmem) + (sizeof(uint32_t) << (2 * ell)); }
+size_t bucket_hist_smem(uint32_t ell) { return sizeof(TileSmem) + (sizeof(uint32_t) << (2 * ell)) + sizeof(uint32_t) * (((1u << (2 * ell)) - 1) / 3); }
 
 cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
                                uint64_t* hist, uint64_t max_tiles, int n_sms, cudaStream_t s) {
@@ -349,20 +393,22 @@ cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint3
 template <typename KeyT, typename IdT>
 cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
                               uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, KeyT* keys, IdT* ids,
-                              uint64_t n_tiles, cudaStream_t s) {
+                              uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, cudaStream_t s) {
     if (n_tiles == 0) return cudaSuccess;
+    uint64_t want = (uint64_t)n_sms * 6;
+    unsigned grid = (unsigned)(n_tiles < want ? n_tiles : want);
     if (tile_base == nullptr)
-        list_write_kernel<KeyT, IdT, true><<<(unsigned)n_tiles, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo,
-                                                                                     bucket_hi, nullptr, keys, ids);
+        list_write_kernel<KeyT, IdT, true><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, nullptr,
+                                                                         keys, ids, n_passes, (unsigned long long*)digit_hist);
     else
-        list_write_kernel<KeyT, IdT, false><<<(unsigned)n_tiles, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo,
-                                                                                      bucket_hi, tile_base, keys, ids);
+        list_write_kernel<KeyT, IdT, false><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
+                                                                          tile_base, keys, ids, n_passes, (unsigned long long*)digit_hist);
     return cudaGetLastError();
 }
 
 #define CX_LIST_INST(K, I)                                                                                                        \
     template cudaError_t launch_list_write<K, I>(const Reads&, const BuildInfo*, const uint32_t*, uint32_t, uint32_t, uint32_t,  \
-                                                 uint32_t, const uint64_t*, K*, I*, uint64_t, cudaStream_t);
+                                                 uint32_t, const uint64_t*, K*, I*, uint64_t, uint32_t, uint64_t*, int, cudaStream_t);
 CX_LIST_INST(uint32_t, uint32_t)
 CX_LIST_INST(uint32_t, uint64_t)
 CX_LIST_INST(uint64_t, uint32_t)
