@@ -52,6 +52,7 @@ def parse_args():
     ap.add_argument("--scale", type=float, default=1.0, help="debug only: scale the workload down")
     ap.add_argument("--impl", default="cx", choices=["cx", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--key-bases", type=int, default=0, help="first-round key window w (0 = the library's default)")
     return ap.parse_args()
 
 
@@ -199,7 +200,7 @@ def run_cx(args) -> None:
     d_off = h_off.to(dev)
     d_packed = torch.empty((total + 31) // 32 + 1, dtype=torch.int64, device=dev)
     d_out = torch.empty(N, dtype=torch.uint8, device=dev)
-    plan = cx.Plan(n_reads, total, max_read_len=coll.max_read_len, profile=1, device=dev)
+    plan = cx.Plan(n_reads, total, max_read_len=coll.max_read_len, profile=1, key_bases=args.key_bases or None, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
     stream = torch.cuda.current_stream()
 
@@ -301,7 +302,7 @@ def run_cx(args) -> None:
         "dtype": "u64", "data": "synthetic",
         "config": {"workload": WORKLOADS.get(args.config, str(args.config)) + (f" x scale {args.scale:g}" if args.scale != 1 else ""),
                    "n_reads": n_reads, "total_bases": total, "n_suffixes": N, "parallelism": "replicas only" if world > 1 else "1 gpu",
-                   "l2": "256 MiB L2-flush write between timed steps; working set >> L2", "prefix_len": 6, "key_bases": "auto (14 in a 32-bit key when the batch is under 2^28 suffixes, else 29 in a 64-bit key)",
+                   "l2": "256 MiB L2-flush write between timed steps; working set >> L2", "prefix_len": 6, "key_bases": "auto (14 bases in a 32-bit key up to 2^30 suffixes, else ceil(log4 N)+1 bases in a 64-bit key)",
                    "id_bytes": stats["id_bytes"], "n_batches": stats["n_batches"], "sort_passes": stats["sort_passes"],
                    "refine_rounds": stats["refine_rounds"], "refine_elements": stats["refine_elements"],
                    "small_group_elems": stats["small_group_elems"]},

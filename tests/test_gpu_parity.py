@@ -1,6 +1,7 @@
 """Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
 same seeded inputs.  Integer/byte work: the bar is bit-exact.  Needs a B200: `pytest -m gpu`."""
 import itertools
+import os
 
 import numpy as np
 import pytest
@@ -91,6 +92,31 @@ def test_config1_full():
 def test_config_shapes_scaled(idx, scale):
     c = gen.config(idx, scale)
     assert_parity(c)
+
+
+def _full_size_check(idx, prefixes, lf_sample):
+    """Full-size parity in the launch configuration bench.py times: the oracle's range-restricted slices
+    (every suffix that begins with a given prefix: a contiguous piece of B_R) must match
+    byte for byte, and the whole output must pass the size-independent checks (symbol counts, first-n
+    rule, LF-mapping inversion of a seeded sample of reads)."""
+    c = gen.config(idx)
+    got = gpu_bwt(c)
+    chk.check_all(got, c, lf_sample=lf_sample)
+    for pfx in prefixes:
+        off, want = oracle.bwt_with_prefix(c.ascii, c.offsets, pfx)
+        assert want.size > 0, pfx
+        assert np.array_equal(got[off:off + want.size], want), f"config {idx}: slice of prefix {pfx} differs"
+
+
+def test_config2_full_size_sampled_slices():
+    # configs[1], 1.01e8 suffixes: the bench workload
+    _full_size_check(1, ["CATG", "TTTTTTT", "AAAAA", "GGC"], lf_sample=20_000)
+
+
+@pytest.mark.skipif(os.environ.get("CX_TEST_LARGE", "0") != "1", reason="set CX_TEST_LARGE=1 (several minutes, ~40 GB host RAM)")
+def test_config3_full_size_sampled_slices():
+    # configs[2], 1.01e9 suffixes
+    _full_size_check(2, ["ACGTACG", "TTGACCA"], lf_sample=2_000)
 
 
 def test_eight_byte_ids():
