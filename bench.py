@@ -37,7 +37,7 @@ WORKLOADS = {
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture named here (None until one exists for this workload).
-NCU_TRAFFIC = {"file": None, "bytes_per_launch": None}
+NCU_TRAFFIC = {"file": "profiles/r01_ncu_full.md (onesweep_pass_kernel<u32,u32>, configs[1])", "bytes_per_launch": 1_890_000_000}
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 CPU_SAMPLE_SCALE = 0.1        # cpu_baseline leg: the workload's recipe at this scale (coverage preserved)
 REF_SAMPLE_SCALE = 0.05       # --impl reference: one step = the oracle on the recipe at this scale
@@ -312,7 +312,7 @@ def run_cx(args) -> None:
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {"kernel": "onesweep_pass_kernel (a6, one radix pass)", "bound": "hbm", "achieved": round(achieved, 1),
-                     "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4), "traffic": NCU_TRAFFIC["bytes_per_launch"],
+                     "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4), "traffic": NCU_TRAFFIC["bytes_per_launch"] if args.config == 1 and args.scale == 1.0 else None,
                      "traffic_from": NCU_TRAFFIC["file"], "peak_source": peak_src, "nominal_peak": 8000.0,
                      "alg_bytes_per_launch": int(bytes_per_launch), "us_per_launch": round(ms_per_launch * 1e3, 2),
                      "launches_per_step": dom["launches"] / args.steps},
