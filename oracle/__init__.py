@@ -48,6 +48,8 @@ def _load():
         lib.cx_oracle_bwt_with_prefix.argtypes = [u8p, u64p, ctypes.c_uint64, u8p, ctypes.c_uint64, u8p,
                                                   ctypes.c_uint64, u64p, u64p]
         lib.cx_oracle_bwt_with_prefix.restype = ctypes.c_int
+        lib.cx_oracle_bwt_of_listed.argtypes = [u8p, u64p, ctypes.c_uint64, u64p, ctypes.c_uint64, u8p]
+        lib.cx_oracle_bwt_of_listed.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -95,6 +97,20 @@ def bwt_with_prefix(ascii_: np.ndarray, offsets: np.ndarray, prefix: str):
         raise OracleError(rc)
     assert int(so.value) + int(sl.value) <= N
     return int(so.value), out[:int(sl.value)].copy()
+
+
+def bwt_of_listed(ascii_: np.ndarray, offsets: np.ndarray, listed: np.ndarray):
+    """Sort the listed suffixes ((k, 2) array of (read, pos)) with the definition's comparator and return their
+    preceding symbols in that order, plus the sorted list."""
+    text, off = _prep(ascii_, offsets)
+    n = int(off.shape[0] - 1) if off.shape[0] else 0
+    lst = np.ascontiguousarray(listed, dtype=np.uint64).reshape(-1, 2).copy()
+    out = np.empty(max(lst.shape[0], 1), dtype=np.uint8)
+    rc = _load().cx_oracle_bwt_of_listed(_ptr(text, ctypes.c_uint8), _ptr(off, ctypes.c_uint64), n,
+                                         _ptr(lst, ctypes.c_uint64), lst.shape[0], _ptr(out, ctypes.c_uint8))
+    if rc:
+        raise OracleError(rc)
+    return out[:lst.shape[0]], lst
 
 
 def bwt_of_strings(reads: list[str]) -> str:

@@ -190,3 +190,26 @@ int cx_oracle_bwt_with_prefix(const uint8_t *text, const uint64_t *offsets, uint
     free(L);
     return CX_ORACLE_OK;
 }
+
+/*
+ * The same steps 3-4 applied to a caller-supplied list of suffixes (read, pos) instead of all of
+ * them: sort the listed suffixes with the definition's comparator and read off their preceding
+ * symbols.  If the list is exactly the set of suffixes that begin with some string, the output is the
+ * corresponding contiguous piece of B_R.  Used by the full-size checks of configs[3..4],
+ * where the listing (a linear scan) is done outside and only the reads that own a listed suffix are
+ * handed over; the read indices must keep the collection's relative order (the tie-break).
+ * list: n_listed pairs (read, pos), overwritten with the sorted order.
+ */
+int cx_oracle_bwt_of_listed(const uint8_t *text, const uint64_t *offsets, uint64_t n_reads, uint64_t *list,
+                            uint64_t n_listed, uint8_t *out) {
+    int rc = validate(text, offsets, n_reads);
+    if (rc) return rc;
+    if (n_listed && (!list || !out)) return CX_ORACLE_ARG;
+    cx_ctx_t ctx = {text, offsets};
+    cx_suffix_t *L = (cx_suffix_t *)list; /* two uint64 per entry, same layout */
+    for (uint64_t k = 0; k < n_listed; ++k)
+        if (L[k].read >= n_reads || L[k].pos > offsets[L[k].read + 1] - offsets[L[k].read]) return CX_ORACLE_ARG;
+    if (n_listed) qsort_r(L, n_listed, sizeof(cx_suffix_t), compare_suffixes, &ctx);
+    for (uint64_t k = 0; k < n_listed; ++k) out[k] = preceding_symbol(&ctx, &L[k]);
+    return CX_ORACLE_OK;
+}

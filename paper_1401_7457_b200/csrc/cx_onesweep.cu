@@ -11,7 +11,6 @@
 // Algorithmic traffic per pass: 2 * (8 + sizeof(id)) bytes per pair; histogram kernel: 8 bytes per pair.
 #include "cx_internal.cuh"
 #include "cx_launch.h"
-#include <stdlib.h>
 
 namespace cx {
 namespace {
@@ -96,9 +95,6 @@ struct PassSmem {
     uint32_t tile;
 };
 
-// Lanes of the warp whose 8-bit digit equals mine.  Eight ballots: constant cost whatever the digit
-// distribution (match.any on sm_100a takes ~25 cycles per DISTINCT value in the warp, ~700 cycles for
-// random digits -- measured).
 // p &= (my bit B set) ? ballot : ~ballot, as LOP3.P, VOTE, SEL, LOP3 (nvcc's own code for the C++ form takes six)
 template <int B>
 __device__ __forceinline__ void ballot_step(uint32_t& p, uint32_t d) {
@@ -118,18 +114,14 @@ __device__ __forceinline__ void ballot_steps(uint32_t& p, uint32_t d) {
     }
 }
 
-template <int MODE>
+// Lanes of the warp whose 8-bit digit equals mine: eight ballot steps.
 __device__ __forceinline__ uint32_t digit_peers(uint32_t d) {
-    // MODE = number of low digit bits resolved by match.any (0, 2, 3, 4, or 22 = two 2-bit matches); the rest by ballots
     uint32_t p = kFull;
-    constexpr int kMatchBits = MODE == 22 ? 4 : MODE;
-    if (MODE == 22) p = __match_any_sync(kFull, d & 3u) & __match_any_sync(kFull, (d >> 2) & 3u);
-    else if (MODE > 0) p = __match_any_sync(kFull, d & ((1u << MODE) - 1));
-    ballot_steps<kMatchBits, kRadixBits>(p, d);
+    ballot_steps<0, kRadixBits>(p, d);
     return p;
 }
 
-template <typename KeyT, typename ValT, int THREADS, int ITEMS, int MIN_BLOCKS, int RANK_MODE>
+template <typename KeyT, typename ValT, int THREADS, int ITEMS, int MIN_BLOCKS>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
 onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ vals_in, KeyT* __restrict__ keys_out,
                      ValT* __restrict__ vals_out, uint64_t n, uint32_t shift, uint32_t digit_mask,
@@ -182,7 +174,7 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ 
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
         const uint32_t d = (uint32_t)(key[k] >> shift) & digit_mask;
-        const uint32_t peers = digit_peers<RANK_MODE>(d);
+        const uint32_t peers = digit_peers(d);
         const uint32_t below = __popc(peers & lt);
         uint32_t old = 0;
         if (below == 0) old = atomicAdd(&sm.warp_count[warp][d], (uint32_t)__popc(peers));   // lowest peer lane
@@ -306,17 +298,14 @@ cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, u
     constexpr int kTile = kSortThreads * ITEMS;
     using Smem = PassSmem<KeyT, ValT, kSortThreads, ITEMS>;
     constexpr int kMinBlocks = 4;
-    auto kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks, 0>;
-    {   // EXPERIMENT: rank mode from the environment
-        static int mode = getenv("CX_RANK_MODE") ? atoi(getenv("CX_RANK_MODE")) : 0;
-        if (mode == 2) kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks, 2>;
-        if (mode == 3) kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks, 3>;
-        if (mode == 4) kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks, 4>;
-        if (mode == 22) kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks, 22>;
-    }
+    auto kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks>;
+    static bool attr_set = false;
     cudaError_t e;
-    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
-    if (e != cudaSuccess) return e;
+    if (!attr_set) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
     const uint32_t n_passes = (end_bit - begin_bit + kRadixBits - 1) / kRadixBits;
     const uint64_t n_tiles = (n + kTile - 1) / kTile;
     if (n_tiles > ws.max_tiles || n_passes > 8 || n > 0xFFFF0000ull) return cudaErrorInvalidValue;

@@ -178,3 +178,30 @@ def test_generators_are_deterministic_and_acgt_only():
     assert lens.min() >= 50 and lens.max() <= 250
     c2 = gen.config(1, 0.001)
     assert len(set(c2.strings())) < c2.n_reads       # 100x coverage: exact duplicate reads exist
+
+
+def test_listed_form_equals_full_and_prefix_forms():
+    """cx_oracle_bwt_of_listed: listing every suffix gives B_R; listing those with a prefix gives the prefix slice;
+    dropping the reads that own no listed suffix (indices kept in order) changes nothing."""
+    c = gen.config(2, 0.0003)
+    off = c.offsets.astype(np.int64)
+    every = np.array([(i, p) for i in range(c.n_reads) for p in range(int(off[i + 1] - off[i]) + 1)], dtype=np.uint64)
+    got, order = oracle.bwt_of_listed(c.ascii, c.offsets, every[::-1])          # any input order
+    want, want_order = oracle.bwt(c.ascii, c.offsets, return_order=True)
+    assert np.array_equal(got, want) and np.array_equal(order, want_order)
+    text = c.ascii.tobytes()
+    for pfx in (b"AC", b"TTG", b"G"):
+        sel = np.array([(i, p) for i, p in every.tolist() if text[off[i] + p: min(off[i] + p + len(pfx), off[i + 1])] == pfx],
+                       dtype=np.uint64).reshape(-1, 2)
+        _, want_slice = oracle.bwt_with_prefix(c.ascii, c.offsets, pfx.decode())
+        got_slice, _ = oracle.bwt_of_listed(c.ascii, c.offsets, sel)
+        assert np.array_equal(got_slice, want_slice)
+        # sub-collection of the owning reads only
+        owners = np.unique(sel[:, 0]).astype(np.int64)
+        sub_off = np.zeros(owners.size + 1, dtype=np.uint64)
+        sub_off[1:] = np.cumsum(off[owners + 1] - off[owners])
+        sub_text = np.concatenate([c.ascii[off[i]:off[i + 1]] for i in owners]) if owners.size else np.zeros(0, np.uint8)
+        remap = sel.copy()
+        remap[:, 0] = np.searchsorted(owners, sel[:, 0].astype(np.int64))
+        got_sub, _ = oracle.bwt_of_listed(sub_text, sub_off, remap)
+        assert np.array_equal(got_sub, want_slice)
