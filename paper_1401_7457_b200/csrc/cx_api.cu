@@ -396,6 +396,8 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     const uint32_t w = sh.w;
     const uint32_t key_bits = 2 * w + key_len_bits(w);
     KeyT* d_keys1[2] = {reinterpret_cast<KeyT*>(d_keys[0]), reinterpret_cast<KeyT*>(d_keys[1])};   // first-round keys
+    // 32-bit key and 32-bit id: one 64-bit word per suffix (key << 32 | id), sorted keys-only over its upper half
+    const bool pack_kv = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
     p->stats.sort_passes = (key_bits + kRadixBits - 1) / kRadixBits;
 
     for (size_t bi = 0; bi < p->batches.size(); ++bi) {
@@ -407,7 +409,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         if (single) {
             ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (sizeof(KeyT) + sizeof(IdT)), s);
             CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, nullptr, d_keys1[0],
-                                                  d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, s)));
+                                                  d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, s)));
         } else {
             {
                 ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + n_tiles * 8, s);
@@ -420,13 +422,16 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             prof->launches[CX_K_LIST] += 2;   // the scan is three kernels
             ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (sizeof(KeyT) + sizeof(IdT)), s);
             CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, d_tile_count,
-                                                  d_keys1[0], d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, s)));
+                                                  d_keys1[0], d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, s)));
         }
         // ---- step 3(c)ii: sort (first w symbols) ------------------------------------------------
         int in_alt = 0;
-        CX_CUDA((sort_pairs<KeyT, IdT>(d_keys1[0], d_ids[0], d_keys1[1], d_ids[1], nb, 0, key_bits, p->sort, &in_alt, prof, s, true)));
+        if (pack_kv)
+            CX_CUDA((sort_pairs<uint64_t, NoVal>(d_keys[0], nullptr, d_keys[1], nullptr, nb, 32, 32 + key_bits, p->sort, &in_alt, prof, s, true)));
+        else
+            CX_CUDA((sort_pairs<KeyT, IdT>(d_keys1[0], d_ids[0], d_keys1[1], d_ids[1], nb, 0, key_bits, p->sort, &in_alt, prof, s, true)));
         const int cur = in_alt;
-        IdT* ids = d_ids[cur];
+        IdT* ids = pack_kv ? d_ids[0] : d_ids[cur];
         // a9: with pinned-host output the batch is emitted into a staging buffer of the workspace
         const int st = (int)(bi & 1);
         uint8_t* dst = sh.host_out ? ws + L.stage[st] : out + B.out_offset;
@@ -438,7 +443,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         CX_CUDA(cudaMemsetAsync(d_heads[0], 0, (n_words + 1) * 4, s));
         {
             ScopedLaunch sl(prof, CX_K_FINISH, nb * (sizeof(KeyT) + sizeof(IdT) + 1) + nb / 8, s);
-            CX_CUDA((launch_finish_first<KeyT, IdT>(R, d_keys1[cur], w, d_heads[0], ids, nb, sh.cap, dst, d_done, s)));
+            CX_CUDA((launch_finish_first<KeyT, IdT>(R, d_keys1[cur], w, d_heads[0], ids, nb, sh.cap, dst, d_done, pack_kv, s)));
         }
         // ---- what is still tied goes through global rounds: re-key, sort, write back ------------------
         uint32_t depth = w, rounds = 0;
@@ -463,7 +468,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             uint32_t w_r = (59 - gbits) / 2;
             if (w_r > 29) w_r = 29;
             uint64_t* kc = d_keys[1 - cur];
-            IdT* ic = d_ids[1 - cur];
+            IdT* ic = pack_kv ? d_ids[1] : d_ids[1 - cur];
             {
                 ScopedLaunch sl(prof, CX_K_REFINE_KEY, nb / 8 + n_act * (2 * sizeof(IdT) + 8 + 8 + 4), s);
                 CX_CUDA(launch_refine_rekey<IdT>(R, d_heads[hc], d_word_counts, ids, nb, depth, w_r, kc, ic, d_pos, s));

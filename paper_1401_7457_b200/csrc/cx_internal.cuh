@@ -19,11 +19,13 @@ constexpr int kRadix = 1 << kRadixBits;
 
 // onesweep tile shapes (threads x items); one per value width so that registers/smem stay balanced
 constexpr int kSortThreads = 256;
+struct NoVal {};   // value type of a keys-only sort (the 32-bit id rides in the low half of a 64-bit key word)
 template <typename KeyT, typename ValT> struct SortShape {
     // pairs staged per tile: 8-byte pairs 8192 (64 KB), 12-byte pairs 6144 (72 KB), 16-byte pairs 5120 (80 KB); 2 blocks per SM
-    static constexpr int items = sizeof(KeyT) + sizeof(ValT) >= 16 ? 10 : sizeof(KeyT) + sizeof(ValT) >= 12 ? 12 : 16;
+    static constexpr int pair_bytes = sizeof(KeyT) + (sizeof(ValT) >= 4 ? sizeof(ValT) : 0);
+    static constexpr int items = pair_bytes >= 16 ? 10 : pair_bytes >= 12 ? 12 : 16;
 };
-constexpr int kSortTileMin = kSortThreads * 10;   // smallest tile: sizes the tile-state array
+constexpr int kSortTileMin = 2560;   // smallest tile: sizes the tile-state array
 
 // tile-state word of the decoupled look-back: [epoch:8][flag:2][count:54]
 constexpr uint64_t kStatusValueMask = (1ull << 54) - 1;
@@ -128,7 +130,7 @@ cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint3
 template <typename KeyT, typename IdT>
 cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
                               uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, KeyT* keys, IdT* ids,
-                              uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, cudaStream_t s);
+                              uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, bool packed, cudaStream_t s);
 
 // cx_onesweep.cu
 struct SortWorkspace {
@@ -162,9 +164,11 @@ template <typename IdT>
 cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, const IdT* ids_c, const uint32_t* pos_c, uint64_t n_c,
                                     uint32_t w, IdT* ids, uint32_t* heads, uint8_t* out, cudaStream_t s);
 // fused head flags + in-block refinement + emit over the freshly sorted first-round keys; heads_out must be zero-filled
+// packed: keys1 holds 64-bit words (32-bit key << 32 | 32-bit id); `ids` is then OUTPUT: the ids of the positions left to
+// the global path are written there (nothing else will need the others).
 template <typename KeyT, typename IdT>
-cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t* heads_out, const IdT* ids, uint64_t n,
-                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, cudaStream_t s);
+cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t* heads_out, IdT* ids, uint64_t n,
+                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, bool packed, cudaStream_t s);
 // in-block refinement + emit of the groups a global round has split to at most group_cap members; heads_out = copy of heads_in
 template <typename IdT>
 cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32_t* heads_out, const IdT* ids, uint64_t n, uint32_t depth,

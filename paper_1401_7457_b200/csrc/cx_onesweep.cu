@@ -11,12 +11,13 @@
 // Algorithmic traffic per pass: 2 * (8 + sizeof(id)) bytes per pair; histogram kernel: 8 bytes per pair.
 #include "cx_internal.cuh"
 #include "cx_launch.h"
+#include <stdlib.h>
 
 namespace cx {
 namespace {
 
 constexpr uint32_t kFull = 0xffffffffu;
-constexpr int kLookWindow = 8;   // tile states fetched per look-back round trip
+constexpr int kLookWindow = 4;   // tile states fetched per look-back round trip
 
 __device__ __forceinline__ uint64_t pack_status(uint32_t epoch, uint32_t flag, uint64_t value) {
     return ((uint64_t)epoch << 56) | ((uint64_t)flag << 54) | value;
@@ -87,8 +88,9 @@ template <typename KeyT, typename ValT, int THREADS, int ITEMS>
 struct PassSmem {
     static constexpr int kTile = THREADS * ITEMS;
     static constexpr int kWarps = THREADS / 32;
+    static constexpr bool kHasVals = sizeof(ValT) >= 4;
     KeyT keys[kTile];
-    ValT vals[kTile];
+    ValT vals[kHasVals ? kTile : 1];
     uint32_t warp_count[kWarps][kRadix];  // per-warp digit counts, then the staged slot of the warp's first pair of that digit
     uint32_t gofs[kRadix];                // output index of staged slot e with digit d = gofs[d] + e (mod 2^32; batches are < 2^32)
     uint32_t warp_total[kRadix / 32];
@@ -130,6 +132,7 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ 
     using Smem = PassSmem<KeyT, ValT, THREADS, ITEMS>;
     constexpr int kTile = Smem::kTile;
     constexpr int kWarps = Smem::kWarps;
+    constexpr bool kHasVals = Smem::kHasVals;
     static_assert(THREADS >= kRadix && THREADS % 32 == 0, "one thread per digit is required");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
@@ -158,30 +161,24 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ 
         if (full) {
 #pragma unroll
             for (int k = 0; k < ITEMS; ++k) key[k] = __ldcs(kp + k * 32);
+            if constexpr (kHasVals) {
 #pragma unroll
-            for (int k = 0; k < ITEMS; ++k) val[k] = __ldcs(vp + k * 32);
+                for (int k = 0; k < ITEMS; ++k) val[k] = __ldcs(vp + k * 32);
+            }
         } else {
 #pragma unroll
             for (int k = 0; k < ITEMS; ++k) key[k] = warp_base + k * 32 + lane < tile_n ? __ldcs(kp + k * 32) : (KeyT)~(KeyT)0;
+            if constexpr (kHasVals) {
 #pragma unroll
-            for (int k = 0; k < ITEMS; ++k) val[k] = warp_base + k * 32 + lane < tile_n ? __ldcs(vp + k * 32) : (ValT)0;
+                for (int k = 0; k < ITEMS; ++k) val[k] = warp_base + k * 32 + lane < tile_n ? __ldcs(vp + k * 32) : ValT{};
+            }
         }
     }
 
-    // rank inside the warp, row by row (keeps element order, hence stability: PAPER.md:99)
-    uint32_t rank[ITEMS];
-    const uint32_t lt = lanemask_lt();
+    // per-(warp, digit) counts first ("early counts"): the tile's digit totals can then be published before the
+    // ranking work, so that by the time a successor looks back they are visible and it does not spin
 #pragma unroll
-    for (int k = 0; k < ITEMS; ++k) {
-        const uint32_t d = (uint32_t)(key[k] >> shift) & digit_mask;
-        const uint32_t peers = digit_peers(d);
-        const uint32_t below = __popc(peers & lt);
-        uint32_t old = 0;
-        if (below == 0) old = atomicAdd(&sm.warp_count[warp][d], (uint32_t)__popc(peers));   // lowest peer lane
-        old = __shfl_sync(kFull, old, __ffs(peers) - 1);
-        rank[k] = old + below;
-        __syncwarp();
-    }
+    for (int k = 0; k < ITEMS; ++k) atomicAdd(&sm.warp_count[warp][(uint32_t)(key[k] >> shift) & digit_mask], 1u);
     __syncthreads();
 
     // per digit: tile count, tile-state publication, staged slot of every (warp, digit)
@@ -215,13 +212,21 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ 
     }
     __syncthreads();
 
-    // stage pairs in digit order (needs only tile-local offsets; overlaps the predecessors' publications)
+    // rank inside the warp, row by row (keeps element order, hence stability: PAPER.md:99), and stage each pair
+    // at once: the lowest lane of every group of equal digits advances the (warp, digit) slot counter
+    const uint32_t lt = lanemask_lt();
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {
         const uint32_t d = (uint32_t)(key[k] >> shift) & digit_mask;
-        const uint32_t slot = sm.warp_count[warp][d] + rank[k];
+        const uint32_t peers = digit_peers(d);
+        const uint32_t below = __popc(peers & lt);
+        uint32_t old = 0;
+        if (below == 0) old = atomicAdd(&sm.warp_count[warp][d], (uint32_t)__popc(peers));
+        old = __shfl_sync(kFull, old, __ffs(peers) - 1);
+        const uint32_t slot = old + below;
         sm.keys[slot] = key[k];
-        sm.vals[slot] = val[k];
+        if constexpr (kHasVals) sm.vals[slot] = val[k];
+        __syncwarp();
     }
 
     // decoupled look-back, kLookWindow predecessors per round trip
@@ -262,7 +267,7 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ 
             const KeyT kk = sm.keys[e];
             const uint32_t dst = sm.gofs[(uint32_t)(kk >> shift) & digit_mask] + e;
             keys_out[dst] = kk;
-            vals_out[dst] = sm.vals[e];
+            if constexpr (kHasVals) vals_out[dst] = sm.vals[e];
         }
     }
 }
@@ -289,15 +294,13 @@ void sort_workspace_carve(SortWorkspace& ws, void* mem, uint64_t n) {
     ws.ticket_base = 0;
 }
 
-template <typename KeyT, typename ValT>
-cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
-                       uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s, bool hist_ready) {
-    *result_in_alt = 0;
-    if (n <= 1 || end_bit <= begin_bit) return cudaSuccess;
-    constexpr int ITEMS = SortShape<KeyT, ValT>::items;
+template <typename KeyT, typename ValT, int THREADS, int ITEMS, int kMinBlocks>
+cudaError_t sort_pairs_shape(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
+                             uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s, bool hist_ready) {
+    constexpr int kSortThreads = THREADS;
     constexpr int kTile = kSortThreads * ITEMS;
+    static_assert(kTile >= kSortTileMin, "the tile-state array is sized for tiles of at least kSortTileMin pairs");
     using Smem = PassSmem<KeyT, ValT, kSortThreads, ITEMS>;
-    constexpr int kMinBlocks = 4;
     auto kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks>;
     static bool attr_set = false;
     cudaError_t e;
@@ -340,7 +343,7 @@ cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, u
         }
         ws.epoch += 1;
         {
-            ScopedLaunch sl(prof, CX_K_SORT_PASS, n * 2 * (sizeof(KeyT) + sizeof(ValT)), s);
+            ScopedLaunch sl(prof, CX_K_SORT_PASS, n * 2 * SortShape<KeyT, ValT>::pair_bytes, s);
             kernel<<<(unsigned)n_tiles, kSortThreads, sizeof(Smem), s>>>(kin, vin, kout, vout, n, lo, (1u << bits) - 1,
                                                                         ws.hist + (uint64_t)p * kRadix, ws.status, ws.ticket,
                                                                         ws.ticket_base, ws.epoch);
@@ -355,11 +358,30 @@ cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, u
     return cudaSuccess;
 }
 
+template <typename KeyT, typename ValT>
+cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
+                       uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s, bool hist_ready) {
+    *result_in_alt = 0;
+    if (n <= 1 || end_bit <= begin_bit) return cudaSuccess;
+    constexpr int ITEMS = SortShape<KeyT, ValT>::items;
+    if constexpr (sizeof(ValT) < 4) {   // EXPERIMENT: tile shape of the keys-only sort from the environment
+        static int shape = getenv("CX_SORT_SHAPE") ? atoi(getenv("CX_SORT_SHAPE")) : 0;
+        if (shape == 1) return sort_pairs_shape<KeyT, ValT, 512, 16, 2>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready);
+        if (shape == 2) return sort_pairs_shape<KeyT, ValT, 256, 32, 2>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready);
+        if (shape == 3) return sort_pairs_shape<KeyT, ValT, 512, 8, 3>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready);
+        if (shape == 4) return sort_pairs_shape<KeyT, ValT, 1024, 8, 2>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready);
+        if (shape == 5) return sort_pairs_shape<KeyT, ValT, 1024, 16, 1>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready);
+        if (shape == 6) return sort_pairs_shape<KeyT, ValT, 384, 16, 2>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready);
+    }
+    return sort_pairs_shape<KeyT, ValT, kSortThreads, ITEMS, 4>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready);
+}
+
 #define CX_SORT_INST(K, V)                                                                                               \
     template cudaError_t sort_pairs<K, V>(K*, V*, K*, V*, uint64_t, uint32_t, uint32_t, SortWorkspace&, int*, Launch*, cudaStream_t, bool);
 CX_SORT_INST(uint32_t, uint32_t)
 CX_SORT_INST(uint32_t, uint64_t)
 CX_SORT_INST(uint64_t, uint32_t)
 CX_SORT_INST(uint64_t, uint64_t)
+CX_SORT_INST(uint64_t, NoVal)
 
 }  // namespace cx

@@ -298,10 +298,10 @@ __device__ __forceinline__ void count_if_less(uint32_t& acc, const uint4& a, con
         : "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w), "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w));
 }
 
-template <typename KeyT, typename IdT, bool FIRST>
+template <typename KeyT, typename IdT, bool FIRST, bool PACKED>
 __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, const KeyT* __restrict__ keys1, uint32_t w1, uint32_t len_mask,
                                                                     const uint32_t* __restrict__ heads_in, uint32_t* __restrict__ heads,
-                                                                    const IdT* __restrict__ ids, uint64_t n,
+                                                                    IdT* __restrict__ ids, uint64_t n,
                                                                     uint32_t depth0, uint32_t cap, uint8_t* __restrict__ out,
                                                                     unsigned long long* elems_done) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -319,9 +319,17 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
             const uint64_t j = base + e;
             bool head = true;   // positions past n count as heads
             if (j < n) {
-                const KeyT kc = __ldcs(keys1 + j);
-                head = j == 0 || kc != __ldg(keys1 + j - 1) || ((uint32_t)kc & len_mask) < w1;
-                sm.id_a[e] = __ldcs(ids + j);
+                if constexpr (PACKED) {
+                    const uint64_t* pairs = reinterpret_cast<const uint64_t*>(keys1);
+                    const uint64_t pc = __ldcs(pairs + j);
+                    const uint32_t kc = (uint32_t)(pc >> 32);
+                    head = j == 0 || kc != (uint32_t)(__ldg(pairs + j - 1) >> 32) || (kc & len_mask) < w1;
+                    sm.id_a[e] = (IdT)(uint32_t)pc;
+                } else {
+                    const KeyT kc = __ldcs(keys1 + j);
+                    head = j == 0 || kc != __ldg(keys1 + j - 1) || ((uint32_t)kc & len_mask) < w1;
+                    sm.id_a[e] = __ldcs(ids + j);
+                }
             }
             const uint32_t word = __ballot_sync(kFull, head);
             if ((tid & 31) == 0) sm.hw[e >> 5] = word;
@@ -371,6 +379,8 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
         sm.gs[e] = s;
         sm.ge[e] = t;
         sm.mine[e] = mine;
+        // packed input carries the ids inside the key words: hand those of the suffixes left to the global path over
+        if (PACKED && FIRST && !mine && e < kLocalTile && base + e < n) ids[base + e] = sm.id_a[e];
     }
     __syncthreads();
 
@@ -504,16 +514,14 @@ cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, cons
 }
 
 template <typename KeyT, typename IdT>
-cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t* heads_out, const IdT* ids, uint64_t n,
-                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, cudaStream_t s) {
+cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t* heads_out, IdT* ids, uint64_t n,
+                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, bool packed, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
-    auto kernel = finish_tile_kernel<KeyT, IdT, true>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem<IdT>));
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
+    if (packed && !kCanPack) return cudaErrorInvalidValue;
+    auto kernel = packed ? finish_tile_kernel<KeyT, IdT, true, kCanPack> : finish_tile_kernel<KeyT, IdT, true, false>;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem<IdT>));
+    if (e != cudaSuccess) return e;
     if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
     uint64_t blocks = (n + kLocalTile - 1) / kLocalTile;
     kernel<<<(unsigned)blocks, kLocalThreads, sizeof(LocalSmem<IdT>), s>>>(R, keys1, w1, (1u << key_len_bits(w1)) - 1, nullptr, heads_out, ids, n,
@@ -525,7 +533,7 @@ template <typename IdT>
 cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32_t* heads_out, const IdT* ids, uint64_t n, uint32_t depth,
                                 uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
-    auto kernel = finish_tile_kernel<uint64_t, IdT, false>;
+    auto kernel = finish_tile_kernel<uint64_t, IdT, false, false>;
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem<IdT>));
@@ -534,7 +542,7 @@ cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32
     }
     if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
     uint64_t blocks = (n + kLocalTile - 1) / kLocalTile;
-    kernel<<<(unsigned)blocks, kLocalThreads, sizeof(LocalSmem<IdT>), s>>>(R, nullptr, 0, 0, heads_in, heads_out, ids, n, depth, group_cap, out,
+    kernel<<<(unsigned)blocks, kLocalThreads, sizeof(LocalSmem<IdT>), s>>>(R, nullptr, 0, 0, heads_in, heads_out, const_cast<IdT*>(ids), n, depth, group_cap, out,
                                                                           elems_done);
     return cudaGetLastError();
 }
@@ -544,10 +552,10 @@ cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32
                                                   uint32_t, uint64_t*, IdT*, uint32_t*, cudaStream_t);                               \
     template cudaError_t launch_refine_writeback<IdT>(const Reads&, const uint64_t*, const IdT*, const uint32_t*, uint64_t,         \
                                                       uint32_t, IdT*, uint32_t*, uint8_t*, cudaStream_t);                            \
-    template cudaError_t launch_finish_first<uint32_t, IdT>(const Reads&, const uint32_t*, uint32_t, uint32_t*, const IdT*,         \
-                                                            uint64_t, uint32_t, uint8_t*, unsigned long long*, cudaStream_t);        \
-    template cudaError_t launch_finish_first<uint64_t, IdT>(const Reads&, const uint64_t*, uint32_t, uint32_t*, const IdT*,         \
-                                                            uint64_t, uint32_t, uint8_t*, unsigned long long*, cudaStream_t);        \
+    template cudaError_t launch_finish_first<uint32_t, IdT>(const Reads&, const uint32_t*, uint32_t, uint32_t*, IdT*, uint64_t,     \
+                                                            uint32_t, uint8_t*, unsigned long long*, bool, cudaStream_t);            \
+    template cudaError_t launch_finish_first<uint64_t, IdT>(const Reads&, const uint64_t*, uint32_t, uint32_t*, IdT*, uint64_t,     \
+                                                            uint32_t, uint8_t*, unsigned long long*, bool, cudaStream_t);            \
     template cudaError_t launch_finish_later<IdT>(const Reads&, const uint32_t*, uint32_t*, const IdT*, uint64_t, uint32_t,         \
                                                   uint32_t, uint8_t*, unsigned long long*, cudaStream_t);
 CX_INSTANTIATE(uint32_t)

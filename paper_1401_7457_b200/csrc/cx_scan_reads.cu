@@ -245,7 +245,9 @@ __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const
 // a4 (write half) + a5: ids of the batch in (read, pos) order, each with its first key.
 // The read is in shared memory already, so the round-1 key costs no gather.
 // ---------------------------------------------------------------------------------------------
-template <typename KeyT, typename IdT, bool ALL>
+// PACKED (32-bit key and id only): one 64-bit word (key << 32 | id) per suffix goes to `keys`, nothing to `ids`;
+// the sort is then keys-only over bits [32, 64) and the id travels with its key for free.
+template <typename KeyT, typename IdT, bool ALL, bool PACKED>
 __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const BuildInfo* __restrict__ info,
                                                                   const uint32_t* __restrict__ tile_first_read, uint32_t ell, uint32_t w,
                                                                   uint32_t bucket_lo, uint32_t bucket_hi,
@@ -302,8 +304,12 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
             for (int k = 0; k < kListItems; ++k) {
                 uint32_t s = k * kListThreads + threadIdx.x;
                 if (take[k]) {
-                    keys[c.g0 + s] = key[k];
-                    ids[c.g0 + s] = id[k];
+                    if constexpr (PACKED) {
+                        reinterpret_cast<uint64_t*>(keys)[c.g0 + s] = ((uint64_t)key[k] << 32) | (uint64_t)id[k];
+                    } else {
+                        keys[c.g0 + s] = key[k];
+                        ids[c.g0 + s] = id[k];
+                    }
                 }
             }
             continue;
@@ -330,8 +336,12 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
         for (int k = 0; k < kListItems; ++k) {
             if (take[k]) {
                 uint64_t dst = base + sm.scan[k * kWarps + warp] + rank[k];
-                keys[dst] = key[k];
-                ids[dst] = id[k];
+                if constexpr (PACKED) {
+                    reinterpret_cast<uint64_t*>(keys)[dst] = ((uint64_t)key[k] << 32) | (uint64_t)id[k];
+                } else {
+                    keys[dst] = key[k];
+                    ids[dst] = id[k];
+                }
             }
         }
     }
@@ -393,22 +403,34 @@ cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint3
 template <typename KeyT, typename IdT>
 cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
                               uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, KeyT* keys, IdT* ids,
-                              uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, cudaStream_t s) {
+                              uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, bool packed, cudaStream_t s) {
     if (n_tiles == 0) return cudaSuccess;
     uint64_t want = (uint64_t)n_sms * 6;
     unsigned grid = (unsigned)(n_tiles < want ? n_tiles : want);
-    if (tile_base == nullptr)
-        list_write_kernel<KeyT, IdT, true><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, nullptr,
-                                                                         keys, ids, n_passes, (unsigned long long*)digit_hist);
-    else
-        list_write_kernel<KeyT, IdT, false><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
-                                                                          tile_base, keys, ids, n_passes, (unsigned long long*)digit_hist);
+    unsigned long long* dh = (unsigned long long*)digit_hist;
+    constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
+    if (packed && !kCanPack) return cudaErrorInvalidValue;
+    if (tile_base == nullptr) {
+        if (packed)
+            list_write_kernel<KeyT, IdT, true, kCanPack><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
+                                                                                       nullptr, keys, ids, n_passes, dh);
+        else
+            list_write_kernel<KeyT, IdT, true, false><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
+                                                                                    nullptr, keys, ids, n_passes, dh);
+    } else {
+        if (packed)
+            list_write_kernel<KeyT, IdT, false, kCanPack><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
+                                                                                        tile_base, keys, ids, n_passes, dh);
+        else
+            list_write_kernel<KeyT, IdT, false, false><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
+                                                                                     tile_base, keys, ids, n_passes, dh);
+    }
     return cudaGetLastError();
 }
 
 #define CX_LIST_INST(K, I)                                                                                                        \
     template cudaError_t launch_list_write<K, I>(const Reads&, const BuildInfo*, const uint32_t*, uint32_t, uint32_t, uint32_t,  \
-                                                 uint32_t, const uint64_t*, K*, I*, uint64_t, uint32_t, uint64_t*, int, cudaStream_t);
+                                                 uint32_t, const uint64_t*, K*, I*, uint64_t, uint32_t, uint64_t*, int, bool, cudaStream_t);
 CX_LIST_INST(uint32_t, uint32_t)
 CX_LIST_INST(uint32_t, uint64_t)
 CX_LIST_INST(uint64_t, uint32_t)
