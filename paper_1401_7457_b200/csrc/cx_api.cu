@@ -358,7 +358,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     // ---- Fig. 2 step 1: scan all suffixes, partition sizes ------------------------------------
     {
         ScopedLaunch sl(prof, CX_K_PREP, (n_reads + 1) * 8, s);
-        CX_CUDA(launch_prep(offsets, n_reads, d_info, s));
+        CX_CUDA(launch_prep(offsets, n_reads, sh.max_bases, d_info, s));
     }
     {
         ScopedLaunch sl(prof, CX_K_PREP, sh.max_tiles * 4, s);
@@ -366,7 +366,21 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     }
     CX_CUDA(cudaMemsetAsync(d_hist, 0, sh.n_buckets * 8, s));
     CX_CUDA(cudaMemsetAsync(d_scalars, 0, 64, s));
-    {
+    // A plan whose largest legal input fits one batch needs no partition sizes to list its suffixes: the listing
+    // scan then counts them on the way (one read of the collection instead of two).
+    const bool fused_scan = sh.max_suffixes <= p->m1;
+    const uint32_t w = sh.w;
+    const uint32_t key_bits = 2 * w + key_len_bits(w);
+    const uint32_t n_passes = (key_bits + kRadixBits - 1) / kRadixBits;
+    KeyT* d_keys1[2] = {reinterpret_cast<KeyT*>(d_keys[0]), reinterpret_cast<KeyT*>(d_keys[1])};   // first-round keys
+    // 32-bit key and 32-bit id: one 64-bit word per suffix (key << 32 | id), sorted keys-only over its upper half
+    const bool pack_kv = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
+    if (fused_scan) {
+        CX_CUDA(cudaMemsetAsync(p->sort.hist, 0, (size_t)n_passes * kRadix * sizeof(uint64_t), s));
+        ScopedLaunch sl(prof, CX_K_LIST, 0, s);
+        CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, 0, 0, nullptr, d_keys1[0], d_ids[0], sh.max_tiles, n_passes,
+                                              p->sort.hist, p->n_sms, pack_kv, d_hist, p->m1, s)));
+    } else {
         ScopedLaunch sl(prof, CX_K_HIST, 0, s);
         CX_CUDA(launch_bucket_hist(R, d_info, d_tile_first, sh.ell, d_hist, sh.max_tiles, p->n_sms, s));
     }
@@ -376,7 +390,8 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     const BuildInfo info = *p->h_info;
     if (info.bad_offsets || info.total_bases > sh.max_bases || (info.max_len >> sh.pos_bits) != 0) return CX_ERR_ARG;
     const uint64_t N = info.n_suffixes;
-    prof->bytes[CX_K_HIST] += info.total_bases / 4 + (n_reads + 1) * 8;
+    if (fused_scan) prof->bytes[CX_K_LIST] += info.total_bases / 4 + (n_reads + 1) * 8 + N * (sizeof(KeyT) + sizeof(IdT));
+    else prof->bytes[CX_K_HIST] += info.total_bases / 4 + (n_reads + 1) * 8;
     R.n_words = (info.total_bases + 31) >> 5;
     R.uniform = info.nonuniform ? 0u : 1u;
     R.uniform_len = info.first_len;
@@ -393,23 +408,20 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     p->stats.n_batches = (uint32_t)p->batches.size();
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
     const bool single = p->batches.size() == 1;
-    const uint32_t w = sh.w;
-    const uint32_t key_bits = 2 * w + key_len_bits(w);
-    KeyT* d_keys1[2] = {reinterpret_cast<KeyT*>(d_keys[0]), reinterpret_cast<KeyT*>(d_keys[1])};   // first-round keys
-    // 32-bit key and 32-bit id: one 64-bit word per suffix (key << 32 | id), sorted keys-only over its upper half
-    const bool pack_kv = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
+    if (fused_scan && !single) return CX_ERR_CUDA;   // cannot happen: N <= max_suffixes <= m1
     p->stats.sort_passes = (key_bits + kRadixBits - 1) / kRadixBits;
 
     for (size_t bi = 0; bi < p->batches.size(); ++bi) {
         const Batch& B = p->batches[bi];
         const uint64_t nb = B.count;
         // ---- step 3(a) + 3(c)i: list the batch's suffixes with their first keys ----------------
-        const uint32_t n_passes = (key_bits + kRadixBits - 1) / kRadixBits;
-        CX_CUDA(cudaMemsetAsync(p->sort.hist, 0, (size_t)n_passes * kRadix * sizeof(uint64_t), s));
-        if (single) {
+        if (!fused_scan) CX_CUDA(cudaMemsetAsync(p->sort.hist, 0, (size_t)n_passes * kRadix * sizeof(uint64_t), s));
+        if (fused_scan) {
+            // listed before the partition sizes were read back
+        } else if (single) {
             ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (sizeof(KeyT) + sizeof(IdT)), s);
             CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, nullptr, d_keys1[0],
-                                                  d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, s)));
+                                                  d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, nullptr, ~0ull, s)));
         } else {
             {
                 ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + n_tiles * 8, s);
@@ -422,7 +434,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             prof->launches[CX_K_LIST] += 2;   // the scan is three kernels
             ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (sizeof(KeyT) + sizeof(IdT)), s);
             CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, d_tile_count,
-                                                  d_keys1[0], d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, s)));
+                                                  d_keys1[0], d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, nullptr, ~0ull, s)));
         }
         // ---- step 3(c)ii: sort (first w symbols) ------------------------------------------------
         int in_alt = 0;

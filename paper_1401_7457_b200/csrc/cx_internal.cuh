@@ -42,7 +42,7 @@ struct BuildInfo {
     uint64_t n_suffixes;
     uint64_t max_len;
     uint64_t first_len;
-    uint32_t bad_offsets;   // offsets[0] != 0 or a decreasing pair
+    uint32_t bad_offsets;   // bit 0: offsets[0] != 0 or a decreasing pair; bit 1: more bases than the plan allows
     uint32_t nonuniform;    // some read differs in length from read 0
 };
 
@@ -116,7 +116,7 @@ cudaError_t launch_pack(const uint8_t* ascii, uint64_t total_bases, uint64_t* pa
 uint32_t* pack_fallback_status();
 
 // cx_scan_reads.cu
-cudaError_t launch_prep(const uint64_t* offsets, uint64_t n_reads, BuildInfo* info, cudaStream_t s);
+cudaError_t launch_prep(const uint64_t* offsets, uint64_t n_reads, uint64_t max_bases, BuildInfo* info, cudaStream_t s);
 cudaError_t launch_tile_table(const uint64_t* offsets, uint64_t n_reads, const BuildInfo* info, uint32_t* tile_first_read,
                               uint64_t max_tiles, cudaStream_t s);
 cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
@@ -130,7 +130,8 @@ cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint3
 template <typename KeyT, typename IdT>
 cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
                               uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, KeyT* keys, IdT* ids,
-                              uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, bool packed, cudaStream_t s);
+                              uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, bool packed, uint64_t* bucket_hist,
+                              uint64_t max_n, cudaStream_t s);
 
 // cx_onesweep.cu
 struct SortWorkspace {

@@ -156,27 +156,37 @@ __device__ __forceinline__ uint8_t preceding_symbol(const Reads& R, IdT id) {
 // ---------------------------------------------------------------------------------------------
 // global path: compact + re-key, write back
 // ---------------------------------------------------------------------------------------------
+// One thread per 32 sorted positions looks for members still tied; the warp then handles every such word together,
+// one lane per position (oversize groups are rare, so nearly all threads leave after one load).
 template <typename IdT>
 __global__ void __launch_bounds__(256) refine_rekey_kernel(Reads R, const uint32_t* __restrict__ heads,
                                                            const uint64_t* __restrict__ word_base, const IdT* __restrict__ ids,
                                                            uint64_t n, uint32_t depth, uint32_t w, uint64_t* __restrict__ keys_c,
                                                            IdT* __restrict__ ids_c, uint32_t* __restrict__ pos_c) {
-    uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= n) return;
-    uint64_t wi = j >> 5;
-    uint32_t bit = (uint32_t)(j & 31);
-    uint32_t act, ah;
-    active_masks(heads[wi], heads[wi + 1], act, ah);
-    if (!((act >> bit) & 1u)) return;
-    uint64_t base = word_base[wi];
-    uint32_t below = (1u << bit) - 1;
-    uint64_t c = (base & 0xffffffffull) + __popc(act & below);
-    uint64_t g = (base >> 32) + __popc(ah & (below | (1u << bit))) - 1;   // ordinal of this element's group
-    IdT id = ids[j];
-    uint64_t key = key_at_depth(R, id, depth, w);
-    keys_c[c] = (g << (2 * w + 5)) | key;
-    ids_c[c] = id;
-    pos_c[c] = (uint32_t)j;
+    const uint64_t n_words = (n + 31) >> 5;
+    const uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t act = 0, ah = 0;
+    if (wi < n_words) active_masks(heads[wi], heads[wi + 1], act, ah);
+    uint64_t base = act ? word_base[wi] : 0ull;
+    uint32_t todo = __ballot_sync(kFull, act != 0);
+    const uint32_t bit = lane_id();
+    while (todo) {
+        const int src = __ffs(todo) - 1;
+        todo &= todo - 1;
+        const uint32_t wact = __shfl_sync(kFull, act, src), wah = __shfl_sync(kFull, ah, src);
+        const uint64_t wbase = __shfl_sync(kFull, base, src);
+        const uint64_t wwi = wi - bit + src;   // word index of lane `src` (lanes hold consecutive words)
+        if ((wact >> bit) & 1u) {
+            const uint64_t j = (wwi << 5) + bit;
+            const uint32_t below = (1u << bit) - 1;
+            const uint64_t c = (wbase & 0xffffffffull) + __popc(wact & below);
+            const uint64_t g = (wbase >> 32) + __popc(wah & (below | (1u << bit))) - 1;   // ordinal of this element's group
+            const IdT id = ids[j];
+            keys_c[c] = (g << (2 * w + 5)) | key_at_depth(R, id, depth, w);
+            ids_c[c] = id;
+            pos_c[c] = (uint32_t)j;
+        }
+    }
 }
 
 template <typename IdT>
@@ -501,7 +511,8 @@ template <typename IdT>
 cudaError_t launch_refine_rekey(const Reads& R, const uint32_t* heads, const uint64_t* word_base, const IdT* ids, uint64_t n,
                                 uint32_t depth, uint32_t w, uint64_t* keys_c, IdT* ids_c, uint32_t* pos_c, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
-    refine_rekey_kernel<IdT><<<(unsigned)((n + 255) / 256), 256, 0, s>>>(R, heads, word_base, ids, n, depth, w, keys_c, ids_c, pos_c);
+    const uint64_t n_words = (n + 31) >> 5;
+    refine_rekey_kernel<IdT><<<(unsigned)((n_words + 255) / 256), 256, 0, s>>>(R, heads, word_base, ids, n, depth, w, keys_c, ids_c, pos_c);
     return cudaGetLastError();
 }
 

@@ -15,7 +15,7 @@ namespace {
 // ---------------------------------------------------------------------------------------------
 // prep
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) prep_kernel(const uint64_t* __restrict__ offsets, uint64_t n_reads, BuildInfo* info) {
+__global__ void __launch_bounds__(256) prep_kernel(const uint64_t* __restrict__ offsets, uint64_t n_reads, uint64_t max_bases, BuildInfo* info) {
     uint64_t first_len = offsets[1] - offsets[0];
     uint64_t local_max = 0;
     uint32_t bad = 0, nonuni = 0;
@@ -42,6 +42,7 @@ __global__ void __launch_bounds__(256) prep_kernel(const uint64_t* __restrict__ 
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         if (offsets[0] != 0) atomicOr(&info->bad_offsets, 1u);
+        if (offsets[n_reads] > max_bases) atomicOr(&info->bad_offsets, 2u);   // more bases than the plan was made for
         info->total_bases = offsets[n_reads];
         info->n_suffixes = offsets[n_reads] + n_reads;
         info->first_len = first_len;
@@ -173,6 +174,7 @@ __global__ void __launch_bounds__(kListThreads) bucket_hist_kernel(Reads R, cons
     uint32_t* s_short = s_hist + n_kmers;
     const uint32_t n_short = (n_kmers - 1) / 3;
     for (uint32_t k = threadIdx.x; k < n_kmers + n_short; k += blockDim.x) s_hist[k] = 0;
+    if (info->bad_offsets) return;   // reported by the host after it reads `info`
     R.n_words = (info->total_bases + 31) >> 5;
     const uint64_t N = info->n_suffixes;
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
@@ -253,11 +255,19 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
                                                                   uint32_t bucket_lo, uint32_t bucket_hi,
                                                                   const uint64_t* __restrict__ tile_base, KeyT* __restrict__ keys,
                                                                   IdT* __restrict__ ids, uint32_t n_passes,
-                                                                  unsigned long long* __restrict__ digit_hist) {
+                                                                  unsigned long long* __restrict__ digit_hist,
+                                                                  unsigned long long* __restrict__ bucket_hist, uint64_t max_n) {
     __shared__ TileSmem sm;
     __shared__ uint32_t s_dh[8][kRadix];   // digit counts of every radix pass of the sort that follows (a6's upfront histogram)
+    // bucket_hist != nullptr (ALL only): this scan also counts the partition sizes (a2), as bucket_hist_kernel does, so that a
+    // build that is known to fit one batch reads the collection once
+    extern __shared__ uint32_t s_bh[];
+    const uint32_t n_kmers = 1u << (2 * ell), n_short = (n_kmers - 1) / 3;
+    if (bucket_hist)
+        for (uint32_t k = threadIdx.x; k < n_kmers + n_short; k += blockDim.x) s_bh[k] = 0;
     R.n_words = (info->total_bases + 31) >> 5;
     const uint64_t N = info->n_suffixes;
+    if (N > max_n || info->bad_offsets) return;   // the host reports both after reading `info`
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
     const uint32_t warp = threadIdx.x >> 5;
     constexpr int kWarps = kListThreads / 32;
@@ -284,6 +294,12 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
                 id[k] = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
                 if (ALL) {
                     take[k] = true;
+                    if (bucket_hist) {
+                        uint32_t kmer, r;
+                        bucket_of(sl, ell, kmer, r);
+                        if (r == ell) atomicAdd(&s_bh[kmer], 1u);
+                        else atomicAdd(&s_bh[n_kmers + (((1u << (2 * r)) - 1) / 3) + (kmer >> (2 * (ell - r)))], 1u);
+                    }
                 } else {
                     uint32_t kmer, r;
                     uint32_t b = bucket_of(sl, ell, kmer, r);
@@ -350,6 +366,19 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
         uint32_t v = (&s_dh[0][0])[i];
         if (v) atomicAdd(digit_hist + i, (unsigned long long)v);
     }
+    if (bucket_hist) {
+        for (uint32_t k = threadIdx.x; k < n_kmers; k += blockDim.x) {
+            uint32_t v = s_bh[k];
+            if (v) atomicAdd(bucket_hist + (uint64_t)k * (ell + 1) + ell, (unsigned long long)v);
+        }
+        for (uint32_t r = 0; r < ell; ++r) {
+            const uint32_t first = n_kmers + ((1u << (2 * r)) - 1) / 3, count = 1u << (2 * r);
+            for (uint32_t k = threadIdx.x; k < count; k += blockDim.x) {
+                uint32_t v = s_bh[first + k];
+                if (v) atomicAdd(bucket_hist + ((uint64_t)k << (2 * (ell - r))) * (ell + 1) + r, (unsigned long long)v);
+            }
+        }
+    }
 }
 
 }  // namespace
@@ -357,12 +386,12 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
 // ---------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------
-cudaError_t launch_prep(const uint64_t* offsets, uint64_t n_reads, BuildInfo* info, cudaStream_t s) {
+cudaError_t launch_prep(const uint64_t* offsets, uint64_t n_reads, uint64_t max_bases, BuildInfo* info, cudaStream_t s) {
     cudaError_t e = cudaMemsetAsync(info, 0, sizeof(BuildInfo), s);
     if (e != cudaSuccess) return e;
     uint64_t blocks = (n_reads + 255) / 256;
     unsigned grid = (unsigned)(blocks < 148ull * 8 ? (blocks ? blocks : 1) : 148ull * 8);
-    prep_kernel<<<grid, 256, 0, s>>>(offsets, n_reads, info);
+    prep_kernel<<<grid, 256, 0, s>>>(offsets, n_reads, max_bases, info);
     return cudaGetLastError();
 }
 
@@ -403,34 +432,31 @@ cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint3
 template <typename KeyT, typename IdT>
 cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
                               uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, KeyT* keys, IdT* ids,
-                              uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, bool packed, cudaStream_t s) {
+                              uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, bool packed, uint64_t* bucket_hist,
+                              uint64_t max_n, cudaStream_t s) {
     if (n_tiles == 0) return cudaSuccess;
-    uint64_t want = (uint64_t)n_sms * 6;
+    uint64_t want = (uint64_t)n_sms * (bucket_hist ? 4 : 6);
     unsigned grid = (unsigned)(n_tiles < want ? n_tiles : want);
     unsigned long long* dh = (unsigned long long*)digit_hist;
+    unsigned long long* bh = (unsigned long long*)bucket_hist;
     constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
-    if (packed && !kCanPack) return cudaErrorInvalidValue;
-    if (tile_base == nullptr) {
-        if (packed)
-            list_write_kernel<KeyT, IdT, true, kCanPack><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
-                                                                                       nullptr, keys, ids, n_passes, dh);
-        else
-            list_write_kernel<KeyT, IdT, true, false><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
-                                                                                    nullptr, keys, ids, n_passes, dh);
-    } else {
-        if (packed)
-            list_write_kernel<KeyT, IdT, false, kCanPack><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
-                                                                                        tile_base, keys, ids, n_passes, dh);
-        else
-            list_write_kernel<KeyT, IdT, false, false><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi,
-                                                                                     tile_base, keys, ids, n_passes, dh);
-    }
-    return cudaGetLastError();
+    if ((packed && !kCanPack) || (bucket_hist && tile_base)) return cudaErrorInvalidValue;
+    const size_t smem = bucket_hist ? bucket_hist_smem(ell) - sizeof(TileSmem) : 0;
+    auto launch = [&](auto kernel) {
+        if (smem) {
+            cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bucket_hist_smem(7) - sizeof(TileSmem)));
+            if (e != cudaSuccess) return e;
+        }
+        kernel<<<grid, kListThreads, smem, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids, n_passes, dh, bh, max_n);
+        return cudaGetLastError();
+    };
+    if (tile_base == nullptr) return packed ? launch(list_write_kernel<KeyT, IdT, true, kCanPack>) : launch(list_write_kernel<KeyT, IdT, true, false>);
+    return packed ? launch(list_write_kernel<KeyT, IdT, false, kCanPack>) : launch(list_write_kernel<KeyT, IdT, false, false>);
 }
 
 #define CX_LIST_INST(K, I)                                                                                                        \
     template cudaError_t launch_list_write<K, I>(const Reads&, const BuildInfo*, const uint32_t*, uint32_t, uint32_t, uint32_t,  \
-                                                 uint32_t, const uint64_t*, K*, I*, uint64_t, uint32_t, uint64_t*, int, bool, cudaStream_t);
+                                                 uint32_t, const uint64_t*, K*, I*, uint64_t, uint32_t, uint64_t*, int, bool, uint64_t*, uint64_t, cudaStream_t);
 CX_LIST_INST(uint32_t, uint32_t)
 CX_LIST_INST(uint32_t, uint64_t)
 CX_LIST_INST(uint64_t, uint32_t)

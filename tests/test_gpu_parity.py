@@ -158,6 +158,31 @@ def test_bucket_too_large_is_reported():
     assert e.value.code == cx.binding.CX_ERR_BUCKET_TOO_LARGE
 
 
+def test_bad_offsets_and_oversize_input_are_reported_not_executed():
+    import paper_1401_7457_b200 as cx
+    c = gen.config(1, 0.002)
+    a = torch.from_numpy(c.ascii).cuda()
+    packed = cx.cx_pack_reads(a)
+    out = torch.empty(c.n_suffixes, dtype=torch.uint8, device="cuda")
+    good = torch.from_numpy(c.offsets.astype(np.int64)).cuda()
+    for kind in ("decreasing", "nonzero_start"):
+        off = good.clone()
+        if kind == "decreasing":
+            off[5] = off[7] + 3
+        else:
+            off[0] = 1
+        p = cx.Plan(c.n_reads, c.total_bases, max_read_len=100)
+        with pytest.raises(cx.CxError) as e:
+            p.build(packed, off, c.n_reads, out)
+        assert e.value.code == cx.binding.CX_ERR_ARG
+        p.build(packed, good, c.n_reads, out)                # the plan is still usable
+        assert np.array_equal(out.cpu().numpy(), oracle.bwt(c.ascii, c.offsets))
+    small = cx.Plan(c.n_reads, c.total_bases // 2, max_read_len=100)      # planned for half the bases
+    with pytest.raises(cx.CxError) as e:
+        small.build(packed, good, c.n_reads, out)
+    assert e.value.code == cx.binding.CX_ERR_ARG
+
+
 def test_deterministic():
     c = gen.config(2, 0.001)
     assert np.array_equal(gpu_bwt(c), gpu_bwt(c))
