@@ -65,7 +65,8 @@ Layout make_layout(const Shape& sh, uint64_t m1) {
     L.info = take(sizeof(BuildInfo));
     L.hist = take(sh.n_buckets * 8);
     L.tile_first = take((sh.max_tiles + 1) * 4);
-    L.tile_count = take((sh.max_tiles + 1) * 8);
+    // per-tile counts of up to kCountGroup batches at a time; a plan that always fits one batch never counts
+    L.tile_count = take((sh.max_tiles + 1) * 8 * (sh.max_suffixes <= m1 ? 1 : kCountGroup));
     L.tile_sums = take((scan_block_count(sh.max_tiles + 1) + 1) * 8);
     L.scalars = take(64);
     for (int i = 0; i < 2; ++i) L.keys[i] = take(m1 * 8);
@@ -423,17 +424,22 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, nullptr, d_keys1[0],
                                                   d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, nullptr, ~0ull, s)));
         } else {
-            {
-                ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + n_tiles * 8, s);
-                CX_CUDA(launch_list_count(R, d_info, d_tile_first, sh.ell, B.bucket_lo, B.bucket_hi, d_tile_count, n_tiles, s));
+            const uint64_t col_stride = sh.max_tiles + 1;
+            if (bi % kCountGroup == 0) {   // one scan counts this batch and the next seven
+                CountRanges cr{};
+                for (size_t q = bi; q < p->batches.size() && cr.n < (uint32_t)kCountGroup; ++q) cr.first[cr.n++] = p->batches[q].bucket_lo;
+                cr.first[cr.n] = p->batches[bi + cr.n - 1].bucket_hi + 1;
+                ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + n_tiles * 8 * cr.n, s);
+                CX_CUDA(launch_list_count(R, d_info, d_tile_first, sh.ell, cr, d_tile_count, col_stride, n_tiles, s));
             }
+            uint64_t* d_col = d_tile_count + (bi % kCountGroup) * col_stride;
             {
                 ScopedLaunch sl(prof, CX_K_LIST, n_tiles * 16, s);
-                CX_CUDA(launch_scan_u64(d_tile_count, n_tiles, d_tile_sums, d_scalars + 2, s));
+                CX_CUDA(launch_scan_u64(d_col, n_tiles, d_tile_sums, d_scalars + 2, s));
             }
             prof->launches[CX_K_LIST] += 2;   // the scan is three kernels
             ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (sizeof(KeyT) + sizeof(IdT)), s);
-            CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, d_tile_count,
+            CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, d_col,
                                                   d_keys1[0], d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, nullptr, ~0ull, s)));
         }
         // ---- step 3(c)ii: sort (first w symbols) ------------------------------------------------
@@ -470,7 +476,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
                 CX_CUDA(launch_scan_u64(d_word_counts, n_words, d_word_sums, d_scalars, s));
             }
             prof->launches[CX_K_REFINE_SCAN] += 2;
-            CX_CUDA(cudaMemcpyAsync(p->h_scalars, d_scalars, 16, cudaMemcpyDeviceToHost, s));
+            CX_CUDA(cudaMemcpyAsync(p->h_scalars, d_scalars, 32, cudaMemcpyDeviceToHost, s));
             CX_CUDA(cudaStreamSynchronize(s));
             const uint64_t n_act = p->h_scalars[0] & 0xffffffffull;
             const uint64_t n_groups = p->h_scalars[0] >> 32;
@@ -503,6 +509,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             }
         }
         p->stats.small_group_elems = p->h_scalars[1];
+        p->stats.compare_ops = p->h_scalars[3];
         p->stats.refine_elements += p->h_scalars[1] - local_before;
         if (rounds > p->stats.refine_rounds) p->stats.refine_rounds = rounds;
 
@@ -534,7 +541,7 @@ extern "C" int cx_bwt_build(cx_bwt_plan_t* p, const uint64_t* packed_reads, cons
     if (!p) return CX_ERR_ARG;
     p->prof.reset();
     memset(&p->stats, 0, sizeof(p->stats));
-    p->h_scalars[0] = p->h_scalars[1] = 0;
+    p->h_scalars[0] = p->h_scalars[1] = p->h_scalars[3] = 0;
     if (n_reads == 0) return CX_OK;
     if (!read_offsets || !out_bwt || n_reads > p->sh.max_reads) return CX_ERR_ARG;
     if (!packed_reads && p->sh.max_bases) return CX_ERR_ARG;

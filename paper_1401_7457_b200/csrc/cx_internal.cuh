@@ -121,9 +121,15 @@ cudaError_t launch_tile_table(const uint64_t* offsets, uint64_t n_reads, const B
                               uint64_t max_tiles, cudaStream_t s);
 cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
                                uint64_t* hist, uint64_t max_tiles, int n_sms, cudaStream_t s);
-// count suffixes of each tile whose bucket lies in [bucket_lo, bucket_hi]
+// count, per tile, the suffixes of up to kCountGroup consecutive batches in one scan; batch j owns partitions
+// [first[j], first[j + 1]); tile_count[j * col_stride + tile]
+constexpr int kCountGroup = 8;
+struct CountRanges {
+    uint32_t n;
+    uint32_t first[kCountGroup + 1];
+};
 cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
-                              uint32_t bucket_lo, uint32_t bucket_hi, uint64_t* tile_count, uint64_t n_tiles, cudaStream_t s);
+                              const CountRanges& ranges, uint64_t* tile_count, uint64_t col_stride, uint64_t n_tiles, cudaStream_t s);
 // write (key, id) of those suffixes in (read, pos) order; tile_base == nullptr means "every suffix, index = slot".
 // Also accumulates the digit counts of the n_passes radix passes over key bits [0, 8 * n_passes) into digit_hist
 // (zeroed by the caller), which is what sort_pairs(..., hist_ready = true) expects.

@@ -362,7 +362,7 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
     __syncthreads();
 
     // ---- classify: groups that start in this tile and have at most cap members are ours -----------
-    uint32_t n_active = 0;
+    uint32_t n_active = 0, n_compares = 0;
 #pragma unroll
     for (int k = 0; k < kLocalItems; ++k) {
         const int e = k * kLocalThreads + tid;
@@ -414,6 +414,7 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
             if (s != kNone) {
                 const int t = sm.ge[e];
                 const uint4 my = reinterpret_cast<const uint4*>(sm.key)[e];
+                n_compares += (uint32_t)(t - s);
                 uint32_t neg = 0;   // minus the number of members whose key is below mine
 #pragma unroll 4
                 for (int q = s; q < t; ++q) count_if_less(neg, reinterpret_cast<const uint4*>(sm.key)[q], my);
@@ -428,9 +429,13 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
             const int e = k * kLocalThreads + tid;
             if (sm.gs[e] != kNone) {
                 const int se = sm.src[e];
-                const u128 kk = sm.key[se] >> 8;
+                const uint4 kk = reinterpret_cast<const uint4*>(sm.key)[se];
                 idn[k] = sm.id_a[se];
-                const bool head = e == sm.gs[e] || kk != (sm.key[sm.src[e - 1]] >> 8) || ((uint32_t)kk & 63u) < kLocalW;
+                bool head = e == sm.gs[e] || ((kk.x >> 8) & 63u) < kLocalW;
+                if (!head) {   // same bases and length as the member ranked just before?  (the low 8 bits are the group index)
+                    const uint4 kp = reinterpret_cast<const uint4*>(sm.key)[sm.src[e - 1]];
+                    head = ((((kk.x ^ kp.x) >> 8) | (kk.y ^ kp.y)) | ((kk.z ^ kp.z) | (kk.w ^ kp.w))) != 0;
+                }
                 headbit |= (uint32_t)head << k;
             }
         }
@@ -450,14 +455,14 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
             const int e = k * kLocalThreads + tid;
             const int s = sm.gs[e];
             if (s != kNone) {
-                const int t = sm.ge[e];
-                const int ps = prev_head(sm.hw, e, s);
-                const int ne = next_head(sm.hw, e, t);
-                if (ne - ps >= 2) {
-                    sm.gs[e] = (uint16_t)ps;
-                    sm.ge[e] = (uint16_t)ne;
-                } else {
+                // head bits of e and e + 1 both set: alone in its group, placed for good
+                const uint32_t lo = sm.hw[e >> 5], hi = sm.hw[(e >> 5) + 1];
+                if (((((uint64_t)hi << 32) | lo) >> (e & 31) & 3u) == 3u) {
                     sm.gs[e] = kNone;
+                } else {
+                    const int t = sm.ge[e];
+                    sm.gs[e] = (uint16_t)prev_head(sm.hw, e, s);
+                    sm.ge[e] = (uint16_t)next_head(sm.hw, e, t);
                 }
             }
         }
@@ -475,13 +480,19 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
         if (add) atomicOr(&heads[w0 + i], add);
     }
     // one statistics update per block (hundreds of thousands of atomics on one address would serialise in L2)
-    __shared__ uint32_t s_done;
-    if (tid == 0) s_done = 0;
+    __shared__ uint32_t s_done, s_cmp;
+    if (tid == 0) s_done = 0, s_cmp = 0;
     __syncthreads();
-    for (int o = 16; o; o >>= 1) n_active += __shfl_xor_sync(kFull, n_active, o);
-    if (lane_id() == 0 && n_active) atomicAdd(&s_done, n_active);
+    for (int o = 16; o; o >>= 1) {
+        n_active += __shfl_xor_sync(kFull, n_active, o);
+        n_compares += __shfl_xor_sync(kFull, n_compares, o);
+    }
+    if (lane_id() == 0 && n_active) atomicAdd(&s_done, n_active), atomicAdd(&s_cmp, n_compares);
     __syncthreads();
-    if (tid == 0 && s_done) atomicAdd(elems_done, (unsigned long long)s_done);
+    if (tid == 0 && s_done) {
+        atomicAdd(elems_done, (unsigned long long)s_done);
+        atomicAdd(elems_done + 2, (unsigned long long)s_cmp);   // 128-bit key comparisons done (the ALU work of this kernel)
+    }
 }
 
 }  // namespace

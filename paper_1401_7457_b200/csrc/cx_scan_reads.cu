@@ -212,21 +212,23 @@ __global__ void __launch_bounds__(kListThreads) bucket_hist_kernel(Reads R, cons
 }
 
 // ---------------------------------------------------------------------------------------------
-// a4 (count half): suffixes per tile whose partition lies in [bucket_lo, bucket_hi]
+// a4 (count half): suffixes per tile that fall in each of up to kCountGroup consecutive batches, in ONE scan of the
+// collection (fewer scans).  Batch j owns the partitions [first[j], first[j + 1]).
+// tile_count is laid out [batch][tile] so that each batch's column can be scanned in place.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const BuildInfo* __restrict__ info,
                                                                   const uint32_t* __restrict__ tile_first_read, uint32_t ell,
-                                                                  uint32_t bucket_lo, uint32_t bucket_hi, uint64_t* __restrict__ tile_count) {
+                                                                  CountRanges ranges, uint64_t* __restrict__ tile_count, uint64_t col_stride) {
     __shared__ TileSmem sm;
-    __shared__ uint32_t s_total;
+    __shared__ uint32_t s_total[kCountGroup];
     R.n_words = (info->total_bases + 31) >> 5;
     const uint64_t N = info->n_suffixes;
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
     uint64_t t = blockIdx.x;
-    if (t >= n_tiles) return;
-    if (threadIdx.x == 0) s_total = 0;
+    if (t >= n_tiles || info->bad_offsets) return;
+    if (threadIdx.x < kCountGroup) s_total[threadIdx.x] = 0;
     TileCtx c = load_tile(R, info, tile_first_read, t, n_tiles, N, sm);
-    uint32_t mine = 0;
+    uint32_t mine = 0;   // eight 4-bit counters (a thread sees at most kListItems = 8 suffixes)
 #pragma unroll
     for (int k = 0; k < kListItems; ++k) {
         uint32_t s = k * kListThreads + threadIdx.x;
@@ -234,13 +236,23 @@ __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const
             Slot sl = decode_slot(c, sm, s);
             uint32_t kmer, r;
             uint32_t b = bucket_of(sl, ell, kmer, r);
-            mine += (b >= bucket_lo && b <= bucket_hi);
+            if (b >= ranges.first[0] && b < ranges.first[ranges.n]) {
+                uint32_t j = 0;
+#pragma unroll
+                for (int q = 1; q < kCountGroup; ++q) j += (q < (int)ranges.n && b >= ranges.first[q]);
+                mine += 1u << (4 * j);
+            }
         }
     }
-    for (int o = 16; o; o >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
-    if (lane_id() == 0 && mine) atomicAdd(&s_total, mine);
+    static_assert(kListItems <= 15, "4-bit per-thread counters");
+#pragma unroll
+    for (int j = 0; j < kCountGroup; ++j) {
+        uint32_t v = (mine >> (4 * j)) & 15u;
+        for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane_id() == 0 && v) atomicAdd(&s_total[j], v);
+    }
     __syncthreads();
-    if (threadIdx.x == 0) tile_count[t] = s_total;
+    if (threadIdx.x < ranges.n) tile_count[(uint64_t)threadIdx.x * col_stride + t] = s_total[threadIdx.x];
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -423,9 +435,9 @@ cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint
 }
 
 cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
-                              uint32_t bucket_lo, uint32_t bucket_hi, uint64_t* tile_count, uint64_t n_tiles, cudaStream_t s) {
-    if (n_tiles == 0) return cudaSuccess;
-    list_count_kernel<<<(unsigned)n_tiles, kListThreads, 0, s>>>(R, info, tile_first_read, ell, bucket_lo, bucket_hi, tile_count);
+                              const CountRanges& ranges, uint64_t* tile_count, uint64_t col_stride, uint64_t n_tiles, cudaStream_t s) {
+    if (n_tiles == 0 || ranges.n == 0) return cudaSuccess;
+    list_count_kernel<<<(unsigned)n_tiles, kListThreads, 0, s>>>(R, info, tile_first_read, ell, ranges, tile_count, col_stride);
     return cudaGetLastError();
 }
 
