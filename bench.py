@@ -169,6 +169,26 @@ def run_reference(args) -> None:
 
 
 # --------------------------------------------------------------------------------------------------
+# multi-rank plumbing (replicas only: no data-path collective; covered on CPU by tests/test_bench_dist.py with gloo)
+# --------------------------------------------------------------------------------------------------
+def replica_seed(config: int, rank: int) -> int:
+    """Every rank sorts its own collection of the same recipe: rank 0 uses the config's base seed."""
+    from workloads import generate as gen
+    return gen.BASE_SEED + config + 1000 * rank
+
+
+def max_over_ranks(values, device) -> list:
+    """Element-wise MAX of per-rank timings (the contract's 'max over ranks'); identity when not distributed."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+# --------------------------------------------------------------------------------------------------
 # the CUDA arm
 # --------------------------------------------------------------------------------------------------
 def run_cx(args) -> None:
@@ -191,7 +211,7 @@ def run_cx(args) -> None:
     cx.lib()
 
     # ---- synthetic input (seeded; replicas differ only in seed) -------------------------------------
-    coll = gen.config(args.config, args.scale, seed=gen.BASE_SEED + args.config + 1000 * rank)
+    coll = gen.config(args.config, args.scale, seed=replica_seed(args.config, rank))
     n_reads, total, N = coll.n_reads, coll.total_bases, coll.n_suffixes
     h_ascii = torch.from_numpy(coll.ascii).pin_memory()
     h_off = torch.from_numpy(coll.offsets.astype(np.int64)).pin_memory()
@@ -273,9 +293,7 @@ def run_cx(args) -> None:
     e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
     barrier()
     if world > 1:
-        t = torch.tensor([dev_ms, e2e_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dev_ms, e2e_ms = float(t[0]), float(t[1])
+        dev_ms, e2e_ms = max_over_ranks([dev_ms, e2e_ms], dev)
     if rank != 0:
         dist.destroy_process_group()
         return

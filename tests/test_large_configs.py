@@ -144,7 +144,10 @@ def check_slices(recipe, probes, out, n_suffixes):
 
 def run_config(index, probes_text, chunk_reads, workspace_bytes, host_out, scale=1.0):
     import paper_1401_7457_b200 as cx
+    import gc
     dev = torch.device("cuda", 0)
+    gc.collect()
+    torch.cuda.empty_cache()                 # a previous config's workspace must not stay cached
     t0 = time.time()
     recipe = gt.ReadRecipe(index, scale, device=dev)
     probes = [PrefixProbe(t) for t in probes_text]
@@ -180,6 +183,9 @@ def run_config(index, probes_text, chunk_reads, workspace_bytes, host_out, scale
     with open(f"gpurun_out/large_config{index}.json", "w") as f:
         json.dump(res, f)
     print(json.dumps(res))
+    del out, packed, offsets, counts, last_base, got, recipe, probes
+    gc.collect()
+    torch.cuda.empty_cache()
     return res
 
 
