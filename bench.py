@@ -34,6 +34,7 @@ WORKLOADS = {
     1: "configs[1]: 1,000,000 reads x 100 bp at 100x over a seeded 1 Mbp genome (1.01e8 suffixes)",
     2: "configs[2]: 10,000,000 reads x 100 bp at 30x over 33 Mbp, both strands, 1% subst. (1.01e9 suffixes)",
     3: "configs[3]: 40,000,000 reads x 50-250 bp over a 50 Mbp repeat genome (~6.04e9 suffixes)",
+    4: "configs[4]: 1,000,000,000 reads x 100 bp at 30x over 3.3 Gbp, both strands, 1% subst. (1.01e11 suffixes)",
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture named here (None until one exists for this workload).
@@ -53,6 +54,7 @@ def parse_args():
     ap.add_argument("--impl", default="cx", choices=["cx", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--key-bases", type=int, default=0, help="first-round key window w (0 = the library's default)")
+    ap.add_argument("--max-batch", type=int, default=0, help="m1: most suffixes per batch (0 = as many as the workspace allows)")
     return ap.parse_args()
 
 
@@ -220,7 +222,8 @@ def run_cx(args) -> None:
     d_off = h_off.to(dev)
     d_packed = torch.empty((total + 31) // 32 + 1, dtype=torch.int64, device=dev)
     d_out = torch.empty(N, dtype=torch.uint8, device=dev)
-    plan = cx.Plan(n_reads, total, max_read_len=coll.max_read_len, profile=1, key_bases=args.key_bases or None, device=dev)
+    plan = cx.Plan(n_reads, total, max_read_len=coll.max_read_len, profile=1, key_bases=args.key_bases or None, max_batch_suffixes=args.max_batch or None,
+                   device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
     stream = torch.cuda.current_stream()
 

@@ -118,6 +118,8 @@ __device__ __forceinline__ TileCtx load_tile(const Reads& R, const BuildInfo* __
 struct Slot {
     uint64_t read, pos, rem;   // suffix (read, pos); rem = bases left = m_i - pos
     uint64_t window;           // the next 32 bases, MSB-first, junk past rem
+    uint64_t b;                // index of its first base in the concatenation
+    uint32_t lo;               // read - r0 (index into the staged offsets of a ragged collection)
 };
 
 __device__ __forceinline__ Slot decode_slot(const TileCtx& c, const TileSmem& sm, uint32_t s) {
@@ -129,6 +131,7 @@ __device__ __forceinline__ Slot decode_slot(const TileCtx& c, const TileSmem& sm
         sl.read = c.r0 + rr;
         sl.pos = x - rr * c.L1;
         sl.rem = (c.L1 - 1) - sl.pos;
+        sl.lo = rr;
         b = sl.read * (c.L1 - 1) + sl.pos;
     } else {
         uint64_t g = c.g0 + s;
@@ -139,6 +142,7 @@ __device__ __forceinline__ Slot decode_slot(const TileCtx& c, const TileSmem& sm
             if (sm.off[mid] + c.r0 + mid <= g) lo = mid; else hi = mid - 1;
         }
         sl.read = c.r0 + lo;
+        sl.lo = lo;
         uint64_t start = sm.off[lo];
         sl.pos = g - (start + sl.read);
         sl.rem = sm.off[lo + 1] - start - sl.pos;
@@ -148,7 +152,28 @@ __device__ __forceinline__ Slot decode_slot(const TileCtx& c, const TileSmem& sm
     uint32_t sh = (uint32_t)(b & 31) * 2;
     uint64_t w0 = sm.packed[wi], w1 = sm.packed[wi + 1];
     sl.window = sh ? (w0 << sh) | (w1 >> (64 - sh)) : w0;
+    sl.b = b;
     return sl;
+}
+
+// Step from a suffix slot to the next one in (read, position) order without decoding it from scratch: inside a read the
+// 32-base window shifts by one base (two bits from the staged words); after a read's end-marker slot the next read starts
+// at the same base index, so the window stays.  A scan that only needs the l-mer of most slots (the multi-batch listing)
+// pays ~10 instructions per slot this way instead of a division or a binary search plus a funnel shift.
+__device__ __forceinline__ void next_slot(const TileCtx& c, const TileSmem& sm, Slot& sl) {
+    if (sl.rem) {
+        const uint64_t nb = sl.b + 32;
+        const uint32_t two = (uint32_t)(sm.packed[(uint32_t)((nb >> 5) - c.word0)] >> (62 - 2 * (uint32_t)(nb & 31))) & 3u;
+        sl.window = (sl.window << 2) | two;
+        sl.b += 1;
+        sl.pos += 1;
+        sl.rem -= 1;
+    } else {
+        sl.read += 1;
+        sl.lo += 1;
+        sl.pos = 0;
+        sl.rem = c.uniform ? (uint64_t)(c.L1 - 1) : sm.off[sl.lo + 1] - sm.off[sl.lo];
+    }
 }
 
 // Partition code of a suffix (reading A4 of PAPER.md:79 "suffixes shorter than l require special
@@ -224,35 +249,114 @@ __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const
     R.n_words = (info->total_bases + 31) >> 5;
     const uint64_t N = info->n_suffixes;
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
-    uint64_t t = blockIdx.x;
-    if (t >= n_tiles || info->bad_offsets) return;
-    if (threadIdx.x < kCountGroup) s_total[threadIdx.x] = 0;
-    TileCtx c = load_tile(R, info, tile_first_read, t, n_tiles, N, sm);
-    uint32_t mine = 0;   // eight 4-bit counters (a thread sees at most kListItems = 8 suffixes)
+    if (info->bad_offsets) return;
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        __syncthreads();   // previous tile done with sm and s_total
+        if (threadIdx.x < kCountGroup) s_total[threadIdx.x] = 0;
+        TileCtx c = load_tile(R, info, tile_first_read, t, n_tiles, N, sm);
+        // thread t walks the kListItems consecutive slots [t * kListItems, ...)
+        uint64_t mine = 0;   // eight 8-bit counters
+        const uint32_t s0 = threadIdx.x * kListItems;
+        if (s0 < c.n_slots) {
+            Slot sl = decode_slot(c, sm, s0);
 #pragma unroll
-    for (int k = 0; k < kListItems; ++k) {
-        uint32_t s = k * kListThreads + threadIdx.x;
-        if (s < c.n_slots) {
-            Slot sl = decode_slot(c, sm, s);
-            uint32_t kmer, r;
-            uint32_t b = bucket_of(sl, ell, kmer, r);
-            if (b >= ranges.first[0] && b < ranges.first[ranges.n]) {
-                uint32_t j = 0;
+            for (int i = 0; i < kListItems; ++i) {
+                if (s0 + i < c.n_slots) {
+                    uint32_t kmer, r;
+                    const uint32_t b = bucket_of(sl, ell, kmer, r);
+                    if (b >= ranges.first[0] && b < ranges.first[ranges.n]) {
+                        uint32_t j = 0;
 #pragma unroll
-                for (int q = 1; q < kCountGroup; ++q) j += (q < (int)ranges.n && b >= ranges.first[q]);
-                mine += 1u << (4 * j);
+                        for (int q = 1; q < kCountGroup; ++q) j += (q < (int)ranges.n && b >= ranges.first[q]);
+                        mine += 1ull << (8 * j);
+                    }
+                    if (s0 + i + 1 < c.n_slots) next_slot(c, sm, sl);
+                }
             }
         }
-    }
-    static_assert(kListItems <= 15, "4-bit per-thread counters");
 #pragma unroll
-    for (int j = 0; j < kCountGroup; ++j) {
-        uint32_t v = (mine >> (4 * j)) & 15u;
-        for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if (lane_id() == 0 && v) atomicAdd(&s_total[j], v);
+        for (int j = 0; j < kCountGroup; ++j) {
+            uint32_t v = (uint32_t)(mine >> (8 * j)) & 255u;
+            for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane_id() == 0 && v) atomicAdd(&s_total[j], v);
+        }
+        __syncthreads();
+        if (threadIdx.x < ranges.n) tile_count[(uint64_t)threadIdx.x * col_stride + t] = s_total[threadIdx.x];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a4 (write half) + a5 for one batch of a multi-batch build: the suffixes whose partition lies in
+// [bucket_lo, bucket_hi], in (read, pos) order, each with its first key.  Most slots belong to other
+// batches, so the scan walks the slots with next_slot() and decodes in full only what it takes.
+// ---------------------------------------------------------------------------------------------
+template <typename KeyT, typename IdT, bool PACKED>
+__global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, const BuildInfo* __restrict__ info,
+                                                                   const uint32_t* __restrict__ tile_first_read, uint32_t ell, uint32_t w,
+                                                                   uint32_t bucket_lo, uint32_t bucket_hi,
+                                                                   const uint64_t* __restrict__ tile_base, KeyT* __restrict__ keys,
+                                                                   IdT* __restrict__ ids, uint32_t n_passes,
+                                                                   unsigned long long* __restrict__ digit_hist) {
+    __shared__ TileSmem sm;
+    __shared__ uint32_t s_dh[8][kRadix];
+    __shared__ uint32_t s_warp[kListThreads / 32];
+    R.n_words = (info->total_bases + 31) >> 5;
+    const uint64_t N = info->n_suffixes;
+    const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
+    const uint32_t len_bits = key_len_bits(w);
+    const uint32_t warp = threadIdx.x >> 5;
+    if (info->bad_offsets) return;
+    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) (&s_dh[0][0])[i] = 0;
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        __syncthreads();   // previous tile done with sm and s_warp
+        TileCtx c = load_tile(R, info, tile_first_read, t, n_tiles, N, sm);
+        const uint32_t s0 = threadIdx.x * kListItems;
+        uint32_t mask = 0;   // which of my kListItems consecutive slots belong to this batch
+        if (s0 < c.n_slots) {
+            Slot sl = decode_slot(c, sm, s0);
+#pragma unroll
+            for (int i = 0; i < kListItems; ++i) {
+                if (s0 + i < c.n_slots) {
+                    uint32_t kmer, r;
+                    const uint32_t b = bucket_of(sl, ell, kmer, r);
+                    mask |= (uint32_t)(b >= bucket_lo && b <= bucket_hi) << i;
+                    if (s0 + i + 1 < c.n_slots) next_slot(c, sm, sl);
+                }
+            }
+        }
+        // exclusive scan of the per-thread counts: slot order = thread order
+        const uint32_t cnt = __popc(mask);
+        uint32_t incl = cnt;
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t up = __shfl_up_sync(0xffffffffu, incl, o);
+            if ((int)lane_id() >= o) incl += up;
+        }
+        if (lane_id() == 31) s_warp[warp] = incl;
+        __syncthreads();
+        uint32_t before = incl - cnt;
+        for (uint32_t q = 0; q < warp; ++q) before += s_warp[q];
+        uint64_t dst = tile_base[t] + before;
+        while (mask) {
+            const int i = __ffs(mask) - 1;
+            mask &= mask - 1;
+            const Slot sl = decode_slot(c, sm, s0 + i);
+            const KeyT key = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
+            const IdT id = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
+            for (uint32_t p = 0; p < n_passes; ++p) atomicAdd(&s_dh[p][(uint32_t)(key >> (p * kRadixBits)) & (kRadix - 1)], 1u);
+            if constexpr (PACKED) {
+                reinterpret_cast<uint64_t*>(keys)[dst] = ((uint64_t)key << 32) | (uint64_t)id;
+            } else {
+                keys[dst] = key;
+                ids[dst] = id;
+            }
+            ++dst;
+        }
     }
     __syncthreads();
-    if (threadIdx.x < ranges.n) tile_count[(uint64_t)threadIdx.x * col_stride + t] = s_total[threadIdx.x];
+    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) {
+        uint32_t v = (&s_dh[0][0])[i];
+        if (v) atomicAdd(digit_hist + i, (unsigned long long)v);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -302,8 +406,6 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
             rank[k] = 0;
             if (s < c.n_slots) {
                 Slot sl = decode_slot(c, sm, s);
-                key[k] = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
-                id[k] = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
                 if (ALL) {
                     take[k] = true;
                     if (bucket_hist) {
@@ -316,6 +418,10 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
                     uint32_t kmer, r;
                     uint32_t b = bucket_of(sl, ell, kmer, r);
                     take[k] = b >= bucket_lo && b <= bucket_hi;
+                }
+                if (take[k]) {   // most suffixes of a multi-batch scan belong to other batches: no key, no id for them
+                    key[k] = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
+                    id[k] = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
                 }
             }
             if (take[k]) {
@@ -437,7 +543,9 @@ cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint
 cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
                               const CountRanges& ranges, uint64_t* tile_count, uint64_t col_stride, uint64_t n_tiles, cudaStream_t s) {
     if (n_tiles == 0 || ranges.n == 0) return cudaSuccess;
-    list_count_kernel<<<(unsigned)n_tiles, kListThreads, 0, s>>>(R, info, tile_first_read, ell, ranges, tile_count, col_stride);
+    uint64_t want = 148ull * 8;
+    list_count_kernel<<<(unsigned)(n_tiles < want ? n_tiles : want), kListThreads, 0, s>>>(R, info, tile_first_read, ell, ranges, tile_count,
+                                                                                         col_stride);
     return cudaGetLastError();
 }
 
@@ -463,7 +571,13 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
         return cudaGetLastError();
     };
     if (tile_base == nullptr) return packed ? launch(list_write_kernel<KeyT, IdT, true, kCanPack>) : launch(list_write_kernel<KeyT, IdT, true, false>);
-    return packed ? launch(list_write_kernel<KeyT, IdT, false, kCanPack>) : launch(list_write_kernel<KeyT, IdT, false, false>);
+    if (packed)
+        list_select_kernel<KeyT, IdT, kCanPack><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids,
+                                                                             n_passes, dh);
+    else
+        list_select_kernel<KeyT, IdT, false><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids,
+                                                                          n_passes, dh);
+    return cudaGetLastError();
 }
 
 #define CX_LIST_INST(K, I)                                                                                                        \
