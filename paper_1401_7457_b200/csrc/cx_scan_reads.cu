@@ -156,31 +156,51 @@ __device__ __forceinline__ Slot decode_slot(const TileCtx& c, const TileSmem& sm
     return sl;
 }
 
-// Step from a suffix slot to the next one in (read, position) order without decoding it from scratch: inside a read the
-// 32-base window shifts by one base (two bits from the staged words); after a read's end-marker slot the next read starts
-// at the same base index, so the window stays.  A scan that only needs the l-mer of most slots (the multi-batch listing)
-// pays ~10 instructions per slot this way instead of a division or a binary search plus a funnel shift.
-__device__ __forceinline__ void next_slot(const TileCtx& c, const TileSmem& sm, Slot& sl) {
-    if (sl.rem) {
-        const uint64_t nb = sl.b + 32;
-        const uint32_t two = (uint32_t)(sm.packed[(uint32_t)((nb >> 5) - c.word0)] >> (62 - 2 * (uint32_t)(nb & 31))) & 3u;
-        sl.window = (sl.window << 2) | two;
-        sl.b += 1;
-        sl.pos += 1;
-        sl.rem -= 1;
-    } else {
-        sl.read += 1;
-        sl.lo += 1;
-        sl.pos = 0;
-        sl.rem = c.uniform ? (uint64_t)(c.L1 - 1) : sm.off[sl.lo + 1] - sm.off[sl.lo];
-    }
-}
-
 // Partition code of a suffix (reading A4 of PAPER.md:79 "suffixes shorter than l require special
 // but easy handling"): (first l bases, A-padded) * (l + 1) + min(rem, l).  Order-preserving.
 __device__ __forceinline__ uint32_t bucket_of(const Slot& sl, uint32_t ell, uint32_t& kmer, uint32_t& r) {
     r = sl.rem < ell ? (uint32_t)sl.rem : ell;
     kmer = r ? (uint32_t)((sl.window >> (64 - 2 * r)) << (2 * (ell - r))) : 0u;
+    return kmer * (ell + 1) + r;
+}
+
+// Lean state for scans that only need the partition code of most slots (the multi-batch listing): stepping from a
+// suffix slot to the next one in (read, position) order needs no decoding from scratch -- inside a read the 32-base
+// window shifts by one base taken from the 32 bases after it (both in registers: four shifts, no shared-memory
+// access); after a read's end-marker slot the next read starts at the same base index, so the window stays.
+struct Walk {
+    uint64_t window, ahead;   // bases [b, b + 32) and [b + 32, b + 64), MSB-first
+    uint32_t rem;             // bases left in the read from this slot
+    uint32_t lo;              // read - r0
+};
+__device__ __forceinline__ Walk walk_init(const TileCtx& c, const TileSmem& sm, uint32_t s) {
+    const Slot sl = decode_slot(c, sm, s);
+    Walk wk;
+    wk.window = sl.window;
+    wk.rem = (uint32_t)sl.rem;
+    wk.lo = sl.lo;
+    const uint64_t nb = sl.b + 32;
+    const uint32_t wi = (uint32_t)((nb >> 5) - c.word0);
+    const uint32_t sh = (uint32_t)(nb & 31) * 2;
+    const uint64_t w0 = sm.packed[wi], w1 = sm.packed[wi + 1];
+    wk.ahead = sh ? (w0 << sh) | (w1 >> (64 - sh)) : w0;
+    return wk;
+}
+// valid for at most 32 steps after walk_init (the scans take kListItems = 8)
+__device__ __forceinline__ void walk_next(const TileCtx& c, const TileSmem& sm, Walk& wk) {
+    if (wk.rem) {
+        wk.window = (wk.window << 2) | (wk.ahead >> 62);
+        wk.ahead <<= 2;
+        wk.rem -= 1;
+    } else {   // end-marker slot: the next read starts at the same base index
+        wk.lo += 1;
+        wk.rem = c.uniform ? c.L1 - 1 : (uint32_t)(sm.off[wk.lo + 1] - sm.off[wk.lo]);
+    }
+}
+__device__ __forceinline__ uint32_t walk_bucket(const Walk& wk, uint32_t ell) {
+    const uint32_t hi = (uint32_t)(wk.window >> 32);
+    const uint32_t r = wk.rem < ell ? wk.rem : ell;
+    const uint32_t kmer = r ? (hi >> (32 - 2 * r)) << (2 * (ell - r)) : 0u;
     return kmer * (ell + 1) + r;
 }
 
@@ -258,19 +278,18 @@ __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const
         uint64_t mine = 0;   // eight 8-bit counters
         const uint32_t s0 = threadIdx.x * kListItems;
         if (s0 < c.n_slots) {
-            Slot sl = decode_slot(c, sm, s0);
+            Walk wk = walk_init(c, sm, s0);
 #pragma unroll
             for (int i = 0; i < kListItems; ++i) {
                 if (s0 + i < c.n_slots) {
-                    uint32_t kmer, r;
-                    const uint32_t b = bucket_of(sl, ell, kmer, r);
+                    const uint32_t b = walk_bucket(wk, ell);
                     if (b >= ranges.first[0] && b < ranges.first[ranges.n]) {
                         uint32_t j = 0;
 #pragma unroll
                         for (int q = 1; q < kCountGroup; ++q) j += (q < (int)ranges.n && b >= ranges.first[q]);
                         mine += 1ull << (8 * j);
                     }
-                    if (s0 + i + 1 < c.n_slots) next_slot(c, sm, sl);
+                    if (s0 + i + 1 < c.n_slots) walk_next(c, sm, wk);
                 }
             }
         }
@@ -313,14 +332,13 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
         const uint32_t s0 = threadIdx.x * kListItems;
         uint32_t mask = 0;   // which of my kListItems consecutive slots belong to this batch
         if (s0 < c.n_slots) {
-            Slot sl = decode_slot(c, sm, s0);
+            Walk wk = walk_init(c, sm, s0);
 #pragma unroll
             for (int i = 0; i < kListItems; ++i) {
                 if (s0 + i < c.n_slots) {
-                    uint32_t kmer, r;
-                    const uint32_t b = bucket_of(sl, ell, kmer, r);
-                    mask |= (uint32_t)(b >= bucket_lo && b <= bucket_hi) << i;
-                    if (s0 + i + 1 < c.n_slots) next_slot(c, sm, sl);
+                    const uint32_t b = walk_bucket(wk, ell);
+                    mask |= (uint32_t)(b - bucket_lo <= bucket_hi - bucket_lo) << i;
+                    if (s0 + i + 1 < c.n_slots) walk_next(c, sm, wk);
                 }
             }
         }
