@@ -159,6 +159,8 @@ extern "C" int cx_bwt_plan(cx_bwt_plan_t** plan_out, uint64_t max_reads, uint64_
     if (hi > kMaxBatch) hi = kMaxBatch;
     if (make_layout(sh, 1).total > workspace_bytes) return CX_ERR_WORKSPACE;
     uint64_t lo = 1;
+    // the largest legal input in one batch needs a smaller count table than any split does, so test it first
+    if (make_layout(sh, hi).total <= workspace_bytes) lo = hi;
     while (lo < hi) {
         uint64_t mid = lo + (hi - lo + 1) / 2;
         if (make_layout(sh, mid).total <= workspace_bytes) lo = mid; else hi = mid - 1;

@@ -183,6 +183,19 @@ def test_bad_offsets_and_oversize_input_are_reported_not_executed():
     assert e.value.code == cx.binding.CX_ERR_ARG
 
 
+def test_default_workspace_gives_one_batch():
+    """cx_bwt_workspace_bytes sizes the workspace for one batch; the plan must then really take one
+    (the listing scan that also counts partition sizes depends on it)."""
+    import paper_1401_7457_b200 as cx
+    c = gen.config(2, 0.002)
+    p = cx.Plan(c.n_reads, c.total_bases, max_read_len=100)
+    out = torch.empty(c.n_suffixes, dtype=torch.uint8, device="cuda")
+    p.build(cx.cx_pack_reads(torch.from_numpy(c.ascii).cuda()), torch.from_numpy(c.offsets.astype(np.int64)).cuda(), c.n_reads, out)
+    st = p.stats()
+    assert st["n_batches"] == 1 and st["max_batch"] == c.n_suffixes
+    assert np.array_equal(out.cpu().numpy(), oracle.bwt(c.ascii, c.offsets))
+
+
 def test_deterministic():
     c = gen.config(2, 0.001)
     assert np.array_equal(gpu_bwt(c), gpu_bwt(c))
