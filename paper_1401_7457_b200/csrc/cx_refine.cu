@@ -226,12 +226,14 @@ static_assert(kLocalElems % kLocalThreads == 0 && kLocalThreads % 32 == 0, "tile
 constexpr uint32_t kLocalW = 57;                            // bases per in-block round
 typedef unsigned __int128 u128;
 constexpr uint16_t kNone = 0xffff;
+constexpr int kSubBlock = 32;                               // members ranked by counting before runs are merged
 
 template <typename IdT>
 struct LocalSmem {
     u128 key[kLocalElems];      // [57 bases, A-padded : 114][min(remaining, 57) : 6][index inside the group : 8]
     IdT id_a[kLocalElems];
-    uint16_t src[kLocalElems];  // src[p] = member that ranks at position p after this round
+    uint16_t ord[2][kLocalElems];  // sorted order of the runs being merged, ping-pong; at the end of a round
+                                   // ord[cur][p] = member that ranks at position p
     uint16_t gs[kLocalElems];   // first position of the element's current group (kNone: not ours / placed)
     uint16_t ge[kLocalElems];   // one past its last position
     uint32_t hw[kLocalWords];   // head bits of the window, updated as groups split
@@ -407,33 +409,79 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
             }
         }
         if (!__syncthreads_or(any)) break;
-#pragma unroll 1
+        // Stable rank inside every group.  Members are first ranked by counting inside sub-blocks of kSubBlock
+        // consecutive members (<= kSubBlock comparisons each); sorted runs are then merged pairwise, each member
+        // finding its rank in the sibling run by binary search (keys are distinct: the group index is part of them),
+        // so a group of g members costs ~kSubBlock + log2(g / kSubBlock) * log2(g) comparisons per member, not g.
+        uint32_t myrank[kLocalItems];
+        uint32_t more = 0;   // some group of mine is longer than one sub-block
+        int cur = 0;
+#pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
             const int e = k * kLocalThreads + tid;
             const int s = sm.gs[e];
+            myrank[k] = 0;
             if (s != kNone) {
                 const int t = sm.ge[e];
+                const int b0 = s + ((e - s) / kSubBlock) * kSubBlock;
+                const int b1 = min(b0 + kSubBlock, t);
                 const uint4 my = reinterpret_cast<const uint4*>(sm.key)[e];
-                n_compares += (uint32_t)(t - s);
-                uint32_t neg = 0;   // minus the number of members whose key is below mine
+                n_compares += (uint32_t)(b1 - b0);
+                uint32_t neg = 0;   // minus the number of sub-block members whose key is below mine
 #pragma unroll 4
-                for (int q = s; q < t; ++q) count_if_less(neg, reinterpret_cast<const uint4*>(sm.key)[q], my);
-                sm.src[s - (int)neg] = (uint16_t)e;
+                for (int q = b0; q < b1; ++q) count_if_less(neg, reinterpret_cast<const uint4*>(sm.key)[q], my);
+                myrank[k] = 0u - neg;
+                sm.ord[0][b0 + myrank[k]] = (uint16_t)e;
+                more |= (uint32_t)(t - s > kSubBlock);
             }
         }
-        __syncthreads();
+        static_assert((kSubBlock & (kSubBlock - 1)) == 0, "runs double from a power of two");
+        for (int run = kSubBlock, sh = 31 - __clz(kSubBlock); __syncthreads_or(more); run *= 2, ++sh) {
+            more = 0;
+#pragma unroll
+            for (int k = 0; k < kLocalItems; ++k) {
+                const int e = k * kLocalThreads + tid;
+                const int s = sm.gs[e];
+                if (s == kNone) continue;
+                const int t = sm.ge[e];
+                const int r = (e - s) >> sh;             // my run, its sibling is r ^ 1
+                uint32_t nr = myrank[k];
+                if (t - s > run) {
+                    const int sb = s + (r ^ 1) * run;    // sibling run [sb, sb + len)
+                    if (sb < t) {
+                        const uint4 my = reinterpret_cast<const uint4*>(sm.key)[e];
+                        int lo = 0, hi = min(run, t - sb);
+                        n_compares += 32 - __clz(hi);
+                        while (lo < hi) {                // lower bound: sibling members below me
+                            const int mid = (lo + hi) >> 1;
+                            uint32_t neg = 0;
+                            count_if_less(neg, reinterpret_cast<const uint4*>(sm.key)[sm.ord[cur][sb + mid]], my);
+                            if (neg) lo = mid + 1; else hi = mid;
+                        }
+                        nr += (uint32_t)lo;
+                    }
+                    myrank[k] = nr;
+                    sm.ord[cur ^ 1][s + (r >> 1) * 2 * run + nr] = (uint16_t)e;
+                    more |= (uint32_t)(t - s > 2 * run);
+                } else {
+                    sm.ord[cur ^ 1][s + nr] = (uint16_t)e;   // already one run: carried over
+                }
+            }
+            cur ^= 1;
+        }
+        const uint16_t* src = sm.ord[cur];
         IdT idn[kLocalItems];
         uint32_t headbit = 0;
 #pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
             const int e = k * kLocalThreads + tid;
             if (sm.gs[e] != kNone) {
-                const int se = sm.src[e];
+                const int se = src[e];
                 const uint4 kk = reinterpret_cast<const uint4*>(sm.key)[se];
                 idn[k] = sm.id_a[se];
                 bool head = e == sm.gs[e] || ((kk.x >> 8) & 63u) < kLocalW;
                 if (!head) {   // same bases and length as the member ranked just before?  (the low 8 bits are the group index)
-                    const uint4 kp = reinterpret_cast<const uint4*>(sm.key)[sm.src[e - 1]];
+                    const uint4 kp = reinterpret_cast<const uint4*>(sm.key)[src[e - 1]];
                     head = ((((kk.x ^ kp.x) >> 8) | (kk.y ^ kp.y)) | ((kk.z ^ kp.z) | (kk.w ^ kp.w))) != 0;
                 }
                 headbit |= (uint32_t)head << k;
