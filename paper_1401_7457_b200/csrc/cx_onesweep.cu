@@ -363,10 +363,11 @@ cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, u
     *result_in_alt = 0;
     if (n <= 1 || end_bit <= begin_bit) return cudaSuccess;
     constexpr int ITEMS = SortShape<KeyT, ValT>::items;
-    // keys-only (packed 32-bit key | id): 512 threads x 16 = 8192 words per tile, 2 blocks per SM (measured best of
-    // 256x16x4, 512x16x2, 256x32x2, 384x16x2, 512x8x3, 1024x8x2, 1024x16x1: 1.95 ms against 2.03-3.1 ms for 4 passes at C2)
+    // keys-only (packed 32-bit key | id): 384 threads x 16 = 6144 words per tile, 3 blocks per SM, 56 registers.  Measured
+    // at C2 (4 passes, ms): 384x16x3 1.91, 512x16x2 1.96, 256x24x3 2.00, 256x16x4 2.03; shapes that need register caps
+    // to fit more blocks (256x16x5/6, 512x16x3) spill and lose: 2.29-2.52.
     if constexpr (sizeof(ValT) < 4)
-        return sort_pairs_shape<KeyT, ValT, 512, 16, 2>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready);
+        return sort_pairs_shape<KeyT, ValT, 384, 16, 3>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready);
     return sort_pairs_shape<KeyT, ValT, kSortThreads, ITEMS, 4>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready);
 }
 
