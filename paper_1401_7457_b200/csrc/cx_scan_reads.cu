@@ -2,7 +2,10 @@
 //   prep        offsets sanity, longest read, uniform-length test
 //   tile table  first read of every tile of kListTile consecutive suffix slots
 //   a2 bucket histogram   (Fig. 2 step 1: "Scan all suffixes ... Store the size of each partition")
-//   a4+a5 list + key build (Fig. 2 steps 3(a), 3(c)i; key = the paper's "stringword")
+//   a4+a5 list + key build (Fig. 2 steps 3(a), 3(c)i; key = the paper's "stringword"):
+//         list_write   the whole collection as one batch (also counts the partition sizes on the way)
+//         list_count   per tile, the suffixes of eight consecutive batches in one scan (fewer scans)
+//         list_select  one batch of several: the suffixes whose partition lies in the batch's range
 //
 // A suffix slot g in [0, N) is suffix (i, p) with g = offsets[i] + i + p: reads laid end to end, each
 // followed by one slot for its end-marker.  Slots ascend in (read, position) order, which is the
@@ -72,7 +75,6 @@ __global__ void __launch_bounds__(256) tile_table_kernel(const uint64_t* __restr
 struct TileSmem {
     uint64_t off[kListTile + 2];           // offsets of the reads that intersect the tile
     uint64_t packed[kListTile / 32 + 4];   // the bases of the tile plus one window of look-ahead
-    uint32_t scan[kListItems * (kListThreads / 32) + 1];
 };
 
 struct TileCtx {
@@ -378,24 +380,22 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
 }
 
 // ---------------------------------------------------------------------------------------------
-// a4 (write half) + a5: ids of the batch in (read, pos) order, each with its first key.
-// The read is in shared memory already, so the round-1 key costs no gather.
+// a4 + a5 (+ a2) for a build that takes the whole collection in one batch: every suffix in (read, pos)
+// order, index = slot, each with its first key.  The read is in shared memory already, so the round-1
+// key costs no gather.  The same scan builds the digit histograms of the sort that follows and, when
+// bucket_hist != nullptr, the partition sizes (as bucket_hist_kernel does): the collection is read once.
+// PACKED (32-bit key and id only): one 64-bit word (key << 32 | id) per suffix goes to `keys`, nothing to
+// `ids`; the sort is then keys-only over bits [32, 64) and the id travels with its key for free.
 // ---------------------------------------------------------------------------------------------
-// PACKED (32-bit key and id only): one 64-bit word (key << 32 | id) per suffix goes to `keys`, nothing to `ids`;
-// the sort is then keys-only over bits [32, 64) and the id travels with its key for free.
-template <typename KeyT, typename IdT, bool ALL, bool PACKED>
+template <typename KeyT, typename IdT, bool PACKED>
 __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const BuildInfo* __restrict__ info,
                                                                   const uint32_t* __restrict__ tile_first_read, uint32_t ell, uint32_t w,
-                                                                  uint32_t bucket_lo, uint32_t bucket_hi,
-                                                                  const uint64_t* __restrict__ tile_base, KeyT* __restrict__ keys,
-                                                                  IdT* __restrict__ ids, uint32_t n_passes,
+                                                                  KeyT* __restrict__ keys, IdT* __restrict__ ids, uint32_t n_passes,
                                                                   unsigned long long* __restrict__ digit_hist,
                                                                   unsigned long long* __restrict__ bucket_hist, uint64_t max_n) {
     __shared__ TileSmem sm;
     __shared__ uint32_t s_dh[8][kRadix];   // digit counts of every radix pass of the sort that follows (a6's upfront histogram)
-    // bucket_hist != nullptr (ALL only): this scan also counts the partition sizes (a2), as bucket_hist_kernel does, so that a
-    // build that is known to fit one batch reads the collection once
-    extern __shared__ uint32_t s_bh[];
+    extern __shared__ uint32_t s_bh[];     // partition counters, laid out as in bucket_hist_kernel
     const uint32_t n_kmers = 1u << (2 * ell), n_short = (n_kmers - 1) / 3;
     if (bucket_hist)
         for (uint32_t k = threadIdx.x; k < n_kmers + n_short; k += blockDim.x) s_bh[k] = 0;
@@ -403,97 +403,31 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
     const uint64_t N = info->n_suffixes;
     if (N > max_n || info->bad_offsets) return;   // the host reports both after reading `info`
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
-    const uint32_t warp = threadIdx.x >> 5;
-    constexpr int kWarps = kListThreads / 32;
     const uint32_t len_bits = key_len_bits(w);
     for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) (&s_dh[0][0])[i] = 0;
 
     for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
         __syncthreads();   // previous tile done with sm
         TileCtx c = load_tile(R, info, tile_first_read, t, n_tiles, N, sm);
-        KeyT key[kListItems];
-        IdT id[kListItems];
-        uint32_t rank[kListItems];
-        bool take[kListItems];
 #pragma unroll
         for (int k = 0; k < kListItems; ++k) {
-            uint32_t s = k * kListThreads + threadIdx.x;
-            take[k] = false;
-            key[k] = 0;
-            id[k] = 0;
-            rank[k] = 0;
-            if (s < c.n_slots) {
-                Slot sl = decode_slot(c, sm, s);
-                if (ALL) {
-                    take[k] = true;
-                    if (bucket_hist) {
-                        uint32_t kmer, r;
-                        bucket_of(sl, ell, kmer, r);
-                        if (r == ell) atomicAdd(&s_bh[kmer], 1u);
-                        else atomicAdd(&s_bh[n_kmers + (((1u << (2 * r)) - 1) / 3) + (kmer >> (2 * (ell - r)))], 1u);
-                    }
-                } else {
-                    uint32_t kmer, r;
-                    uint32_t b = bucket_of(sl, ell, kmer, r);
-                    take[k] = b >= bucket_lo && b <= bucket_hi;
-                }
-                if (take[k]) {   // most suffixes of a multi-batch scan belong to other batches: no key, no id for them
-                    key[k] = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
-                    id[k] = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
-                }
+            const uint32_t s = k * kListThreads + threadIdx.x;
+            if (s >= c.n_slots) continue;
+            const Slot sl = decode_slot(c, sm, s);
+            if (bucket_hist) {
+                uint32_t kmer, r;
+                bucket_of(sl, ell, kmer, r);
+                if (r == ell) atomicAdd(&s_bh[kmer], 1u);
+                else atomicAdd(&s_bh[n_kmers + (((1u << (2 * r)) - 1) / 3) + (kmer >> (2 * (ell - r)))], 1u);
             }
-            if (take[k]) {
-                for (uint32_t p = 0; p < n_passes; ++p) atomicAdd(&s_dh[p][(uint32_t)(key[k] >> (p * kRadixBits)) & (kRadix - 1)], 1u);
-            }
-            if (!ALL) {
-                uint32_t m = __ballot_sync(0xffffffffu, take[k]);
-                rank[k] = __popc(m & lanemask_lt());
-                if (lane_id() == 0) sm.scan[k * kWarps + warp] = __popc(m);
-            }
-        }
-        if (ALL) {
-#pragma unroll
-            for (int k = 0; k < kListItems; ++k) {
-                uint32_t s = k * kListThreads + threadIdx.x;
-                if (take[k]) {
-                    if constexpr (PACKED) {
-                        reinterpret_cast<uint64_t*>(keys)[c.g0 + s] = ((uint64_t)key[k] << 32) | (uint64_t)id[k];
-                    } else {
-                        keys[c.g0 + s] = key[k];
-                        ids[c.g0 + s] = id[k];
-                    }
-                }
-            }
-            continue;
-        }
-        __syncthreads();
-        // exclusive scan of the kListItems * kWarps row counts (slot order = item-major, then warp)
-        if (threadIdx.x < 32) {
-            uint32_t carry = 0;
-            for (int base = 0; base < kListItems * kWarps; base += 32) {
-                uint32_t idx = base + threadIdx.x;
-                uint32_t v = idx < kListItems * kWarps ? sm.scan[idx] : 0;
-                uint32_t incl = v;
-                for (int o = 1; o < 32; o <<= 1) {
-                    uint32_t up = __shfl_up_sync(0xffffffffu, incl, o);
-                    if ((int)threadIdx.x >= o) incl += up;
-                }
-                if (idx < kListItems * kWarps) sm.scan[idx] = carry + incl - v;
-                carry += __shfl_sync(0xffffffffu, incl, 31);
-            }
-        }
-        __syncthreads();
-        const uint64_t base = tile_base[t];
-#pragma unroll
-        for (int k = 0; k < kListItems; ++k) {
-            if (take[k]) {
-                uint64_t dst = base + sm.scan[k * kWarps + warp] + rank[k];
-                if constexpr (PACKED) {
-                    reinterpret_cast<uint64_t*>(keys)[dst] = ((uint64_t)key[k] << 32) | (uint64_t)id[k];
-                } else {
-                    keys[dst] = key[k];
-                    ids[dst] = id[k];
-                }
+            const KeyT key = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
+            const IdT id = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
+            for (uint32_t p = 0; p < n_passes; ++p) atomicAdd(&s_dh[p][(uint32_t)(key >> (p * kRadixBits)) & (kRadix - 1)], 1u);
+            if constexpr (PACKED) {
+                reinterpret_cast<uint64_t*>(keys)[c.g0 + s] = ((uint64_t)key << 32) | (uint64_t)id;
+            } else {
+                keys[c.g0 + s] = key;
+                ids[c.g0 + s] = id;
             }
         }
     }
@@ -585,10 +519,10 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
             cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bucket_hist_smem(7) - sizeof(TileSmem)));
             if (e != cudaSuccess) return e;
         }
-        kernel<<<grid, kListThreads, smem, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids, n_passes, dh, bh, max_n);
+        kernel<<<grid, kListThreads, smem, s>>>(R, info, tile_first_read, ell, w, keys, ids, n_passes, dh, bh, max_n);
         return cudaGetLastError();
     };
-    if (tile_base == nullptr) return packed ? launch(list_write_kernel<KeyT, IdT, true, kCanPack>) : launch(list_write_kernel<KeyT, IdT, true, false>);
+    if (tile_base == nullptr) return packed ? launch(list_write_kernel<KeyT, IdT, kCanPack>) : launch(list_write_kernel<KeyT, IdT, false>);
     if (packed)
         list_select_kernel<KeyT, IdT, kCanPack><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids,
                                                                              n_passes, dh);
