@@ -36,8 +36,8 @@ enum {
                                      starting at 0 or decreasing */
     CX_ERR_BAD_BASE = -2,         /* cx_pack_reads saw a byte outside "ACGT" (reads are ACGT only) */
     CX_ERR_WORKSPACE = -3,        /* workspace too small for even one bucket-sized batch */
-    CX_ERR_BUCKET_TOO_LARGE = -4, /* one l-prefix partition exceeds m1; the paper refines it recursively
-                                     (Fig. 2 step 1) -- not built yet, reported instead */
+    CX_ERR_BUCKET_TOO_LARGE = -4, /* a partition still exceeds m1 after refining it by its next l characters down to
+                                     2^20 bases (Fig. 2 step 1); not reachable with sane inputs */
     CX_ERR_CUDA = -5,             /* CUDA runtime error (or no device); text via cx_strerror */
     CX_ERR_NOMEM = -6             /* host allocation failed */
 };
@@ -74,6 +74,7 @@ typedef struct cx_bwt_stats_s {
     uint32_t refine_rounds;     /* global refinement rounds, max over batches                           */
     uint32_t max_read_len;      /* longest read seen                                                    */
     uint32_t uniform_len;       /* 1 if every read has the same length (the paper's setting)*/
+    uint32_t refined_partitions;/* l-prefix partitions larger than m1 that were partitioned again */
 } cx_bwt_stats_t;
 
 /* Kernel classes for cx_bwt_kernel_time; one per row of the hot path. */

@@ -3,6 +3,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <functional>
 #include <new>
 #include <vector>
 
@@ -35,21 +36,35 @@ uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
 
 constexpr uint64_t kMaxBatch = 0xFFFF0000ull;   // positions inside a batch are 32-bit
 
-struct Batch {
-    uint32_t bucket_lo, bucket_hi;
-    uint64_t count, out_offset;
+// A region on the host: the partition prefix it stands for (an oversize partition is partitioned again by
+// its next l characters, recursively).  Region 0 is the whole collection.
+struct RegionHost {
+    uint32_t depth = 0;
+    std::vector<uint64_t> prefix;   // depth bases, 2 bit/base, MSB-first words
 };
+
+struct Batch {
+    uint32_t bucket_lo, bucket_hi;   // partitions (codes at the region's depth) sorted together
+    uint64_t count, out_offset;
+    uint32_t region;                 // index into the plan's regions
+    uint64_t ord_lo, ord_hi;         // slice of the listing order taken (a partition of identical suffixes cut into batches)
+    uint32_t col;                    // column of the per-tile count table that holds this batch's counts
+    bool count_here, scan_here;      // this batch launches the counting scan of its group / scans its column
+    CountRanges ranges;              // the group counted when count_here
+};
+
+constexpr uint32_t kMaxRegionDepth = 1u << 20;   // bases; deeper refinement is reported as CX_ERR_BUCKET_TOO_LARGE
 
 // Byte offsets of every region of the workspace for a given m1.
 struct Layout {
-    uint64_t info, hist, tile_first, tile_count, tile_sums, scalars;
+    uint64_t info, hist, tile_first, tile_count, tile_sums, scalars, prefix;
     uint64_t keys[2], ids[3], pos, heads[2], word_counts, word_sums, sort, stage[2];
     uint64_t total;
 };
 
 struct Shape {
     uint64_t max_reads, max_bases, max_suffixes, max_tiles;
-    uint32_t ell, w, cap, id_bytes, pos_bits;
+    uint32_t ell, w, cap, id_bytes, pos_bits, prefix_words;
     uint64_t n_buckets;
     bool host_out;
 };
@@ -69,6 +84,7 @@ Layout make_layout(const Shape& sh, uint64_t m1) {
     L.tile_count = take((sh.max_tiles + 1) * 8 * (sh.max_suffixes <= m1 ? 1 : kCountGroup));
     L.tile_sums = take((scan_block_count(sh.max_tiles + 1) + 1) * 8);
     L.scalars = take(64);
+    L.prefix = take((uint64_t)(sh.prefix_words) * 8);
     for (int i = 0; i < 2; ++i) L.keys[i] = take(m1 * 8);
     for (int i = 0; i < 3; ++i) L.ids[i] = take(m1 * sh.id_bytes);
     L.pos = take(m1 * 4);
@@ -99,6 +115,7 @@ int make_shape(uint64_t max_reads, uint64_t max_bases, const cx_bwt_opts_t* o, S
     uint64_t max_len = o->max_read_len ? o->max_read_len : max_bases;
     if (max_len > max_bases) max_len = max_bases;
     sh.pos_bits = bit_width64(max_len);
+    sh.prefix_words = (uint32_t)((max_len < kMaxRegionDepth ? max_len : kMaxRegionDepth) / 32 + 2);   // region prefix of a refined partition
     uint32_t read_bits = bit_width64(max_reads ? max_reads - 1 : 0);
     if (sh.pos_bits + read_bits > 64) return CX_ERR_ARG;
     sh.id_bytes = sh.pos_bits + read_bits <= 32 ? 4 : 8;
@@ -123,6 +140,8 @@ struct cx_bwt_plan_s {
     uint64_t* h_scalars;
     uint64_t* h_hist;
     std::vector<Batch> batches;
+    std::vector<RegionHost> regions;
+    uint64_t* h_hist2;   // pinned: sizes of the sub-partitions of the partition being refined
     Launch prof;
     cx_bwt_stats_t stats;
     cudaStream_t copy_stream;
@@ -200,7 +219,7 @@ extern "C" int cx_bwt_plan(cx_bwt_plan_t** plan_out, uint64_t max_reads, uint64_
     p->copy_stream = nullptr;
     p->emit_done = p->stage_free[0] = p->stage_free[1] = nullptr;
 
-    size_t host_bytes = sizeof(BuildInfo) + 64 + sh.n_buckets * 8;
+    size_t host_bytes = sizeof(BuildInfo) + 64 + 2 * sh.n_buckets * 8;
     cudaError_t e = cudaMallocHost((void**)&p->h_pinned, host_bytes);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->emit_done, cudaEventDisableTiming);
@@ -216,6 +235,7 @@ extern "C" int cx_bwt_plan(cx_bwt_plan_t** plan_out, uint64_t max_reads, uint64_
     p->h_info = reinterpret_cast<BuildInfo*>(p->h_pinned);
     p->h_scalars = reinterpret_cast<uint64_t*>(p->h_pinned + sizeof(BuildInfo));
     p->h_hist = reinterpret_cast<uint64_t*>(p->h_pinned + sizeof(BuildInfo) + 64);
+    p->h_hist2 = p->h_hist + sh.n_buckets;
     sort_workspace_carve(p->sort, p->ws + p->L.sort, lo);
     *plan_out = p;
     return CX_OK;
@@ -262,7 +282,7 @@ extern "C" const char* cx_strerror(int code) {
     case CX_ERR_ARG: return "invalid argument (null pointer, bad option, size above the plan's maximum, or bad offsets)";
     case CX_ERR_BAD_BASE: return "input contains a byte outside ACGT";
     case CX_ERR_WORKSPACE: return "workspace too small";
-    case CX_ERR_BUCKET_TOO_LARGE: return "one prefix partition exceeds the batch limit m1 (recursive refinement not built)";
+    case CX_ERR_BUCKET_TOO_LARGE: return "a partition still exceeds the batch limit m1 after refinement to the depth limit";
     case CX_ERR_CUDA: return g_cuda_msg;
     case CX_ERR_NOMEM: return "host allocation failed";
     default: return "unknown error code";
@@ -296,41 +316,109 @@ extern "C" int cx_bwt_kernel_time(const cx_bwt_plan_t* p, int cls, double* ms_ou
 // ---------------------------------------------------------------------------------------------
 namespace {
 
-// Fig. 2 steps 2 and 3(b) ("merging a consecutive range of partitions"):
-// greedy ranges of consecutive partitions with total size <= m1.
-int plan_batches(cx_bwt_plan_t* p, uint64_t N) {
-    p->batches.clear();
-    const uint64_t nb = p->sh.n_buckets;
-    uint64_t largest = 0, out = 0;
-    Batch cur{0, 0, 0, 0};
+// Fig. 2 steps 1, 2 and 3(b): consecutive partitions are merged into batches of total size
+// <= m1; a partition larger than m1 is "further partition[ed] by looking at the next l characters ... recursively":
+// its sub-partition sizes come from `sub_hist` (a device scan confined to the partition's region) and are planned the
+// same way, in place, so that batches stay in BWT order.  A partition of suffixes that END inside the prefix holds
+// identical strings, whose order is the listing order: it is simply cut into slices of that order.
+struct Planner {
+    cx_bwt_plan_t* p;
+    std::function<int(uint32_t, uint64_t*)> sub_hist;   // sizes of the sub-partitions of region #i into p->h_hist2-sized array
+    uint64_t out = 0;
+    Batch cur{};
     bool open = false;
-    for (uint64_t b = 0; b < nb; ++b) {
-        uint64_t c = p->h_hist[b];
-        if (c == 0) continue;
-        if (c > largest) largest = c;
-        if (c > p->m1) {
-            p->stats.largest_bucket = largest;
-            return CX_ERR_BUCKET_TOO_LARGE;
-        }
-        if (open && cur.count + c > p->m1) {
-            p->batches.push_back(cur);
-            out += cur.count;
-            open = false;
-        }
-        if (!open) {
-            cur = Batch{(uint32_t)b, (uint32_t)b, 0, out};
-            open = true;
-        }
-        cur.bucket_hi = (uint32_t)b;
-        cur.count += c;
-    }
-    if (open) {
+
+    void flush() {
+        if (!open) return;
         p->batches.push_back(cur);
         out += cur.count;
+        open = false;
     }
-    p->stats.largest_bucket = largest;
-    return out == N ? CX_OK : CX_ERR_CUDA;   // a mismatch means the histogram kernel misbehaved
-}
+    int region(uint32_t ri, const uint64_t* hist, bool top) {
+        const Shape& sh = p->sh;
+        const uint64_t nb = sh.n_buckets, m1 = p->m1;
+        for (uint64_t b = 0; b < nb; ++b) {
+            const uint64_t c = hist[b];
+            if (c == 0) continue;
+            if (top && c > p->stats.largest_bucket) p->stats.largest_bucket = c;
+            if (c > m1) {
+                flush();
+                const uint32_t r = (uint32_t)(b % (sh.ell + 1)), kmer = (uint32_t)(b / (sh.ell + 1));
+                if (r < sh.ell) {   // identical suffixes: slices of the listing order
+                    for (uint64_t k0 = 0; k0 < c; k0 += m1) {
+                        const uint64_t n = c - k0 < m1 ? c - k0 : m1;
+                        Batch s{};
+                        s.bucket_lo = s.bucket_hi = (uint32_t)b;
+                        s.count = n, s.out_offset = out, s.region = ri, s.ord_lo = k0, s.ord_hi = k0 + n;
+                        p->batches.push_back(s);
+                        out += n;
+                    }
+                } else {            // refine by the next l characters
+                    const uint32_t depth = p->regions[ri].depth, child_depth = depth + sh.ell;
+                    if (child_depth > kMaxRegionDepth || (child_depth + 31) / 32 + 1 > sh.prefix_words) return CX_ERR_BUCKET_TOO_LARGE;
+                    RegionHost child;
+                    child.depth = child_depth;
+                    child.prefix = p->regions[ri].prefix;
+                    child.prefix.resize((child_depth + 31) / 32 + 1, 0ull);
+                    for (uint32_t i = 0; i < sh.ell; ++i) {
+                        const uint64_t code = (kmer >> (2 * (sh.ell - 1 - i))) & 3u;
+                        const uint32_t j = depth + i;
+                        child.prefix[j / 32] |= code << (62 - 2 * (j % 32));
+                    }
+                    p->regions.push_back(child);
+                    const uint32_t ci = (uint32_t)p->regions.size() - 1;
+                    std::vector<uint64_t> h(nb);
+                    int rc = sub_hist(ci, h.data());
+                    if (rc) return rc;
+                    uint64_t total = 0;
+                    for (uint64_t q = 0; q < nb; ++q) total += h[q];
+                    if (total != c) return CX_ERR_CUDA;   // the region scan and the partition scan disagree
+                    p->stats.refined_partitions += 1;
+                    rc = region(ci, h.data(), false);
+                    if (rc) return rc;
+                    flush();
+                }
+                continue;
+            }
+            if (open && cur.count + c > m1) flush();
+            if (!open) {
+                cur = Batch{};
+                cur.bucket_lo = (uint32_t)b, cur.out_offset = out, cur.region = ri, cur.ord_lo = 0, cur.ord_hi = ~0ull;
+                open = true;
+            }
+            cur.bucket_hi = (uint32_t)b;
+            cur.count += c;
+        }
+        flush();
+        return CX_OK;
+    }
+    // which batch launches the counting scan, which column of the count table each batch reads
+    void assign_count_groups() {
+        std::vector<Batch>& B = p->batches;
+        for (size_t i = 0; i < B.size();) {
+            if (B[i].ord_hi != ~0ull) {   // slices of one partition share one counted and scanned column
+                size_t j = i;
+                while (j < B.size() && B[j].ord_hi != ~0ull && B[j].region == B[i].region && B[j].bucket_lo == B[i].bucket_lo) {
+                    B[j].col = 0, B[j].count_here = B[j].scan_here = (j == i);
+                    ++j;
+                }
+                B[i].ranges.n = 1, B[i].ranges.first[0] = B[i].bucket_lo, B[i].ranges.first[1] = B[i].bucket_lo + 1;
+                i = j;
+                continue;
+            }
+            size_t j = i;
+            CountRanges cr{};
+            while (j < B.size() && cr.n < (uint32_t)kCountGroup && B[j].ord_hi == ~0ull && B[j].region == B[i].region) {
+                B[j].col = cr.n, B[j].count_here = (j == i), B[j].scan_here = true;
+                cr.first[cr.n++] = B[j].bucket_lo;
+                ++j;
+            }
+            cr.first[cr.n] = B[j - 1].bucket_hi + 1;
+            B[i].ranges = cr;
+            i = j;
+        }
+    }
+};
 
 template <typename KeyT, typename IdT>
 int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets, uint64_t n_reads, uint8_t* out, cudaStream_t s) {
@@ -382,10 +470,10 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         CX_CUDA(cudaMemsetAsync(p->sort.hist, 0, (size_t)n_passes * kRadix * sizeof(uint64_t), s));
         ScopedLaunch sl(prof, CX_K_LIST, 0, s);
         CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, 0, 0, nullptr, d_keys1[0], d_ids[0], sh.max_tiles, n_passes,
-                                              p->sort.hist, p->n_sms, pack_kv, d_hist, p->m1, s)));
+                                              p->sort.hist, p->n_sms, pack_kv, d_hist, p->m1, Region{}, 0, ~0ull, s)));
     } else {
         ScopedLaunch sl(prof, CX_K_HIST, 0, s);
-        CX_CUDA(launch_bucket_hist(R, d_info, d_tile_first, sh.ell, d_hist, sh.max_tiles, p->n_sms, s));
+        CX_CUDA(launch_bucket_hist(R, d_info, d_tile_first, sh.ell, Region{}, d_hist, sh.max_tiles, p->n_sms, s));
     }
     CX_CUDA(cudaMemcpyAsync(p->h_info, d_info, sizeof(BuildInfo), cudaMemcpyDeviceToHost, s));
     CX_CUDA(cudaMemcpyAsync(p->h_hist, d_hist, sh.n_buckets * 8, cudaMemcpyDeviceToHost, s));
@@ -405,18 +493,49 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     p->stats.uniform_len = R.uniform;
     p->built = true;
 
-    // ---- steps 2, 3(b): batch ranges -----------------------------------------------------------
-    int rc = plan_batches(p, N);
+    // ---- steps 1-2, 3(b): batch ranges, oversize partitions refined by their next l characters ----------
+    uint64_t* d_prefix = reinterpret_cast<uint64_t*>(ws + L.prefix);
+    uint32_t region_on_device = 0;   // region 0 (depth 0) needs no prefix
+    auto use_region = [&](uint32_t ri, Region& dev) -> cudaError_t {
+        const RegionHost& rh = p->regions[ri];
+        dev.prefix = d_prefix;
+        dev.depth = rh.depth;
+        if (rh.depth == 0 || ri == region_on_device) return cudaSuccess;
+        region_on_device = ri;
+        return cudaMemcpyAsync(d_prefix, rh.prefix.data(), rh.prefix.size() * 8, cudaMemcpyHostToDevice, s);   // pageable: staged at once
+    };
+    p->regions.clear();
+    p->regions.push_back(RegionHost{});
+    p->batches.clear();
+    Planner planner{p, nullptr};
+    planner.sub_hist = [&](uint32_t ri, uint64_t* hist_out) -> int {
+        Region dev{};
+        CX_CUDA(use_region(ri, dev));
+        CX_CUDA(cudaMemsetAsync(d_hist, 0, sh.n_buckets * 8, s));
+        {
+            ScopedLaunch sl(prof, CX_K_HIST, info.total_bases / 4 + (n_reads + 1) * 8, s);
+            CX_CUDA(launch_bucket_hist(R, d_info, d_tile_first, sh.ell, dev, d_hist, sh.max_tiles, p->n_sms, s));
+        }
+        CX_CUDA(cudaMemcpyAsync(p->h_hist2, d_hist, sh.n_buckets * 8, cudaMemcpyDeviceToHost, s));
+        CX_CUDA(cudaStreamSynchronize(s));
+        memcpy(hist_out, p->h_hist2, sh.n_buckets * 8);
+        return CX_OK;
+    };
+    int rc = planner.region(0, p->h_hist, true);
     if (rc) return rc;
+    if (planner.out != N) return CX_ERR_CUDA;   // a mismatch means the partition scan misbehaved
+    planner.assign_count_groups();
     p->stats.n_batches = (uint32_t)p->batches.size();
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
-    const bool single = p->batches.size() == 1;
+    const bool single = p->batches.size() == 1 && p->batches[0].ord_hi == ~0ull;
     if (fused_scan && !single) return CX_ERR_CUDA;   // cannot happen: N <= max_suffixes <= m1
     p->stats.sort_passes = (key_bits + kRadixBits - 1) / kRadixBits;
 
     for (size_t bi = 0; bi < p->batches.size(); ++bi) {
         const Batch& B = p->batches[bi];
         const uint64_t nb = B.count;
+        Region region{};
+        const uint32_t depth_base = p->regions[B.region].depth;   // symbols every suffix of the batch shares
         // ---- step 3(a) + 3(c)i: list the batch's suffixes with their first keys ----------------
         if (!fused_scan) CX_CUDA(cudaMemsetAsync(p->sort.hist, 0, (size_t)n_passes * kRadix * sizeof(uint64_t), s));
         if (fused_scan) {
@@ -424,25 +543,25 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         } else if (single) {
             ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (sizeof(KeyT) + sizeof(IdT)), s);
             CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, nullptr, d_keys1[0],
-                                                  d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, nullptr, ~0ull, s)));
+                                                  d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, nullptr, ~0ull, Region{}, 0, ~0ull,
+                                                  s)));
         } else {
             const uint64_t col_stride = sh.max_tiles + 1;
-            if (bi % kCountGroup == 0) {   // one scan counts this batch and the next seven
-                CountRanges cr{};
-                for (size_t q = bi; q < p->batches.size() && cr.n < (uint32_t)kCountGroup; ++q) cr.first[cr.n++] = p->batches[q].bucket_lo;
-                cr.first[cr.n] = p->batches[bi + cr.n - 1].bucket_hi + 1;
-                ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + n_tiles * 8 * cr.n, s);
-                CX_CUDA(launch_list_count(R, d_info, d_tile_first, sh.ell, cr, d_tile_count, col_stride, n_tiles, s));
+            CX_CUDA(use_region(B.region, region));
+            if (B.count_here) {   // one scan counts this batch and up to seven that follow it in the same region
+                ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + n_tiles * 8 * B.ranges.n, s);
+                CX_CUDA(launch_list_count(R, d_info, d_tile_first, sh.ell, region, B.ranges, d_tile_count, col_stride, n_tiles, s));
             }
-            uint64_t* d_col = d_tile_count + (bi % kCountGroup) * col_stride;
-            {
+            uint64_t* d_col = d_tile_count + B.col * col_stride;
+            if (B.scan_here) {
                 ScopedLaunch sl(prof, CX_K_LIST, n_tiles * 16, s);
                 CX_CUDA(launch_scan_u64(d_col, n_tiles, d_tile_sums, d_scalars + 2, s));
+                prof->launches[CX_K_LIST] += 2;   // the scan is three kernels
             }
-            prof->launches[CX_K_LIST] += 2;   // the scan is three kernels
             ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (sizeof(KeyT) + sizeof(IdT)), s);
-            CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, d_col,
-                                                  d_keys1[0], d_ids[0], n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, nullptr, ~0ull, s)));
+            CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, d_col, d_keys1[0], d_ids[0],
+                                                  n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, nullptr, ~0ull, region, B.ord_lo, B.ord_hi,
+                                                  s)));
         }
         // ---- step 3(c)ii: sort (first w symbols) ------------------------------------------------
         int in_alt = 0;
@@ -463,10 +582,10 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         CX_CUDA(cudaMemsetAsync(d_heads[0], 0, (n_words + 1) * 4, s));
         {
             ScopedLaunch sl(prof, CX_K_FINISH, nb * (sizeof(KeyT) + sizeof(IdT) + 1) + nb / 8, s);
-            CX_CUDA((launch_finish_first<KeyT, IdT>(R, d_keys1[cur], w, d_heads[0], ids, nb, sh.cap, dst, d_done, pack_kv, s)));
+            CX_CUDA((launch_finish_first<KeyT, IdT>(R, d_keys1[cur], w, depth_base + w, d_heads[0], ids, nb, sh.cap, dst, d_done, pack_kv, s)));
         }
         // ---- what is still tied goes through global rounds: re-key, sort, write back ------------------
-        uint32_t depth = w, rounds = 0;
+        uint32_t depth = depth_base + w, rounds = 0;
         uint64_t local_before = p->h_scalars[1];
         while (true) {
             {

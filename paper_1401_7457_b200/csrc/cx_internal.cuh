@@ -57,6 +57,14 @@ struct Reads {
     uint32_t uniform;          // 1: all reads have the same length, offsets need not be gathered
 };
 
+// A region of the suffix space: the suffixes whose first `depth` bases spell `prefix`.  depth = 0 is the whole
+// collection.  An l-prefix partition that is larger than a batch is partitioned again by its NEXT l characters,
+// recursively (Fig. 2 step 1): the scans then work inside the region of that partition.
+struct Region {
+    const uint64_t* prefix;   // DEVICE: depth bases, 2 bit/base, MSB-first in each word
+    uint32_t depth;
+};
+
 // ---------------------------------------------------------------------------------------------
 // device helpers
 // ---------------------------------------------------------------------------------------------
@@ -99,6 +107,23 @@ __device__ __forceinline__ uint64_t make_key(uint64_t window, uint64_t rem, uint
     return (bases << len_bits) | r;
 }
 
+// Is the suffix that starts at base index b, with `rem` bases left and `window` = its next 32 bases, inside the region?
+// If so, (window, rem) are advanced to describe the suffix at the region's depth.
+__device__ __forceinline__ bool enter_region(const uint64_t* __restrict__ packed, uint64_t n_words, const Region& g, uint64_t b,
+                                             uint64_t& window, uint32_t& rem) {
+    if (g.depth == 0) return true;
+    if (rem < g.depth) return false;
+    for (uint32_t j = 0; j * 32 < g.depth; ++j) {
+        const uint64_t wj = j == 0 ? window : load_window(packed, n_words, b + 32ull * j);
+        const uint32_t nb = g.depth - j * 32 < 32 ? g.depth - j * 32 : 32;
+        const uint64_t mask = nb == 32 ? ~0ull : ~0ull << (64 - 2 * nb);
+        if ((wj ^ __ldg(g.prefix + j)) & mask) return false;
+    }
+    window = load_window(packed, n_words, b + g.depth);
+    rem -= g.depth;
+    return true;
+}
+
 template <typename IdT>
 __device__ __forceinline__ IdT make_id(uint64_t read, uint64_t pos, uint32_t pos_bits) {
     return (IdT)((read << pos_bits) | pos);
@@ -119,7 +144,7 @@ uint32_t* pack_fallback_status();
 cudaError_t launch_prep(const uint64_t* offsets, uint64_t n_reads, uint64_t max_bases, BuildInfo* info, cudaStream_t s);
 cudaError_t launch_tile_table(const uint64_t* offsets, uint64_t n_reads, const BuildInfo* info, uint32_t* tile_first_read,
                               uint64_t max_tiles, cudaStream_t s);
-cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
+cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, const Region& region,
                                uint64_t* hist, uint64_t max_tiles, int n_sms, cudaStream_t s);
 // count, per tile, the suffixes of up to kCountGroup consecutive batches in one scan; batch j owns partitions
 // [first[j], first[j + 1]); tile_count[j * col_stride + tile]
@@ -128,7 +153,7 @@ struct CountRanges {
     uint32_t n;
     uint32_t first[kCountGroup + 1];
 };
-cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
+cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, const Region& region,
                               const CountRanges& ranges, uint64_t* tile_count, uint64_t col_stride, uint64_t n_tiles, cudaStream_t s);
 // write (key, id) of those suffixes in (read, pos) order; tile_base == nullptr means "every suffix, index = slot".
 // Also accumulates the digit counts of the n_passes radix passes over key bits [0, 8 * n_passes) into digit_hist
@@ -137,7 +162,7 @@ template <typename KeyT, typename IdT>
 cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
                               uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, KeyT* keys, IdT* ids,
                               uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, bool packed, uint64_t* bucket_hist,
-                              uint64_t max_n, cudaStream_t s);
+                              uint64_t max_n, const Region& region, uint64_t ord_lo, uint64_t ord_hi, cudaStream_t s);
 
 // cx_onesweep.cu
 struct SortWorkspace {
@@ -171,10 +196,11 @@ template <typename IdT>
 cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, const IdT* ids_c, const uint32_t* pos_c, uint64_t n_c,
                                     uint32_t w, IdT* ids, uint32_t* heads, uint8_t* out, cudaStream_t s);
 // fused head flags + in-block refinement + emit over the freshly sorted first-round keys; heads_out must be zero-filled
+// depth0: symbols the first-round sort has settled (region depth + w1).
 // packed: keys1 holds 64-bit words (32-bit key << 32 | 32-bit id); `ids` is then OUTPUT: the ids of the positions left to
 // the global path are written there (nothing else will need the others).
 template <typename KeyT, typename IdT>
-cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t* heads_out, IdT* ids, uint64_t n,
+cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t depth0, uint32_t* heads_out, IdT* ids, uint64_t n,
                                 uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, bool packed, cudaStream_t s);
 // in-block refinement + emit of the groups a global round has split to at most group_cap members; heads_out = copy of heads_in
 template <typename IdT>

@@ -584,7 +584,7 @@ cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, cons
 }
 
 template <typename KeyT, typename IdT>
-cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t* heads_out, IdT* ids, uint64_t n,
+cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t depth0, uint32_t* heads_out, IdT* ids, uint64_t n,
                                 uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, bool packed, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
     constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
@@ -595,7 +595,7 @@ cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, 
     if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
     uint64_t blocks = (n + kLocalTile - 1) / kLocalTile;
     kernel<<<(unsigned)blocks, kLocalThreads, sizeof(LocalSmem<IdT>), s>>>(R, keys1, w1, (1u << key_len_bits(w1)) - 1, nullptr, heads_out, ids, n,
-                                                                          w1, group_cap, out, elems_done);
+                                                                          depth0, group_cap, out, elems_done);
     return cudaGetLastError();
 }
 
@@ -622,9 +622,9 @@ cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32
                                                   uint32_t, uint64_t*, IdT*, uint32_t*, cudaStream_t);                               \
     template cudaError_t launch_refine_writeback<IdT>(const Reads&, const uint64_t*, const IdT*, const uint32_t*, uint64_t,         \
                                                       uint32_t, IdT*, uint32_t*, uint8_t*, cudaStream_t);                            \
-    template cudaError_t launch_finish_first<uint32_t, IdT>(const Reads&, const uint32_t*, uint32_t, uint32_t*, IdT*, uint64_t,     \
+    template cudaError_t launch_finish_first<uint32_t, IdT>(const Reads&, const uint32_t*, uint32_t, uint32_t, uint32_t*, IdT*, uint64_t, \
                                                             uint32_t, uint8_t*, unsigned long long*, bool, cudaStream_t);            \
-    template cudaError_t launch_finish_first<uint64_t, IdT>(const Reads&, const uint64_t*, uint32_t, uint32_t*, IdT*, uint64_t,     \
+    template cudaError_t launch_finish_first<uint64_t, IdT>(const Reads&, const uint64_t*, uint32_t, uint32_t, uint32_t*, IdT*, uint64_t, \
                                                             uint32_t, uint8_t*, unsigned long long*, bool, cudaStream_t);            \
     template cudaError_t launch_finish_later<IdT>(const Reads&, const uint32_t*, uint32_t*, const IdT*, uint64_t, uint32_t,         \
                                                   uint32_t, uint8_t*, unsigned long long*, cudaStream_t);

@@ -172,6 +172,7 @@ __device__ __forceinline__ uint32_t bucket_of(const Slot& sl, uint32_t ell, uint
 // access); after a read's end-marker slot the next read starts at the same base index, so the window stays.
 struct Walk {
     uint64_t window, ahead;   // bases [b, b + 32) and [b + 32, b + 64), MSB-first
+    uint64_t b;               // base index of the slot's first base
     uint32_t rem;             // bases left in the read from this slot
     uint32_t lo;              // read - r0
 };
@@ -179,6 +180,7 @@ __device__ __forceinline__ Walk walk_init(const TileCtx& c, const TileSmem& sm, 
     const Slot sl = decode_slot(c, sm, s);
     Walk wk;
     wk.window = sl.window;
+    wk.b = sl.b;
     wk.rem = (uint32_t)sl.rem;
     wk.lo = sl.lo;
     const uint64_t nb = sl.b + 32;
@@ -193,17 +195,26 @@ __device__ __forceinline__ void walk_next(const TileCtx& c, const TileSmem& sm, 
     if (wk.rem) {
         wk.window = (wk.window << 2) | (wk.ahead >> 62);
         wk.ahead <<= 2;
+        wk.b += 1;
         wk.rem -= 1;
     } else {   // end-marker slot: the next read starts at the same base index
         wk.lo += 1;
         wk.rem = c.uniform ? c.L1 - 1 : (uint32_t)(sm.off[wk.lo + 1] - sm.off[wk.lo]);
     }
 }
-__device__ __forceinline__ uint32_t walk_bucket(const Walk& wk, uint32_t ell) {
-    const uint32_t hi = (uint32_t)(wk.window >> 32);
-    const uint32_t r = wk.rem < ell ? wk.rem : ell;
+__device__ __forceinline__ uint32_t window_bucket(uint64_t window, uint32_t rem, uint32_t ell) {
+    const uint32_t hi = (uint32_t)(window >> 32);
+    const uint32_t r = rem < ell ? rem : ell;
     const uint32_t kmer = r ? (hi >> (32 - 2 * r)) << (2 * (ell - r)) : 0u;
     return kmer * (ell + 1) + r;
+}
+// partition code of the walker's slot inside `region` (at the region's depth); false if the slot is outside it
+__device__ __forceinline__ bool walk_bucket(const Reads& R, const Region& region, const Walk& wk, uint32_t ell, uint32_t& code) {
+    uint64_t window = wk.window;
+    uint32_t rem = wk.rem;
+    if (region.depth && !enter_region(R.packed, R.n_words, region, wk.b, window, rem)) return false;
+    code = window_bucket(window, rem, ell);
+    return true;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -211,7 +222,7 @@ __device__ __forceinline__ uint32_t walk_bucket(const Walk& wk, uint32_t ell) {
 // shared-memory histogram with warp-aggregated updates, the few short ones go straight to global.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kListThreads) bucket_hist_kernel(Reads R, const BuildInfo* __restrict__ info,
-                                                                   const uint32_t* __restrict__ tile_first_read, uint32_t ell,
+                                                                   const uint32_t* __restrict__ tile_first_read, uint32_t ell, Region region,
                                                                    unsigned long long* __restrict__ hist) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem& sm = *reinterpret_cast<TileSmem*>(smem_raw);
@@ -235,6 +246,11 @@ __global__ void __launch_bounds__(kListThreads) bucket_hist_kernel(Reads R, cons
             if (valid) {
                 uint32_t kmer = 0, r = 0;
                 Slot sl = decode_slot(c, sm, s);
+                if (region.depth) {   // sizes of the sub-partitions of an oversize partition
+                    uint32_t rem = (uint32_t)sl.rem;
+                    if (!enter_region(R.packed, R.n_words, region, sl.b, sl.window, rem)) continue;
+                    sl.rem = rem;
+                }
                 uint32_t b = bucket_of(sl, ell, kmer, r);
                 // consecutive suffixes rarely share an l-mer, so one shared-memory atomic per suffix beats warp
                 // aggregation here (match.any costs ~25 cycles per distinct value on sm_100a)
@@ -264,7 +280,7 @@ __global__ void __launch_bounds__(kListThreads) bucket_hist_kernel(Reads R, cons
 // tile_count is laid out [batch][tile] so that each batch's column can be scanned in place.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const BuildInfo* __restrict__ info,
-                                                                  const uint32_t* __restrict__ tile_first_read, uint32_t ell,
+                                                                  const uint32_t* __restrict__ tile_first_read, uint32_t ell, Region region,
                                                                   CountRanges ranges, uint64_t* __restrict__ tile_count, uint64_t col_stride) {
     __shared__ TileSmem sm;
     __shared__ uint32_t s_total[kCountGroup];
@@ -284,8 +300,8 @@ __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const
 #pragma unroll
             for (int i = 0; i < kListItems; ++i) {
                 if (s0 + i < c.n_slots) {
-                    const uint32_t b = walk_bucket(wk, ell);
-                    if (b >= ranges.first[0] && b < ranges.first[ranges.n]) {
+                    uint32_t b = 0;
+                    if (walk_bucket(R, region, wk, ell, b) && b >= ranges.first[0] && b < ranges.first[ranges.n]) {
                         uint32_t j = 0;
 #pragma unroll
                         for (int q = 1; q < kCountGroup; ++q) j += (q < (int)ranges.n && b >= ranges.first[q]);
@@ -317,7 +333,11 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
                                                                    uint32_t bucket_lo, uint32_t bucket_hi,
                                                                    const uint64_t* __restrict__ tile_base, KeyT* __restrict__ keys,
                                                                    IdT* __restrict__ ids, uint32_t n_passes,
-                                                                   unsigned long long* __restrict__ digit_hist) {
+                                                                   unsigned long long* __restrict__ digit_hist, Region region,
+                                                                   uint64_t ord_lo, uint64_t ord_hi) {
+    // region: the scan is confined to the suffixes of an oversize partition and keys start at its depth.
+    // [ord_lo, ord_hi): of the selected suffixes, in listing order, only these ordinals are written (at ordinal - ord_lo):
+    // a partition of IDENTICAL suffixes larger than a batch is cut this way, its order being the listing order anyway.
     __shared__ TileSmem sm;
     __shared__ uint32_t s_dh[8][kRadix];
     __shared__ uint32_t s_warp[kListThreads / 32];
@@ -338,8 +358,8 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
 #pragma unroll
             for (int i = 0; i < kListItems; ++i) {
                 if (s0 + i < c.n_slots) {
-                    const uint32_t b = walk_bucket(wk, ell);
-                    mask |= (uint32_t)(b - bucket_lo <= bucket_hi - bucket_lo) << i;
+                    uint32_t b = 0;
+                    mask |= (uint32_t)(walk_bucket(R, region, wk, ell, b) && b - bucket_lo <= bucket_hi - bucket_lo) << i;
                     if (s0 + i + 1 < c.n_slots) walk_next(c, sm, wk);
                 }
             }
@@ -359,15 +379,22 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
         while (mask) {
             const int i = __ffs(mask) - 1;
             mask &= mask - 1;
-            const Slot sl = decode_slot(c, sm, s0 + i);
-            const KeyT key = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
-            const IdT id = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
-            for (uint32_t p = 0; p < n_passes; ++p) atomicAdd(&s_dh[p][(uint32_t)(key >> (p * kRadixBits)) & (kRadix - 1)], 1u);
-            if constexpr (PACKED) {
-                reinterpret_cast<uint64_t*>(keys)[dst] = ((uint64_t)key << 32) | (uint64_t)id;
-            } else {
-                keys[dst] = key;
-                ids[dst] = id;
+            if (dst >= ord_lo && dst < ord_hi) {
+                Slot sl = decode_slot(c, sm, s0 + i);
+                if (region.depth) {
+                    sl.window = load_window(R.packed, R.n_words, sl.b + region.depth);
+                    sl.rem -= region.depth;
+                }
+                const KeyT key = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
+                const IdT id = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
+                for (uint32_t p = 0; p < n_passes; ++p) atomicAdd(&s_dh[p][(uint32_t)(key >> (p * kRadixBits)) & (kRadix - 1)], 1u);
+                const uint64_t at = dst - ord_lo;
+                if constexpr (PACKED) {
+                    reinterpret_cast<uint64_t*>(keys)[at] = ((uint64_t)key << 32) | (uint64_t)id;
+                } else {
+                    keys[at] = key;
+                    ids[at] = id;
+                }
             }
             ++dst;
         }
@@ -475,7 +502,7 @@ cudaError_t launch_tile_table(const uint64_t* offsets, uint64_t n_reads, const B
 
 size_t bucket_hist_smem(uint32_t ell) { return sizeof(TileSmem) + (sizeof(uint32_t) << (2 * ell)) + sizeof(uint32_t) * (((1u << (2 * ell)) - 1) / 3); }
 
-cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
+cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, const Region& region,
                                uint64_t* hist, uint64_t max_tiles, int n_sms, cudaStream_t s) {
     if (max_tiles == 0) return cudaSuccess;
     size_t smem = bucket_hist_smem(ell);
@@ -488,15 +515,15 @@ cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint
     int per_sm = ell <= 6 ? 4 : 2;
     uint64_t want = (uint64_t)n_sms * per_sm;
     unsigned grid = (unsigned)(max_tiles < want ? max_tiles : want);
-    bucket_hist_kernel<<<grid, kListThreads, smem, s>>>(R, info, tile_first_read, ell, (unsigned long long*)hist);
+    bucket_hist_kernel<<<grid, kListThreads, smem, s>>>(R, info, tile_first_read, ell, region, (unsigned long long*)hist);
     return cudaGetLastError();
 }
 
-cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell,
+cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, const Region& region,
                               const CountRanges& ranges, uint64_t* tile_count, uint64_t col_stride, uint64_t n_tiles, cudaStream_t s) {
     if (n_tiles == 0 || ranges.n == 0) return cudaSuccess;
     uint64_t want = 148ull * 8;
-    list_count_kernel<<<(unsigned)(n_tiles < want ? n_tiles : want), kListThreads, 0, s>>>(R, info, tile_first_read, ell, ranges, tile_count,
+    list_count_kernel<<<(unsigned)(n_tiles < want ? n_tiles : want), kListThreads, 0, s>>>(R, info, tile_first_read, ell, region, ranges, tile_count,
                                                                                          col_stride);
     return cudaGetLastError();
 }
@@ -505,7 +532,7 @@ template <typename KeyT, typename IdT>
 cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
                               uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, KeyT* keys, IdT* ids,
                               uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, bool packed, uint64_t* bucket_hist,
-                              uint64_t max_n, cudaStream_t s) {
+                              uint64_t max_n, const Region& region, uint64_t ord_lo, uint64_t ord_hi, cudaStream_t s) {
     if (n_tiles == 0) return cudaSuccess;
     uint64_t want = (uint64_t)n_sms * (bucket_hist ? 4 : 6);
     unsigned grid = (unsigned)(n_tiles < want ? n_tiles : want);
@@ -525,16 +552,17 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
     if (tile_base == nullptr) return packed ? launch(list_write_kernel<KeyT, IdT, kCanPack>) : launch(list_write_kernel<KeyT, IdT, false>);
     if (packed)
         list_select_kernel<KeyT, IdT, kCanPack><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids,
-                                                                             n_passes, dh);
+                                                                             n_passes, dh, region, ord_lo, ord_hi);
     else
         list_select_kernel<KeyT, IdT, false><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids,
-                                                                          n_passes, dh);
+                                                                          n_passes, dh, region, ord_lo, ord_hi);
     return cudaGetLastError();
 }
 
 #define CX_LIST_INST(K, I)                                                                                                        \
     template cudaError_t launch_list_write<K, I>(const Reads&, const BuildInfo*, const uint32_t*, uint32_t, uint32_t, uint32_t,  \
-                                                 uint32_t, const uint64_t*, K*, I*, uint64_t, uint32_t, uint64_t*, int, bool, uint64_t*, uint64_t, cudaStream_t);
+                                                 uint32_t, const uint64_t*, K*, I*, uint64_t, uint32_t, uint64_t*, int, bool, uint64_t*, uint64_t, const Region&,     \
+                                                 uint64_t, uint64_t, cudaStream_t);
 CX_LIST_INST(uint32_t, uint32_t)
 CX_LIST_INST(uint32_t, uint64_t)
 CX_LIST_INST(uint64_t, uint32_t)

@@ -150,12 +150,50 @@ def test_pinned_host_output_streams_batches():
     assert np.array_equal(out.numpy(), want)
 
 
-def test_bucket_too_large_is_reported():
+# ---- NEXT-1: partitions larger than a batch are partitioned again by their next l characters ------------
+
+def _stats_of(coll, **opts):
     import paper_1401_7457_b200 as cx
+    p = cx.Plan(coll.n_reads, coll.total_bases, max_read_len=max(coll.max_read_len, 1), **opts)
+    out = torch.empty(coll.n_suffixes, dtype=torch.uint8, device="cuda")
+    a = torch.from_numpy(coll.ascii).cuda()
+    packed = cx.cx_pack_reads(a) if coll.total_bases else torch.zeros(1, dtype=torch.int64, device="cuda")
+    p.build(packed, torch.from_numpy(coll.offsets.astype(np.int64)).cuda(), coll.n_reads, out)
+    return out.cpu().numpy(), p.stats()
+
+
+@pytest.mark.parametrize("m1", [1000, 150, 37])
+def test_homopolymer_collection_with_tiny_batches(m1):
+    # every suffix falls in the AAAAAA partition or a partition of identical short suffixes: refinement down to the
+    # read length, and (m1 < n_reads) partitions of identical suffixes cut into slices of the listing order
     c = gen.from_strings(["A" * 100] * 200)
-    with pytest.raises(cx.CxError) as e:
-        gpu_bwt(c, max_batch_suffixes=1000)
-    assert e.value.code == cx.binding.CX_ERR_BUCKET_TOO_LARGE
+    got, st = _stats_of(c, max_batch_suffixes=m1)
+    assert np.array_equal(got, oracle.bwt(c.ascii, c.offsets))
+    assert st["refined_partitions"] >= 10 and st["n_batches"] > 10
+
+
+def test_tandem_repeats_and_duplicates_with_tiny_batches():
+    c = gen.from_strings(["ACGT" * 50] * 40 + ["CGTA" * 30 + "T"] * 25 + ["G" * 77] * 30 + ["", "A", "AC"] * 20)
+    for m1 in (500, 90):
+        got, st = _stats_of(c, max_batch_suffixes=m1, prefix_len=3)
+        assert np.array_equal(got, oracle.bwt(c.ascii, c.offsets)), m1
+        assert st["refined_partitions"] > 0
+
+
+@pytest.mark.parametrize("idx,scale,m1,ell", [(1, 0.01, 20_000, 2), (2, 0.001, 9_000, 1), (3, 0.0003, 30_000, 2)])
+def test_config_shapes_with_forced_refinement(idx, scale, m1, ell):
+    c = gen.config(idx, scale)
+    got, st = _stats_of(c, max_batch_suffixes=m1, prefix_len=ell)
+    assert np.array_equal(got, oracle.bwt(c.ascii, c.offsets))
+    assert st["refined_partitions"] > 0
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_random_skewed_collections_with_tiny_batches(seed):
+    c = gen.random_collection(100 + seed, n_reads=20 + (seed * 29) % 200, max_len=1 + (seed * 17) % 120, alphabet=["A", "AC", "ACGT", "GT"][seed % 4])
+    for m1 in (64, 11):
+        got, _ = _stats_of(c, max_batch_suffixes=m1, prefix_len=1 + seed % 4, small_group_max=[0, 1][seed % 2])
+        assert np.array_equal(got, oracle.bwt(c.ascii, c.offsets)), (seed, m1)
 
 
 def test_bad_offsets_and_oversize_input_are_reported_not_executed():
