@@ -54,6 +54,8 @@ def parse_args():
     ap.add_argument("--impl", default="cx", choices=["cx", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--key-bases", type=int, default=0, help="first-round key window w (0 = the library's default)")
+    ap.add_argument("--table4", type=int, default=0, help="NEXT-3: the paper's read-length experiment instead of a config: read length 100/200/400, "
+                    "1e10 x --scale bases (PAPER.md:184-189)")
     ap.add_argument("--max-batch", type=int, default=0, help="m1: most suffixes per batch (0 = as many as the workspace allows)")
     return ap.parse_args()
 
@@ -213,7 +215,10 @@ def run_cx(args) -> None:
     cx.lib()
 
     # ---- synthetic input (seeded; replicas differ only in seed) -------------------------------------
-    coll = gen.config(args.config, args.scale, seed=replica_seed(args.config, rank))
+    if args.table4:
+        coll = gen.table4(args.table4, args.scale)
+    else:
+        coll = gen.config(args.config, args.scale, seed=replica_seed(args.config, rank))
     n_reads, total, N = coll.n_reads, coll.total_bases, coll.n_suffixes
     h_ascii = torch.from_numpy(coll.ascii).pin_memory()
     h_off = torch.from_numpy(coll.offsets.astype(np.int64)).pin_memory()
@@ -321,7 +326,8 @@ def run_cx(args) -> None:
         "metric": METRIC, "value": world * N / (dev_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": dev_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u64", "data": "synthetic",
-        "config": {"workload": WORKLOADS.get(args.config, str(args.config)) + (f" x scale {args.scale:g}" if args.scale != 1 else ""),
+        "config": {"workload": (f"Table 4 shape (PAPER.md:184-189): reads of {args.table4} bp, 30x, both strands, 1% subst." if args.table4
+                                else WORKLOADS.get(args.config, str(args.config))) + (f" x scale {args.scale:g}" if args.scale != 1 else ""),
                    "n_reads": n_reads, "total_bases": total, "n_suffixes": N, "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": "256 MiB L2-flush write between timed steps; working set >> L2", "prefix_len": 6, "key_bases": "auto (14 bases in a 32-bit key up to 2^30 suffixes, else ceil(log4 N)+1 bases in a 64-bit key)",
                    "id_bytes": stats["id_bytes"], "n_batches": stats["n_batches"], "sort_passes": stats["sort_passes"],

@@ -119,6 +119,14 @@ def test_config3_full_size_sampled_slices():
     _full_size_check(2, ["ACGTACG", "TTGACCA"], lf_sample=2_000)
 
 
+@pytest.mark.parametrize("read_len", [200, 400, 1000])
+def test_longer_reads_table4_shape(read_len):
+    # NEXT-3: the paper's read-length experiment (Table 4) at reduced scale; deeper refinement
+    c = gen.table4(read_len, 0.0002)
+    assert_parity(c)
+    assert_parity(c, small_group_max=1)
+
+
 def test_eight_byte_ids():
     c = gen.config(1, 0.02)
     assert_parity(c, max_read_len=0)                     # unknown read length -> 64-bit suffix ids

@@ -194,6 +194,18 @@ def config(index: int, scale: float = 1.0, seed: int | None = None) -> Collectio
     raise ValueError("config index must be 0..4")
 
 
+def table4(read_len: int, scale: float = 1.0, seed: int | None = None) -> Collection:
+    """Stand-in for the paper's read-length experiment (Table 4; Section 4.3): equal
+    total bases (1e10 at scale 1) in reads of 100, 200 or 400 bp -- 100M x 100, 50M x 200, 25M x 400 in the paper.
+    Same structure as configs[2]: 30x over an iid genome, both strands, 1 % substitutions."""
+    if seed is None:
+        seed = BASE_SEED + 40 + read_len
+    total = max(read_len, int(round(10_000_000_000 * scale)))
+    n = max(1, total // read_len)
+    G = max(2 * read_len, total // 30)
+    return _sample_reads(seed, _iid_codes(seed, 1, 0, G), n, read_len, read_len, True, 1, 100, f"T4-{read_len}x{scale:g}")
+
+
 def random_collection(seed: int, n_reads: int, max_len: int, alphabet: str = "ACGT",
                       min_len: int = 0) -> Collection:
     """Small adversarial collections for tests: short alphabets and ragged (possibly empty) reads."""
