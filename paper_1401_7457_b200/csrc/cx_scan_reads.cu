@@ -209,10 +209,11 @@ __device__ __forceinline__ uint32_t window_bucket(uint64_t window, uint32_t rem,
     return kmer * (ell + 1) + r;
 }
 // partition code of the walker's slot inside `region` (at the region's depth); false if the slot is outside it
+template <bool REGION>
 __device__ __forceinline__ bool walk_bucket(const Reads& R, const Region& region, const Walk& wk, uint32_t ell, uint32_t& code) {
     uint64_t window = wk.window;
     uint32_t rem = wk.rem;
-    if (region.depth && !enter_region(R.packed, R.n_words, region, wk.b, window, rem)) return false;
+    if (REGION && !enter_region(R.packed, R.n_words, region, wk.b, window, rem)) return false;
     code = window_bucket(window, rem, ell);
     return true;
 }
@@ -279,6 +280,7 @@ __global__ void __launch_bounds__(kListThreads) bucket_hist_kernel(Reads R, cons
 // collection (fewer scans).  Batch j owns the partitions [first[j], first[j + 1]).
 // tile_count is laid out [batch][tile] so that each batch's column can be scanned in place.
 // ---------------------------------------------------------------------------------------------
+template <bool REGION>   // REGION = false: the whole collection, no region code in the loop
 __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const BuildInfo* __restrict__ info,
                                                                   const uint32_t* __restrict__ tile_first_read, uint32_t ell, Region region,
                                                                   CountRanges ranges, uint64_t* __restrict__ tile_count, uint64_t col_stride) {
@@ -301,7 +303,7 @@ __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const
             for (int i = 0; i < kListItems; ++i) {
                 if (s0 + i < c.n_slots) {
                     uint32_t b = 0;
-                    if (walk_bucket(R, region, wk, ell, b) && b >= ranges.first[0] && b < ranges.first[ranges.n]) {
+                    if (walk_bucket<REGION>(R, region, wk, ell, b) && b >= ranges.first[0] && b < ranges.first[ranges.n]) {
                         uint32_t j = 0;
 #pragma unroll
                         for (int q = 1; q < kCountGroup; ++q) j += (q < (int)ranges.n && b >= ranges.first[q]);
@@ -327,7 +329,7 @@ __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const
 // [bucket_lo, bucket_hi], in (read, pos) order, each with its first key.  Most slots belong to other
 // batches, so the scan walks the slots with next_slot() and decodes in full only what it takes.
 // ---------------------------------------------------------------------------------------------
-template <typename KeyT, typename IdT, bool PACKED>
+template <typename KeyT, typename IdT, bool PACKED, bool REGION>
 __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, const BuildInfo* __restrict__ info,
                                                                    const uint32_t* __restrict__ tile_first_read, uint32_t ell, uint32_t w,
                                                                    uint32_t bucket_lo, uint32_t bucket_hi,
@@ -359,7 +361,7 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
             for (int i = 0; i < kListItems; ++i) {
                 if (s0 + i < c.n_slots) {
                     uint32_t b = 0;
-                    mask |= (uint32_t)(walk_bucket(R, region, wk, ell, b) && b - bucket_lo <= bucket_hi - bucket_lo) << i;
+                    mask |= (uint32_t)(walk_bucket<REGION>(R, region, wk, ell, b) && b - bucket_lo <= bucket_hi - bucket_lo) << i;
                     if (s0 + i + 1 < c.n_slots) walk_next(c, sm, wk);
                 }
             }
@@ -381,7 +383,7 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
             mask &= mask - 1;
             if (dst >= ord_lo && dst < ord_hi) {
                 Slot sl = decode_slot(c, sm, s0 + i);
-                if (region.depth) {
+                if (REGION) {
                     sl.window = load_window(R.packed, R.n_words, sl.b + region.depth);
                     sl.rem -= region.depth;
                 }
@@ -523,8 +525,11 @@ cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint3
                               const CountRanges& ranges, uint64_t* tile_count, uint64_t col_stride, uint64_t n_tiles, cudaStream_t s) {
     if (n_tiles == 0 || ranges.n == 0) return cudaSuccess;
     uint64_t want = 148ull * 8;
-    list_count_kernel<<<(unsigned)(n_tiles < want ? n_tiles : want), kListThreads, 0, s>>>(R, info, tile_first_read, ell, region, ranges, tile_count,
-                                                                                         col_stride);
+    const unsigned grid = (unsigned)(n_tiles < want ? n_tiles : want);
+    if (region.depth)
+        list_count_kernel<true><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, region, ranges, tile_count, col_stride);
+    else
+        list_count_kernel<false><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, region, ranges, tile_count, col_stride);
     return cudaGetLastError();
 }
 
@@ -550,13 +555,13 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
         return cudaGetLastError();
     };
     if (tile_base == nullptr) return packed ? launch(list_write_kernel<KeyT, IdT, kCanPack>) : launch(list_write_kernel<KeyT, IdT, false>);
-    if (packed)
-        list_select_kernel<KeyT, IdT, kCanPack><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids,
-                                                                             n_passes, dh, region, ord_lo, ord_hi);
-    else
-        list_select_kernel<KeyT, IdT, false><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids,
-                                                                          n_passes, dh, region, ord_lo, ord_hi);
-    return cudaGetLastError();
+    auto select = [&](auto kernel) {
+        kernel<<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids, n_passes, dh, region, ord_lo,
+                                             ord_hi);
+        return cudaGetLastError();
+    };
+    if (region.depth) return packed ? select(list_select_kernel<KeyT, IdT, kCanPack, true>) : select(list_select_kernel<KeyT, IdT, false, true>);
+    return packed ? select(list_select_kernel<KeyT, IdT, kCanPack, false>) : select(list_select_kernel<KeyT, IdT, false, false>);
 }
 
 #define CX_LIST_INST(K, I)                                                                                                        \
