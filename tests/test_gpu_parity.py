@@ -127,6 +127,24 @@ def test_longer_reads_table4_shape(read_len):
     assert_parity(c, small_group_max=1)
 
 
+def test_one_long_read_and_word_aligned_lengths():
+    # a single 200 kbp read (18 position bits; the textbook BWT of S$), then reads whose lengths sit on packed-word edges
+    rng = np.random.default_rng(5)
+    long_read = "".join("ACGT"[i] for i in rng.integers(0, 4, 200_000))
+    assert_parity(gen.from_strings([long_read]))
+    assert_parity(gen.from_strings([long_read[:70_000], long_read[:70_000], "ACGT" * 8000]), max_batch_suffixes=30_000, prefix_len=3)
+    edge = ["".join("ACGT"[i] for i in rng.integers(0, 4, n)) for n in (31, 32, 33, 63, 64, 65, 0, 1, 96, 128, 127, 57, 58, 14, 15, 71, 72)] * 9
+    assert_parity(gen.from_strings(edge))
+    assert_parity(gen.from_strings(edge), max_batch_suffixes=700, prefix_len=2)
+
+
+def test_empty_reads_everywhere():
+    reads = ["", "", "ACGTACGT", "", "T", "", ""] * 300 + [""] * 500
+    assert_parity(gen.from_strings(reads))
+    assert_parity(gen.from_strings(reads), max_batch_suffixes=1000)     # fewer than n_reads: the end-marker partition is sliced
+    assert_parity(gen.from_strings([""] * 5000), max_batch_suffixes=999)
+
+
 def test_eight_byte_ids():
     c = gen.config(1, 0.02)
     assert_parity(c, max_read_len=0)                     # unknown read length -> 64-bit suffix ids
