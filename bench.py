@@ -344,8 +344,8 @@ def run_cx(args) -> None:
                      "alg_bytes_per_launch": int(bytes_per_launch), "us_per_launch": round(ms_per_launch * 1e3, 2),
                      "launches_per_step": dom["launches"] / args.steps},
         # The in-block refinement (finish) is the largest share of the step and is bound by integer ALU issue, not HBM: its
-        # algorithmic work is the number of 128-bit key comparisons its stable counting rank makes (counted by the kernel),
-        # six issue slots each (LDS.128 + a five-instruction borrow chain); peak = SMs x 128 lanes x SM clock / 6.
+        # algorithmic work is the number of 192-bit key comparisons its stable rank makes (counted by the kernel), nine
+        # issue slots each (LDS.128 + LDS.64 + a seven-instruction borrow chain); peak = SMs x 128 lanes x SM clock / 9.
         "roofline_finish": finish_roofline(classes["finish"], stats, clocks, args.steps),
         "pipeline": {"alg_bytes_per_step": int(total_alg), "alg_bytes_per_suffix": round(total_alg / N, 1),
                      "gb_s": round(total_alg / (dev_ms * 1e-3) / 1e9, 1), "frac_of_peak": round(total_alg / (dev_ms * 1e-3) / 1e9 / peak, 4),
@@ -365,12 +365,12 @@ def finish_roofline(cls: dict, stats: dict, clocks: dict, steps: int) -> dict:
     import torch
     n_sms = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
     mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0
-    peak = n_sms * 128 * mhz * 1e6 / 6.0
+    peak = n_sms * 128 * mhz * 1e6 / 9.0
     ms = cls["ms"] / max(steps, 1)
     achieved = stats["compare_ops"] / (ms * 1e-3) if ms > 0 else 0.0
-    return {"kernel": "finish_tile_kernel (a7+a8)", "bound": "alu", "achieved": achieved, "peak": peak, "unit": "128-bit key comparisons/s",
+    return {"kernel": "finish_tile_kernel (a7+a8)", "bound": "alu", "achieved": achieved, "peak": peak, "unit": "192-bit key comparisons/s",
             "frac": round(achieved / peak, 4), "compare_ops_per_step": stats["compare_ops"], "ms_per_step": round(ms, 4),
-            "peak_derivation": f"{n_sms} SMs x 128 lanes x {mhz:.0f} MHz / 6 issue slots per comparison"}
+            "peak_derivation": f"{n_sms} SMs x 128 lanes x {mhz:.0f} MHz / 9 issue slots per comparison"}
 
 
 def main():

@@ -67,7 +67,7 @@ typedef struct cx_bwt_stats_s {
     uint64_t refine_elements;   /* suffixes re-keyed, summed over refinement rounds and batches          */
     uint64_t small_group_elems; /* of those, finished by the in-block path                               */
     uint64_t kernel_launches;   /* kernels launched by the build                                        */
-    uint64_t compare_ops;       /* 128-bit key comparisons of the in-block refinement (its ALU work)     */
+    uint64_t compare_ops;       /* 192-bit key comparisons of the in-block refinement (its ALU work)     */
     uint32_t n_batches;         /* GPU batches (the paper's "small rounds", Fig. 2 step 3(c))            */
     uint32_t id_bytes;          /* 4 or 8: width of a suffix id                                         */
     uint32_t sort_passes;       /* radix passes of the first sort of a batch                            */

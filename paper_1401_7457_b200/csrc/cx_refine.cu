@@ -8,8 +8,9 @@
 // iterations over all suffixes; here only the groups still tied are re-keyed:
 //
 //   local path : groups of at most kLocalGroupCap suffixes are finished inside one thread block --
-//                ids in shared memory, one window gather per member per round, stable rank by
-//                counting, looping over depth until every member is placed;
+//                ids in shared memory, one 88-base gather per member per round (192-bit key: bases, length,
+//                index in the group), stable rank by counting inside sub-blocks and rank-merging them,
+//                looping over depth until every member is placed;
 //   global path: larger groups are compacted, re-keyed as (group ordinal | next w' bases | length)
 //                in one 64-bit key, sorted by the onesweep sorter, and written back in place.
 //
@@ -223,14 +224,15 @@ constexpr int kLocalElems = kLocalTile + kLocalGroupCap;   // positions a block 
 constexpr int kLocalWords = kLocalElems / 32 + 2;
 constexpr int kLocalItems = kLocalElems / kLocalThreads;
 static_assert(kLocalElems % kLocalThreads == 0 && kLocalThreads % 32 == 0, "tile shape");
-constexpr uint32_t kLocalW = 57;                            // bases per in-block round
-typedef unsigned __int128 u128;
+constexpr uint32_t kLocalW = 88;                            // bases per in-block round (192-bit round key)
 constexpr uint16_t kNone = 0xffff;
 constexpr int kSubBlock = 32;                               // members ranked by counting before runs are merged
 
 template <typename IdT>
 struct LocalSmem {
-    u128 key[kLocalElems];      // [57 bases, A-padded : 114][min(remaining, 57) : 6][index inside the group : 8]
+    // round key, 192 bits: [88 bases, A-padded : 176][0 : 1][min(remaining, 88) : 7][index inside the group : 8]
+    uint4 key_lo[kLocalElems];  // bits 0..127, .x least significant
+    uint2 key_hi[kLocalElems];  // bits 128..191 = the first 32 bases
     IdT id_a[kLocalElems];
     uint16_t ord[2][kLocalElems];  // sorted order of the runs being merged, ping-pong; at the end of a round
                                    // ord[cur][p] = member that ranks at position p
@@ -270,10 +272,15 @@ __device__ __forceinline__ int next_head(const uint32_t* hw, int e, int hi) {
     }
 }
 
-// 128-bit round key of suffix `id` at depth d: the next 57 bases (A-padded), then min(remaining, 57), then the
-// member's index inside its tie group -- so that one unsigned compare orders the group stably
+// 192-bit round key of suffix `id` at depth d: the next 88 bases (A-padded), then min(remaining, 88), then the member's
+// index inside its tie group -- so that one unsigned compare orders the group stably.  One round covers a
+// 100 bp read after a 14-base first sort.
+struct Key192 {
+    uint4 lo;   // bits 0..127
+    uint2 hi;   // bits 128..191
+};
 template <typename IdT>
-__device__ __forceinline__ u128 key128_at_depth(const Reads& R, IdT id, uint32_t depth, uint32_t idx) {
+__device__ __forceinline__ Key192 key192_at_depth(const Reads& R, IdT id, uint32_t depth, uint32_t idx) {
     const uint64_t read = (uint64_t)id >> R.pos_bits;
     const uint64_t pos = (uint64_t)id & ((1ull << R.pos_bits) - 1);
     uint64_t start, len;
@@ -281,33 +288,45 @@ __device__ __forceinline__ u128 key128_at_depth(const Reads& R, IdT id, uint32_t
     const uint64_t at = pos + depth;
     const uint64_t rem = at < len ? len - at : 0;
     const uint32_t r = rem < kLocalW ? (uint32_t)rem : kLocalW;
-    uint64_t hi = 0, mid = 0;
+    uint64_t p0 = 0, p1 = 0, p2 = 0;   // bases [0,32), [32,64), [64,88) of the window
     if (r) {
         const uint64_t b = start + at;
         const uint64_t wi = b >> 5;
         const uint32_t sh = (uint32_t)(b & 31) * 2;
+        const uint64_t last = R.n_words - 1 - wi;   // words after wi that exist
         const uint64_t w0 = __ldg(R.packed + wi);
-        const uint64_t w1 = (sh || r > 32) && wi + 1 < R.n_words ? __ldg(R.packed + wi + 1) : 0ull;
-        hi = sh ? (w0 << sh) | (w1 >> (64 - sh)) : w0;
+        const uint64_t w1 = (sh || r > 32) && last >= 1 ? __ldg(R.packed + wi + 1) : 0ull;
+        p0 = sh ? (w0 << sh) | (w1 >> (64 - sh)) : w0;
         if (r < 32) {
-            hi &= ~0ull << (64 - 2 * r);
+            p0 &= ~0ull << (64 - 2 * r);
         } else if (r > 32) {
-            const uint64_t w2 = sh && wi + 2 < R.n_words ? __ldg(R.packed + wi + 2) : 0ull;
-            mid = sh ? (w1 << sh) | (w2 >> (64 - sh)) : w1;
-            mid &= ~0ull << (64 - 2 * (r - 32));   // at most 25 bases: the low 14 bits are clear
+            const uint64_t w2 = ((sh && r > 32) || r > 64) && last >= 2 ? __ldg(R.packed + wi + 2) : 0ull;
+            p1 = sh ? (w1 << sh) | (w2 >> (64 - sh)) : w1;
+            if (r < 64) {
+                p1 &= ~0ull << (64 - 2 * (r - 32));
+            } else if (r > 64) {
+                const uint64_t w3 = sh && last >= 3 ? __ldg(R.packed + wi + 3) : 0ull;
+                p2 = sh ? (w2 << sh) | (w3 >> (64 - sh)) : w2;
+                p2 &= ~0ull << (64 - 2 * (r - 64));   // at most 24 bases: the low 16 bits are clear
+            }
         }
     }
-    const uint64_t lo = mid | ((uint64_t)r << 8) | idx;
-    return ((u128)hi << 64) | lo;
+    const uint64_t k0 = p2 | ((uint64_t)r << 8) | idx;
+    Key192 k;
+    k.lo = make_uint4((uint32_t)k0, (uint32_t)(k0 >> 32), (uint32_t)p1, (uint32_t)(p1 >> 32));
+    k.hi = make_uint2((uint32_t)p0, (uint32_t)(p0 >> 32));
+    return k;
 }
 
-// acc -= (a < b) for 128-bit unsigned a, b (x = least significant word): the borrow of a - b, five instructions
-__device__ __forceinline__ void count_if_less(uint32_t& acc, const uint4& a, const uint4& b) {
+// acc -= (a < b) for 192-bit unsigned a, b: the borrow of a - b, seven instructions
+__device__ __forceinline__ void count_if_less(uint32_t& acc, const uint4& alo, const uint2& ahi, const uint4& blo, const uint2& bhi) {
     asm("{\n\t.reg .u32 t;\n\t"
-        "sub.cc.u32 t, %1, %5;\n\tsubc.cc.u32 t, %2, %6;\n\tsubc.cc.u32 t, %3, %7;\n\tsubc.cc.u32 t, %4, %8;\n\t"
+        "sub.cc.u32 t, %1, %7;\n\tsubc.cc.u32 t, %2, %8;\n\tsubc.cc.u32 t, %3, %9;\n\tsubc.cc.u32 t, %4, %10;\n\t"
+        "subc.cc.u32 t, %5, %11;\n\tsubc.cc.u32 t, %6, %12;\n\t"
         "subc.u32 %0, %0, 0;\n\t}"
         : "+r"(acc)
-        : "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w), "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w));
+        : "r"(alo.x), "r"(alo.y), "r"(alo.z), "r"(alo.w), "r"(ahi.x), "r"(ahi.y), "r"(blo.x), "r"(blo.y), "r"(blo.z), "r"(blo.w), "r"(bhi.x),
+          "r"(bhi.y));
 }
 
 template <typename KeyT, typename IdT, bool FIRST, bool PACKED>
@@ -396,7 +415,7 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
     }
     __syncthreads();
 
-    // ---- rounds: one 57-base gather per member still tied, stable rank by counting -------------------
+    // ---- rounds: one 88-base gather per member still tied, stable rank (see below) ----------------------
     for (uint32_t depth = depth0;; depth += kLocalW) {
         uint32_t any = 0;
 #pragma unroll
@@ -404,7 +423,9 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
             const int e = k * kLocalThreads + tid;
             const int s = sm.gs[e];
             if (s != kNone) {
-                sm.key[e] = key128_at_depth(R, sm.id_a[e], depth, (uint32_t)(e - s));
+                const Key192 kk = key192_at_depth(R, sm.id_a[e], depth, (uint32_t)(e - s));
+                sm.key_lo[e] = kk.lo;
+                sm.key_hi[e] = kk.hi;
                 any = 1;
             }
         }
@@ -425,11 +446,12 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
                 const int t = sm.ge[e];
                 const int b0 = s + ((e - s) / kSubBlock) * kSubBlock;
                 const int b1 = min(b0 + kSubBlock, t);
-                const uint4 my = reinterpret_cast<const uint4*>(sm.key)[e];
+                const uint4 my = sm.key_lo[e];
+                const uint2 myh = sm.key_hi[e];
                 n_compares += (uint32_t)(b1 - b0);
                 uint32_t neg = 0;   // minus the number of sub-block members whose key is below mine
 #pragma unroll 4
-                for (int q = b0; q < b1; ++q) count_if_less(neg, reinterpret_cast<const uint4*>(sm.key)[q], my);
+                for (int q = b0; q < b1; ++q) count_if_less(neg, sm.key_lo[q], sm.key_hi[q], my, myh);
                 myrank[k] = 0u - neg;
                 sm.ord[0][b0 + myrank[k]] = (uint16_t)e;
                 more |= (uint32_t)(t - s > kSubBlock);
@@ -449,13 +471,15 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
                 if (t - s > run) {
                     const int sb = s + (r ^ 1) * run;    // sibling run [sb, sb + len)
                     if (sb < t) {
-                        const uint4 my = reinterpret_cast<const uint4*>(sm.key)[e];
+                        const uint4 my = sm.key_lo[e];
+                        const uint2 myh = sm.key_hi[e];
                         int lo = 0, hi = min(run, t - sb);
                         n_compares += 32 - __clz(hi);
                         while (lo < hi) {                // lower bound: sibling members below me
                             const int mid = (lo + hi) >> 1;
                             uint32_t neg = 0;
-                            count_if_less(neg, reinterpret_cast<const uint4*>(sm.key)[sm.ord[cur][sb + mid]], my);
+                            const int qi = sm.ord[cur][sb + mid];
+                            count_if_less(neg, sm.key_lo[qi], sm.key_hi[qi], my, myh);
                             if (neg) lo = mid + 1; else hi = mid;
                         }
                         nr += (uint32_t)lo;
@@ -477,12 +501,14 @@ __global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, con
             const int e = k * kLocalThreads + tid;
             if (sm.gs[e] != kNone) {
                 const int se = src[e];
-                const uint4 kk = reinterpret_cast<const uint4*>(sm.key)[se];
+                const uint4 kk = sm.key_lo[se];
                 idn[k] = sm.id_a[se];
-                bool head = e == sm.gs[e] || ((kk.x >> 8) & 63u) < kLocalW;
+                bool head = e == sm.gs[e] || ((kk.x >> 8) & 127u) < kLocalW;
                 if (!head) {   // same bases and length as the member ranked just before?  (the low 8 bits are the group index)
-                    const uint4 kp = reinterpret_cast<const uint4*>(sm.key)[src[e - 1]];
-                    head = ((((kk.x ^ kp.x) >> 8) | (kk.y ^ kp.y)) | ((kk.z ^ kp.z) | (kk.w ^ kp.w))) != 0;
+                    const int sp = src[e - 1];
+                    const uint4 kp = sm.key_lo[sp];
+                    const uint2 hk = sm.key_hi[se], hp = sm.key_hi[sp];
+                    head = (((((kk.x ^ kp.x) >> 8) | (kk.y ^ kp.y)) | ((kk.z ^ kp.z) | (kk.w ^ kp.w))) | ((hk.x ^ hp.x) | (hk.y ^ hp.y))) != 0;
                 }
                 headbit |= (uint32_t)head << k;
             }
