@@ -33,7 +33,7 @@ constexpr uint32_t kFlagAggregate = 1, kFlagInclusive = 2;
 
 // in-block refinement
 constexpr int kLocalThreads = 256;
-constexpr int kLocalTile = 1024;         // sorted positions owned by one block (measured at C2: 512 -> 6.2 ms, 1024 -> 5.7, 1536 -> 5.8, 2048 -> 6.3)
+constexpr int kLocalTile = 768;          // sorted positions owned by one block (measured at C2 with 192-bit keys: 768 -> 5.13 ms, 1024 -> 5.23; with 128-bit keys 512 -> 6.2, 1024 -> 5.7, 1536 -> 5.8, 2048 -> 6.3)
 constexpr int kLocalGroupCap = 256;      // largest tie group the in-block path accepts
 
 // Facts about one build, produced by the prep kernel and read by later kernels and by the host.

@@ -330,7 +330,7 @@ __device__ __forceinline__ void count_if_less(uint32_t& acc, const uint4& alo, c
 }
 
 template <typename KeyT, typename IdT, bool FIRST, bool PACKED>
-__global__ void __launch_bounds__(kLocalThreads) finish_tile_kernel(Reads R, const KeyT* __restrict__ keys1, uint32_t w1, uint32_t len_mask,
+__global__ void __launch_bounds__(kLocalThreads, 5) finish_tile_kernel(Reads R, const KeyT* __restrict__ keys1, uint32_t w1, uint32_t len_mask,
                                                                     const uint32_t* __restrict__ heads_in, uint32_t* __restrict__ heads,
                                                                     IdT* __restrict__ ids, uint64_t n,
                                                                     uint32_t depth0, uint32_t cap, uint8_t* __restrict__ out,
