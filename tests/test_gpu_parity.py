@@ -260,6 +260,31 @@ def test_default_workspace_gives_one_batch():
     assert np.array_equal(out.cpu().numpy(), oracle.bwt(c.ascii, c.offsets))
 
 
+def test_plan_reuse_many_builds_and_side_stream():
+    """One plan, many builds of different collections (more than 255 radix passes in total, so the look-back epoch of
+    the tile states wraps), on a non-default stream."""
+    import paper_1401_7457_b200 as cx
+    colls = [gen.config(1, 0.003), gen.config(2, 0.0008), gen.random_collection(3, 150, 90), gen.from_strings(["A" * 100] * 300),
+             gen.config(0, 0.3), gen.from_strings(["ACGT", "TAGT", "GGAA"])]
+    wants = [oracle.bwt(c.ascii, c.offsets) for c in colls]
+    max_reads = max(c.n_reads for c in colls)
+    max_bases = max(c.total_bases for c in colls)
+    plan = cx.Plan(max_reads, max_bases, max_read_len=100)
+    stream = torch.cuda.Stream()
+    passes = 0
+    with torch.cuda.stream(stream):
+        for it in range(14):
+            for c, want in zip(colls, wants):
+                a = torch.from_numpy(c.ascii).cuda()
+                off = torch.from_numpy(c.offsets.astype(np.int64)).cuda()
+                out = torch.empty(c.n_suffixes, dtype=torch.uint8, device="cuda")
+                plan.build(cx.cx_pack_reads(a, stream=stream), off, c.n_reads, out, stream=stream)
+                stream.synchronize()
+                assert np.array_equal(out.cpu().numpy(), want), (it, c.name)
+                passes += plan.stats()["sort_passes"]
+    assert passes > 255
+
+
 def test_deterministic():
     c = gen.config(2, 0.001)
     assert np.array_equal(gpu_bwt(c), gpu_bwt(c))
