@@ -157,7 +157,7 @@ def run_config(index, probes_text, chunk_reads, workspace_bytes, host_out, scale
     torch.cuda.synchronize()
     t_gen = time.time() - t0
     torch.cuda.empty_cache()
-    opts = dict(max_read_len=max_len, out_is_host_pinned=1 if host_out else 0)
+    opts = dict(max_read_len=max_len, out_is_host_pinned=1 if host_out else 0, profile=1)
     plan = cx.Plan(n, total, workspace_bytes=workspace_bytes, **opts)
     out = torch.empty(N, dtype=torch.uint8, pin_memory=True) if host_out else torch.empty(N, dtype=torch.uint8, device=dev)
     torch.cuda.synchronize()
@@ -166,6 +166,7 @@ def run_config(index, probes_text, chunk_reads, workspace_bytes, host_out, scale
     torch.cuda.synchronize()
     t_build = time.time() - t1
     stats = plan.stats()
+    kernel_ms = {k: round(v["ms"], 2) for k, v in plan.kernel_times().items() if v["launches"]}
     plan.free()
     del plan
     # whole-output properties
@@ -178,7 +179,7 @@ def run_config(index, probes_text, chunk_reads, workspace_bytes, host_out, scale
     slices = check_slices(recipe, probes, out, N)
     res = {"config": index, "scale": scale, "n_reads": n, "total_bases": total, "n_suffixes": N, "generate_s": round(t_gen, 1),
            "build_s": round(t_build, 3), "suffixes_per_s": N / t_build, "gbases_per_hour": total / t_build * 3600 / 1e9,
-           "stats": stats, "slices": slices, "host_out": host_out}
+           "stats": stats, "kernel_ms": kernel_ms, "slices": slices, "host_out": host_out}
     os.makedirs("gpurun_out", exist_ok=True)
     with open(f"gpurun_out/large_config{index}.json", "w") as f:
         json.dump(res, f)
