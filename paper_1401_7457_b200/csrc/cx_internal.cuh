@@ -33,7 +33,13 @@ constexpr uint32_t kFlagAggregate = 1, kFlagInclusive = 2;
 
 // in-block refinement
 constexpr int kLocalThreads = 256;
-constexpr int kLocalTile = 768;          // sorted positions owned by one block (measured at C2 with 192-bit keys: 768 -> 5.13 ms, 1024 -> 5.23; with 128-bit keys 512 -> 6.2, 1024 -> 5.7, 1536 -> 5.8, 2048 -> 6.3)
+// Sorted positions owned by one block.  The kernel is bound by random gathers, and what limits those is the L1 left
+// beside the shared-memory carve-out: 512 + 256 positions x 5 blocks/SM fit the 164 KB carve-out (92 KB of L1);
+// 768 + 256 needs 228 KB (28 KB of L1) and runs 1.5x slower on collections larger than L2.  Measured finish times,
+// configs[1] / configs[2] / configs[3] x 0.25: 512 -> 5.38 / 35.7 / 116.6 ms; 768 -> 5.47 / 59.3 / 185.2 ms;
+// 640 with 224 threads (196 KB carve-out) -> 5.31 / 39.8 / 130.6 ms.
+constexpr int kLocalTile = 512;
+constexpr int kLocalBlocksPerSM = 5;
 constexpr int kLocalGroupCap = 256;      // largest tie group the in-block path accepts
 
 // Facts about one build, produced by the prep kernel and read by later kernels and by the host.

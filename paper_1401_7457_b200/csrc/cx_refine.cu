@@ -8,9 +8,11 @@
 // iterations over all suffixes; here only the groups still tied are re-keyed:
 //
 //   local path : groups of at most kLocalGroupCap suffixes are finished inside one thread block --
-//                ids in shared memory, one 88-base gather per member per round (192-bit key: bases, length,
-//                index in the group), stable rank by counting inside sub-blocks and rank-merging them,
-//                looping over depth until every member is placed;
+//                one locator per member in shared memory (first base, bases left, preceding symbol: the
+//                offsets table and the word before the suffix are gathered once), one 88-base gather per
+//                member per round (192-bit key: bases, length, index in the group), stable rank by
+//                counting inside sub-blocks and rank-merging them, looping over depth until every member
+//                is placed; the BWT symbols then come straight from the locators;
 //   global path: larger groups are compacted, re-keyed as (group ordinal | next w' bases | length)
 //                in one 64-bit key, sorted by the onesweep sorter, and written back in place.
 //
@@ -233,14 +235,14 @@ struct LocalSmem {
     // round key, 192 bits: [88 bases, A-padded : 176][0 : 1][min(remaining, 88) : 7][index inside the group : 8]
     uint4 key_lo[kLocalElems];  // bits 0..127, .x least significant
     uint2 key_hi[kLocalElems];  // bits 128..191 = the first 32 bases
-    IdT id_a[kLocalElems];
+    uint64_t loc[kLocalElems];  // locator of the suffix now at this position (layout above); 0: not ours.  Holds the raw
+                                // id between the head pass and the classify pass
     uint16_t ord[2][kLocalElems];  // sorted order of the runs being merged, ping-pong; at the end of a round
                                    // ord[cur][p] = member that ranks at position p
     uint16_t gs[kLocalElems];   // first position of the element's current group (kNone: not ours / placed)
     uint16_t ge[kLocalElems];   // one past its last position
     uint32_t hw[kLocalWords];   // head bits of the window, updated as groups split
     uint32_t hw0[kLocalWords];  // as loaded
-    uint8_t mine[kLocalElems];  // 1: this block emits the position
 };
 
 // nearest set bit at or below position e, not lower than `lo`; -1 if none
@@ -272,46 +274,40 @@ __device__ __forceinline__ int next_head(const uint32_t* hw, int e, int hi) {
     }
 }
 
-// 192-bit round key of suffix `id` at depth d: the next 88 bases (A-padded), then min(remaining, 88), then the member's
-// index inside its tie group -- so that one unsigned compare orders the group stably.  One round covers a
-// 100 bp read after a 14-base first sort.
+// Locator of a suffix this block owns: everything the rounds and the emit need, so that the offsets table and the
+// word before the suffix are read once per suffix, not once per round and again at the emit (each such gather is a
+// 64-byte DRAM fetch on a collection larger than L2):
+//   [code of the preceding symbol, 1 = $, 2..5 = A C G T : 3][bases from its first base to the end of the read : 21]
+//   [index of its first base in the packed text : 40]
+constexpr uint32_t kLocBaseBits = 40, kLocRemBits = 21;
+__device__ __forceinline__ uint8_t loc_symbol(uint64_t loc) {
+    return (uint8_t)(0x544743412400ull >> (8 * (uint32_t)(loc >> (kLocBaseBits + kLocRemBits))));
+}
+
+// 192-bit round key of the suffix with locator `loc` at depth d: the next 88 bases (A-padded), then min(remaining, 88),
+// then the member's index inside its tie group -- so that one unsigned compare orders the group stably.
+// One round covers a 100 bp read after a 14-base first sort.
 struct Key192 {
     uint4 lo;   // bits 0..127
     uint2 hi;   // bits 128..191
 };
-template <typename IdT>
-__device__ __forceinline__ Key192 key192_at_depth(const Reads& R, IdT id, uint32_t depth, uint32_t idx) {
-    const uint64_t read = (uint64_t)id >> R.pos_bits;
-    const uint64_t pos = (uint64_t)id & ((1ull << R.pos_bits) - 1);
-    uint64_t start, len;
-    read_span(R, read, start, len);
-    const uint64_t at = pos + depth;
-    const uint64_t rem = at < len ? len - at : 0;
-    const uint32_t r = rem < kLocalW ? (uint32_t)rem : kLocalW;
-    uint64_t p0 = 0, p1 = 0, p2 = 0;   // bases [0,32), [32,64), [64,88) of the window
-    if (r) {
-        const uint64_t b = start + at;
-        const uint64_t wi = b >> 5;
-        const uint32_t sh = (uint32_t)(b & 31) * 2;
-        const uint64_t last = R.n_words - 1 - wi;   // words after wi that exist
-        const uint64_t w0 = __ldg(R.packed + wi);
-        const uint64_t w1 = (sh || r > 32) && last >= 1 ? __ldg(R.packed + wi + 1) : 0ull;
-        p0 = sh ? (w0 << sh) | (w1 >> (64 - sh)) : w0;
-        if (r < 32) {
-            p0 &= ~0ull << (64 - 2 * r);
-        } else if (r > 32) {
-            const uint64_t w2 = ((sh && r > 32) || r > 64) && last >= 2 ? __ldg(R.packed + wi + 2) : 0ull;
-            p1 = sh ? (w1 << sh) | (w2 >> (64 - sh)) : w1;
-            if (r < 64) {
-                p1 &= ~0ull << (64 - 2 * (r - 32));
-            } else if (r > 64) {
-                const uint64_t w3 = sh && last >= 3 ? __ldg(R.packed + wi + 3) : 0ull;
-                p2 = sh ? (w2 << sh) | (w3 >> (64 - sh)) : w2;
-                p2 &= ~0ull << (64 - 2 * (r - 64));   // at most 24 bases: the low 16 bits are clear
-            }
-        }
+// x with only its first cnt bases kept (cnt may be <= 0 or >= 32)
+__device__ __forceinline__ uint64_t keep_bases(uint64_t x, int cnt) {
+    return cnt >= 32 ? x : (cnt <= 0 ? 0ull : x & (~0ull << (64 - 2 * cnt)));
+}
+// w: the four packed words from the one that holds the window's first base (words the window does not touch are 0);
+// shift: bit offset of that base in w[0]; take: bases of the window that exist (<= 88)
+__device__ __forceinline__ Key192 key192_of_words(const uint64_t (&w)[4], uint32_t shift, uint32_t take, uint32_t idx) {
+    uint64_t p0 = w[0], p1 = w[1], p2 = w[2];   // bases [0,32), [32,64), [64,88) of the window
+    if (shift) {
+        p0 = (w[0] << shift) | (w[1] >> (64 - shift));
+        p1 = (w[1] << shift) | (w[2] >> (64 - shift));
+        p2 = (w[2] << shift) | (w[3] >> (64 - shift));
     }
-    const uint64_t k0 = p2 | ((uint64_t)r << 8) | idx;
+    p0 = keep_bases(p0, (int)take);
+    p1 = keep_bases(p1, (int)take - 32);
+    p2 = keep_bases(p2, (int)take - 64);        // at most 24 bases: the low 16 bits are clear
+    const uint64_t k0 = p2 | ((uint64_t)take << 8) | idx;
     Key192 k;
     k.lo = make_uint4((uint32_t)k0, (uint32_t)(k0 >> 32), (uint32_t)p1, (uint32_t)(p1 >> 32));
     k.hi = make_uint2((uint32_t)p0, (uint32_t)(p0 >> 32));
@@ -330,7 +326,7 @@ __device__ __forceinline__ void count_if_less(uint32_t& acc, const uint4& alo, c
 }
 
 template <typename KeyT, typename IdT, bool FIRST, bool PACKED>
-__global__ void __launch_bounds__(kLocalThreads, 5) finish_tile_kernel(Reads R, const KeyT* __restrict__ keys1, uint32_t w1, uint32_t len_mask,
+__global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_kernel(Reads R, const KeyT* __restrict__ keys1, uint32_t w1, uint32_t len_mask,
                                                                     const uint32_t* __restrict__ heads_in, uint32_t* __restrict__ heads,
                                                                     IdT* __restrict__ ids, uint64_t n,
                                                                     uint32_t depth0, uint32_t cap, uint8_t* __restrict__ out,
@@ -355,11 +351,11 @@ __global__ void __launch_bounds__(kLocalThreads, 5) finish_tile_kernel(Reads R, 
                     const uint64_t pc = __ldcs(pairs + j);
                     const uint32_t kc = (uint32_t)(pc >> 32);
                     head = j == 0 || kc != (uint32_t)(__ldg(pairs + j - 1) >> 32) || (kc & len_mask) < w1;
-                    sm.id_a[e] = (IdT)(uint32_t)pc;
+                    sm.loc[e] = (uint32_t)pc;
                 } else {
                     const KeyT kc = __ldcs(keys1 + j);
                     head = j == 0 || kc != __ldg(keys1 + j - 1) || ((uint32_t)kc & len_mask) < w1;
-                    sm.id_a[e] = __ldcs(ids + j);
+                    sm.loc[e] = (uint64_t)__ldcs(ids + j);
                 }
             }
             const uint32_t word = __ballot_sync(kFull, head);
@@ -383,12 +379,17 @@ __global__ void __launch_bounds__(kLocalThreads, 5) finish_tile_kernel(Reads R, 
     __syncthreads();
 
     // ---- classify: groups that start in this tile and have at most cap members are ours -----------
+    // The kernel lives on random gathers (the offsets table, the word before the suffix, the key words); every batch
+    // of them is issued for all of a thread's positions before the first is used, so their latencies overlap.
     uint32_t n_active = 0, n_compares = 0;
+    IdT idv[kLocalItems];
+    uint32_t state = 0;   // 2 bits per position: 0 not ours, 1 alone in its group (final), 2 member of a group refined here
 #pragma unroll
     for (int k = 0; k < kLocalItems; ++k) {
         const int e = k * kLocalThreads + tid;
         uint16_t s = kNone, t = kNone;
-        uint8_t mine = 0;
+        uint32_t st = 0;
+        idv[k] = 0;
         if (base + e < n) {
             const int lo = e - (int)cap + 1;
             const int ps = prev_head(sm.hw, e, lo < 0 ? 0 : lo);
@@ -398,20 +399,67 @@ __global__ void __launch_bounds__(kLocalThreads, 5) finish_tile_kernel(Reads R, 
                     if (ne - ps >= 2) {
                         s = (uint16_t)ps;
                         t = (uint16_t)ne;
-                        mine = 1;
+                        st = 2;
                         ++n_active;
-                        if (!FIRST) sm.id_a[e] = ids[base + e];
                     } else if (FIRST) {
-                        mine = 1;   // alone in its group after the first sort: final
+                        st = 1;
                     }
                 }
+            }
+            if (FIRST) {
+                idv[k] = (IdT)sm.loc[e];
+                // packed input carries the ids inside the key words: hand those of the suffixes left to the global path over
+                if (PACKED && !st && e < kLocalTile) ids[base + e] = idv[k];
+            } else if (st) {
+                idv[k] = ids[base + e];
             }
         }
         sm.gs[e] = s;
         sm.ge[e] = t;
-        sm.mine[e] = mine;
-        // packed input carries the ids inside the key words: hand those of the suffixes left to the global path over
-        if (PACKED && FIRST && !mine && e < kLocalTile && base + e < n) ids[base + e] = sm.id_a[e];
+        state |= st << (2 * k);
+    }
+    {
+        uint64_t first_base[kLocalItems];   // index of the suffix's first base in the packed text
+        uint32_t left[kLocalItems];         // bases from there to the end of its read
+        const uint64_t pos_mask = (1ull << R.pos_bits) - 1;
+        if (R.uniform) {
+#pragma unroll
+            for (int k = 0; k < kLocalItems; ++k) {
+                const uint64_t read = (uint64_t)idv[k] >> R.pos_bits, pos = (uint64_t)idv[k] & pos_mask;
+                first_base[k] = read * R.uniform_len + pos;
+                left[k] = (uint32_t)(R.uniform_len - pos);
+            }
+        } else {
+            uint64_t lo[kLocalItems], hi[kLocalItems];
+#pragma unroll
+            for (int k = 0; k < kLocalItems; ++k) {
+                const uint64_t* p = R.offsets + (((state >> (2 * k)) & 3u) ? (uint64_t)idv[k] >> R.pos_bits : 0ull);
+                lo[k] = __ldg(p);
+                hi[k] = __ldg(p + 1);
+            }
+#pragma unroll
+            for (int k = 0; k < kLocalItems; ++k) {
+                const uint64_t pos = (uint64_t)idv[k] & pos_mask;
+                first_base[k] = lo[k] + pos;
+                left[k] = (uint32_t)(hi[k] - lo[k] - pos);
+            }
+        }
+        uint64_t before[kLocalItems];       // the word that holds the base before the suffix
+#pragma unroll
+        for (int k = 0; k < kLocalItems; ++k) {
+            const bool want = ((state >> (2 * k)) & 3u) && ((uint64_t)idv[k] & pos_mask);
+            before[k] = __ldg(R.packed + (want ? (first_base[k] - 1) >> 5 : 0ull));
+        }
+#pragma unroll
+        for (int k = 0; k < kLocalItems; ++k) {
+            const int e = k * kLocalThreads + tid;
+            const uint32_t st = (state >> (2 * k)) & 3u;
+            uint64_t code = 1;   // $: the suffix starts its read
+            if ((uint64_t)idv[k] & pos_mask) code = 2 + ((before[k] >> (62 - 2 * ((first_base[k] - 1) & 31))) & 3u);
+            const uint64_t loc = (code << (kLocBaseBits + kLocRemBits)) | ((uint64_t)left[k] << kLocBaseBits) | first_base[k];
+            if (FIRST && st == 1) out[base + e] = loc_symbol(loc);   // alone in its group after the first sort: final
+            sm.loc[e] = st == 2 ? loc : 0ull;
+        }
     }
     __syncthreads();
 
@@ -419,13 +467,33 @@ __global__ void __launch_bounds__(kLocalThreads, 5) finish_tile_kernel(Reads R, 
     for (uint32_t depth = depth0;; depth += kLocalW) {
         uint32_t any = 0;
 #pragma unroll
-        for (int k = 0; k < kLocalItems; ++k) {
-            const int e = k * kLocalThreads + tid;
-            const int s = sm.gs[e];
-            if (s != kNone) {
-                const Key192 kk = key192_at_depth(R, sm.id_a[e], depth, (uint32_t)(e - s));
-                sm.key_lo[e] = kk.lo;
-                sm.key_hi[e] = kk.hi;
+        for (int kk = 0; kk < kLocalItems; kk += 2) {
+            uint64_t w[2][4];
+            uint32_t take[2], shift[2];
+            int start[2];
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int e = (kk + j) * kLocalThreads + tid;
+                const bool exists = kk + j < kLocalItems;
+                start[j] = exists ? sm.gs[e] : kNone;
+                const uint64_t loc = exists ? sm.loc[e] : 0ull;
+                const uint32_t remaining = start[j] != kNone ? (uint32_t)(loc >> kLocBaseBits) & ((1u << kLocRemBits) - 1) : 0u;
+                const uint32_t rem = remaining > depth ? remaining - depth : 0u;
+                take[j] = rem < kLocalW ? rem : kLocalW;
+                const uint64_t b = (loc & ((1ull << kLocBaseBits) - 1)) + depth;
+                shift[j] = (uint32_t)(b & 31) * 2;
+                const uint32_t n_w = take[j] ? (shift[j] + 2 * take[j] + 63) >> 6 : 0u;   // words the window touches
+                const uint64_t* p = R.packed + (n_w ? b >> 5 : 0ull);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) w[j][i] = i < (int)n_w ? __ldg(p + i) : 0ull;
+            }
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                if (start[j] == kNone) continue;
+                const int e = (kk + j) * kLocalThreads + tid;
+                const Key192 key = key192_of_words(w[j], shift[j], take[j], (uint32_t)(e - start[j]));
+                sm.key_lo[e] = key.lo;
+                sm.key_hi[e] = key.hi;
                 any = 1;
             }
         }
@@ -494,7 +562,7 @@ __global__ void __launch_bounds__(kLocalThreads, 5) finish_tile_kernel(Reads R, 
             cur ^= 1;
         }
         const uint16_t* src = sm.ord[cur];
-        IdT idn[kLocalItems];
+        uint64_t locn[kLocalItems];
         uint32_t headbit = 0;
 #pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
@@ -502,7 +570,7 @@ __global__ void __launch_bounds__(kLocalThreads, 5) finish_tile_kernel(Reads R, 
             if (sm.gs[e] != kNone) {
                 const int se = src[e];
                 const uint4 kk = sm.key_lo[se];
-                idn[k] = sm.id_a[se];
+                locn[k] = sm.loc[se];
                 bool head = e == sm.gs[e] || ((kk.x >> 8) & 127u) < kLocalW;
                 if (!head) {   // same bases and length as the member ranked just before?  (the low 8 bits are the group index)
                     const int sp = src[e - 1];
@@ -518,7 +586,7 @@ __global__ void __launch_bounds__(kLocalThreads, 5) finish_tile_kernel(Reads R, 
         for (int k = 0; k < kLocalItems; ++k) {
             const int e = k * kLocalThreads + tid;
             if (sm.gs[e] != kNone) {
-                sm.id_a[e] = idn[k];
+                sm.loc[e] = locn[k];
                 if ((headbit >> k) & 1u) atomicOr(&sm.hw[e >> 5], 1u << (e & 31));
             }
         }
@@ -546,7 +614,8 @@ __global__ void __launch_bounds__(kLocalThreads, 5) finish_tile_kernel(Reads R, 
 #pragma unroll
     for (int k = 0; k < kLocalItems; ++k) {
         const int e = k * kLocalThreads + tid;
-        if (sm.mine[e]) out[base + e] = preceding_symbol(R, sm.id_a[e]);
+        const uint64_t loc = sm.loc[e];
+        if (loc) out[base + e] = loc_symbol(loc);
     }
     for (int i = tid; i < kLocalWords; i += kLocalThreads) {
         if (w0 + i > n_words) continue;
