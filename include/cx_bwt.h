@@ -57,6 +57,13 @@ typedef struct cx_bwt_opts_s {
     uint32_t small_group_max;    /* tie refinement: groups up to this many suffixes are finished inside one
                                     thread block; 0 = default (256); 1 = use only the global re-key + sort   */
     uint32_t profile;            /* 1: bracket every kernel with CUDA events (see cx_bwt_kernel_time)         */
+    uint32_t shard_index;        /* with shard_count > 1: which contiguous range of partitions this plan sorts     */
+    uint32_t shard_count;        /* 0 or 1: the whole collection.  W > 1: the paper's distributed scheme (PAPER.md:103,
+                                    Section 3.3): every worker holds all reads and computes the same partition sizes;
+                                    partition b belongs to worker floor(first_output_position(b) * W / N), so each
+                                    worker gets consecutive partitions of about N / W suffixes, sorts only those, and
+                                    writes them at their final positions of out_bwt; the pieces are disjoint and
+                                    "can be simply concatenated".  W <= 65536                    */
 } cx_bwt_opts_t;
 
 /* What the last cx_bwt_build on a plan did (HOST struct, filled by cx_bwt_get_stats). */
@@ -75,6 +82,8 @@ typedef struct cx_bwt_stats_s {
     uint32_t max_read_len;      /* longest read seen                                                    */
     uint32_t uniform_len;       /* 1 if every read has the same length (the paper's setting)*/
     uint32_t refined_partitions;/* l-prefix partitions larger than m1 that were partitioned again */
+    uint64_t shard_offset;      /* first position of out_bwt this build wrote (0 unless shard_count > 1)  */
+    uint64_t shard_suffixes;    /* positions written from there: the shard's piece of the BWT (N if unsharded) */
 } cx_bwt_stats_t;
 
 /* Kernel classes for cx_bwt_kernel_time; one per row of the hot path. */
@@ -131,6 +140,8 @@ int cx_pack_reads(const uint8_t *ascii_dev, uint64_t total_bases, uint64_t *pack
  *   read_offsets: DEVICE, n_reads+1 base offsets, [0] = 0, non-decreasing; total_bases = [n_reads]
  *   out_bwt     : N = total_bases + n_reads bytes over "$ACGT" (ASCII), equal to B_R of
  *                 PAPER.md:55.  DEVICE, or pinned HOST if the plan was made with out_is_host_pinned.
+ * With opts.shard_count = W > 1 only the bytes [stats.shard_offset, + stats.shard_suffixes) of out_bwt are
+ * written (the piece of worker opts.shard_index); out_bwt is still addressed from position 0.
  * Reads may have different lengths, including 0 (one suffix, preceded by '$').  n_reads = 0 is a
  * successful no-op.  Work is enqueued on `stream` (and joined side streams); the call synchronises
  * `stream` to read the partition sizes and once per refinement round, and returns after the last

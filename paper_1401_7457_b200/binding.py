@@ -28,14 +28,15 @@ class CxError(RuntimeError):
 class cx_bwt_opts_t(ctypes.Structure):
     _fields_ = [("prefix_len", ctypes.c_uint32), ("key_bases", ctypes.c_uint32), ("max_batch_suffixes", ctypes.c_uint64),
                 ("max_read_len", ctypes.c_uint32), ("out_is_host_pinned", ctypes.c_int32), ("small_group_max", ctypes.c_uint32),
-                ("profile", ctypes.c_uint32)]
+                ("profile", ctypes.c_uint32), ("shard_index", ctypes.c_uint32), ("shard_count", ctypes.c_uint32)]
 
 
 class cx_bwt_stats_t(ctypes.Structure):
     _fields_ = [("n_suffixes", ctypes.c_uint64), ("max_batch", ctypes.c_uint64), ("largest_bucket", ctypes.c_uint64),
                 ("refine_elements", ctypes.c_uint64), ("small_group_elems", ctypes.c_uint64), ("kernel_launches", ctypes.c_uint64), ("compare_ops", ctypes.c_uint64),
                 ("n_batches", ctypes.c_uint32), ("id_bytes", ctypes.c_uint32), ("sort_passes", ctypes.c_uint32),
-                ("refine_rounds", ctypes.c_uint32), ("max_read_len", ctypes.c_uint32), ("uniform_len", ctypes.c_uint32), ("refined_partitions", ctypes.c_uint32)]
+                ("refine_rounds", ctypes.c_uint32), ("max_read_len", ctypes.c_uint32), ("uniform_len", ctypes.c_uint32), ("refined_partitions", ctypes.c_uint32),
+                ("shard_offset", ctypes.c_uint64), ("shard_suffixes", ctypes.c_uint64)]
 
     def as_dict(self) -> dict:
         return {k: int(getattr(self, k)) for k, _ in self._fields_}

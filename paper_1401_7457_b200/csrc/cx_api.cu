@@ -67,6 +67,8 @@ struct Shape {
     uint32_t ell, w, cap, id_bytes, pos_bits, prefix_words;
     uint64_t n_buckets;
     bool host_out;
+    uint32_t shard_index, shard_count;   // NEXT-2: this plan sorts one of shard_count contiguous partition ranges
+    bool sharded() const { return shard_count > 1; }
 };
 
 Layout make_layout(const Shape& sh, uint64_t m1) {
@@ -81,7 +83,7 @@ Layout make_layout(const Shape& sh, uint64_t m1) {
     L.hist = take(sh.n_buckets * 8);
     L.tile_first = take((sh.max_tiles + 1) * 4);
     // per-tile counts of up to kCountGroup batches at a time; a plan that always fits one batch never counts
-    L.tile_count = take((sh.max_tiles + 1) * 8 * (sh.max_suffixes <= m1 ? 1 : kCountGroup));
+    L.tile_count = take((sh.max_tiles + 1) * 8 * (sh.max_suffixes <= m1 && !sh.sharded() ? 1 : kCountGroup));
     L.tile_sums = take((scan_block_count(sh.max_tiles + 1) + 1) * 8);
     L.scalars = take(64);
     L.prefix = take((uint64_t)(sh.prefix_words) * 8);
@@ -121,6 +123,9 @@ int make_shape(uint64_t max_reads, uint64_t max_bases, const cx_bwt_opts_t* o, S
     sh.id_bytes = sh.pos_bits + read_bits <= 32 ? 4 : 8;
     sh.n_buckets = (1ull << (2 * sh.ell)) * (sh.ell + 1);
     sh.host_out = o->out_is_host_pinned != 0;
+    sh.shard_count = o->shard_count ? o->shard_count : 1;
+    sh.shard_index = o->shard_index;
+    if (sh.shard_count > 65536 || sh.shard_index >= sh.shard_count) return CX_ERR_ARG;
     return CX_OK;
 }
 
@@ -327,6 +332,8 @@ struct Planner {
     uint64_t out = 0;
     Batch cur{};
     bool open = false;
+    uint64_t n_total = 0;                    // N, for the shard rule
+    uint64_t shard_lo = ~0ull, shard_n = 0;  // output range of this plan's shard
 
     void flush() {
         if (!open) return;
@@ -337,10 +344,24 @@ struct Planner {
     int region(uint32_t ri, const uint64_t* hist, bool top) {
         const Shape& sh = p->sh;
         const uint64_t nb = sh.n_buckets, m1 = p->m1;
+        uint64_t seen = 0;   // suffixes in the partitions before b (top level: their first position in the BWT)
         for (uint64_t b = 0; b < nb; ++b) {
             const uint64_t c = hist[b];
             if (c == 0) continue;
             if (top && c > p->stats.largest_bucket) p->stats.largest_bucket = c;
+            if (top && sh.sharded()) {
+                // "a contiguous range of partitions of roughly equal total size" per worker: a partition
+                // goes to the shard that its first output position falls in when [0, N) is cut into shard_count equal parts
+                const uint64_t owner = (uint64_t)(((unsigned __int128)seen * sh.shard_count) / n_total);
+                seen += c;
+                if (owner != sh.shard_index) {
+                    flush();
+                    out += c;
+                    continue;
+                }
+                if (shard_lo == ~0ull) shard_lo = seen - c;
+                shard_n += c;
+            }
             if (c > m1) {
                 flush();
                 const uint32_t r = (uint32_t)(b % (sh.ell + 1)), kmer = (uint32_t)(b / (sh.ell + 1));
@@ -459,7 +480,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     CX_CUDA(cudaMemsetAsync(d_scalars, 0, 64, s));
     // A plan whose largest legal input fits one batch needs no partition sizes to list its suffixes: the listing
     // scan then counts them on the way (one read of the collection instead of two).
-    const bool fused_scan = sh.max_suffixes <= p->m1;
+    const bool fused_scan = sh.max_suffixes <= p->m1 && !sh.sharded();
     const uint32_t w = sh.w;
     const uint32_t key_bits = 2 * w + key_len_bits(w);
     const uint32_t n_passes = (key_bits + kRadixBits - 1) / kRadixBits;
@@ -521,13 +542,16 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         memcpy(hist_out, p->h_hist2, sh.n_buckets * 8);
         return CX_OK;
     };
+    planner.n_total = N;
     int rc = planner.region(0, p->h_hist, true);
     if (rc) return rc;
     if (planner.out != N) return CX_ERR_CUDA;   // a mismatch means the partition scan misbehaved
     planner.assign_count_groups();
     p->stats.n_batches = (uint32_t)p->batches.size();
+    p->stats.shard_offset = sh.sharded() ? (planner.shard_n ? planner.shard_lo : N) : 0;
+    p->stats.shard_suffixes = sh.sharded() ? planner.shard_n : N;
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
-    const bool single = p->batches.size() == 1 && p->batches[0].ord_hi == ~0ull;
+    const bool single = p->batches.size() == 1 && p->batches[0].ord_hi == ~0ull && p->batches[0].count == N;
     if (fused_scan && !single) return CX_ERR_CUDA;   // cannot happen: N <= max_suffixes <= m1
     p->stats.sort_passes = (key_bits + kRadixBits - 1) / kRadixBits;
 
