@@ -54,6 +54,10 @@ def parse_args():
     ap.add_argument("--impl", default="cx", choices=["cx", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--key-bases", type=int, default=0, help="first-round key window w (0 = the library's default)")
+    ap.add_argument("--shard", action="store_true", help="NEXT-2, with --gpus N > 1 under torchrun: ONE collection, rank k sorts the k-th of N contiguous "
+                    "partition ranges (PAPER.md:103) and the pieces are exchanged (all-gather-v); strong scaling.  Default: independent replicas")
+    ap.add_argument("--shard-of", type=int, default=0, help="one GPU: time ONE shard of a W-way partition-range split (no exchange); with --shard-index")
+    ap.add_argument("--shard-index", type=int, default=0)
     ap.add_argument("--table4", type=int, default=0, help="NEXT-3: the paper's read-length experiment instead of a config: read length 100/200/400, "
                     "1e10 x --scale bases (PAPER.md:184-189)")
     ap.add_argument("--max-batch", type=int, default=0, help="m1: most suffixes per batch (0 = as many as the workspace allows)")
@@ -218,7 +222,7 @@ def run_cx(args) -> None:
     if args.table4:
         coll = gen.table4(args.table4, args.scale)
     else:
-        coll = gen.config(args.config, args.scale, seed=replica_seed(args.config, rank))
+        coll = gen.config(args.config, args.scale, seed=replica_seed(args.config, 0 if args.shard else rank))
     n_reads, total, N = coll.n_reads, coll.total_bases, coll.n_suffixes
     h_ascii = torch.from_numpy(coll.ascii).pin_memory()
     h_off = torch.from_numpy(coll.offsets.astype(np.int64)).pin_memory()
@@ -227,20 +231,30 @@ def run_cx(args) -> None:
     d_off = h_off.to(dev)
     d_packed = torch.empty((total + 31) // 32 + 1, dtype=torch.int64, device=dev)
     d_out = torch.empty(N, dtype=torch.uint8, device=dev)
+    sharded = bool(args.shard) and world > 1
     plan = cx.Plan(n_reads, total, max_read_len=coll.max_read_len, profile=1, key_bases=args.key_bases or None, max_batch_suffixes=args.max_batch or None,
-                   device=dev)
+                   shard_index=rank if sharded else (args.shard_index if args.shard_of > 1 else None),
+                   shard_count=world if sharded else (args.shard_of if args.shard_of > 1 else None), device=dev)
+    one_shard = args.shard_of > 1 and not sharded
+    units = 1 if sharded else world      # collections sorted per step by the whole job
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
     stream = torch.cuda.current_stream()
 
+    def build():
+        if sharded:
+            cx.build_sharded(plan, d_packed, d_off, n_reads, d_out)   # this rank's partition range, then the exchange of the pieces
+        else:
+            plan.build(d_packed, d_off, n_reads, d_out)
+
     def step_device():
         cx.cx_pack_reads(d_ascii, d_packed, check=False)
-        plan.build(d_packed, d_off, n_reads, d_out)
+        build()
 
     def step_e2e():
         d_ascii.copy_(h_ascii, non_blocking=True)
         d_off.copy_(h_off, non_blocking=True)
         cx.cx_pack_reads(d_ascii, d_packed, check=False)
-        plan.build(d_packed, d_off, n_reads, d_out)
+        build()
         h_out.copy_(d_out, non_blocking=True)
         stream.synchronize()
 
@@ -259,7 +273,9 @@ def run_cx(args) -> None:
     got = torch.bincount(d_out.to(torch.int64), minlength=128).cpu().numpy()
     want = np.bincount(coll.ascii, minlength=128)
     want[ord("$")] += n_reads
-    if not np.array_equal(got[:128], want[:128]):
+    if one_shard:
+        N = stats["shard_suffixes"]          # the piece this run sorts; its parity is tests/test_shard.py
+    elif not np.array_equal(got[:128], want[:128]):
         raise SystemExit("bench.py: output symbol counts differ from the input's")
 
     # ---- device-resident timing -----------------------------------------------------------------------
@@ -276,7 +292,7 @@ def run_cx(args) -> None:
         pack_ev[i][0].record(stream)
         cx.cx_pack_reads(d_ascii, d_packed, check=False)
         pack_ev[i][1].record(stream)
-        plan.build(d_packed, d_off, n_reads, d_out)
+        build()
         ev[i][1].record(stream)
         stream.synchronize()
         for k, v in plan.kernel_times().items():
@@ -323,18 +339,20 @@ def run_cx(args) -> None:
     total_alg = sum(v["bytes"] for v in classes.values()) / args.steps
     kern_ms = sum(v["ms"] for v in classes.values()) / args.steps
     line = {
-        "metric": METRIC, "value": world * N / (dev_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": dev_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": units * N / (dev_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": dev_ms, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
         "dtype": "u64", "data": "synthetic",
         "config": {"workload": (f"Table 4 shape (PAPER.md:184-189): reads of {args.table4} bp, 30x, both strands, 1% subst." if args.table4
                                 else WORKLOADS.get(args.config, str(args.config))) + (f" x scale {args.scale:g}" if args.scale != 1 else ""),
-                   "n_reads": n_reads, "total_bases": total, "n_suffixes": N, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "n_reads": n_reads, "total_bases": total, "n_suffixes": N, "parallelism": (f"{world} contiguous partition ranges (PAPER.md:103) + all-gather-v of the pieces" if sharded
+                                                                                       else "replicas only" if world > 1 else
+                                                                                       f"1 gpu, shard {args.shard_index} of {args.shard_of} only (its piece: {N} suffixes)" if one_shard else "1 gpu"),
                    "l2": "256 MiB L2-flush write between timed steps; working set >> L2", "prefix_len": 6, "key_bases": "auto (14 bases in a 32-bit key up to 2^30 suffixes, else ceil(log4 N)+1 bases in a 64-bit key)",
                    "id_bytes": stats["id_bytes"], "n_batches": stats["n_batches"], "sort_passes": stats["sort_passes"],
                    "refine_rounds": stats["refine_rounds"], "refine_elements": stats["refine_elements"],
                    "small_group_elems": stats["small_group_elems"]},
-        "gbases_per_hour": world * total / (dev_ms * 1e-3) * 3600 / 1e9,
-        "e2e": {"value": world * N / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+        "gbases_per_hour": units * total / (dev_ms * 1e-3) * 3600 / 1e9,
+        "e2e": {"value": units * N / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
                 "h2d_bytes_per_step": int(h_ascii.numel() + h_off.numel() * 8), "d2h_bytes_per_step": int(h_out.numel())},
         "gpu_launches": int(launches),
         "clocks": clocks,

@@ -40,6 +40,10 @@ def test_workspace_bytes_and_argument_errors():
     assert e.value.code == -1
     with pytest.raises(cx.CxError):
         cx.cx_bwt_workspace_bytes(10, 1000, key_bases=30)
+    with pytest.raises(cx.CxError):
+        cx.cx_bwt_workspace_bytes(10, 1000, shard_index=2, shard_count=2)       # NEXT-2: index must be below the count
+    # a sharded plan always needs the multi-batch count table, so it asks for a little more than the unsharded one
+    assert cx.cx_bwt_workspace_bytes(10_000, 1_000_000, max_read_len=100, shard_index=1, shard_count=2) > a
     L = cx.lib()
     assert L.cx_bwt_plan(None, 1, 1, None, None, 0) == -1
     assert L.cx_bwt_build(None, None, None, 1, None, None) == -1
