@@ -56,6 +56,8 @@ def parse_args():
     ap.add_argument("--key-bases", type=int, default=0, help="first-round key window w (0 = the library's default)")
     ap.add_argument("--shard", action="store_true", help="NEXT-2, with --gpus N > 1 under torchrun: ONE collection, rank k sorts the k-th of N contiguous "
                     "partition ranges (PAPER.md:103) and the pieces are exchanged (all-gather-v); strong scaling.  Default: independent replicas")
+    ap.add_argument("--fasta", action="store_true", help="NEXT-4: the step starts from the collection's FASTA text (resident in HBM; pinned host for e2e): "
+                    "cx_fasta_parse + pack + build")
     ap.add_argument("--shard-of", type=int, default=0, help="one GPU: time ONE shard of a W-way partition-range split (no exchange); with --shard-index")
     ap.add_argument("--shard-index", type=int, default=0)
     ap.add_argument("--table4", type=int, default=0, help="NEXT-3: the paper's read-length experiment instead of a config: read length 100/200/400, "
@@ -240,6 +242,23 @@ def run_cx(args) -> None:
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
     stream = torch.cuda.current_stream()
 
+    fasta_ev = []
+    if args.fasta:
+        h_text = torch.from_numpy(np.frombuffer(gen.to_fasta(coll, line_width=0), dtype=np.uint8).copy()).pin_memory()
+        d_text = h_text.to(dev)
+
+    def ingest(timed=False):
+        """ASCII bases + offsets of the step: resident already, or parsed from the FASTA text (NEXT-4)"""
+        if not args.fasta:
+            return d_ascii, d_off
+        if timed:
+            fasta_ev.append((torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)))
+            fasta_ev[-1][0].record(stream)
+        bases, offs = cx.cx_fasta_parse(d_text, max_reads=n_reads)
+        if timed:
+            fasta_ev[-1][1].record(stream)
+        return bases, offs
+
     def build():
         if sharded:
             cx.build_sharded(plan, d_packed, d_off, n_reads, d_out)   # this rank's partition range, then the exchange of the pieces
@@ -247,14 +266,21 @@ def run_cx(args) -> None:
             plan.build(d_packed, d_off, n_reads, d_out)
 
     def step_device():
-        cx.cx_pack_reads(d_ascii, d_packed, check=False)
-        build()
+        a, o = ingest()
+        cx.cx_pack_reads(a, d_packed, check=False)
+        build() if not args.fasta else plan.build(d_packed, o, n_reads, d_out)
 
     def step_e2e():
-        d_ascii.copy_(h_ascii, non_blocking=True)
-        d_off.copy_(h_off, non_blocking=True)
-        cx.cx_pack_reads(d_ascii, d_packed, check=False)
-        build()
+        if args.fasta:
+            d_text.copy_(h_text, non_blocking=True)
+            a, o = ingest()
+            cx.cx_pack_reads(a, d_packed, check=False)
+            plan.build(d_packed, o, n_reads, d_out)
+        else:
+            d_ascii.copy_(h_ascii, non_blocking=True)
+            d_off.copy_(h_off, non_blocking=True)
+            cx.cx_pack_reads(d_ascii, d_packed, check=False)
+            build()
         h_out.copy_(d_out, non_blocking=True)
         stream.synchronize()
 
@@ -289,10 +315,11 @@ def run_cx(args) -> None:
     for i in range(args.steps):
         flush.fill_(i)                       # L2 flush between timed iterations (outside the events)
         ev[i][0].record(stream)
+        a, o = ingest(timed=True)
         pack_ev[i][0].record(stream)
-        cx.cx_pack_reads(d_ascii, d_packed, check=False)
+        cx.cx_pack_reads(a, d_packed, check=False)
         pack_ev[i][1].record(stream)
-        build()
+        build() if not args.fasta else plan.build(d_packed, o, n_reads, d_out)
         ev[i][1].record(stream)
         stream.synchronize()
         for k, v in plan.kernel_times().items():
@@ -305,6 +332,10 @@ def run_cx(args) -> None:
     classes["pack"]["ms"] = sum(a.elapsed_time(b) for a, b in pack_ev)
     classes["pack"]["launches"] = args.steps
     classes["pack"]["bytes"] = args.steps * (total + total // 4)
+    if args.fasta:      # two reads of the text, one write of the bases, 8 B per read (cx_fasta.cu)
+        classes["fasta"] = {"ms": sum(a.elapsed_time(b) for a, b in fasta_ev), "launches": 10 * args.steps,
+                            "bytes": args.steps * (2 * h_text.numel() + total + 8 * n_reads)}
+        launches += 10 * args.steps
 
     # ---- end to end: pinned host in, pinned host out ----------------------------------------------------
     for _ in range(2):
@@ -343,7 +374,8 @@ def run_cx(args) -> None:
         "warmup": max(args.warmup, 3), "ms_per_step": dev_ms, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
         "dtype": "u64", "data": "synthetic",
         "config": {"workload": (f"Table 4 shape (PAPER.md:184-189): reads of {args.table4} bp, 30x, both strands, 1% subst." if args.table4
-                                else WORKLOADS.get(args.config, str(args.config))) + (f" x scale {args.scale:g}" if args.scale != 1 else ""),
+                                else WORKLOADS.get(args.config, str(args.config))) + (f" x scale {args.scale:g}" if args.scale != 1 else "")
+                               + (" [input: FASTA text, parsed on the device]" if args.fasta else ""),
                    "n_reads": n_reads, "total_bases": total, "n_suffixes": N, "parallelism": (f"{world} contiguous partition ranges (PAPER.md:103) + all-gather-v of the pieces" if sharded
                                                                                        else "replicas only" if world > 1 else
                                                                                        f"1 gpu, shard {args.shard_index} of {args.shard_of} only (its piece: {N} suffixes)" if one_shard else "1 gpu"),
@@ -353,7 +385,7 @@ def run_cx(args) -> None:
                    "small_group_elems": stats["small_group_elems"]},
         "gbases_per_hour": units * total / (dev_ms * 1e-3) * 3600 / 1e9,
         "e2e": {"value": units * N / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
-                "h2d_bytes_per_step": int(h_ascii.numel() + h_off.numel() * 8), "d2h_bytes_per_step": int(h_out.numel())},
+                "h2d_bytes_per_step": int(h_text.numel()) if args.fasta else int(h_ascii.numel() + h_off.numel() * 8), "d2h_bytes_per_step": int(h_out.numel())},
         "gpu_launches": int(launches),
         "clocks": clocks,
         "roofline": {"kernel": "onesweep_pass_kernel (a6, one radix pass)", "bound": "hbm", "achieved": round(achieved, 1),

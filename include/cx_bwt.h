@@ -134,6 +134,27 @@ int cx_pack_reads(const uint8_t *ascii_dev, uint64_t total_bases, uint64_t *pack
                   uint32_t *status_dev, cx_stream_t stream);
 
 /*
+ * NEXT-4, ingest: FASTA text -> the inputs of cx_pack_reads / cx_bwt_build, on the device.  "The input was in FASTA
+ * format"; loading is "more than 16 minutes" of the paper's 6,886 s.  Grammar taken (the
+ * paper gives none): lines end with '\n' (the last may lack it); a line whose first byte is '>' is a header and starts
+ * a new read; every other line is a sequence line whose bytes, except '\r', are appended to the current read (a read
+ * may span several lines, or none: length 0).  Bytes are copied as they are: cx_pack_reads rejects what is not ACGT.
+ *   text_dev       : DEVICE, n_bytes of FASTA text
+ *   bases_out_dev  : DEVICE, capacity n_bytes; receives the reads' bases, concatenated (the ascii_dev of cx_pack_reads)
+ *   offsets_out_dev: DEVICE, max_reads + 1 entries; receives read_offsets (entries past max_reads are never written)
+ *   counts_out_dev : DEVICE uint64[3]: reads found, bases found, sequence bytes met before the first header (these
+ *                    belong to no read: non-zero means the text is not FASTA and the other outputs are meaningless).
+ *                    The call is asynchronous; the caller reads counts after synchronising and must treat
+ *                    counts[0] > max_reads or counts[2] != 0 as an error.
+ *   workspace_dev  : DEVICE, cx_fasta_workspace_bytes(n_bytes) bytes, 256-byte aligned
+ * Errors: CX_ERR_ARG (null pointers, workspace too small), CX_ERR_CUDA.
+ */
+int cx_fasta_workspace_bytes(uint64_t n_bytes, uint64_t *bytes_out);
+int cx_fasta_parse(const uint8_t *text_dev, uint64_t n_bytes, uint8_t *bases_out_dev, uint64_t *offsets_out_dev,
+                   uint64_t max_reads, uint64_t *counts_out_dev, void *workspace_dev, uint64_t workspace_bytes,
+                   cx_stream_t stream);
+
+/*
  * The whole of Figure 2 on the device: partition sizes, batch ranges, and per
  * batch: list suffix ids, build keys, radix sort, refine ties, emit preceding symbols.
  *   packed_reads: DEVICE, ceil(total_bases/32) words in the cx_pack_reads layout

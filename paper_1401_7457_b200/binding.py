@@ -62,10 +62,13 @@ def lib() -> ctypes.CDLL:
         L.cx_bwt_kernel_time.argtypes = [vp, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(u64), ctypes.POINTER(u64)]
         L.cx_sort_pairs_workspace_bytes.argtypes = [u64, ctypes.POINTER(u64)]
         L.cx_sort_pairs.argtypes = [vp, vp, vp, vp, u64, u32, u32, u32, vp, u64, ctypes.POINTER(i32), vp]
+        L.cx_fasta_workspace_bytes.argtypes = [u64, ctypes.POINTER(u64)]
+        L.cx_fasta_parse.argtypes = [vp, u64, vp, vp, u64, vp, vp, u64, vp]
         L.cx_strerror.argtypes = [i32]
         L.cx_strerror.restype = ctypes.c_char_p
         for name in ("cx_bwt_workspace_bytes", "cx_bwt_plan", "cx_pack_reads", "cx_bwt_build", "cx_bwt_free", "cx_bwt_get_stats",
-                     "cx_bwt_get_histogram", "cx_bwt_kernel_time", "cx_sort_pairs_workspace_bytes", "cx_sort_pairs"):
+                     "cx_bwt_get_histogram", "cx_bwt_kernel_time", "cx_sort_pairs_workspace_bytes", "cx_sort_pairs",
+                     "cx_fasta_workspace_bytes", "cx_fasta_parse"):
             getattr(L, name).restype = i32
         _lib = L
     return _lib
@@ -200,6 +203,49 @@ def cx_sort_pairs(keys: torch.Tensor, vals: torch.Tensor, begin_bit: int = 0, en
     _check(lib().cx_sort_pairs(k0.data_ptr(), v0.data_ptr(), k1.data_ptr(), v1.data_ptr(), n, vals.element_size(), begin_bit,
                                end_bit, ws.data_ptr(), int(wsb.value), ctypes.byref(alt), _stream_ptr(stream)))
     return (k1, v1) if alt.value else (k0, v0)
+
+
+def cx_fasta_parse(text_dev: torch.Tensor, max_reads: int | None = None, stream=None):
+    """cx_fasta_parse: FASTA text (uint8, device) -> (bases uint8[total], read_offsets int64[n_reads + 1]), both on the device.
+    max_reads bounds the offsets buffer (default: one read per two bytes of text, the most a FASTA text can hold)."""
+    assert text_dev.is_cuda and text_dev.dtype == torch.uint8 and text_dev.is_contiguous()
+    n = text_dev.numel()
+    if max_reads is None:
+        max_reads = n // 2 + 1
+    wsb = ctypes.c_uint64(0)
+    _check(lib().cx_fasta_workspace_bytes(n, ctypes.byref(wsb)))
+    ws = torch.empty(int(wsb.value) + 256, dtype=torch.uint8, device=text_dev.device)
+    ws_ptr = (ws.data_ptr() + 255) // 256 * 256
+    bases = torch.empty(max(n, 1), dtype=torch.uint8, device=text_dev.device)
+    offsets = torch.empty(max_reads + 1, dtype=torch.int64, device=text_dev.device)
+    counts = torch.empty(3, dtype=torch.int64, device=text_dev.device)
+    with torch.cuda.device(text_dev.device):
+        _check(lib().cx_fasta_parse(text_dev.data_ptr(), n, bases.data_ptr(), offsets.data_ptr(), max_reads, counts.data_ptr(), ws_ptr,
+                                    int(wsb.value), _stream_ptr(stream)))
+        n_reads, total, orphans = (int(x) for x in counts.cpu())     # synchronises
+    if orphans:
+        raise CxError(-1, f"not FASTA: {orphans} sequence bytes before the first '>' header")
+    if n_reads > max_reads:
+        raise CxError(-1, f"{n_reads} reads in the text, max_reads = {max_reads}")
+    return bases[:total], offsets[:n_reads + 1]
+
+
+def bwt_of_fasta(text_host, device="cuda", **opts):
+    """Host FASTA bytes -> host BWT bytes (numpy): H2D copy, cx_fasta_parse, cx_pack_reads, cx_bwt_build, D2H copy."""
+    import numpy as np
+    t = torch.from_numpy(np.frombuffer(bytes(text_host), dtype=np.uint8).copy()).to(device)
+    bases, offsets = cx_fasta_parse(t)
+    n_reads, total = offsets.numel() - 1, bases.numel()
+    if n_reads <= 0:
+        return np.zeros(0, dtype=np.uint8)
+    packed = cx_pack_reads(bases) if total else torch.zeros(1, dtype=torch.int64, device=device)
+    opts.setdefault("max_read_len", max(int((offsets[1:] - offsets[:-1]).max()), 1))
+    plan = Plan(n_reads, total, **opts)
+    out = torch.empty(total + n_reads, dtype=torch.uint8, device=device)
+    plan.build(packed, offsets, n_reads, out)
+    res = out.cpu().numpy()
+    plan.free()
+    return res
 
 
 def bwt_of_collection(ascii_host, offsets_host, device="cuda", **opts):

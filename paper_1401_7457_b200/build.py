@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcxbwt.so")
-SOURCES = ["cx_pack.cu", "cx_scan_reads.cu", "cx_onesweep.cu", "cx_refine.cu", "cx_api.cu"]
+SOURCES = ["cx_pack.cu", "cx_fasta.cu", "cx_scan_reads.cu", "cx_onesweep.cu", "cx_refine.cu", "cx_api.cu"]
 HEADERS = ["cx_internal.cuh", "cx_launch.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I" + os.path.join(ROOT, "include"), "-I" + CSRC]

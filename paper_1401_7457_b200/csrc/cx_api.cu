@@ -281,6 +281,22 @@ extern "C" int cx_pack_reads(const uint8_t* ascii_dev, uint64_t total_bases, uin
     return CX_OK;
 }
 
+extern "C" int cx_fasta_workspace_bytes(uint64_t n_bytes, uint64_t* bytes_out) {
+    if (!bytes_out) return CX_ERR_ARG;
+    *bytes_out = fasta_workspace_bytes(n_bytes);
+    return CX_OK;
+}
+
+extern "C" int cx_fasta_parse(const uint8_t* text_dev, uint64_t n_bytes, uint8_t* bases_out_dev, uint64_t* offsets_out_dev, uint64_t max_reads,
+                              uint64_t* counts_out_dev, void* workspace_dev, uint64_t workspace_bytes, cx_stream_t stream) {
+    if (!offsets_out_dev || !counts_out_dev || (n_bytes && (!text_dev || !bases_out_dev || !workspace_dev))) return CX_ERR_ARG;
+    if (n_bytes && (workspace_bytes < fasta_workspace_bytes(n_bytes) || (reinterpret_cast<uintptr_t>(workspace_dev) & 255))) return CX_ERR_ARG;
+    if (n_bytes > (1ull << 43)) return CX_ERR_ARG;   // tiles are launched as one grid dimension
+    CX_CUDA(launch_fasta_parse(text_dev, n_bytes, bases_out_dev, offsets_out_dev, max_reads, counts_out_dev,
+                               static_cast<unsigned char*>(workspace_dev), stream));
+    return CX_OK;
+}
+
 extern "C" const char* cx_strerror(int code) {
     switch (code) {
     case CX_OK: return "ok";

@@ -143,6 +143,10 @@ __device__ __forceinline__ IdT make_id(uint64_t read, uint64_t pos, uint32_t pos
 struct Launch;   // profiling hook, defined in cx_api.cu
 
 // cx_pack.cu
+// NEXT-4: FASTA text -> bases + read offsets (cx_fasta.cu)
+uint64_t fasta_workspace_bytes(uint64_t n_bytes);
+cudaError_t launch_fasta_parse(const uint8_t* text, uint64_t n, uint8_t* bases_out, uint64_t* offsets_out, uint64_t max_reads, uint64_t* counts,
+                               unsigned char* ws, cudaStream_t s);
 cudaError_t launch_pack(const uint8_t* ascii, uint64_t total_bases, uint64_t* packed, uint32_t* status, cudaStream_t s);
 uint32_t* pack_fallback_status();
 

@@ -217,3 +217,35 @@ def random_collection(seed: int, n_reads: int, max_len: int, alphabet: str = "AC
     letters = np.frombuffer(alphabet.encode("ascii"), dtype=np.uint8)
     draws = H(seed, 21, np.arange(total, dtype=_U64)) % _U64(len(letters))
     return Collection(letters[draws.astype(np.int64)], offsets, f"rand{seed}")
+
+
+# ----------------------------------------------------------------------------------------------
+# FASTA text of a collection (input of the ingest step, NEXT-4; "The input was in FASTA format")
+# ----------------------------------------------------------------------------------------------
+def to_fasta(coll: Collection, line_width: int = 0, crlf: bool = False, final_newline: bool = True, seed: int | None = None) -> bytes:
+    """One record per read: a '>' header line, then the bases on lines of at most `line_width` bytes (0: one line;
+    an empty read has no sequence line).  With a seed, header texts vary in length and a few blank lines are strewn in
+    (both legal under the grammar of DESIGN.md section 16)."""
+    eol = b"\r\n" if crlf else b"\n"
+    parts = []
+    draws = H(seed, 9, np.arange(coll.n_reads, dtype=np.uint64)) if seed is not None else None
+    for i in range(coll.n_reads):
+        r = coll.ascii[int(coll.offsets[i]):int(coll.offsets[i + 1])].tobytes()
+        if draws is None:
+            parts.append(b">r%d" % i)
+        else:
+            d = int(draws[i])
+            parts.append(b">read_%d %s" % (i, b"x" * (d % 23)))
+            if d % 11 == 0:
+                parts.append(eol)      # a blank line after the header
+        parts.append(eol)
+        if r:
+            if line_width:
+                parts.append(eol.join(r[k:k + line_width] for k in range(0, len(r), line_width)))
+            else:
+                parts.append(r)
+            parts.append(eol)
+    text = b"".join(parts)
+    if not final_newline and text.endswith(eol):
+        text = text[:-len(eol)]
+    return text
