@@ -7,7 +7,7 @@
 // Every other line is a sequence line: its bytes, except '\r', are appended to the current read.  Sequence bytes
 // before the first header belong to no read ("orphans"): they are counted and the caller treats that as an error.
 //
-// Three steps, each a streaming pass over tiles of 4096 bytes (thread t owns 16 consecutive bytes):
+// Three steps, each a streaming pass over tiles of 16 KB (thread t owns 64 consecutive bytes):
 //   summarise : per tile, the kind of its last line start, its header count, and its base count split into the part
 //               whose kind is known inside the tile and the part that continues a line begun in an earlier tile;
 //   resolve   : per tile, the kind of the line it starts in (walk back over the tile kinds: one step unless a line
@@ -23,8 +23,9 @@ namespace {
 __host__ __device__ constexpr uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
 
 constexpr int kFaThreads = 256;
-constexpr int kFaBytes = 16;                       // per thread
-constexpr int kFaTile = kFaThreads * kFaBytes;     // 4096
+constexpr int kFaVec = 4;                          // 16-byte loads per thread
+constexpr int kFaBytes = 16 * kFaVec;              // consecutive bytes owned by a thread
+constexpr int kFaTile = kFaThreads * kFaBytes;     // 16384
 constexpr uint32_t kNone = 0, kHeader = 1, kSeq = 2;
 
 struct ThreadDecode {
@@ -34,29 +35,41 @@ struct ThreadDecode {
     uint32_t n_headers;   // header lines that start among my bytes
 };
 
-__device__ __forceinline__ uint8_t byte_of(const uint4& v, int i) {
-    const uint32_t w = i < 4 ? v.x : i < 8 ? v.y : i < 12 ? v.z : v.w;
-    return (uint8_t)(w >> (8 * (i & 3)));
+struct Chunk {
+    uint4 v[kFaVec];
+};
+__device__ __forceinline__ uint8_t byte_of(const Chunk& c, int i) {
+    const uint4& v = c.v[i >> 4];
+    const int j = i & 15;
+    const uint32_t w = j < 4 ? v.x : j < 8 ? v.y : j < 12 ? v.z : v.w;
+    return (uint8_t)(w >> (8 * (j & 3)));
 }
 
-// my 16 bytes (zero-filled past the end) and the byte before them ('\n' before the text: byte 0 starts a line)
-__device__ __forceinline__ void load_chunk(const uint8_t* __restrict__ text, uint64_t n, uint64_t at, uint4& v, uint8_t& prev, uint32_t& cnt) {
-    v = make_uint4(0, 0, 0, 0);
+// my bytes (zero-filled past the end) and the byte before them ('\n' before the text: byte 0 starts a line)
+__device__ __forceinline__ void load_chunk(const uint8_t* __restrict__ text, uint64_t n, uint64_t at, Chunk& c, uint8_t& prev, uint32_t& cnt) {
+#pragma unroll
+    for (int q = 0; q < kFaVec; ++q) c.v[q] = make_uint4(0, 0, 0, 0);
     cnt = 0;
     prev = '\n';
     if (at >= n) return;
     cnt = (uint32_t)min((uint64_t)kFaBytes, n - at);
     if (at) prev = text[at - 1];
     if (cnt == kFaBytes && ((reinterpret_cast<uintptr_t>(text) + at) & 15) == 0) {
-        v = __ldg(reinterpret_cast<const uint4*>(text + at));
+#pragma unroll
+        for (int q = 0; q < kFaVec; ++q) c.v[q] = __ldg(reinterpret_cast<const uint4*>(text + at) + q);
     } else {
-        uint32_t w[4] = {0, 0, 0, 0};
-        for (uint32_t i = 0; i < cnt; ++i) w[i >> 2] |= (uint32_t)text[at + i] << (8 * (i & 3));
-        v = make_uint4(w[0], w[1], w[2], w[3]);
+        uint32_t w[4 * kFaVec];
+#pragma unroll
+        for (int q = 0; q < 4 * kFaVec; ++q) w[q] = 0;
+#pragma unroll
+        for (int i = 0; i < kFaBytes; ++i)
+            if ((uint32_t)i < cnt) w[i >> 2] |= (uint32_t)text[at + i] << (8 * (i & 3));
+#pragma unroll
+        for (int q = 0; q < kFaVec; ++q) c.v[q] = make_uint4(w[4 * q], w[4 * q + 1], w[4 * q + 2], w[4 * q + 3]);
     }
 }
 
-__device__ __forceinline__ ThreadDecode decode(const uint4& v, uint8_t prev, uint32_t cnt) {
+__device__ __forceinline__ ThreadDecode decode(const Chunk& v, uint8_t prev, uint32_t cnt) {
     ThreadDecode d{kNone, 0, 0, 0};
     uint32_t kind = kNone;
 #pragma unroll
@@ -95,27 +108,27 @@ __device__ __forceinline__ uint32_t incoming_kind(uint32_t my_last, uint32_t* s_
     return k;
 }
 
-__device__ __forceinline__ uint32_t block_sum(uint32_t v, uint32_t* s_part) {
+__device__ __forceinline__ uint64_t block_sum(uint64_t v, uint64_t* s_part) {
     for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     __syncthreads();
     if (lane_id() == 0) s_part[threadIdx.x >> 5] = v;
     __syncthreads();
-    uint32_t t = 0;
+    uint64_t t = 0;
     for (int q = 0; q < kFaThreads / 32; ++q) t += s_part[q];
     return t;
 }
 
 // exclusive prefix of v over the block's threads
-__device__ __forceinline__ uint32_t block_excl(uint32_t v, uint32_t* s_part) {
-    uint32_t incl = v;
+__device__ __forceinline__ uint64_t block_excl(uint64_t v, uint64_t* s_part) {
+    uint64_t incl = v;
     for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t up = __shfl_up_sync(0xffffffffu, incl, o);
+        const uint64_t up = __shfl_up_sync(0xffffffffu, incl, o);
         if ((int)lane_id() >= o) incl += up;
     }
     __syncthreads();
     if (lane_id() == 31) s_part[threadIdx.x >> 5] = incl;
     __syncthreads();
-    uint32_t carry = 0;
+    uint64_t carry = 0;
     for (uint32_t q = 0; q < (threadIdx.x >> 5); ++q) carry += s_part[q];
     return carry + incl - v;
 }
@@ -129,17 +142,19 @@ struct TileSummary {
 
 __global__ void __launch_bounds__(kFaThreads) fasta_summarise_kernel(const uint8_t* __restrict__ text, uint64_t n, TileSummary* __restrict__ sums,
                                                                      uint8_t* __restrict__ tile_kind) {
-    __shared__ uint32_t s_last[kFaThreads / 32], s_part[kFaThreads / 32];
+    __shared__ uint32_t s_last[kFaThreads / 32];
+    __shared__ uint64_t s_part[kFaThreads / 32];
     const uint64_t at = (uint64_t)blockIdx.x * kFaTile + (uint64_t)threadIdx.x * kFaBytes;
-    uint4 v;
+    Chunk v;
     uint8_t prev;
     uint32_t cnt;
     load_chunk(text, n, at, v, prev, cnt);
     const ThreadDecode d = decode(v, prev, cnt);
     const uint32_t inc = incoming_kind(d.last_kind, s_last);
-    const uint32_t pre = block_sum(inc == kNone ? d.pre_cnt : 0u, s_part);
-    const uint32_t post = block_sum(d.post_bases + (inc == kSeq ? d.pre_cnt : 0u), s_part);
-    const uint32_t heads = block_sum(d.n_headers, s_part);
+    // three sums in one: each is at most kFaTile < 2^20
+    const uint64_t all = block_sum((uint64_t)(inc == kNone ? d.pre_cnt : 0u) | ((uint64_t)(d.post_bases + (inc == kSeq ? d.pre_cnt : 0u)) << 20) |
+                                   ((uint64_t)d.n_headers << 40), s_part);
+    const uint32_t pre = (uint32_t)all & 0xfffffu, post = (uint32_t)(all >> 20) & 0xfffffu, heads = (uint32_t)(all >> 40);
     if (threadIdx.x == kFaThreads - 1) {
         const uint32_t last = d.last_kind != kNone ? d.last_kind : inc;
         sums[blockIdx.x] = TileSummary{pre, post, heads, last};
@@ -170,9 +185,10 @@ __global__ void __launch_bounds__(kFaThreads) fasta_write_kernel(const uint8_t* 
                                                                  const uint64_t* __restrict__ base_at, const uint64_t* __restrict__ head_at,
                                                                  uint8_t* __restrict__ bases_out, uint64_t* __restrict__ offsets_out, uint64_t max_reads,
                                                                  unsigned long long* __restrict__ orphans) {
-    __shared__ uint32_t s_last[kFaThreads / 32], s_part[kFaThreads / 32];
+    __shared__ uint32_t s_last[kFaThreads / 32];
+    __shared__ uint64_t s_part[kFaThreads / 32];
     const uint64_t at = (uint64_t)blockIdx.x * kFaTile + (uint64_t)threadIdx.x * kFaBytes;
-    uint4 v;
+    Chunk v;
     uint8_t prev;
     uint32_t cnt;
     load_chunk(text, n, at, v, prev, cnt);
@@ -182,10 +198,11 @@ __global__ void __launch_bounds__(kFaThreads) fasta_write_kernel(const uint8_t* 
     const uint32_t my_bases = d.post_bases + (kind == kSeq ? d.pre_cnt : 0u);
     __shared__ uint8_t s_bases[kFaTile];   // the tile's bases in order: staged so that they leave as runs of consecutive bytes
     __shared__ uint32_t s_total;
-    uint32_t lb = block_excl(my_bases, s_part);                           // index of my first base among the tile's
+    const uint64_t both = block_excl((uint64_t)my_bases | ((uint64_t)d.n_headers << 32), s_part);   // two prefix sums in one
+    uint32_t lb = (uint32_t)both;                                         // index of my first base among the tile's
     if (threadIdx.x == kFaThreads - 1) s_total = lb + my_bases;
     const uint64_t tile_b = base_at[blockIdx.x];                          // index of the tile's first base in the output
-    uint64_t r = head_at[blockIdx.x] + block_excl(d.n_headers, s_part);   // reads started before my bytes
+    uint64_t r = head_at[blockIdx.x] + (both >> 32);                      // reads started before my bytes
     uint32_t lost = 0;
 #pragma unroll
     for (int i = 0; i < kFaBytes; ++i) {
