@@ -196,13 +196,16 @@ __global__ void __launch_bounds__(kFaThreads) fasta_write_kernel(const uint8_t* 
     uint32_t kind = incoming_kind(d.last_kind, s_last);
     if (kind == kNone) kind = tile_in[blockIdx.x];
     const uint32_t my_bases = d.post_bases + (kind == kSeq ? d.pre_cnt : 0u);
-    __shared__ uint8_t s_bases[kFaTile];   // the tile's bases in order: staged so that they leave as runs of consecutive bytes
+    // the tile's bases in order, staged so that they leave as aligned 16-byte stores: staged index i + skew holds the base
+    // that goes to bases_out[tile_b + i], skew = the low four address bits of that destination
+    __shared__ __align__(16) uint8_t s_bases[kFaTile + 16];
     __shared__ uint32_t s_total;
     const uint64_t both = block_excl((uint64_t)my_bases | ((uint64_t)d.n_headers << 32), s_part);   // two prefix sums in one
     uint32_t lb = (uint32_t)both;                                         // index of my first base among the tile's
     if (threadIdx.x == kFaThreads - 1) s_total = lb + my_bases;
     const uint64_t tile_b = base_at[blockIdx.x];                          // index of the tile's first base in the output
     uint64_t r = head_at[blockIdx.x] + (both >> 32);                      // reads started before my bytes
+    const uint32_t skew = (uint32_t)(reinterpret_cast<uintptr_t>(bases_out + tile_b) & 15);
     uint32_t lost = 0;
 #pragma unroll
     for (int i = 0; i < kFaBytes; ++i) {
@@ -217,27 +220,20 @@ __global__ void __launch_bounds__(kFaThreads) fasta_write_kernel(const uint8_t* 
             }
             if (kind == kSeq && c != '\n' && c != '\r') {
                 if (r == 0) ++lost;   // no header yet: the byte belongs to no read
-                s_bases[lb++] = c;
+                s_bases[skew + lb++] = c;
             }
             prev = c;
         }
     }
     __syncthreads();
     {
-        // aligned 16-byte stores for the body, single bytes for the ragged ends
-        const uint32_t total = s_total;
-        uint8_t* dst = bases_out + tile_b;
-        const uint32_t head = min(total, (uint32_t)((16 - (reinterpret_cast<uintptr_t>(dst) & 15)) & 15));
-        for (uint32_t i = threadIdx.x; i < head; i += kFaThreads) dst[i] = s_bases[i];
-        const uint32_t n16 = (total - head) / 16;
-        for (uint32_t q = threadIdx.x; q < n16; q += kFaThreads) {
-            const uint8_t* sp = s_bases + head + q * 16;
-            uint32_t w[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) w[k] = (uint32_t)sp[4 * k] | ((uint32_t)sp[4 * k + 1] << 8) | ((uint32_t)sp[4 * k + 2] << 16) | ((uint32_t)sp[4 * k + 3] << 24);
-            *reinterpret_cast<uint4*>(dst + head + q * 16) = make_uint4(w[0], w[1], w[2], w[3]);
-        }
-        for (uint32_t i = head + n16 * 16 + threadIdx.x; i < total; i += kFaThreads) dst[i] = s_bases[i];
+        const uint32_t end = skew + s_total;                 // staged bytes are [skew, end)
+        uint8_t* dst = bases_out + tile_b - skew;            // 16-byte aligned; dst[j] <- s_bases[j]
+        const uint32_t body_lo = skew ? 16u : 0u, body_hi = end & ~15u;
+        for (uint32_t j = skew + threadIdx.x; j < min(end, body_lo); j += kFaThreads) dst[j] = s_bases[j];
+        for (uint32_t j = body_lo + 16 * threadIdx.x; j + 16 <= body_hi; j += 16 * kFaThreads)
+            *reinterpret_cast<uint4*>(dst + j) = *reinterpret_cast<const uint4*>(s_bases + j);
+        for (uint32_t j = max(body_hi, body_lo) + threadIdx.x; j < end; j += kFaThreads) dst[j] = s_bases[j];
     }
     if (lost) atomicAdd(orphans, (unsigned long long)lost);
 }
