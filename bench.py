@@ -38,7 +38,7 @@ WORKLOADS = {
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture named here (None until one exists for this workload).
-NCU_TRAFFIC = {"file": "profiles/r01_ncu_full.md (onesweep_pass_kernel<u64 key|id word, keys-only>, configs[1])", "bytes_per_launch": 1_593_000_000}
+NCU_TRAFFIC = {"file": "profiles/r01_ncu_full.md (onesweep_pass_kernel<u64 key|id word, keys-only>, configs[1])", "bytes_per_launch": 1_592_000_000}
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 CPU_SAMPLE_SCALE = 0.1        # cpu_baseline leg: the workload's recipe at this scale (coverage preserved)
 REF_SAMPLE_SCALE = 0.05       # --impl reference: one step = the oracle on the recipe at this scale
