@@ -86,6 +86,7 @@ struct TileCtx {
     uint32_t uniform;   // every read has length L: slot -> (read, pos) by division, no offsets needed
     uint32_t L1;        // L + 1
     uint32_t pos0;      // position of slot g0 inside read r0 (uniform only)
+    float inv_L1;       // 1 / L1: slot -> read by a multiply and a one-step correction instead of an integer division
 };
 
 __device__ __forceinline__ TileCtx load_tile(const Reads& R, const BuildInfo* __restrict__ info,
@@ -96,6 +97,7 @@ __device__ __forceinline__ TileCtx load_tile(const Reads& R, const BuildInfo* __
     c.n_slots = (uint32_t)min((uint64_t)kListTile, N - c.g0);
     c.uniform = info->nonuniform ? 0u : 1u;
     c.L1 = (uint32_t)info->first_len + 1u;
+    c.inv_L1 = 1.0f / (float)c.L1;
     c.r0 = tile_first_read[t];
     c.pos0 = 0;
     c.n_tile_reads = 0;
@@ -129,7 +131,11 @@ __device__ __forceinline__ Slot decode_slot(const TileCtx& c, const TileSmem& sm
     uint64_t b;
     if (c.uniform) {
         const uint32_t x = c.pos0 + s;
-        const uint32_t rr = x / c.L1;
+        // x < L1 + kListTile, so x / L1 <= kListTile + 1: the float estimate is within one of it (the integer division
+        // this replaces was 8 % of the multi-batch listing's instructions)
+        uint32_t rr = (uint32_t)((float)x * c.inv_L1);
+        if ((uint64_t)rr * c.L1 > x) --rr;
+        else if ((uint64_t)(rr + 1) * c.L1 <= x) ++rr;
         sl.read = c.r0 + rr;
         sl.pos = x - rr * c.L1;
         sl.rem = (c.L1 - 1) - sl.pos;
@@ -205,7 +211,8 @@ __device__ __forceinline__ void walk_next(const TileCtx& c, const TileSmem& sm, 
 __device__ __forceinline__ uint32_t window_bucket(uint64_t window, uint32_t rem, uint32_t ell) {
     const uint32_t hi = (uint32_t)(window >> 32);
     const uint32_t r = rem < ell ? rem : ell;
-    const uint32_t kmer = r ? (hi >> (32 - 2 * r)) << (2 * (ell - r)) : 0u;
+    // the first l bases with those past the end of the read cleared (A-padded); no branch, valid for r = 0
+    const uint32_t kmer = (hi >> (32 - 2 * ell)) & (0xffffffffu << (2 * (ell - r)));
     return kmer * (ell + 1) + r;
 }
 // partition code of the walker's slot inside `region` (at the region's depth); false if the slot is outside it
@@ -216,6 +223,15 @@ __device__ __forceinline__ bool walk_bucket(const Reads& R, const Region& region
     if (REGION && !enter_region(R.packed, R.n_words, region, wk.b, window, rem)) return false;
     code = window_bucket(window, rem, ell);
     return true;
+}
+
+// digit histograms of the sort that follows (one shared-memory counter per pass and digit): constant shifts, so a
+// pass costs an extract and an atomic instead of a variable 64-bit shift inside a counted loop
+template <typename KeyT>
+__device__ __forceinline__ void digit_counts(uint32_t (*s_dh)[kRadix], KeyT key, uint32_t n_passes) {
+#pragma unroll
+    for (uint32_t p = 0; p < sizeof(KeyT); ++p)
+        if (p < n_passes) atomicAdd(&s_dh[p][(uint32_t)(key >> (p * kRadixBits)) & (kRadix - 1)], 1u);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -343,6 +359,7 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
     __shared__ TileSmem sm;
     __shared__ uint32_t s_dh[8][kRadix];
     __shared__ uint32_t s_warp[kListThreads / 32];
+    __shared__ uint16_t s_taken[kListTile];   // slots of the tile that belong to the batch, in slot order
     R.n_words = (info->total_bases + 31) >> 5;
     const uint64_t N = info->n_suffixes;
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
@@ -375,21 +392,33 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
         }
         if (lane_id() == 31) s_warp[warp] = incl;
         __syncthreads();
-        uint32_t before = incl - cnt;
-        for (uint32_t q = 0; q < warp; ++q) before += s_warp[q];
-        uint64_t dst = tile_base[t] + before;
+        uint32_t before = incl - cnt, total = 0;
+        for (uint32_t q = 0; q < kListThreads / 32; ++q) {
+            const uint32_t v = s_warp[q];
+            if (q < warp) before += v;
+            total += v;
+        }
+        // The taken slots are few and scattered over the threads: decoding them where they were found runs every warp
+        // for as many rounds as its busiest lane has slots, one or two lanes at a time.  They are compacted first (slot
+        // order = thread order) and then decoded one per thread: full warps, consecutive output addresses.
         while (mask) {
             const int i = __ffs(mask) - 1;
             mask &= mask - 1;
+            s_taken[before++] = (uint16_t)(s0 + i);
+        }
+        __syncthreads();
+        const uint64_t tile_dst = tile_base[t];
+        for (uint32_t j = threadIdx.x; j < total; j += kListThreads) {
+            const uint64_t dst = tile_dst + j;
             if (dst >= ord_lo && dst < ord_hi) {
-                Slot sl = decode_slot(c, sm, s0 + i);
+                Slot sl = decode_slot(c, sm, s_taken[j]);
                 if (REGION) {
                     sl.window = load_window(R.packed, R.n_words, sl.b + region.depth);
                     sl.rem -= region.depth;
                 }
                 const KeyT key = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
                 const IdT id = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
-                for (uint32_t p = 0; p < n_passes; ++p) atomicAdd(&s_dh[p][(uint32_t)(key >> (p * kRadixBits)) & (kRadix - 1)], 1u);
+                digit_counts(s_dh, key, n_passes);
                 const uint64_t at = dst - ord_lo;
                 if constexpr (PACKED) {
                     reinterpret_cast<uint64_t*>(keys)[at] = ((uint64_t)key << 32) | (uint64_t)id;
@@ -398,7 +427,6 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
                     ids[at] = id;
                 }
             }
-            ++dst;
         }
     }
     __syncthreads();
@@ -451,7 +479,7 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
             }
             const KeyT key = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
             const IdT id = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
-            for (uint32_t p = 0; p < n_passes; ++p) atomicAdd(&s_dh[p][(uint32_t)(key >> (p * kRadixBits)) & (kRadix - 1)], 1u);
+            digit_counts(s_dh, key, n_passes);
             if constexpr (PACKED) {
                 reinterpret_cast<uint64_t*>(keys)[c.g0 + s] = ((uint64_t)key << 32) | (uint64_t)id;
             } else {
@@ -556,6 +584,13 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
     };
     if (tile_base == nullptr) return packed ? launch(list_write_kernel<KeyT, IdT, kCanPack>) : launch(list_write_kernel<KeyT, IdT, false>);
     auto select = [&](auto kernel) {
+        // persistent blocks: exactly as many as are resident at once (48 registers: five per SM); a sixth per SM would
+        // run as a second wave on an almost empty machine
+        int per_sm = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kListThreads, 0);
+        if (e != cudaSuccess) return e;
+        const uint64_t resident = (uint64_t)n_sms * (per_sm > 0 ? per_sm : 1);
+        const unsigned grid = (unsigned)(n_tiles < resident ? n_tiles : resident);
         kernel<<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids, n_passes, dh, region, ord_lo,
                                              ord_hi);
         return cudaGetLastError();
