@@ -208,12 +208,33 @@ __device__ __forceinline__ void walk_next(const TileCtx& c, const TileSmem& sm, 
         wk.rem = c.uniform ? c.L1 - 1 : (uint32_t)(sm.off[wk.lo + 1] - sm.off[wk.lo]);
     }
 }
-__device__ __forceinline__ uint32_t window_bucket(uint64_t window, uint32_t rem, uint32_t ell) {
-    const uint32_t hi = (uint32_t)(window >> 32);
+// hi: the next 16 bases of the suffix (the high word of its window)
+__device__ __forceinline__ uint32_t window_bucket32(uint32_t hi, uint32_t rem, uint32_t ell) {
     const uint32_t r = rem < ell ? rem : ell;
     // the first l bases with those past the end of the read cleared (A-padded); no branch, valid for r = 0
     const uint32_t kmer = (hi >> (32 - 2 * ell)) & (0xffffffffu << (2 * (ell - r)));
     return kmer * (ell + 1) + r;
+}
+__device__ __forceinline__ uint32_t window_bucket(uint64_t window, uint32_t rem, uint32_t ell) {
+    return window_bucket32((uint32_t)(window >> 32), rem, ell);
+}
+// Outside a region the partition code needs only the first l <= 7 bases of a suffix, and a thread walks kListItems = 8
+// consecutive slots: the 16 bases in the high word of the first slot's window serve all of them (7 shifts of one base
+// leave 9 >= l), so the walk is one 32-bit shift per slot instead of two 64-bit funnel shifts.
+struct Walk32 {
+    uint32_t top, rem, lo;
+};
+static_assert(16 - (kListItems - 1) >= 7, "the high word must still hold l bases at the last slot of a thread");
+__device__ __forceinline__ Walk32 walk32_of(const Walk& wk) { return Walk32{(uint32_t)(wk.window >> 32), wk.rem, wk.lo}; }
+// step to the next slot; `more`: that slot is still inside the tile (its read's length is staged)
+__device__ __forceinline__ void walk32_next(const TileCtx& c, const TileSmem& sm, Walk32& w, bool more) {
+    if (w.rem) {
+        w.top <<= 2;
+        w.rem -= 1;
+    } else if (more) {   // end-marker slot: the next read starts at the same base index
+        w.lo += 1;
+        w.rem = c.uniform ? c.L1 - 1 : (uint32_t)(sm.off[w.lo + 1] - sm.off[w.lo]);
+    }
 }
 // partition code of the walker's slot inside `region` (at the region's depth); false if the slot is outside it
 template <bool REGION>
@@ -315,17 +336,26 @@ __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const
         const uint32_t s0 = threadIdx.x * kListItems;
         if (s0 < c.n_slots) {
             Walk wk = walk_init(c, sm, s0);
+            Walk32 w32 = walk32_of(wk);
+            const uint32_t n_here = min((uint32_t)kListItems, c.n_slots - s0);
 #pragma unroll
             for (int i = 0; i < kListItems; ++i) {
-                if (s0 + i < c.n_slots) {
+                if ((uint32_t)i < n_here) {
                     uint32_t b = 0;
-                    if (walk_bucket<REGION>(R, region, wk, ell, b) && b >= ranges.first[0] && b < ranges.first[ranges.n]) {
+                    bool in;
+                    if constexpr (REGION) in = walk_bucket<true>(R, region, wk, ell, b);
+                    else in = true, b = window_bucket32(w32.top, w32.rem, ell);
+                    if (in && b >= ranges.first[0] && b < ranges.first[ranges.n]) {
                         uint32_t j = 0;
 #pragma unroll
                         for (int q = 1; q < kCountGroup; ++q) j += (q < (int)ranges.n && b >= ranges.first[q]);
                         mine += 1ull << (8 * j);
                     }
-                    if (s0 + i + 1 < c.n_slots) walk_next(c, sm, wk);
+                    if constexpr (REGION) {
+                        if ((uint32_t)i + 1 < n_here) walk_next(c, sm, wk);
+                    } else {
+                        walk32_next(c, sm, w32, (uint32_t)i + 1 < n_here);
+                    }
                 }
             }
         }
@@ -374,12 +404,19 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
         uint32_t mask = 0;   // which of my kListItems consecutive slots belong to this batch
         if (s0 < c.n_slots) {
             Walk wk = walk_init(c, sm, s0);
+            Walk32 w32 = walk32_of(wk);
+            const uint32_t n_here = min((uint32_t)kListItems, c.n_slots - s0);
 #pragma unroll
             for (int i = 0; i < kListItems; ++i) {
-                if (s0 + i < c.n_slots) {
-                    uint32_t b = 0;
-                    mask |= (uint32_t)(walk_bucket<REGION>(R, region, wk, ell, b) && b - bucket_lo <= bucket_hi - bucket_lo) << i;
-                    if (s0 + i + 1 < c.n_slots) walk_next(c, sm, wk);
+                if ((uint32_t)i < n_here) {
+                    if constexpr (REGION) {
+                        uint32_t b = 0;
+                        mask |= (uint32_t)(walk_bucket<true>(R, region, wk, ell, b) && b - bucket_lo <= bucket_hi - bucket_lo) << i;
+                        if ((uint32_t)i + 1 < n_here) walk_next(c, sm, wk);
+                    } else {
+                        mask |= (uint32_t)(window_bucket32(w32.top, w32.rem, ell) - bucket_lo <= bucket_hi - bucket_lo) << i;
+                        walk32_next(c, sm, w32, (uint32_t)i + 1 < n_here);
+                    }
                 }
             }
         }
