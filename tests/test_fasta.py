@@ -122,3 +122,18 @@ def test_fasta_text_to_bwt_end_to_end():
     assert np.array_equal(got, oracle.bwt(c.ascii, c.offsets))
     with pytest.raises(cx.CxError):
         cx.bwt_of_fasta(b">r0\nACNT\n")                      # A8: bytes outside ACGT are rejected by the pack step
+
+
+@pytest.mark.gpu
+def test_parse_texts_around_the_tile_size():
+    """Texts of exactly one tile (16 KB), one byte less and one more; a header and a CRLF pair straddling a tile edge;
+    a tile of nothing but line ends."""
+    tile = 16384
+    for n in (tile - 1, tile, tile + 1, 2 * tile, 2 * tile + 17):
+        body = (b"ACGT" * (n // 4 + 1))[:n - 3]
+        _assert_parse_parity(b">x\n" + body)                                   # one read, no final newline, n bytes in all
+    head = b">" + b"h" * 40 + b"\n"
+    for cut in range(tile - 45, tile + 3, 7):                                 # the header line slides across the tile edge
+        pre = (b">a\n" + b"ACGT" * (tile // 4))[:cut - 1] + b"\n"
+        _assert_parse_parity(pre + head + b"GGAA\r\nTT\r\n")
+    _assert_parse_parity(b">a\nAC" + b"\r\n" * (tile // 2 + 5) + b"GT\n>b\n" + b"\n" * tile + b"T")

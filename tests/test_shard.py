@@ -133,3 +133,27 @@ def test_check_pieces():
     for bad in ([(0, 5), (6, 6)], [(0, 5), (5, 6)], [(1, 11)]):
         with pytest.raises(RuntimeError):
             shard.check_pieces(bad, 12)
+
+
+@pytest.mark.gpu
+def test_shards_stream_to_pinned_host_and_slice_the_end_marker_partition():
+    """Pinned-host output (a9) inside a shard, and m1 below n_reads so that the partition of bare end-markers (identical
+    suffixes) is cut into slices of the listing order inside the shard that owns it."""
+    import paper_1401_7457_b200 as cx
+    c = gen.config(1, 0.005)                                   # 5,000 reads
+    want = oracle.bwt(c.ascii, c.offsets)
+    a = torch.from_numpy(c.ascii).cuda()
+    off = torch.from_numpy(c.offsets.astype(np.int64)).cuda()
+    packed = cx.cx_pack_reads(a)
+    out = torch.full((c.n_suffixes,), ord("?"), dtype=torch.uint8).pin_memory()
+    pieces = []
+    for k in range(3):
+        p = cx.Plan(c.n_reads, c.total_bases, max_read_len=100, max_batch_suffixes=3_000, out_is_host_pinned=1, shard_index=k, shard_count=3)
+        p.build(packed, off, c.n_reads, out)
+        torch.cuda.synchronize()
+        st = p.stats()
+        pieces.append((st["shard_offset"], st["shard_suffixes"]))
+        assert st["n_batches"] > 3
+        p.free()
+    cx.check_pieces(pieces, c.n_suffixes)
+    assert np.array_equal(out.numpy(), want)
