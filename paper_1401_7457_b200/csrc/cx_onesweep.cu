@@ -265,8 +265,9 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ 
         if (full || e < tile_n) {
             const KeyT kk = sm.keys[e];
             const uint32_t dst = sm.gofs[(uint32_t)(kk >> shift) & digit_mask] + e;
-            keys_out[dst] = kk;
-            if constexpr (kHasVals) vals_out[dst] = sm.vals[e];
+            // streaming stores: a pass's output is next read by the following launch, long after it has left L2
+            __stcs(keys_out + dst, kk);
+            if constexpr (kHasVals) __stcs(vals_out + dst, sm.vals[e]);
         }
     }
 }
