@@ -157,3 +157,49 @@ def test_shards_stream_to_pinned_host_and_slice_the_end_marker_partition():
         p.free()
     cx.check_pieces(pieces, c.n_suffixes)
     assert np.array_equal(out.numpy(), want)
+
+
+# ---- build_sharded end to end on CPU: two gloo ranks, a stand-in plan that writes the oracle's piece ----------------
+class _PieceWriter:
+    """Stands in for cx.Plan on a machine without a GPU: `build` writes this rank's piece of a BWT computed by the oracle
+    (cut at a fixed position) and `stats` reports it, which is all build_sharded needs to drive the exchange."""
+
+    def __init__(self, full, lo, hi):
+        self.full, self.lo, self.hi = full, lo, hi
+
+    def build(self, packed, offsets, n_reads, out, stream=None):
+        out[self.lo:self.hi] = self.full[self.lo:self.hi]
+
+    def stats(self):
+        return {"shard_offset": self.lo, "shard_suffixes": self.hi - self.lo}
+
+
+def _sharded_worker(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import sys
+    sys.path.insert(0, ROOT)
+    from paper_1401_7457_b200 import shard
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    c = gen.config(0, 0.01)                                                  # every rank holds the same reads (PAPER.md:103)
+    full = torch.from_numpy(oracle.bwt(c.ascii, c.offsets))
+    cut = [0, c.n_suffixes // 3, c.n_suffixes]
+    out = torch.zeros(c.n_suffixes, dtype=torch.uint8)
+    pieces = shard.build_sharded(_PieceWriter(full, cut[rank], cut[rank + 1]), None, None, c.n_reads, out)
+    ok = bool(torch.equal(out, full))
+    dist.barrier()
+    dist.destroy_process_group()
+    q.put((rank, ok, pieces == [(cut[0], cut[1] - cut[0]), (cut[1], cut[2] - cut[1])]))
+
+
+def test_build_sharded_two_gloo_ranks_with_a_stand_in_plan():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 33500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_sharded_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=180) for _ in procs)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    assert all(ok and pieces_ok for _, ok, pieces_ok in res)
