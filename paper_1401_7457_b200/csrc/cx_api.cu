@@ -518,6 +518,9 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     const BuildInfo info = *p->h_info;
     if (info.bad_offsets || info.total_bases > sh.max_bases || (info.max_len >> sh.pos_bits) != 0) return CX_ERR_ARG;
     const uint64_t N = info.n_suffixes;
+    // the in-block path keeps (bases left : 21 bits, first base : 40 bits) per suffix in one locator word; a collection
+    // outside those widths is refined by the global path only, which works on ids
+    const uint32_t cap = (info.max_len >= (1ull << 21) || info.total_bases >= (1ull << 40)) ? 1u : sh.cap;
     if (fused_scan) prof->bytes[CX_K_LIST] += info.total_bases / 4 + (n_reads + 1) * 8 + N * (sizeof(KeyT) + sizeof(IdT));
     else prof->bytes[CX_K_HIST] += info.total_bases / 4 + (n_reads + 1) * 8;
     R.n_words = (info.total_bases + 31) >> 5;
@@ -622,7 +625,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         CX_CUDA(cudaMemsetAsync(d_heads[0], 0, (n_words + 1) * 4, s));
         {
             ScopedLaunch sl(prof, CX_K_FINISH, nb * (sizeof(KeyT) + sizeof(IdT) + 1) + nb / 8, s);
-            CX_CUDA((launch_finish_first<KeyT, IdT>(R, d_keys1[cur], w, depth_base + w, d_heads[0], ids, nb, sh.cap, dst, d_done, pack_kv, s)));
+            CX_CUDA((launch_finish_first<KeyT, IdT>(R, d_keys1[cur], w, depth_base + w, d_heads[0], ids, nb, cap, dst, d_done, pack_kv, s)));
         }
         // ---- what is still tied goes through global rounds: re-key, sort, write back ------------------
         uint32_t depth = depth_base + w, rounds = 0;
@@ -662,10 +665,10 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             p->stats.refine_elements += n_act;
             depth += w_r;
             ++rounds;
-            if (sh.cap > 1) {
+            if (cap > 1) {
                 CX_CUDA(cudaMemcpyAsync(d_heads[1 - hc], d_heads[hc], (n_words + 1) * 4, cudaMemcpyDeviceToDevice, s));
                 ScopedLaunch sl(prof, CX_K_FINISH, nb / 4, s);
-                CX_CUDA(launch_finish_later<IdT>(R, d_heads[hc], d_heads[1 - hc], ids, nb, depth, sh.cap, dst, d_done, s));
+                CX_CUDA(launch_finish_later<IdT>(R, d_heads[hc], d_heads[1 - hc], ids, nb, depth, cap, dst, d_done, s));
                 hc = 1 - hc;
             }
         }

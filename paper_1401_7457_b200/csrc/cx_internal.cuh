@@ -142,6 +142,13 @@ __device__ __forceinline__ IdT make_id(uint64_t read, uint64_t pos, uint32_t pos
 // ---------------------------------------------------------------------------------------------
 struct Launch;   // profiling hook, defined in cx_api.cu
 
+// SMs of the current device (grids of the persistent kernels are sized from it; nothing assumes 148)
+inline int sm_count() {
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return 1;
+    return n;
+}
+
 // cx_pack.cu
 // NEXT-4: FASTA text -> bases + read offsets (cx_fasta.cu)
 uint64_t fasta_workspace_bytes(uint64_t n_bytes);

@@ -302,13 +302,9 @@ cudaError_t sort_pairs_shape(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_
     static_assert(kTile >= kSortTileMin, "the tile-state array is sized for tiles of at least kSortTileMin pairs");
     using Smem = PassSmem<KeyT, ValT, kSortThreads, ITEMS>;
     auto kernel = onesweep_pass_kernel<KeyT, ValT, kSortThreads, ITEMS, kMinBlocks>;
-    static bool attr_set = false;
-    cudaError_t e;
-    if (!attr_set) {
-        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    // per device and context, and cheap: set on every call (a cached flag would be wrong on a second GPU)
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
+    if (e != cudaSuccess) return e;
     const uint32_t n_passes = (end_bit - begin_bit + kRadixBits - 1) / kRadixBits;
     const uint64_t n_tiles = (n + kTile - 1) / kTile;
     if (n_tiles > ws.max_tiles || n_passes > 8 || n > 0xFFFF0000ull) return cudaErrorInvalidValue;
@@ -318,7 +314,8 @@ cudaError_t sort_pairs_shape(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_
         if (e != cudaSuccess) return e;
         uint64_t chunk = (uint64_t)kHistThreads * kHistItems;
         uint64_t blocks = (n + chunk - 1) / chunk;
-        unsigned grid = (unsigned)(blocks < 148ull * 4 ? blocks : 148ull * 4);
+        const uint64_t want = (uint64_t)sm_count() * 4;
+        unsigned grid = (unsigned)(blocks < want ? blocks : want);
         ScopedLaunch sl(prof, CX_K_SORT_HIST, n * sizeof(KeyT), s);
         digit_hist_kernel<KeyT><<<grid, kHistThreads, 0, s>>>(keys, n, begin_bit, end_bit, n_passes, (unsigned long long*)ws.hist);
     }

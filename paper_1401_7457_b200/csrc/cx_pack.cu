@@ -59,7 +59,8 @@ cudaError_t launch_pack(const uint8_t* ascii, uint64_t total_bases, uint64_t* pa
     uint64_t n_words = (total_bases + 31) >> 5;
     if (n_words == 0) return cudaSuccess;
     uint64_t blocks = (n_words + 255) / 256;
-    unsigned grid = (unsigned)(blocks < 148ull * 32 ? blocks : 148ull * 32);
+    const uint64_t want = (uint64_t)sm_count() * 32;
+    unsigned grid = (unsigned)(blocks < want ? blocks : want);
     if ((reinterpret_cast<uintptr_t>(ascii) & 15) == 0)
         pack_kernel<true><<<grid, 256, 0, s>>>(ascii, total_bases, packed, status);
     else

@@ -448,7 +448,7 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
 #pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
             const bool want = ((state >> (2 * k)) & 3u) && ((uint64_t)idv[k] & pos_mask);
-            before[k] = __ldg(R.packed + (want ? (first_base[k] - 1) >> 5 : 0ull));
+            before[k] = want ? __ldg(R.packed + ((first_base[k] - 1) >> 5)) : 0ull;   // no load at all for a read's first suffix (packed may hold no word)
         }
 #pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
@@ -483,7 +483,7 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
                 const uint64_t b = (loc & ((1ull << kLocBaseBits) - 1)) + depth;
                 shift[j] = (uint32_t)(b & 31) * 2;
                 const uint32_t n_w = take[j] ? (shift[j] + 2 * take[j] + 63) >> 6 : 0u;   // words the window touches
-                const uint64_t* p = R.packed + (n_w ? b >> 5 : 0ull);
+                const uint64_t* p = R.packed + (b >> 5);
 #pragma unroll
                 for (int i = 0; i < 4; ++i) w[j][i] = i < (int)n_w ? __ldg(p + i) : 0ull;
             }
@@ -700,12 +700,8 @@ cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32
                                 uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
     auto kernel = finish_tile_kernel<uint64_t, IdT, false, false>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem<IdT>));
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem<IdT>));
+    if (e != cudaSuccess) return e;
     if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
     uint64_t blocks = (n + kLocalTile - 1) / kLocalTile;
     kernel<<<(unsigned)blocks, kLocalThreads, sizeof(LocalSmem<IdT>), s>>>(R, nullptr, 0, 0, heads_in, heads_out, const_cast<IdT*>(ids), n, depth, group_cap, out,

@@ -554,7 +554,8 @@ cudaError_t launch_prep(const uint64_t* offsets, uint64_t n_reads, uint64_t max_
     cudaError_t e = cudaMemsetAsync(info, 0, sizeof(BuildInfo), s);
     if (e != cudaSuccess) return e;
     uint64_t blocks = (n_reads + 255) / 256;
-    unsigned grid = (unsigned)(blocks < 148ull * 8 ? (blocks ? blocks : 1) : 148ull * 8);
+    const uint64_t want = (uint64_t)sm_count() * 8;
+    unsigned grid = (unsigned)(blocks < want ? (blocks ? blocks : 1) : want);
     prep_kernel<<<grid, 256, 0, s>>>(offsets, n_reads, max_bases, info);
     return cudaGetLastError();
 }
@@ -573,12 +574,8 @@ cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint
                                uint64_t* hist, uint64_t max_tiles, int n_sms, cudaStream_t s) {
     if (max_tiles == 0) return cudaSuccess;
     size_t smem = bucket_hist_smem(ell);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(bucket_hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bucket_hist_smem(7));
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    cudaError_t e = cudaFuncSetAttribute(bucket_hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bucket_hist_smem(7));
+    if (e != cudaSuccess) return e;
     int per_sm = ell <= 6 ? 4 : 2;
     uint64_t want = (uint64_t)n_sms * per_sm;
     unsigned grid = (unsigned)(max_tiles < want ? max_tiles : want);
@@ -589,7 +586,7 @@ cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint
 cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, const Region& region,
                               const CountRanges& ranges, uint64_t* tile_count, uint64_t col_stride, uint64_t n_tiles, cudaStream_t s) {
     if (n_tiles == 0 || ranges.n == 0) return cudaSuccess;
-    uint64_t want = 148ull * 8;
+    uint64_t want = (uint64_t)sm_count() * 8;
     const unsigned grid = (unsigned)(n_tiles < want ? n_tiles : want);
     if (region.depth)
         list_count_kernel<true><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, region, ranges, tile_count, col_stride);

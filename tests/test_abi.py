@@ -62,3 +62,33 @@ def test_no_cpu_fallback_in_product():
         if f.endswith((".py", ".c")):
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_1401_7457_b200" not in src and "from paper_1401_7457_b200" not in src
+
+
+# ---- a C-language consumer of the header (the boundary is a C ABI, not a Python one) --------------------------------
+_C_SRC = os.path.join(ROOT, "tests", "c_consumer", "figure1.c")
+_CUDA_INC = os.environ.get("CUDA_HOME", "/usr/local/cuda") + "/include"
+_CUDA_LIB = os.environ.get("CUDA_HOME", "/usr/local/cuda") + "/lib64"
+
+
+def _compile_c_consumer(tmp_path):
+    import subprocess
+    import paper_1401_7457_b200 as cx
+    cx.lib()                                             # builds libcxbwt.so if stale
+    pkg = os.path.join(ROOT, "paper_1401_7457_b200")
+    exe = str(tmp_path / "figure1")
+    # strict C99: the header must not rely on C++ (extern "C" is guarded, cx_stream_t is an incomplete struct pointer)
+    subprocess.check_call(["gcc", "-std=c99", "-pedantic", "-Wall", "-Werror", "-I" + os.path.join(ROOT, "include"), "-isystem", _CUDA_INC,
+                           _C_SRC, "-o", exe, "-L" + pkg, "-lcxbwt", "-L" + _CUDA_LIB, "-lcudart", "-Wl,-rpath," + pkg, "-Wl,-rpath," + _CUDA_LIB])
+    return exe
+
+
+def test_header_compiles_as_c_and_links(tmp_path):
+    assert os.path.exists(_compile_c_consumer(tmp_path))
+
+
+@pytest.mark.gpu
+def test_c_consumer_runs_figure1(tmp_path):
+    import subprocess
+    r = subprocess.run([_compile_c_consumer(tmp_path)], capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert r.stdout.split() == ["TTAAG$TAG$CAGG$", "15"]          # PAPER.md:59, Figure 1

@@ -358,3 +358,12 @@ def test_partition_sizes_match_linear_scan():
     assert np.array_equal(got, want)
     # partitions are contiguous and ordered in the output: per-partition symbol multiset check
     chk.check_all(out.cpu().numpy(), c)
+
+
+def test_read_longer_than_2_pow_21_in_tie_groups():
+    """A read of 2.2 Mbp whose suffixes sit in tie groups with short reads copied out of it: the in-block refinement must
+    carry 'bases left' beyond 21 bits (a 21-bit field silently corrupted the emitted symbols)."""
+    rng = np.random.default_rng(21)
+    long_read = "".join(np.frombuffer(b"ACGT", np.uint8)[rng.integers(0, 4, 2_200_000)].tobytes().decode())
+    reads = [long_read, long_read[100:160], long_read[100:160], long_read[5000:5100], long_read[2_199_900:], ""]
+    assert_parity(gen.from_strings(reads))
