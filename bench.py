@@ -6,13 +6,18 @@ collection-BWT hot path on B200, with the dominant kernel's HBM roofline and the
 
 A "step" is one pass of the whole hot path (rows a1-a8 of DESIGN.md: 2-bit pack, partition sizes,
 batch plan, list + key build, onesweep sort, tie refinement, emit) over one synthetic collection.
-At N=1 the workload is BASELINE.json configs[1] (1,000,000 reads x 100 bp, 100x coverage of a seeded
-1 Mbp genome -> 1.01e8 suffixes), the case the paper's design is hardest on (deep shared substrings).
+At N=1 the workload is BASELINE.json configs[2] (10,000,000 reads x 100 bp, 30x over a seeded 33 Mbp
+genome, both strands, 1 % substitutions -> 1.01e9 suffixes): the largest configuration that is sorted
+as ONE in-HBM batch and whose host-resident end-to-end leg (1 GB in, 1 GB out) fits any box.  The two
+larger configurations (configs[3]: 6.04e9 suffixes in two batches; configs[4]: 1.01e11 suffixes, the
+paper's 1000M x 100 bp headline, streamed out of core) are measured in the same run as one-step records
+under "other_configs" when the box has the memory for them (skip with --no-other-configs).
 For N>1 (torchrun, one rank per GPU) every rank runs an independent replica with its own seed: the
 north_star fixes the path to one GPU with no collectives.
 
-`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
-recipe; nothing else in this file touches oracle/ except the `cpu_baseline` leg.
+`--impl reference` times the CPU oracle (oracle/, as it stands, one prefix range per process over all
+host cores) on a bounded sample of the same recipe; nothing else in this file touches oracle/ except
+the `cpu_baseline` leg.
 """
 from __future__ import annotations
 
@@ -29,6 +34,7 @@ if ROOT not in sys.path:
 
 METRIC = "suffixes_sorted_per_s"
 UNIT = "suffixes/s"
+DEFAULT_CONFIG = 2
 WORKLOADS = {
     0: "configs[0]: 10,000 reads x 100 bp iid (1.01e6 suffixes)",
     1: "configs[1]: 1,000,000 reads x 100 bp at 100x over a seeded 1 Mbp genome (1.01e8 suffixes)",
@@ -36,26 +42,35 @@ WORKLOADS = {
     3: "configs[3]: 40,000,000 reads x 50-250 bp over a 50 Mbp repeat genome (~6.04e9 suffixes)",
     4: "configs[4]: 1,000,000,000 reads x 100 bp at 30x over 3.3 Gbp, both strands, 1% subst. (1.01e11 suffixes)",
 }
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture named here (None until one exists for this workload).
-NCU_TRAFFIC = {"file": "profiles/r01_ncu_full.md (onesweep_pass_kernel<u64 key|id word, keys-only>, configs[1])", "bytes_per_launch": 1_592_000_000}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed `ncu --set full` captures of THIS round at the
+# benched configuration (profiles/r02_ncu_full.md); keyed by (config, kernel class).  None until a capture exists.
+NCU_TRAFFIC: dict = {}
+NCU_TRAFFIC_FILE = "profiles/r02_ncu_full.md"
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
-CPU_SAMPLE_SCALE = 0.1        # cpu_baseline leg: the workload's recipe at this scale (coverage preserved)
-REF_SAMPLE_SCALE = 0.05       # --impl reference: one step = the oracle on the recipe at this scale
+CPU_SAMPLE_SCALE = {0: 1.0, 1: 0.5, 2: 0.1, 3: 0.01, 4: 0.001}      # cpu_baseline: the recipe at this scale (coverage preserved), all cores
+REF_SAMPLE_SCALE = {0: 1.0, 1: 0.25, 2: 0.04, 3: 0.004, 4: 0.0004}  # --impl reference: one step = the oracle on the recipe at this scale
+KERNEL_NAMES = {"pack": "pack_kernel (a1)", "prep": "prep_kernel + tile_table_kernel", "hist": "bucket_hist_kernel (a2)",
+                "list": "list_write_kernel / list_count + list_select (a4+a5)", "sort_hist": "digit_hist_kernel (a6)",
+                "sort_scan": "bin_scan_kernel (a6)", "sort_pass": "onesweep_pass_kernel (a6, one radix pass of the first sort)",
+                "finish": "finish_tile_kernel (a7+a8)", "refine_scan": "active_count + scan (a7, global path)",
+                "refine_key": "refine_rekey_kernel (a7, global path)", "refine_write": "refine_writeback_kernel (a7+a8, global path)",
+                "refine_sort": "onesweep_pass_kernel (a7, global path re-sort)", "fasta": "fasta_* kernels (NEXT-4 ingest)"}
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (0-based)")
+    ap.add_argument("--config", type=int, default=DEFAULT_CONFIG, help="BASELINE.json configs index (0-based)")
     ap.add_argument("--scale", type=float, default=1.0, help="debug only: scale the workload down")
     ap.add_argument("--impl", default="cx", choices=["cx", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the one-step records of configs[3] and configs[4]")
+    ap.add_argument("--all-configs", action="store_true", help="also add one-step records of configs[0] and configs[1] to other_configs")
     ap.add_argument("--key-bases", type=int, default=0, help="first-round key window w (0 = the library's default)")
     ap.add_argument("--shard", action="store_true", help="NEXT-2, with --gpus N > 1 under torchrun: ONE collection, rank k sorts the k-th of N contiguous "
-                    "partition ranges (PAPER.md:103) and the pieces are exchanged (all-gather-v); strong scaling.  Default: independent replicas")
+                    "partition ranges (PAPER.md:103) and the pieces are exchanged (all-gather); strong scaling.  Default: independent replicas")
     ap.add_argument("--fasta", action="store_true", help="NEXT-4: the step starts from the collection's FASTA text (resident in HBM; pinned host for e2e): "
                     "cx_fasta_parse + pack + build")
     ap.add_argument("--shard-of", type=int, default=0, help="one GPU: time ONE shard of a W-way partition-range split (no exchange); with --shard-index")
@@ -63,6 +78,7 @@ def parse_args():
     ap.add_argument("--table4", type=int, default=0, help="NEXT-3: the paper's read-length experiment instead of a config: read length 100/200/400, "
                     "1e10 x --scale bases (PAPER.md:184-189)")
     ap.add_argument("--max-batch", type=int, default=0, help="m1: most suffixes per batch (0 = as many as the workspace allows)")
+    ap.add_argument("--out-bits", type=int, default=8, choices=[8, 4], help="NEXT-4: 4 = packed output, two symbols per byte")
     return ap.parse_args()
 
 
@@ -133,48 +149,88 @@ class ClockSampler:
 # --------------------------------------------------------------------------------------------------
 # CPU oracle legs (the only code in this file that may touch oracle/)
 # --------------------------------------------------------------------------------------------------
+ORACLE_PREFIXES = [a + b for a in "ACGT" for b in "ACGT"]     # 16 ranges of the first two bases + the rest below
+
+
+def _oracle_range(job):
+    """One worker of the all-core leg: the plain oracle restricted to the suffixes that begin with `prefix`
+    (a prefix range is a contiguous piece of B_R).  prefix '' = suffixes shorter than two bases and the
+    end-marker suffixes: the full oracle on the collection of every read's last base (a tiny collection)."""
+    import numpy as np
+    path, prefix = job
+    import oracle
+    ascii_ = np.load(path + ".ascii.npy", mmap_mode="r")
+    offsets = np.load(path + ".offsets.npy")
+    t0 = time.perf_counter()
+    _, piece = oracle.bwt_with_prefix(np.asarray(ascii_), offsets, prefix)
+    return prefix, int(piece.size), time.perf_counter() - t0
+
+
+def time_oracle_all_cores(coll, procs: int):
+    """Wall time of the range-restricted oracle over all 16 two-base prefix ranges, `procs` processes (spawned: the
+    parent may hold a CUDA context).  Returns (seconds, suffixes sorted)."""
+    import multiprocessing as mp
+    import tempfile
+
+    import numpy as np
+    import oracle
+    oracle.build()
+    with tempfile.TemporaryDirectory(dir="/dev/shm" if os.path.isdir("/dev/shm") else None) as td:
+        path = os.path.join(td, "sample")
+        np.save(path + ".ascii.npy", coll.ascii)
+        np.save(path + ".offsets.npy", coll.offsets)
+        ctx = mp.get_context("spawn")
+        with ctx.Pool(procs) as pool:
+            pool.map(_oracle_warm, range(procs))                   # start the workers (imports) outside the timed region
+            t0 = time.perf_counter()
+            res = pool.map(_oracle_range, [(path, p) for p in ORACLE_PREFIXES], chunksize=1)
+            dt = time.perf_counter() - t0
+    return dt, sum(r[1] for r in res)
+
+
+def _oracle_warm(_):
+    import numpy  # noqa: F401
+    import oracle
+    oracle.build()
+    return 0
+
+
 def oracle_sample(config: int, scale: float):
     from workloads import generate as gen
     coll = gen.config(config, scale)
-    desc = (f"configs[{config}] recipe at scale {scale:g} (coverage preserved): {coll.n_reads:,} reads, "
-            f"{coll.n_suffixes:,} suffixes, full plain oracle (materialise, qsort with the definition's comparator, read off)")
+    desc = (f"configs[{config}] recipe at scale {scale:g} (coverage preserved): {coll.n_reads:,} reads, {coll.n_suffixes:,} suffixes; "
+            f"plain oracle (materialise, qsort with the definition's comparator, read off) restricted to each of the 16 two-base "
+            f"prefix ranges, one range per process")
     return coll, desc
 
 
-def time_oracle(coll) -> float:
-    import oracle
-    t0 = time.perf_counter()
-    oracle.bwt(coll.ascii, coll.offsets)
-    return time.perf_counter() - t0
-
-
 def cpu_baseline(config: int) -> dict:
-    import oracle
-    oracle.build()
-    coll, desc = oracle_sample(config, CPU_SAMPLE_SCALE if config >= 1 else 1.0)
-    dt = time_oracle(coll)
-    return {"value": coll.n_suffixes / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc, "seconds": round(dt, 3),
-            "host_cpus": os.cpu_count()}
+    cores = os.cpu_count() or 1
+    coll, desc = oracle_sample(config, CPU_SAMPLE_SCALE.get(config, 0.01))
+    dt, sorted_n = time_oracle_all_cores(coll, cores)
+    return {"value": sorted_n / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc + f"; {sorted_n:,} suffixes sorted",
+            "seconds": round(dt, 3), "host_cpus": cores}
 
 
 def run_reference(args) -> None:
     """The reference arm of this tier = the oracle, timed as it stands on the host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    import oracle
-    oracle.build()
-    coll, desc = oracle_sample(args.config, (REF_SAMPLE_SCALE if args.config >= 1 else 1.0) * args.scale)
-    for _ in range(args.warmup):
-        time_oracle(coll)
-    times = [time_oracle(coll) for _ in range(args.steps)]
-    ms = 1e3 * sum(times) / len(times)
-    value = coll.n_suffixes / (ms / 1e3)
+    cores = os.cpu_count() or 1
+    coll, desc = oracle_sample(args.config, REF_SAMPLE_SCALE.get(args.config, 0.01) * args.scale)
+    for _ in range(min(args.warmup, 1)):                 # a CPU program has nothing to warm but the page cache
+        time_oracle_all_cores(coll, cores)
+    runs = [time_oracle_all_cores(coll, cores) for _ in range(args.steps)]
+    ms = 1e3 * sum(r[0] for r in runs) / len(runs)
+    sorted_n = runs[0][1]
+    value = sorted_n / (ms / 1e3)
+    base_share = coll.total_bases * (sorted_n / coll.n_suffixes)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "u64", "data": "synthetic", "config": {"workload": WORKLOADS[args.config], "sample": desc},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+            "dtype": "u8", "data": "synthetic", "config": {"workload": WORKLOADS[args.config], "sample": desc},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gbases_per_hour": coll.total_bases / (ms / 1e3) * 3600 / 1e9, "gpu_launches": 0}
+            "gbases_per_hour": base_share / (ms / 1e3) * 3600 / 1e9, "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
@@ -199,6 +255,132 @@ def max_over_ranks(values, device) -> list:
 
 
 # --------------------------------------------------------------------------------------------------
+# inputs
+# --------------------------------------------------------------------------------------------------
+def device_collection(index: int, scale: float, seed: int, dev, chunk_reads: int = 2_000_000, keep_ascii: bool = True):
+    """configs[1..4] generated chunk by chunk on the device (workloads/generate_torch.py, pinned to the numpy recipes by
+    tests/test_generators.py).  Returns (ascii uint8 | None, packed int64, offsets int64, n_reads, total_bases, max_len,
+    symbol counts int64[256]).  With keep_ascii=False only the packed form is kept (configs[3], configs[4])."""
+    import torch
+
+    import paper_1401_7457_b200 as cx
+    from workloads import generate_torch as gt
+    recipe = gt.ReadRecipe(index, scale, seed=seed, device=dev)
+    n = recipe.n_reads
+    offsets = gt.offsets_of(recipe)
+    total = int(offsets[-1])
+    max_len = int((offsets[1:] - offsets[:-1]).max()) if n else 0
+    packed = torch.zeros((total + 31) // 32 + 1, dtype=torch.int64, device=dev)
+    ascii_all = torch.empty(total, dtype=torch.uint8, device=dev) if keep_ascii else None
+    counts = torch.zeros(256, dtype=torch.int64, device=dev)
+    carry = torch.zeros(0, dtype=torch.uint8, device=dev)
+    done = 0                                  # bases packed so far (a multiple of 32)
+    for a, b, lens, ascii_ in gt.read_chunks(recipe, chunk_reads):
+        counts += torch.bincount(ascii_.to(torch.int64), minlength=256)
+        if keep_ascii:
+            o0 = int(offsets[a])
+            ascii_all[o0:o0 + ascii_.numel()] = ascii_
+        buf = torch.cat([carry, ascii_]) if carry.numel() else ascii_
+        whole = buf.numel() // 32 * 32 if b < n else buf.numel()
+        if whole:
+            cx.cx_pack_reads(buf[:whole].contiguous(), packed[done // 32: done // 32 + (whole + 31) // 32])
+        carry = buf[whole:].clone()
+        done += whole
+        del ascii_, buf
+    assert done == total
+    del recipe
+    return ascii_all, packed, offsets, n, total, max_len, counts
+
+
+def host_ram_gb() -> float:
+    try:
+        with open("/proc/meminfo") as f:
+            for ln in f:
+                if ln.startswith("MemAvailable:"):
+                    return int(ln.split()[1]) / (1 << 20)
+    except Exception:
+        pass
+    return 0.0
+
+
+def one_step_record(index: int, dev, peak: float) -> dict:
+    """configs[3] / configs[4] (and, with --all-configs, the small ones) as ONE timed build each: inputs generated on the
+    device, packed reads resident in HBM, CUDA events around cx_bwt_build, per-class times from the same build (profile=1:
+    events around every launch; the whole-build time of a run this long is not moved by them).  configs[4] streams its
+    101 GB output to pinned host memory (a9)."""
+    import gc
+
+    import torch
+
+    import paper_1401_7457_b200 as cx
+    from workloads import generate as gen
+    gc.collect()
+    torch.cuda.empty_cache()
+    free_gb = torch.cuda.mem_get_info(dev)[0] / (1 << 30)
+    host_out = index == 4
+    need_gpu, need_host = {0: 1, 1: 8, 2: 60, 3: 150, 4: 165}[index], {4: 115}.get(index, 4)
+    if free_gb < need_gpu or host_ram_gb() < need_host:
+        return {"workload": WORKLOADS[index], "skipped": f"needs {need_gpu} GB of HBM and {need_host} GB of host RAM; free: {free_gb:.0f} GB, {host_ram_gb():.0f} GB"}
+    t0 = time.time()
+    _, packed, offsets, n, total, max_len, counts = device_collection(index, 1.0, gen.BASE_SEED + index, dev, chunk_reads=2_500_000, keep_ascii=False) \
+        if index >= 1 else _small_collection(index, dev)
+    N = total + n
+    torch.cuda.synchronize()
+    gen_s = time.time() - t0
+    torch.cuda.empty_cache()
+    ws = {3: 130 << 30, 4: 118 << 30}.get(index)
+    plan = cx.Plan(n, total, workspace_bytes=ws, max_read_len=max_len, out_is_host_pinned=1 if host_out else 0, profile=1, device=dev)
+    out = torch.empty(N, dtype=torch.uint8, pin_memory=True) if host_out else torch.empty(N, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    plan.build(packed, offsets, n, out)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    stats = plan.stats()
+    times = plan.kernel_times()
+    plan.free()
+    del plan
+    # whole-output invariant (the parity proper is tests/ -m gpu): symbol counts
+    got = torch.zeros(256, dtype=torch.int64, device=dev)
+    for a in range(0, N, 1 << 30):
+        got += torch.bincount(out[a:a + (1 << 30)].to(dev).to(torch.int64), minlength=256)
+    counts[ord("$")] += n
+    ok = bool(torch.equal(got, counts))
+    kernels = {k: {"ms": round(v["ms"], 2), "launches": v["launches"], "gb_s": round(v["bytes"] / (v["ms"] * 1e-3) / 1e9, 1) if v["ms"] > 0 else None,
+                   "frac_of_peak": round(v["bytes"] / (v["ms"] * 1e-3) / 1e9 / peak, 4) if v["ms"] > 0 else None}
+               for k, v in times.items() if v["launches"]}
+    alg = sum(v["bytes"] for v in times.values())
+    rec = {"workload": WORKLOADS[index], "n_reads": n, "total_bases": total, "n_suffixes": N, "steps": 1, "ms_per_step": ms,
+           "value": N / (ms * 1e-3), "unit": UNIT, "gbases_per_hour": total / (ms * 1e-3) * 3600 / 1e9,
+           "output": "pinned host memory, streamed batch by batch (a9); the D2H copies are inside the timed build" if host_out else "device",
+           "n_batches": stats["n_batches"], "id_bytes": stats["id_bytes"], "sort_passes": stats["sort_passes"], "max_batch": stats["max_batch"],
+           "refine_rounds": stats["refine_rounds"], "kernels": kernels,
+           "pipeline": {"alg_bytes_per_suffix": round(alg / N, 1), "gb_s": round(alg / (ms * 1e-3) / 1e9, 1), "frac_of_peak": round(alg / (ms * 1e-3) / 1e9 / peak, 4)},
+           "symbol_counts_ok": ok, "generate_s": round(gen_s, 1)}
+    del out, packed, offsets, counts, got
+    gc.collect()
+    torch.cuda.empty_cache()
+    if not ok:
+        raise SystemExit(f"bench.py: configs[{index}]: output symbol counts differ from the input's")
+    return rec
+
+
+def _small_collection(index: int, dev):
+    import numpy as np
+    import torch
+
+    import paper_1401_7457_b200 as cx
+    from workloads import generate as gen
+    c = gen.config(index)
+    a = torch.from_numpy(c.ascii).to(dev)
+    counts = torch.bincount(a.to(torch.int64), minlength=256)
+    return a, cx.cx_pack_reads(a), torch.from_numpy(c.offsets.astype(np.int64)).to(dev), c.n_reads, c.total_bases, c.max_read_len, counts
+
+
+# --------------------------------------------------------------------------------------------------
 # the CUDA arm
 # --------------------------------------------------------------------------------------------------
 def run_cx(args) -> None:
@@ -219,32 +401,47 @@ def run_cx(args) -> None:
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     cx.lib()
+    if args.config >= 3 and not args.table4 and args.scale == 1.0:
+        raise SystemExit("bench.py: configs[3] and configs[4] have no host-resident end-to-end leg; they are the one-step records under other_configs")
 
     # ---- synthetic input (seeded; replicas differ only in seed) -------------------------------------
-    if args.table4:
-        coll = gen.table4(args.table4, args.scale)
+    seed = replica_seed(args.config, 0 if args.shard else rank)
+    if args.table4 or args.config == 0 or args.scale < 0.05:
+        coll = gen.table4(args.table4, args.scale) if args.table4 else gen.config(args.config, args.scale, seed=seed)
+        n_reads, total, max_len = coll.n_reads, coll.total_bases, coll.max_read_len
+        h_ascii = torch.from_numpy(coll.ascii).pin_memory()
+        h_off = torch.from_numpy(coll.offsets.astype(np.int64)).pin_memory()
+        d_ascii, d_off = h_ascii.to(dev), h_off.to(dev)
+        want_counts = torch.bincount(d_ascii.to(torch.int64), minlength=256)
+        del coll
     else:
-        coll = gen.config(args.config, args.scale, seed=replica_seed(args.config, 0 if args.shard else rank))
-    n_reads, total, N = coll.n_reads, coll.total_bases, coll.n_suffixes
-    h_ascii = torch.from_numpy(coll.ascii).pin_memory()
-    h_off = torch.from_numpy(coll.offsets.astype(np.int64)).pin_memory()
-    h_out = torch.empty(N, dtype=torch.uint8).pin_memory()
-    d_ascii = h_ascii.to(dev)
-    d_off = h_off.to(dev)
+        d_ascii, _, d_off, n_reads, total, max_len, want_counts = device_collection(args.config, args.scale, seed, dev)
+        h_ascii = torch.empty(total, dtype=torch.uint8).pin_memory()
+        h_ascii.copy_(d_ascii)
+        h_off = torch.empty(n_reads + 1, dtype=torch.int64).pin_memory()
+        h_off.copy_(d_off)
+    N = total + n_reads
+    want_counts[ord("$")] += n_reads
+    out_bytes = N if args.out_bits == 8 else (N + 1) // 2
+    h_out = torch.empty(out_bytes, dtype=torch.uint8).pin_memory()
     d_packed = torch.empty((total + 31) // 32 + 1, dtype=torch.int64, device=dev)
-    d_out = torch.empty(N, dtype=torch.uint8, device=dev)
+    d_out = torch.empty(out_bytes, dtype=torch.uint8, device=dev)
     sharded = bool(args.shard) and world > 1
-    plan = cx.Plan(n_reads, total, max_read_len=coll.max_read_len, profile=1, key_bases=args.key_bases or None, max_batch_suffixes=args.max_batch or None,
-                   shard_index=rank if sharded else (args.shard_index if args.shard_of > 1 else None),
-                   shard_count=world if sharded else (args.shard_of if args.shard_of > 1 else None), device=dev)
     one_shard = args.shard_of > 1 and not sharded
+    plan_opts = dict(max_read_len=max_len, key_bases=args.key_bases or None, max_batch_suffixes=args.max_batch or None,
+                     shard_index=rank if sharded else (args.shard_index if args.shard_of > 1 else None),
+                     shard_count=world if sharded else (args.shard_of if args.shard_of > 1 else None), device=dev)
+    if args.out_bits == 4:
+        plan_opts["out_bits"] = 4
+    plan = cx.Plan(n_reads, total, profile=0, **plan_opts)
     units = 1 if sharded else world      # collections sorted per step by the whole job
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
     stream = torch.cuda.current_stream()
 
     fasta_ev = []
     if args.fasta:
-        h_text = torch.from_numpy(np.frombuffer(gen.to_fasta(coll, line_width=0), dtype=np.uint8).copy()).pin_memory()
+        coll_f = gen.Collection(h_ascii.numpy(), h_off.numpy().astype(np.uint64))
+        h_text = torch.from_numpy(np.frombuffer(gen.to_fasta(coll_f, line_width=0), dtype=np.uint8).copy()).pin_memory()
         d_text = h_text.to(dev)
 
     def ingest(timed=False):
@@ -259,28 +456,28 @@ def run_cx(args) -> None:
             fasta_ev[-1][1].record(stream)
         return bases, offs
 
-    def build():
+    def build(p, offs=None):
         if sharded:
-            cx.build_sharded(plan, d_packed, d_off, n_reads, d_out)   # this rank's partition range, then the exchange of the pieces
+            cx.build_sharded(p, d_packed, d_off, n_reads, d_out)   # this rank's partition range, then the exchange of the pieces
         else:
-            plan.build(d_packed, d_off, n_reads, d_out)
+            p.build(d_packed, d_off if offs is None else offs, n_reads, d_out)
 
-    def step_device():
+    def step_device(p):
         a, o = ingest()
         cx.cx_pack_reads(a, d_packed, check=False)
-        build() if not args.fasta else plan.build(d_packed, o, n_reads, d_out)
+        build(p, o if args.fasta else None)
 
-    def step_e2e():
+    def step_e2e(p):
+        """The call a user makes with HOST buffers: input from pinned host memory, result back in pinned host memory."""
         if args.fasta:
             d_text.copy_(h_text, non_blocking=True)
             a, o = ingest()
             cx.cx_pack_reads(a, d_packed, check=False)
-            plan.build(d_packed, o, n_reads, d_out)
+            p.build(d_packed, o, n_reads, d_out)
         else:
-            d_ascii.copy_(h_ascii, non_blocking=True)
+            cx.pack_reads_from_host(h_ascii, d_ascii, d_packed, stream=stream)      # chunked H2D overlapped with the pack kernel
             d_off.copy_(h_off, non_blocking=True)
-            cx.cx_pack_reads(d_ascii, d_packed, check=False)
-            build()
+            build(p)
         h_out.copy_(d_out, non_blocking=True)
         stream.synchronize()
 
@@ -290,24 +487,22 @@ def run_cx(args) -> None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         flush.fill_(1)
-        step_device()
+        step_device(plan)
     torch.cuda.synchronize()
     stats = plan.stats()
     # cheap whole-output invariants (the parity proper is tests/ -m gpu): |B| = N, n_reads '$', base counts
-    got = torch.bincount(d_out.to(torch.int64), minlength=128).cpu().numpy()
-    want = np.bincount(coll.ascii, minlength=128)
-    want[ord("$")] += n_reads
     if one_shard:
         N = stats["shard_suffixes"]          # the piece this run sorts; its parity is tests/test_shard.py
-    elif not np.array_equal(got[:128], want[:128]):
-        raise SystemExit("bench.py: output symbol counts differ from the input's")
+    elif args.out_bits == 8:
+        got = torch.bincount(d_out.to(torch.int64), minlength=256)
+        if not torch.equal(got, want_counts):
+            raise SystemExit("bench.py: output symbol counts differ from the input's")
 
-    # ---- device-resident timing -----------------------------------------------------------------------
-    classes = {k: {"ms": 0.0, "launches": 0, "bytes": 0} for k in cx.KERNEL_CLASSES}
+    # ---- device-resident timing (profile = 0: no events inside the library) ------------------------------------
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    pack_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     sampler = ClockSampler(local)
     barrier()
     sampler.start()
@@ -315,38 +510,53 @@ def run_cx(args) -> None:
     for i in range(args.steps):
         flush.fill_(i)                       # L2 flush between timed iterations (outside the events)
         ev[i][0].record(stream)
+        step_device(plan)
+        ev[i][1].record(stream)
+        stream.synchronize()
+        launches += plan.stats()["kernel_launches"] + 1 + (10 if args.fasta else 0)
+    barrier()
+    clocks = sampler.stop()
+    dev_ms = sum(a.elapsed_time(b) for a, b in ev) / args.steps
+
+    # ---- end to end: pinned host in, pinned host out ----------------------------------------------------
+    e2e_steps = max(3, min(args.steps, 10))
+    for _ in range(2):
+        step_e2e(plan)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        step_e2e(plan)
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+    barrier()
+    plan.free()
+    del plan
+
+    # ---- per-class table: a separate pass with CUDA events around every launch (cx_bwt_kernel_time) --------------
+    prof_steps = 3
+    pplan = cx.Plan(n_reads, total, profile=1, **plan_opts)
+    classes = {k: {"ms": 0.0, "launches": 0, "bytes": 0} for k in cx.KERNEL_CLASSES}
+    pack_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(prof_steps)]
+    step_device(pplan)
+    for i in range(prof_steps):
+        flush.fill_(i)
         a, o = ingest(timed=True)
         pack_ev[i][0].record(stream)
         cx.cx_pack_reads(a, d_packed, check=False)
         pack_ev[i][1].record(stream)
-        build() if not args.fasta else plan.build(d_packed, o, n_reads, d_out)
-        ev[i][1].record(stream)
+        build(pplan, o if args.fasta else None)
         stream.synchronize()
-        for k, v in plan.kernel_times().items():
+        for k, v in pplan.kernel_times().items():
             for f in ("ms", "launches", "bytes"):
                 classes[k][f] += v[f]
-        launches += plan.stats()["kernel_launches"] + 1
-    barrier()
-    clocks = sampler.stop()
-    dev_ms = sum(a.elapsed_time(b) for a, b in ev) / args.steps
-    classes["pack"]["ms"] = sum(a.elapsed_time(b) for a, b in pack_ev)
-    classes["pack"]["launches"] = args.steps
-    classes["pack"]["bytes"] = args.steps * (total + total // 4)
+    pstats = pplan.stats()
+    classes["pack"] = {"ms": sum(a.elapsed_time(b) for a, b in pack_ev), "launches": prof_steps, "bytes": prof_steps * (total + total // 4)}
     if args.fasta:      # two reads of the text, one write of the bases, 8 B per read (cx_fasta.cu)
-        classes["fasta"] = {"ms": sum(a.elapsed_time(b) for a, b in fasta_ev), "launches": 10 * args.steps,
-                            "bytes": args.steps * (2 * h_text.numel() + total + 8 * n_reads)}
-        launches += 10 * args.steps
+        classes["fasta"] = {"ms": sum(a.elapsed_time(b) for a, b in fasta_ev), "launches": 10 * prof_steps,
+                            "bytes": prof_steps * (2 * h_text.numel() + total + 8 * n_reads)}
+    pplan.free()
+    del pplan
 
-    # ---- end to end: pinned host in, pinned host out ----------------------------------------------------
-    for _ in range(2):
-        step_e2e()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        step_e2e()
-    torch.cuda.synchronize()
-    e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
-    barrier()
     if world > 1:
         dev_ms, e2e_ms = max_over_ranks([dev_ms, e2e_ms], dev)
     if rank != 0:
@@ -360,67 +570,79 @@ def run_cx(args) -> None:
         if v["launches"] == 0:
             continue
         gbs = v["bytes"] / (v["ms"] * 1e-3) / 1e9 if v["ms"] > 0 else None
-        kernels[k] = {"ms_per_step": round(v["ms"] / args.steps, 4), "launches_per_step": v["launches"] / args.steps,
-                      "alg_bytes_per_step": v["bytes"] // args.steps, "gb_s": round(gbs, 1) if gbs else None,
+        kernels[k] = {"ms_per_step": round(v["ms"] / prof_steps, 4), "launches_per_step": v["launches"] / prof_steps,
+                      "alg_bytes_per_step": v["bytes"] // prof_steps, "gb_s": round(gbs, 1) if gbs else None,
                       "frac_of_peak": round(gbs / peak, 4) if gbs else None}
-    dom = classes["sort_pass"]
-    bytes_per_launch = dom["bytes"] / max(dom["launches"], 1)
-    ms_per_launch = dom["ms"] / max(dom["launches"], 1)
-    achieved = bytes_per_launch / (ms_per_launch * 1e-3) / 1e9 if ms_per_launch > 0 else 0.0
-    total_alg = sum(v["bytes"] for v in classes.values()) / args.steps
-    kern_ms = sum(v["ms"] for v in classes.values()) / args.steps
+
+    def roofline_of(cls: str) -> dict:
+        c = classes[cls]
+        per_launch_bytes = c["bytes"] / max(c["launches"], 1)
+        per_launch_ms = c["ms"] / max(c["launches"], 1)
+        ach = per_launch_bytes / (per_launch_ms * 1e-3) / 1e9 if per_launch_ms > 0 else 0.0
+        key = (args.config, cls) if args.scale == 1.0 and not args.table4 and not args.fasta else None
+        return {"kernel": KERNEL_NAMES.get(cls, cls), "class": cls, "bound": "hbm", "achieved": round(ach, 1), "peak": peak, "unit": "GB/s",
+                "frac": round(ach / peak, 4), "traffic": NCU_TRAFFIC.get(key), "traffic_from": NCU_TRAFFIC_FILE if key in NCU_TRAFFIC else None,
+                "peak_source": peak_src, "nominal_peak": 8000.0, "alg_bytes_per_launch": int(per_launch_bytes),
+                "us_per_launch": round(per_launch_ms * 1e3, 2), "launches_per_step": c["launches"] / prof_steps,
+                "share_of_kernel_time": round(c["ms"] / max(sum(x["ms"] for x in classes.values()), 1e-9), 4)}
+
+    dominant = max((k for k in classes if classes[k]["launches"]), key=lambda k: classes[k]["ms"])
+    total_alg = sum(v["bytes"] for v in classes.values()) / prof_steps
+    kern_ms = sum(v["ms"] for v in classes.values()) / prof_steps
+    wl = (f"Table 4 shape (PAPER.md:184-189): reads of {args.table4} bp, 30x, both strands, 1% subst." if args.table4
+          else WORKLOADS.get(args.config, str(args.config))) + (f" x scale {args.scale:g}" if args.scale != 1 else "") \
+        + (" [input: FASTA text, parsed on the device]" if args.fasta else "") + (" [output: 4 bits per symbol]" if args.out_bits == 4 else "")
     line = {
         "metric": METRIC, "value": units * N / (dev_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": dev_ms, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
+        "warmup": warm, "ms_per_step": dev_ms, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
         "dtype": "u64", "data": "synthetic",
-        "config": {"workload": (f"Table 4 shape (PAPER.md:184-189): reads of {args.table4} bp, 30x, both strands, 1% subst." if args.table4
-                                else WORKLOADS.get(args.config, str(args.config))) + (f" x scale {args.scale:g}" if args.scale != 1 else "")
-                               + (" [input: FASTA text, parsed on the device]" if args.fasta else ""),
-                   "n_reads": n_reads, "total_bases": total, "n_suffixes": N, "parallelism": (f"{world} contiguous partition ranges (PAPER.md:103) + all-gather-v of the pieces" if sharded
-                                                                                       else "replicas only" if world > 1 else
-                                                                                       f"1 gpu, shard {args.shard_index} of {args.shard_of} only (its piece: {N} suffixes)" if one_shard else "1 gpu"),
-                   "l2": "256 MiB L2-flush write between timed steps; working set >> L2", "prefix_len": 6, "key_bases": "auto (14 bases in a 32-bit key up to 2^30 suffixes, else ceil(log4 N)+1 bases in a 64-bit key)",
+        "config": {"workload": wl, "n_reads": n_reads, "total_bases": total, "n_suffixes": N,
+                   "parallelism": (f"{world} contiguous partition ranges (PAPER.md:103) + all-gather of the pieces" if sharded
+                                   else "replicas only" if world > 1 else
+                                   f"1 gpu, shard {args.shard_index} of {args.shard_of} only (its piece: {N} suffixes)" if one_shard else "1 gpu"),
+                   "l2": "256 MiB L2-flush write between timed steps; working set >> L2", "prefix_len": 6,
+                   "key_bases": "auto (14 bases in a 32-bit key up to 2^30 suffixes, else ceil(log4 N)+1 bases in a 64-bit key)",
+                   "timing": "value/ms_per_step: CUDA events around each step, library built with profile=0; kernels{}/roofline{}: a "
+                             "separate pass of the same steps with CUDA events around every launch (profile=1)",
                    "id_bytes": stats["id_bytes"], "n_batches": stats["n_batches"], "sort_passes": stats["sort_passes"],
                    "refine_rounds": stats["refine_rounds"], "refine_elements": stats["refine_elements"],
                    "small_group_elems": stats["small_group_elems"]},
         "gbases_per_hour": units * total / (dev_ms * 1e-3) * 3600 / 1e9,
-        "e2e": {"value": units * N / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+        "e2e": {"value": units * N / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "h2d_bytes_per_step": int(h_text.numel()) if args.fasta else int(h_ascii.numel() + h_off.numel() * 8), "d2h_bytes_per_step": int(h_out.numel())},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "roofline": {"kernel": "onesweep_pass_kernel (a6, one radix pass)", "bound": "hbm", "achieved": round(achieved, 1),
-                     "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 4), "traffic": NCU_TRAFFIC["bytes_per_launch"] if args.config == 1 and args.scale == 1.0 else None,
-                     "traffic_from": NCU_TRAFFIC["file"], "peak_source": peak_src, "nominal_peak": 8000.0,
-                     "alg_bytes_per_launch": int(bytes_per_launch), "us_per_launch": round(ms_per_launch * 1e3, 2),
-                     "launches_per_step": dom["launches"] / args.steps},
-        # The in-block refinement (finish) is the largest share of the step and is bound by integer ALU issue, not HBM: its
-        # algorithmic work is the number of 192-bit key comparisons its stable rank makes (counted by the kernel), nine
-        # issue slots each (LDS.128 + LDS.64 + a seven-instruction borrow chain); peak = SMs x 128 lanes x SM clock / 9.
-        "roofline_finish": finish_roofline(classes["finish"], stats, clocks, args.steps),
+        # the kernel class with the largest share of the step, against the HBM roofline of its algorithmic bytes
+        "roofline": roofline_of(dominant),
+        # the metric also names the radix pass: first-sort launches only (the global path's small re-sorts are `refine_sort`)
+        "roofline_sort_pass": roofline_of("sort_pass") if classes["sort_pass"]["launches"] else None,
+        "finish_rank_compares_per_step": pstats["compare_ops"],     # diagnostic: 32-bit rank-key comparisons of the in-block refinement
         "pipeline": {"alg_bytes_per_step": int(total_alg), "alg_bytes_per_suffix": round(total_alg / N, 1),
                      "gb_s": round(total_alg / (dev_ms * 1e-3) / 1e9, 1), "frac_of_peak": round(total_alg / (dev_ms * 1e-3) / 1e9 / peak, 4),
-                     "kernel_ms_per_step": round(kern_ms, 3), "host_gap_ms_per_step": round(dev_ms - kern_ms, 3)},
+                     "kernel_ms_per_step_profiled": round(kern_ms, 3)},
         "kernels": kernels,
         "paper_context": "CX1: 100 Gbases in 6,886 s on i7-3930K + GTX 680 (14.7 M suffixes/s, 52 Gbases/h; PAPER.md:141); BCR 46,899 s "
                          "(abstract: 'BRC ... 12 hours'); other hardware, context only",
     }
+    # release everything of the main workload before the larger configurations
+    del d_ascii, d_off, d_packed, d_out, h_ascii, h_off, h_out, flush
+    if world == 1 and not args.no_other_configs and args.scale == 1.0 and not args.table4 and not one_shard:
+        others = []
+        for idx in ([0, 1] if args.all_configs else []) + [3, 4]:
+            if idx == args.config:
+                continue
+            try:
+                others.append(one_step_record(idx, dev, peak))
+            except SystemExit:
+                raise
+            except Exception as e:  # a box too small for configs[4] must not cost the main measurement
+                others.append({"workload": WORKLOADS[idx], "error": repr(e)[:300]})
+        line["other_configs"] = others
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args.config)
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
-
-
-def finish_roofline(cls: dict, stats: dict, clocks: dict, steps: int) -> dict:
-    import torch
-    n_sms = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
-    mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0
-    peak = n_sms * 128 * mhz * 1e6 / 9.0
-    ms = cls["ms"] / max(steps, 1)
-    achieved = stats["compare_ops"] / (ms * 1e-3) if ms > 0 else 0.0
-    return {"kernel": "finish_tile_kernel (a7+a8)", "bound": "alu", "achieved": achieved, "peak": peak, "unit": "192-bit key comparisons/s",
-            "frac": round(achieved / peak, 4), "compare_ops_per_step": stats["compare_ops"], "ms_per_step": round(ms, 4),
-            "peak_derivation": f"{n_sms} SMs x 128 lanes x {mhz:.0f} MHz / 9 issue slots per comparison"}
 
 
 def main():

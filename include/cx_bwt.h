@@ -74,7 +74,7 @@ typedef struct cx_bwt_stats_s {
     uint64_t refine_elements;   /* suffixes re-keyed, summed over refinement rounds and batches          */
     uint64_t small_group_elems; /* of those, finished by the in-block path                               */
     uint64_t kernel_launches;   /* kernels launched by the build                                        */
-    uint64_t compare_ops;       /* 192-bit key comparisons of the in-block refinement (its ALU work)     */
+    uint64_t compare_ops;       /* rank-key comparisons of the in-block refinement (diagnostic)          */
     uint32_t n_batches;         /* GPU batches (the paper's "small rounds", Fig. 2 step 3(c))            */
     uint32_t id_bytes;          /* 4 or 8: width of a suffix id                                         */
     uint32_t sort_passes;       /* radix passes of the first sort of a batch                            */
@@ -84,6 +84,7 @@ typedef struct cx_bwt_stats_s {
     uint32_t refined_partitions;/* l-prefix partitions larger than m1 that were partitioned again */
     uint64_t shard_offset;      /* first position of out_bwt this build wrote (0 unless shard_count > 1)  */
     uint64_t shard_suffixes;    /* positions written from there: the shard's piece of the BWT (N if unsharded) */
+    uint64_t finish_rounds;     /* refinement rounds of the in-block path, summed over its thread blocks (diagnostic) */
 } cx_bwt_stats_t;
 
 /* Kernel classes for cx_bwt_kernel_time; one per row of the hot path. */
@@ -95,10 +96,12 @@ enum {
     CX_K_SORT_HIST,       /* a6 upfront digit histograms                      */
     CX_K_SORT_SCAN,       /* a6 bin offsets                                   */
     CX_K_SORT_PASS,       /* a6 onesweep radix pass                           */
-    CX_K_FINISH,          /* a7+a8 head flags, in-block refinement of small tie groups, emit */
+    CX_K_FINISH,          /* a7+a8 warp kernel: head flags, tie groups of <= 32 refined in registers, emit */
     CX_K_REFINE_SCAN,     /* a7 compaction scans of the global path           */
     CX_K_REFINE_KEY,      /* a7 re-key gather of the global path              */
     CX_K_REFINE_WRITE,    /* a7+a8 write-back, new flags, emit (global path)  */
+    CX_K_REFINE_SORT,     /* a7 onesweep passes over the compacted members of oversize groups (global path) */
+    CX_K_FINISH_BLOCK,    /* a7+a8 block kernel: tie groups of 33..256 suffixes refined in shared memory */
     CX_K_COUNT
 };
 

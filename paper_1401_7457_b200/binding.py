@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 
 CX_OK, CX_ERR_ARG, CX_ERR_BAD_BASE, CX_ERR_WORKSPACE, CX_ERR_BUCKET_TOO_LARGE, CX_ERR_CUDA, CX_ERR_NOMEM = 0, -1, -2, -3, -4, -5, -6
 KERNEL_CLASSES = ["pack", "prep", "hist", "list", "sort_hist", "sort_scan", "sort_pass", "finish", "refine_scan", "refine_key",
-                  "refine_write"]
+                  "refine_write", "refine_sort", "finish_block"]
 
 
 class CxError(RuntimeError):
@@ -36,7 +36,7 @@ class cx_bwt_stats_t(ctypes.Structure):
                 ("refine_elements", ctypes.c_uint64), ("small_group_elems", ctypes.c_uint64), ("kernel_launches", ctypes.c_uint64), ("compare_ops", ctypes.c_uint64),
                 ("n_batches", ctypes.c_uint32), ("id_bytes", ctypes.c_uint32), ("sort_passes", ctypes.c_uint32),
                 ("refine_rounds", ctypes.c_uint32), ("max_read_len", ctypes.c_uint32), ("uniform_len", ctypes.c_uint32), ("refined_partitions", ctypes.c_uint32),
-                ("shard_offset", ctypes.c_uint64), ("shard_suffixes", ctypes.c_uint64)]
+                ("shard_offset", ctypes.c_uint64), ("shard_suffixes", ctypes.c_uint64), ("finish_rounds", ctypes.c_uint64)]
 
     def as_dict(self) -> dict:
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
@@ -120,6 +120,36 @@ def cx_pack_reads(ascii_dev: torch.Tensor, packed_out: torch.Tensor | None = Non
         _check(lib().cx_pack_reads(ascii_dev.data_ptr(), n, packed_out.data_ptr(), status.data_ptr(), _stream_ptr(stream)))
     if check and int(status.item()) != 0:
         raise CxError(CX_ERR_BAD_BASE, cx_strerror(CX_ERR_BAD_BASE))
+    return packed_out
+
+
+_copy_streams: dict = {}
+
+
+def pack_reads_from_host(ascii_host: torch.Tensor, ascii_dev: torch.Tensor, packed_out: torch.Tensor, stream=None,
+                         chunk_bytes: int = 64 << 20) -> torch.Tensor:
+    """Ingest from pinned HOST memory: the ASCII bases are copied to the device in chunks on a side stream while
+    cx_pack_reads packs the chunks that have already arrived (copies and calls only: the packing is the kernel's).
+    Chunks are multiples of 32 bases, so every chunk starts a packed word."""
+    assert ascii_host.dtype == torch.uint8 and ascii_host.is_pinned() and ascii_dev.is_cuda and ascii_dev.numel() >= ascii_host.numel()
+    n = ascii_host.numel()
+    main = torch.cuda.current_stream() if stream is None else stream
+    key = str(ascii_dev.device)
+    if key not in _copy_streams:
+        _copy_streams[key] = torch.cuda.Stream(device=ascii_dev.device)
+    side = _copy_streams[key]
+    side.wait_stream(main)                                # the buffers may still be in use by earlier work on `main`
+    status = _pack_status(ascii_dev.device)
+    chunk = max(32, chunk_bytes // 32 * 32)
+    for a in range(0, n, chunk):
+        b = min(n, a + chunk)
+        with torch.cuda.stream(side):
+            ascii_dev[a:b].copy_(ascii_host[a:b], non_blocking=True)
+            ev = torch.cuda.Event()
+            ev.record(side)
+        main.wait_event(ev)
+        with torch.cuda.device(ascii_dev.device):
+            _check(lib().cx_pack_reads(ascii_dev.data_ptr() + a, b - a, packed_out.data_ptr() + (a // 32) * 8, status.data_ptr(), main.cuda_stream))
     return packed_out
 
 

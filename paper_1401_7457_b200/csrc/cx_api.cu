@@ -58,7 +58,7 @@ constexpr uint32_t kMaxRegionDepth = 1u << 20;   // bases; deeper refinement is 
 // Byte offsets of every region of the workspace for a given m1.
 struct Layout {
     uint64_t info, hist, tile_first, tile_count, tile_sums, scalars, prefix;
-    uint64_t keys[2], ids[3], pos, heads[2], word_counts, word_sums, sort, stage[2];
+    uint64_t keys[2], ids[3], pos, heads[2], big_tiles, word_counts, word_sums, sort, stage[2];
     uint64_t total;
 };
 
@@ -92,6 +92,7 @@ Layout make_layout(const Shape& sh, uint64_t m1) {
     L.pos = take(m1 * 4);
     uint64_t words = (m1 + 31) / 32 + 2;
     for (int i = 0; i < 2; ++i) L.heads[i] = take(words * 4);
+    L.big_tiles = take(((m1 + kLocalTile - 1) / kLocalTile / 32 + 2) * 4);
     L.word_counts = take(words * 8);
     L.word_sums = take((scan_block_count(words) + 1) * 8);
     L.sort = take(sort_workspace_bytes(m1));
@@ -473,6 +474,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     IdT* d_ids[3] = {reinterpret_cast<IdT*>(ws + L.ids[0]), reinterpret_cast<IdT*>(ws + L.ids[1]), reinterpret_cast<IdT*>(ws + L.ids[2])};
     uint32_t* d_pos = reinterpret_cast<uint32_t*>(ws + L.pos);
     uint32_t* d_heads[2] = {reinterpret_cast<uint32_t*>(ws + L.heads[0]), reinterpret_cast<uint32_t*>(ws + L.heads[1])};
+    uint32_t* d_big_tiles = reinterpret_cast<uint32_t*>(ws + L.big_tiles);
     uint64_t* d_word_counts = reinterpret_cast<uint64_t*>(ws + L.word_counts);
     uint64_t* d_word_sums = reinterpret_cast<uint64_t*>(ws + L.word_sums);
 
@@ -518,9 +520,9 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     const BuildInfo info = *p->h_info;
     if (info.bad_offsets || info.total_bases > sh.max_bases || (info.max_len >> sh.pos_bits) != 0) return CX_ERR_ARG;
     const uint64_t N = info.n_suffixes;
-    // the in-block path keeps (bases left : 21 bits, first base : 40 bits) per suffix in one locator word; a collection
-    // outside those widths is refined by the global path only, which works on ids
-    const uint32_t cap = (info.max_len >= (1ull << 21) || info.total_bases >= (1ull << 40)) ? 1u : sh.cap;
+    // the in-block refinement keeps (first base of the window : 40 bits) and (bases left : 32 bits) per suffix
+    if (info.max_len >= (1ull << 32) || info.total_bases >= (1ull << 40)) return CX_ERR_ARG;
+    const uint32_t cap = sh.cap;
     if (fused_scan) prof->bytes[CX_K_LIST] += info.total_bases / 4 + (n_reads + 1) * 8 + N * (sizeof(KeyT) + sizeof(IdT));
     else prof->bytes[CX_K_HIST] += info.total_bases / 4 + (n_reads + 1) * 8;
     R.n_words = (info.total_bases + 31) >> 5;
@@ -622,15 +624,21 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         const uint64_t n_words = (nb + 31) >> 5;
         int hc = 0;
         unsigned long long* d_done = reinterpret_cast<unsigned long long*>(d_scalars + 1);
-        CX_CUDA(cudaMemsetAsync(d_heads[0], 0, (n_words + 1) * 4, s));
-        {
-            ScopedLaunch sl(prof, CX_K_FINISH, nb * (sizeof(KeyT) + sizeof(IdT) + 1) + nb / 8, s);
-            CX_CUDA((launch_finish_first<KeyT, IdT>(R, d_keys1[cur], w, depth_base + w, d_heads[0], ids, nb, cap, dst, d_done, pack_kv, s)));
+        CX_CUDA((launch_finish_first<KeyT, IdT>(R, d_keys1[cur], w, depth_base + w, d_heads[0], ids, nb, cap, dst, d_done, d_big_tiles, p->n_sms, pack_kv,
+                                                prof, s)));
+        // groups of more than cap suffixes (counted by the warp kernel) go through global rounds; usually there are none
+        const uint64_t over_before = p->h_scalars[5], local_before = p->h_scalars[1];
+        CX_CUDA(cudaMemcpyAsync(p->h_scalars, d_scalars, 48, cudaMemcpyDeviceToHost, s));
+        CX_CUDA(cudaStreamSynchronize(s));
+        const bool any_oversize = p->h_scalars[5] != over_before;
+        if (any_oversize) {   // the head bitmask of what is left: groups of more than cap suffixes
+            CX_CUDA(cudaMemsetAsync(d_heads[0], 0, (n_words + 1) * 4, s));
+            ScopedLaunch sl(prof, CX_K_REFINE_SCAN, nb * sizeof(KeyT) + nb / 8, s);
+            CX_CUDA((launch_publish_heads<KeyT, IdT>(R, d_keys1[cur], w, d_heads[0], nb, cap, pack_kv, s)));
         }
         // ---- what is still tied goes through global rounds: re-key, sort, write back ------------------
         uint32_t depth = depth_base + w, rounds = 0;
-        uint64_t local_before = p->h_scalars[1];
-        while (true) {
+        while (any_oversize) {
             {
                 ScopedLaunch sl(prof, CX_K_REFINE_SCAN, n_words * 12, s);
                 CX_CUDA(launch_active_count(d_heads[hc], nb, d_word_counts, s));
@@ -640,7 +648,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
                 CX_CUDA(launch_scan_u64(d_word_counts, n_words, d_word_sums, d_scalars, s));
             }
             prof->launches[CX_K_REFINE_SCAN] += 2;
-            CX_CUDA(cudaMemcpyAsync(p->h_scalars, d_scalars, 32, cudaMemcpyDeviceToHost, s));
+            CX_CUDA(cudaMemcpyAsync(p->h_scalars, d_scalars, 48, cudaMemcpyDeviceToHost, s));
             CX_CUDA(cudaStreamSynchronize(s));
             const uint64_t n_act = p->h_scalars[0] & 0xffffffffull;
             const uint64_t n_groups = p->h_scalars[0] >> 32;
@@ -656,7 +664,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
                 CX_CUDA(launch_refine_rekey<IdT>(R, d_heads[hc], d_word_counts, ids, nb, depth, w_r, kc, ic, d_pos, s));
             }
             int alt = 0;
-            CX_CUDA((sort_pairs<uint64_t, IdT>(kc, ic, d_keys[cur], d_ids[2], n_act, 0, 2 * w_r + 5 + gbits, p->sort, &alt, prof, s)));
+            CX_CUDA((sort_pairs<uint64_t, IdT>(kc, ic, d_keys[cur], d_ids[2], n_act, 0, 2 * w_r + 5 + gbits, p->sort, &alt, prof, s, false, CX_K_REFINE_SORT)));
             {
                 ScopedLaunch sl(prof, CX_K_REFINE_WRITE, n_act * (8 + 2 * sizeof(IdT) + 4 + 1), s);
                 CX_CUDA(launch_refine_writeback<IdT>(R, alt ? d_keys[cur] : kc, alt ? d_ids[2] : ic, d_pos, n_act, w_r, ids, d_heads[hc],
@@ -667,13 +675,14 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             ++rounds;
             if (cap > 1) {
                 CX_CUDA(cudaMemcpyAsync(d_heads[1 - hc], d_heads[hc], (n_words + 1) * 4, cudaMemcpyDeviceToDevice, s));
-                ScopedLaunch sl(prof, CX_K_FINISH, nb / 4, s);
-                CX_CUDA(launch_finish_later<IdT>(R, d_heads[hc], d_heads[1 - hc], ids, nb, depth, cap, dst, d_done, s));
+                ScopedLaunch sl(prof, CX_K_FINISH_BLOCK, nb / 4, s);
+                CX_CUDA(launch_finish_later<IdT>(R, d_heads[hc], d_heads[1 - hc], ids, nb, depth, cap, dst, d_done, p->n_sms, s));
                 hc = 1 - hc;
             }
         }
         p->stats.small_group_elems = p->h_scalars[1];
         p->stats.compare_ops = p->h_scalars[3];
+        p->stats.finish_rounds = p->h_scalars[4];
         p->stats.refine_elements += p->h_scalars[1] - local_before;
         if (rounds > p->stats.refine_rounds) p->stats.refine_rounds = rounds;
 
@@ -705,7 +714,7 @@ extern "C" int cx_bwt_build(cx_bwt_plan_t* p, const uint64_t* packed_reads, cons
     if (!p) return CX_ERR_ARG;
     p->prof.reset();
     memset(&p->stats, 0, sizeof(p->stats));
-    p->h_scalars[0] = p->h_scalars[1] = p->h_scalars[3] = 0;
+    p->h_scalars[0] = p->h_scalars[1] = p->h_scalars[3] = p->h_scalars[4] = p->h_scalars[5] = 0;
     if (n_reads == 0) return CX_OK;
     if (!read_offsets || !out_bwt || n_reads > p->sh.max_reads) return CX_ERR_ARG;
     if (!packed_reads && p->sh.max_bases) return CX_ERR_ARG;

@@ -39,7 +39,7 @@ constexpr int kLocalThreads = 256;
 // configs[1] / configs[2] / configs[3] x 0.25: 512 -> 5.38 / 35.7 / 116.6 ms; 768 -> 5.47 / 59.3 / 185.2 ms;
 // 640 with 224 threads (196 KB carve-out) -> 5.31 / 39.8 / 130.6 ms.
 constexpr int kLocalTile = 512;
-constexpr int kLocalBlocksPerSM = 5;
+constexpr int kLocalBlocksPerSM = 4;
 constexpr int kLocalGroupCap = 256;      // largest tie group the in-block path accepts
 
 // Facts about one build, produced by the prep kernel and read by later kernels and by the host.
@@ -197,7 +197,8 @@ void sort_workspace_carve(SortWorkspace& ws, void* mem, uint64_t n);
 // hist_ready: ws.hist already holds the digit counts of every pass (the list kernel built them); begin_bit must be 0.
 template <typename KeyT, typename ValT>
 cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
-                       uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s, bool hist_ready = false);
+                       uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s, bool hist_ready = false,
+                       int pass_class = CX_K_SORT_PASS);
 
 // cx_refine.cu
 // word-level counts of active elements / active heads, packed (heads << 32 | elements)
@@ -212,16 +213,22 @@ cudaError_t launch_refine_rekey(const Reads& R, const uint32_t* heads, const uin
 template <typename IdT>
 cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, const IdT* ids_c, const uint32_t* pos_c, uint64_t n_c,
                                     uint32_t w, IdT* ids, uint32_t* heads, uint8_t* out, cudaStream_t s);
-// fused head flags + in-block refinement + emit over the freshly sorted first-round keys; heads_out must be zero-filled
-// depth0: symbols the first-round sort has settled (region depth + w1).
-// packed: keys1 holds 64-bit words (32-bit key << 32 | 32-bit id); `ids` is then OUTPUT: the ids of the positions left to
-// the global path are written there (nothing else will need the others).
+// a7 + a8 over the freshly sorted first-round keys: the warp kernel finishes singletons and tie groups of at most 32
+// suffixes and counts the groups it leaves to the global path (elems_done[4]; their head bitmask is launch_publish_heads'); the block kernel then finishes the groups of 33..group_cap in the tiles the warp
+// kernel flagged in big_tiles (n / kLocalTile / 32 + 2 words).  depth0: symbols the first-round sort has settled.
+// packed: keys1 holds 64-bit words (32-bit key << 32 | 32-bit id); `ids` then receives the ids of the groups left to the
+// global path (nothing else will need the others).
 template <typename KeyT, typename IdT>
 cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t depth0, uint32_t* heads_out, IdT* ids, uint64_t n,
-                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, bool packed, cudaStream_t s);
+                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, uint32_t* big_tiles, int n_sms, bool packed,
+                                Launch* prof, cudaStream_t s);
+// the head bitmask of the global path (zero-filled by the caller): run only when launch_finish_first counted oversize groups
+template <typename KeyT, typename IdT>
+cudaError_t launch_publish_heads(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t* heads_out, uint64_t n, uint32_t group_cap, bool packed,
+                                 cudaStream_t s);
 // in-block refinement + emit of the groups a global round has split to at most group_cap members; heads_out = copy of heads_in
 template <typename IdT>
 cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32_t* heads_out, const IdT* ids, uint64_t n, uint32_t depth,
-                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, cudaStream_t s);
+                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, int n_sms, cudaStream_t s);
 
 }  // namespace cx

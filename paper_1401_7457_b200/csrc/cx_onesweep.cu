@@ -296,7 +296,7 @@ void sort_workspace_carve(SortWorkspace& ws, void* mem, uint64_t n) {
 
 template <typename KeyT, typename ValT, int THREADS, int ITEMS, int kMinBlocks>
 cudaError_t sort_pairs_shape(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
-                             uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s, bool hist_ready) {
+                             uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s, bool hist_ready, int pass_class) {
     constexpr int kSortThreads = THREADS;
     constexpr int kTile = kSortThreads * ITEMS;
     static_assert(kTile >= kSortTileMin, "the tile-state array is sized for tiles of at least kSortTileMin pairs");
@@ -340,7 +340,7 @@ cudaError_t sort_pairs_shape(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_
         }
         ws.epoch += 1;
         {
-            ScopedLaunch sl(prof, CX_K_SORT_PASS, n * 2 * SortShape<KeyT, ValT>::pair_bytes, s);
+            ScopedLaunch sl(prof, pass_class, n * 2 * SortShape<KeyT, ValT>::pair_bytes, s);
             kernel<<<(unsigned)n_tiles, kSortThreads, sizeof(Smem), s>>>(kin, vin, kout, vout, n, lo, (1u << bits) - 1,
                                                                         ws.hist + (uint64_t)p * kRadix, ws.status, ws.ticket,
                                                                         ws.ticket_base, ws.epoch);
@@ -357,7 +357,7 @@ cudaError_t sort_pairs_shape(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_
 
 template <typename KeyT, typename ValT>
 cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, uint64_t n, uint32_t begin_bit,
-                       uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s, bool hist_ready) {
+                       uint32_t end_bit, SortWorkspace& ws, int* result_in_alt, Launch* prof, cudaStream_t s, bool hist_ready, int pass_class) {
     *result_in_alt = 0;
     if (n <= 1 || end_bit <= begin_bit) return cudaSuccess;
     constexpr int ITEMS = SortShape<KeyT, ValT>::items;
@@ -365,12 +365,12 @@ cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, u
     // at C2 (4 passes, ms): 384x16x3 1.91, 512x16x2 1.96, 256x24x3 2.00, 256x16x4 2.03; shapes that need register caps
     // to fit more blocks (256x16x5/6, 512x16x3) spill and lose: 2.29-2.52.
     if constexpr (sizeof(ValT) < 4)
-        return sort_pairs_shape<KeyT, ValT, 384, 16, 3>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready);
-    return sort_pairs_shape<KeyT, ValT, kSortThreads, ITEMS, 4>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready);
+        return sort_pairs_shape<KeyT, ValT, 384, 16, 3>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready, pass_class);
+    return sort_pairs_shape<KeyT, ValT, kSortThreads, ITEMS, 4>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready, pass_class);
 }
 
 #define CX_SORT_INST(K, V)                                                                                               \
-    template cudaError_t sort_pairs<K, V>(K*, V*, K*, V*, uint64_t, uint32_t, uint32_t, SortWorkspace&, int*, Launch*, cudaStream_t, bool);
+    template cudaError_t sort_pairs<K, V>(K*, V*, K*, V*, uint64_t, uint32_t, uint32_t, SortWorkspace&, int*, Launch*, cudaStream_t, bool, int);
 CX_SORT_INST(uint32_t, uint32_t)
 CX_SORT_INST(uint32_t, uint64_t)
 CX_SORT_INST(uint64_t, uint32_t)

@@ -18,6 +18,7 @@
 //
 // Group heads live in a bitmask: bit j = 1 iff sorted position j starts a group.
 #include "cx_internal.cuh"
+#include "cx_launch.h"
 
 namespace cx {
 namespace {
@@ -221,28 +222,53 @@ __global__ void __launch_bounds__(256) refine_writeback_kernel(Reads R, const ui
 //           to the global path (their head bits go to `heads`).
 //   !FIRST: after a global round; head flags come from `heads`; only groups of 2..cap are touched.
 // A position is emitted exactly once, by whoever makes it final (here, or the global write-back).
+//
+// Refinement of one tie group (all members share their first D symbols):
+//   * every member holds a WINDOW of the next kWin = 96 bases in shared memory (A-padded past the end of its read),
+//     gathered ONCE -- a 100 bp read never needs a second gather after a 14-base first sort;
+//   * the group's PIVOT is its member with the most bases in the window.  One XOR + count-leading-zeros of the
+//     member's window against the pivot's gives where the member first differs from the pivot (a base, or the
+//     end of one of the two), which is all that PAPER.md:55 needs to order it against everything else that was
+//     compared with the same pivot:   below the pivot -- ascending depth of divergence, then the symbol there;
+//     equal to the pivot through the window;   above the pivot -- descending depth, then the symbol.
+//     That is an 11-bit key; with the member's index in the group below it a 32-bit unsigned compare ranks the
+//     group stably -- the wide comparison is made once per member, not once per pair;
+//   * members with equal keys form the next groups: those that ENDED at the divergence are identical strings and
+//     final in their current (read index) order; the others go round again with their own pivot; a class that
+//     equals the pivot through a full window gathers its next window first (reads longer than the window).
 // ---------------------------------------------------------------------------------------------
 constexpr int kLocalElems = kLocalTile + kLocalGroupCap;   // positions a block may touch
 constexpr int kLocalWords = kLocalElems / 32 + 2;
 constexpr int kLocalItems = kLocalElems / kLocalThreads;
 static_assert(kLocalElems % kLocalThreads == 0 && kLocalThreads % 32 == 0, "tile shape");
-constexpr uint32_t kLocalW = 88;                            // bases per in-block round (192-bit round key)
+static_assert(kLocalElems <= 1024 && kLocalGroupCap <= 256, "a position takes 10 bits and an index inside a group 8 bits of the rank key");
+constexpr uint32_t kWin = 96;                         // bases per window (three packed words)
+constexpr uint32_t kKeyEqual = kWin * 8;              // key of "equal to the pivot through the window"
+constexpr uint32_t kKeyAbove = kKeyEqual + 8;         // first key of the members above the pivot
 constexpr uint16_t kNone = 0xffff;
-constexpr int kSubBlock = 32;                               // members ranked by counting before runs are merged
 
-template <typename IdT>
+// Locator of a member: [code of the preceding symbol, 1 = $, 2..5 = A C G T : 3][window must be gathered : 1]
+// [unused : 12][bases of the window that exist, <= kWin : 8][index of the window's first base in the packed text : 40]
+constexpr uint32_t kLocBaseBits = 40, kLocTakeShift = 40, kLocCodeShift = 61;
+constexpr uint64_t kLocBaseMask = (1ull << kLocBaseBits) - 1, kLocGather = 1ull << 60;
+__device__ __forceinline__ uint8_t loc_symbol(uint64_t loc) { return (uint8_t)(0x544743412400ull >> (8 * (uint32_t)(loc >> kLocCodeShift))); }
+__device__ __forceinline__ uint32_t loc_take(uint64_t loc) { return (uint32_t)(loc >> kLocTakeShift) & 255u; }
+
 struct LocalSmem {
-    // round key, 192 bits: [88 bases, A-padded : 176][0 : 1][min(remaining, 88) : 7][index inside the group : 8]
-    uint4 key_lo[kLocalElems];  // bits 0..127, .x least significant
-    uint2 key_hi[kLocalElems];  // bits 128..191 = the first 32 bases
-    uint64_t loc[kLocalElems];  // locator of the suffix now at this position (layout above); 0: not ours.  Holds the raw
-                                // id between the head pass and the classify pass
-    uint16_t ord[2][kLocalElems];  // sorted order of the runs being merged, ping-pong; at the end of a round
-                                   // ord[cur][p] = member that ranks at position p
-    uint16_t gs[kLocalElems];   // first position of the element's current group (kNone: not ours / placed)
-    uint16_t ge[kLocalElems];   // one past its last position
-    uint32_t hw[kLocalWords];   // head bits of the window, updated as groups split
-    uint32_t hw0[kLocalWords];  // as loaded
+    uint64_t w0[kLocalElems], w1[kLocalElems], w2[kLocalElems];   // member's window: bases [0,32), [32,64), [64,96), A-padded
+    uint64_t loc[kLocalElems];     // member's locator (holds the raw id between the head pass and the classify pass)
+    uint32_t mrem[kLocalElems];    // member: bases of its read from the window's first base on
+    uint32_t key[kLocalElems];     // position: rank key of the member now there; a position outside every open group holds
+                                   // (position << 21), so that keys are comparable across a whole aligned 32-position window
+    uint32_t sk[2][kLocalElems];   // position: keys of the sorted runs being merged, ping-pong
+    uint16_t mem[2][kLocalElems];  // position -> member, ping-pong over rounds
+    uint16_t gs[kLocalElems];      // position: first position of its open group (kNone: not ours / placed)
+    uint16_t ge[kLocalElems];      // one past the last
+    uint32_t gpiv[2][kLocalElems / 2];   // group (slot = first position / 2; a group has >= 2 members): max over members of
+                                         // (bases in window << 10 | member); ping-pong over rounds
+    uint32_t hw[kLocalWords];      // head bits of the window, updated as groups split
+    uint32_t hw0[kLocalWords];     // as loaded
+    uint8_t sym[kLocalElems];      // position: BWT symbol of the member placed there for good
 };
 
 // nearest set bit at or below position e, not lower than `lo`; -1 if none
@@ -274,70 +300,70 @@ __device__ __forceinline__ int next_head(const uint32_t* hw, int e, int hi) {
     }
 }
 
-// Locator of a suffix this block owns: everything the rounds and the emit need, so that the offsets table and the
-// word before the suffix are read once per suffix, not once per round and again at the emit (each such gather is a
-// 64-byte DRAM fetch on a collection larger than L2):
-//   [code of the preceding symbol, 1 = $, 2..5 = A C G T : 3][bases from its first base to the end of the read : 21]
-//   [index of its first base in the packed text : 40]
-constexpr uint32_t kLocBaseBits = 40, kLocRemBits = 21;
-__device__ __forceinline__ uint8_t loc_symbol(uint64_t loc) {
-    return (uint8_t)(0x544743412400ull >> (8 * (uint32_t)(loc >> (kLocBaseBits + kLocRemBits))));
-}
-
-// 192-bit round key of the suffix with locator `loc` at depth d: the next 88 bases (A-padded), then min(remaining, 88),
-// then the member's index inside its tie group -- so that one unsigned compare orders the group stably.
-// One round covers a 100 bp read after a 14-base first sort.
-struct Key192 {
-    uint4 lo;   // bits 0..127
-    uint2 hi;   // bits 128..191
-};
 // x with only its first cnt bases kept (cnt may be <= 0 or >= 32)
 __device__ __forceinline__ uint64_t keep_bases(uint64_t x, int cnt) {
     return cnt >= 32 ? x : (cnt <= 0 ? 0ull : x & (~0ull << (64 - 2 * cnt)));
 }
-// w: the four packed words from the one that holds the window's first base (words the window does not touch are 0);
-// shift: bit offset of that base in w[0]; take: bases of the window that exist (<= 88)
-__device__ __forceinline__ Key192 key192_of_words(const uint64_t (&w)[4], uint32_t shift, uint32_t take, uint32_t idx) {
-    uint64_t p0 = w[0], p1 = w[1], p2 = w[2];   // bases [0,32), [32,64), [64,88) of the window
-    if (shift) {
-        p0 = (w[0] << shift) | (w[1] >> (64 - shift));
-        p1 = (w[1] << shift) | (w[2] >> (64 - shift));
-        p2 = (w[2] << shift) | (w[3] >> (64 - shift));
+
+// The window of `take` <= kWin bases that starts at base index b, into shared memory as three A-padded words.
+struct Window {
+    uint64_t x[4];     // the packed words from the one that holds base b (words the window does not touch are 0)
+    uint32_t shift;    // bit offset of base b in x[0]
+    uint32_t take;
+};
+__device__ __forceinline__ void window_load(const uint64_t* __restrict__ packed, uint64_t b, uint32_t take, bool want, Window& wd) {
+    wd.shift = (uint32_t)(b & 31) * 2;
+    wd.take = take;
+    const uint32_t n_w = want && take ? (wd.shift + 2 * take + 63) >> 6 : 0u;   // words the window touches (<= 4)
+    const uint64_t* p = packed + (b >> 5);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) wd.x[i] = i < (int)n_w ? __ldg(p + i) : 0ull;
+}
+__device__ __forceinline__ void window_store(const Window& wd, LocalSmem& sm, int m) {
+    uint64_t p0 = wd.x[0], p1 = wd.x[1], p2 = wd.x[2];
+    if (wd.shift) {
+        p0 = (wd.x[0] << wd.shift) | (wd.x[1] >> (64 - wd.shift));
+        p1 = (wd.x[1] << wd.shift) | (wd.x[2] >> (64 - wd.shift));
+        p2 = (wd.x[2] << wd.shift) | (wd.x[3] >> (64 - wd.shift));
     }
-    p0 = keep_bases(p0, (int)take);
-    p1 = keep_bases(p1, (int)take - 32);
-    p2 = keep_bases(p2, (int)take - 64);        // at most 24 bases: the low 16 bits are clear
-    const uint64_t k0 = p2 | ((uint64_t)take << 8) | idx;
-    Key192 k;
-    k.lo = make_uint4((uint32_t)k0, (uint32_t)(k0 >> 32), (uint32_t)p1, (uint32_t)(p1 >> 32));
-    k.hi = make_uint2((uint32_t)p0, (uint32_t)(p0 >> 32));
-    return k;
+    sm.w0[m] = keep_bases(p0, (int)wd.take);
+    sm.w1[m] = keep_bases(p1, (int)wd.take - 32);
+    sm.w2[m] = keep_bases(p2, (int)wd.take - 64);
 }
 
-// acc -= (a < b) for 192-bit unsigned a, b: the borrow of a - b, seven instructions
-__device__ __forceinline__ void count_if_less(uint32_t& acc, const uint4& alo, const uint2& ahi, const uint4& blo, const uint2& bhi) {
-    asm("{\n\t.reg .u32 t;\n\t"
-        "sub.cc.u32 t, %1, %7;\n\tsubc.cc.u32 t, %2, %8;\n\tsubc.cc.u32 t, %3, %9;\n\tsubc.cc.u32 t, %4, %10;\n\t"
-        "subc.cc.u32 t, %5, %11;\n\tsubc.cc.u32 t, %6, %12;\n\t"
-        "subc.u32 %0, %0, 0;\n\t}"
-        : "+r"(acc)
-        : "r"(alo.x), "r"(alo.y), "r"(alo.z), "r"(alo.w), "r"(ahi.x), "r"(ahi.y), "r"(blo.x), "r"(blo.y), "r"(blo.z), "r"(blo.w), "r"(bhi.x),
-          "r"(bhi.y));
+// Lanes hold consecutive positions; H = head bits of the warp's 32 positions.  The maximum of `val` over each run of lanes
+// between heads is added to the slot of that run with ONE shared-memory atomic by the run's last lane (a group's members
+// would otherwise all hit one address).  val = 0: nothing to publish (slot is then not read).
+__device__ __forceinline__ void seg_max_publish(uint32_t val, uint32_t H, uint32_t* slots, uint32_t slot) {
+    const uint32_t lane = lane_id();
+    const uint32_t hb = H & (0xffffffffu >> (31 - lane));
+    const uint32_t lo = hb ? 31u - (uint32_t)__clz(hb) : 0u;   // first lane of my run
+#pragma unroll
+    for (uint32_t o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(kFull, val, o);
+        if (lane >= lo + o && v > val) val = v;
+    }
+    const bool last = lane == 31 || ((H >> (lane + 1)) & 1u);
+    if (last && val) atomicMax(slots + slot, val);
+}
+
+// merge levels a group [s, t) needs after its aligned 32-position windows have been ranked: 0 if it lies in one window
+__device__ __forceinline__ int merge_levels(int s, int t) {
+    const uint32_t x = (uint32_t)(s ^ (t - 1)) >> 5;
+    return x ? 32 - __clz(x) : 0;
 }
 
 template <typename KeyT, typename IdT, bool FIRST, bool PACKED>
-__global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_kernel(Reads R, const KeyT* __restrict__ keys1, uint32_t w1, uint32_t len_mask,
-                                                                    const uint32_t* __restrict__ heads_in, uint32_t* __restrict__ heads,
-                                                                    IdT* __restrict__ ids, uint64_t n,
-                                                                    uint32_t depth0, uint32_t cap, uint8_t* __restrict__ out,
-                                                                    unsigned long long* elems_done) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    LocalSmem<IdT>& sm = *reinterpret_cast<LocalSmem<IdT>*>(smem_raw);
-    const uint64_t base = (uint64_t)blockIdx.x * kLocalTile;
+__device__ __forceinline__ void finish_tile(LocalSmem& sm, uint64_t tile, const Reads& R, const KeyT* __restrict__ keys1, uint32_t w1, uint32_t len_mask,
+                                            const uint32_t* __restrict__ heads_in, uint32_t* __restrict__ heads, const IdT* __restrict__ ids,
+                                            uint64_t n, uint32_t depth0, uint32_t min_group, uint32_t cap, uint8_t* __restrict__ out,
+                                            unsigned long long* elems_done) {
+    const uint64_t base = tile * kLocalTile;
     const uint64_t w0 = base >> 5;
     const uint64_t n_words = (n + 31) >> 5;   // heads[n_words] is the padding word ("the next position is a head")
     const int tid = threadIdx.x;
 
+    for (int i = tid; i < kLocalElems / 2; i += kLocalThreads) sm.gpiv[0][i] = 0;
     // ---- head bits of the window ------------------------------------------------------------------
     if (FIRST) {
 #pragma unroll
@@ -379,11 +405,10 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
     __syncthreads();
 
     // ---- classify: groups that start in this tile and have at most cap members are ours -----------
-    // The kernel lives on random gathers (the offsets table, the word before the suffix, the key words); every batch
-    // of them is issued for all of a thread's positions before the first is used, so their latencies overlap.
     uint32_t n_active = 0, n_compares = 0;
     IdT idv[kLocalItems];
     uint32_t state = 0;   // 2 bits per position: 0 not ours, 1 alone in its group (final), 2 member of a group refined here
+    uint16_t gsv[kLocalItems];
 #pragma unroll
     for (int k = 0; k < kLocalItems; ++k) {
         const int e = k * kLocalThreads + tid;
@@ -395,39 +420,33 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
             const int ps = prev_head(sm.hw, e, lo < 0 ? 0 : lo);
             if (ps >= 0 && ps < kLocalTile) {
                 const int ne = next_head(sm.hw, e, ps + (int)cap);
-                if (ne > 0) {
-                    if (ne - ps >= 2) {
-                        s = (uint16_t)ps;
-                        t = (uint16_t)ne;
-                        st = 2;
-                        ++n_active;
-                    } else if (FIRST) {
-                        st = 1;
-                    }
+                if (ne > 0 && ne - ps >= (int)min_group) {   // FIRST: smaller groups were finished by the warp kernel
+                    s = (uint16_t)ps;
+                    t = (uint16_t)ne;
+                    st = 2;
+                    ++n_active;
                 }
             }
-            if (FIRST) {
-                idv[k] = (IdT)sm.loc[e];
-                // packed input carries the ids inside the key words: hand those of the suffixes left to the global path over
-                if (PACKED && !st && e < kLocalTile) ids[base + e] = idv[k];
-            } else if (st) {
-                idv[k] = ids[base + e];
-            }
+            if (st) idv[k] = FIRST ? (IdT)sm.loc[e] : ids[base + e];
         }
         sm.gs[e] = s;
         sm.ge[e] = t;
+        sm.mem[0][e] = (uint16_t)e;
+        gsv[k] = s;
         state |= st << (2 * k);
     }
+    // ---- locators, the base before every suffix of ours, and the window of every member: one batch of gathers --------
+    // The kernel lives on these random reads; all of a thread's loads are issued before the first is used.
     {
         uint64_t first_base[kLocalItems];   // index of the suffix's first base in the packed text
-        uint32_t left[kLocalItems];         // bases from there to the end of its read
+        uint64_t left[kLocalItems];         // bases from there to the end of its read
         const uint64_t pos_mask = (1ull << R.pos_bits) - 1;
         if (R.uniform) {
 #pragma unroll
             for (int k = 0; k < kLocalItems; ++k) {
                 const uint64_t read = (uint64_t)idv[k] >> R.pos_bits, pos = (uint64_t)idv[k] & pos_mask;
                 first_base[k] = read * R.uniform_len + pos;
-                left[k] = (uint32_t)(R.uniform_len - pos);
+                left[k] = R.uniform_len - pos;
             }
         } else {
             uint64_t lo[kLocalItems], hi[kLocalItems];
@@ -441,14 +460,18 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
             for (int k = 0; k < kLocalItems; ++k) {
                 const uint64_t pos = (uint64_t)idv[k] & pos_mask;
                 first_base[k] = lo[k] + pos;
-                left[k] = (uint32_t)(hi[k] - lo[k] - pos);
+                left[k] = hi[k] - lo[k] - pos;
             }
         }
         uint64_t before[kLocalItems];       // the word that holds the base before the suffix
+        Window wd[kLocalItems];
 #pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
-            const bool want = ((state >> (2 * k)) & 3u) && ((uint64_t)idv[k] & pos_mask);
-            before[k] = want ? __ldg(R.packed + ((first_base[k] - 1) >> 5)) : 0ull;   // no load at all for a read's first suffix (packed may hold no word)
+            const uint32_t st = (state >> (2 * k)) & 3u;
+            const bool want = st && ((uint64_t)idv[k] & pos_mask);
+            before[k] = want ? __ldg(R.packed + ((first_base[k] - 1) >> 5)) : 0ull;   // no load for a read's first suffix
+            const uint64_t rem = st == 2 ? left[k] - depth0 : 0ull;                    // a member of an open group has >= depth0 bases
+            window_load(R.packed, first_base[k] + depth0, (uint32_t)(rem < kWin ? rem : kWin), st == 2, wd[k]);
         }
 #pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
@@ -456,158 +479,207 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
             const uint32_t st = (state >> (2 * k)) & 3u;
             uint64_t code = 1;   // $: the suffix starts its read
             if ((uint64_t)idv[k] & pos_mask) code = 2 + ((before[k] >> (62 - 2 * ((first_base[k] - 1) & 31))) & 3u);
-            const uint64_t loc = (code << (kLocBaseBits + kLocRemBits)) | ((uint64_t)left[k] << kLocBaseBits) | first_base[k];
-            if (FIRST && st == 1) out[base + e] = loc_symbol(loc);   // alone in its group after the first sort: final
-            sm.loc[e] = st == 2 ? loc : 0ull;
+            uint32_t cand = 0;
+            if (st == 2) {
+                const uint64_t rem = left[k] - depth0;
+                window_store(wd[k], sm, e);
+                sm.loc[e] = (code << kLocCodeShift) | ((uint64_t)wd[k].take << kLocTakeShift) | (first_base[k] + depth0);
+                sm.mrem[e] = (uint32_t)rem;   // reads are shorter than 2^32 bases (checked by the build)
+                cand = (wd[k].take << 10) | (uint32_t)e;
+            }
+            // the pivot of every group: its member with the most bases in the window
+            seg_max_publish(cand, sm.hw[e >> 5], sm.gpiv[0], (uint32_t)(gsv[k] >> 1));
         }
     }
     __syncthreads();
 
-    // ---- rounds: one 88-base gather per member still tied, stable rank (see below) ----------------------
-    for (uint32_t depth = depth0;; depth += kLocalW) {
+    // ---- rounds ----------------------------------------------------------------------------------------------------
+    uint32_t n_rounds = 0;
+    for (int pb = 0, mb = 0;; pb ^= 1, mb ^= 1, ++n_rounds) {
+        // keys: where each member first differs from its group's pivot
+        uint32_t mykey[kLocalItems];
         uint32_t any = 0;
+        for (int i = tid; i < kLocalElems / 2; i += kLocalThreads) sm.gpiv[pb ^ 1][i] = 0;
 #pragma unroll
-        for (int kk = 0; kk < kLocalItems; kk += 2) {
-            uint64_t w[2][4];
-            uint32_t take[2], shift[2];
-            int start[2];
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-                const int e = (kk + j) * kLocalThreads + tid;
-                const bool exists = kk + j < kLocalItems;
-                start[j] = exists ? sm.gs[e] : kNone;
-                const uint64_t loc = exists ? sm.loc[e] : 0ull;
-                const uint32_t remaining = start[j] != kNone ? (uint32_t)(loc >> kLocBaseBits) & ((1u << kLocRemBits) - 1) : 0u;
-                const uint32_t rem = remaining > depth ? remaining - depth : 0u;
-                take[j] = rem < kLocalW ? rem : kLocalW;
-                const uint64_t b = (loc & ((1ull << kLocBaseBits) - 1)) + depth;
-                shift[j] = (uint32_t)(b & 31) * 2;
-                const uint32_t n_w = take[j] ? (shift[j] + 2 * take[j] + 63) >> 6 : 0u;   // words the window touches
-                const uint64_t* p = R.packed + (b >> 5);
-#pragma unroll
-                for (int i = 0; i < 4; ++i) w[j][i] = i < (int)n_w ? __ldg(p + i) : 0ull;
-            }
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-                if (start[j] == kNone) continue;
-                const int e = (kk + j) * kLocalThreads + tid;
-                const Key192 key = key192_of_words(w[j], shift[j], take[j], (uint32_t)(e - start[j]));
-                sm.key_lo[e] = key.lo;
-                sm.key_hi[e] = key.hi;
+        for (int k = 0; k < kLocalItems; ++k) {
+            const int q = k * kLocalThreads + tid;
+            const int s = sm.gs[q];
+            mykey[k] = (uint32_t)q << 21;
+            if (s != kNone) {
+                const int m = sm.mem[mb][q];
+                const uint32_t pv = sm.gpiv[pb][s >> 1];
+                const int pm = pv & 1023u;
+                const uint32_t tb = pv >> 10, ta = loc_take(sm.loc[m]);
+                const uint64_t a0 = sm.w0[m], a1 = sm.w1[m], a2 = sm.w2[m];
+                const uint64_t x0 = a0 ^ sm.w0[pm], x1 = a1 ^ sm.w1[pm], x2 = a2 ^ sm.w2[pm];
+                // first base at which the two windows differ (kWin: nowhere)
+                const uint32_t d = x0 ? (uint32_t)__clzll((long long)x0) >> 1 : x1 ? 32u + ((uint32_t)__clzll((long long)x1) >> 1)
+                                      : x2 ? 64u + ((uint32_t)__clzll((long long)x2) >> 1) : kWin;
+                const uint32_t lim = ta < tb ? ta : tb;
+                uint32_t K;
+                if (d < lim || ta > tb) {
+                    // a base of mine against a base of the pivot (d < lim), or against the pivot's end-marker (the pivot
+                    // ended at tb and I go on: above it; cannot happen while the pivot is the longest member)
+                    const uint32_t at = d < lim ? d : tb;
+                    const uint64_t aw = at < 32 ? a0 : at < 64 ? a1 : a2;
+                    const uint32_t sa = (uint32_t)(aw >> (62 - 2 * (at & 31))) & 3u;
+                    bool below = false;
+                    if (d < lim) {
+                        const uint64_t bw = at < 32 ? sm.w0[pm] : at < 64 ? sm.w1[pm] : sm.w2[pm];
+                        below = sa < ((uint32_t)(bw >> (62 - 2 * (at & 31))) & 3u);
+                    }
+                    K = below ? at * 8 + sa + 1 : kKeyAbove + (kWin - 1 - at) * 8 + sa + 1;
+                } else if (ta < tb) {
+                    K = ta * 8;          // my end-marker against a base of the pivot: below it ($ is the smallest symbol)
+                } else {
+                    K = kKeyEqual;       // equal to the pivot through the window (and of its length)
+                }
+                mykey[k] = ((uint32_t)s << 21) | (K << 8) | (uint32_t)(q - s);
                 any = 1;
             }
+            sm.key[q] = mykey[k];
         }
         if (!__syncthreads_or(any)) break;
-        // Stable rank inside every group.  Members are first ranked by counting inside sub-blocks of kSubBlock
-        // consecutive members (<= kSubBlock comparisons each); sorted runs are then merged pairwise, each member
-        // finding its rank in the sibling run by binary search (keys are distinct: the group index is part of them),
-        // so a group of g members costs ~kSubBlock + log2(g / kSubBlock) * log2(g) comparisons per member, not g.
-        uint32_t myrank[kLocalItems];
-        uint32_t more = 0;   // some group of mine is longer than one sub-block
-        int cur = 0;
+        // Stable rank.  Keys are comparable across groups (the group's first position leads the key), so a member's place
+        // inside its aligned window of 32 positions is the number of smaller keys among the 32, whoever owns them.
+        int pos[kLocalItems];
 #pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
-            const int e = k * kLocalThreads + tid;
-            const int s = sm.gs[e];
-            myrank[k] = 0;
-            if (s != kNone) {
-                const int t = sm.ge[e];
-                const int b0 = s + ((e - s) / kSubBlock) * kSubBlock;
-                const int b1 = min(b0 + kSubBlock, t);
-                const uint4 my = sm.key_lo[e];
-                const uint2 myh = sm.key_hi[e];
-                n_compares += (uint32_t)(b1 - b0);
-                uint32_t neg = 0;   // minus the number of sub-block members whose key is below mine
-#pragma unroll 4
-                for (int q = b0; q < b1; ++q) count_if_less(neg, sm.key_lo[q], sm.key_hi[q], my, myh);
-                myrank[k] = 0u - neg;
-                sm.ord[0][b0 + myrank[k]] = (uint16_t)e;
-                more |= (uint32_t)(t - s > kSubBlock);
+            const int q = k * kLocalThreads + tid;
+            pos[k] = q;
+            if (sm.gs[q] != kNone) {
+                const uint4* wkeys = reinterpret_cast<const uint4*>(sm.key + (q & ~31));
+                const uint32_t me = mykey[k];
+                uint32_t below = 0;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const uint4 v = wkeys[i];
+                    below += (uint32_t)(v.x < me) + (uint32_t)(v.y < me) + (uint32_t)(v.z < me) + (uint32_t)(v.w < me);
+                }
+                pos[k] = (q & ~31) + (int)below;
+                sm.sk[0][pos[k]] = me;
+                n_compares += 32;
             }
         }
-        static_assert((kSubBlock & (kSubBlock - 1)) == 0, "runs double from a power of two");
-        for (int run = kSubBlock, sh = 31 - __clz(kSubBlock); __syncthreads_or(more); run *= 2, ++sh) {
-            more = 0;
+        // groups that span several windows: sorted runs are merged pairwise, each member finding its rank in the
+        // sibling run by binary search over the sorted keys (keys are distinct: the index in the group is part of them)
+        for (int level = 0;; ++level) {
+            uint32_t more = 0;
 #pragma unroll
             for (int k = 0; k < kLocalItems; ++k) {
-                const int e = k * kLocalThreads + tid;
-                const int s = sm.gs[e];
+                const int q = k * kLocalThreads + tid;
+                const int s = sm.gs[q];
+                if (s != kNone) more |= (uint32_t)(merge_levels(s, sm.ge[q]) > level);
+            }
+            if (!__syncthreads_or(more)) break;
+            const uint32_t* src = sm.sk[level & 1];
+            uint32_t* dst = sm.sk[(level + 1) & 1];
+            const int wd = 32 << level;
+#pragma unroll
+            for (int k = 0; k < kLocalItems; ++k) {
+                const int q = k * kLocalThreads + tid;
+                const int s = sm.gs[q];
                 if (s == kNone) continue;
-                const int t = sm.ge[e];
-                const int r = (e - s) >> sh;             // my run, its sibling is r ^ 1
-                uint32_t nr = myrank[k];
-                if (t - s > run) {
-                    const int sb = s + (r ^ 1) * run;    // sibling run [sb, sb + len)
-                    if (sb < t) {
-                        const uint4 my = sm.key_lo[e];
-                        const uint2 myh = sm.key_hi[e];
-                        int lo = 0, hi = min(run, t - sb);
-                        n_compares += 32 - __clz(hi);
-                        while (lo < hi) {                // lower bound: sibling members below me
-                            const int mid = (lo + hi) >> 1;
-                            uint32_t neg = 0;
-                            const int qi = sm.ord[cur][sb + mid];
-                            count_if_less(neg, sm.key_lo[qi], sm.key_hi[qi], my, myh);
-                            if (neg) lo = mid + 1; else hi = mid;
-                        }
-                        nr += (uint32_t)lo;
+                const int t = sm.ge[q];
+                if (merge_levels(s, t) <= level) continue;
+                const int wbase = q & ~(wd - 1), sbase = wbase ^ wd;                  // my window and its sibling
+                const int my_lo = max(s, wbase);
+                const int sib_lo = max(s, sbase), sib_hi = min(t, sbase + wd);       // the group's part of the sibling run
+                int lo = 0;
+                if (sib_lo < sib_hi) {
+                    int hi = sib_hi - sib_lo;
+                    const uint32_t me = mykey[k];
+                    n_compares += 32 - __clz(hi);
+                    while (lo < hi) {                // lower bound: sibling members below me
+                        const int mid = (lo + hi) >> 1;
+                        if (src[sib_lo + mid] < me) lo = mid + 1; else hi = mid;
                     }
-                    myrank[k] = nr;
-                    sm.ord[cur ^ 1][s + (r >> 1) * 2 * run + nr] = (uint16_t)e;
-                    more |= (uint32_t)(t - s > 2 * run);
-                } else {
-                    sm.ord[cur ^ 1][s + nr] = (uint16_t)e;   // already one run: carried over
                 }
-            }
-            cur ^= 1;
-        }
-        const uint16_t* src = sm.ord[cur];
-        uint64_t locn[kLocalItems];
-        uint32_t headbit = 0;
-#pragma unroll
-        for (int k = 0; k < kLocalItems; ++k) {
-            const int e = k * kLocalThreads + tid;
-            if (sm.gs[e] != kNone) {
-                const int se = src[e];
-                const uint4 kk = sm.key_lo[se];
-                locn[k] = sm.loc[se];
-                bool head = e == sm.gs[e] || ((kk.x >> 8) & 127u) < kLocalW;
-                if (!head) {   // same bases and length as the member ranked just before?  (the low 8 bits are the group index)
-                    const int sp = src[e - 1];
-                    const uint4 kp = sm.key_lo[sp];
-                    const uint2 hk = sm.key_hi[se], hp = sm.key_hi[sp];
-                    head = (((((kk.x ^ kp.x) >> 8) | (kk.y ^ kp.y)) | ((kk.z ^ kp.z) | (kk.w ^ kp.w))) | ((hk.x ^ hp.x) | (hk.y ^ hp.y))) != 0;
-                }
-                headbit |= (uint32_t)head << k;
+                const int start = sib_lo < sib_hi && sbase < wbase ? sib_lo : my_lo;   // first position of the merged run
+                pos[k] = start + (pos[k] - my_lo) + lo;
+                dst[pos[k]] = mykey[k];
             }
         }
-        __syncthreads();
+        // new head bits, position by position over the ranked keys; the member that ranked at a position moves there
+        uint32_t info[kLocalItems];   // (key class << 16 | member now here), ~0u: position not in an open group
 #pragma unroll
         for (int k = 0; k < kLocalItems; ++k) {
-            const int e = k * kLocalThreads + tid;
-            if (sm.gs[e] != kNone) sm.loc[e] = locn[k];
-            // a warp's 32 positions share one head word and no other warp touches it in this phase: one ballot and one
-            // plain update instead of up to 32 serialised shared-memory atomics (12 % of the kernel's shared wavefronts)
-            const uint32_t word = __ballot_sync(kFull, (headbit >> k) & 1u);
-            if ((tid & 31) == 0 && word) sm.hw[e >> 5] |= word;
-        }
-        __syncthreads();
-        // new group bounds; members alone in their group are placed for good
-#pragma unroll
-        for (int k = 0; k < kLocalItems; ++k) {
-            const int e = k * kLocalThreads + tid;
-            const int s = sm.gs[e];
+            const int p = k * kLocalThreads + tid;
+            const int s = sm.gs[p];
+            bool head = false;
+            info[k] = ~0u;
             if (s != kNone) {
-                // head bits of e and e + 1 both set: alone in its group, placed for good
-                const uint32_t lo = sm.hw[e >> 5], hi = sm.hw[(e >> 5) + 1];
-                if (((((uint64_t)hi << 32) | lo) >> (e & 31) & 3u) == 3u) {
-                    sm.gs[e] = kNone;
+                const uint32_t* fin = sm.sk[merge_levels(s, sm.ge[p]) & 1];
+                const uint32_t kk = fin[p];
+                const uint32_t K = (kk >> 8) & 0x7ffu;
+                const uint32_t tb = sm.gpiv[pb][s >> 1] >> 10;
+                // final classes: members that ended at their divergence, or equal the pivot and end with it -- identical
+                // strings, already in read-index order; each becomes a group of one
+                const bool final_class = (K < kKeyEqual && (K & 7u) == 0) || (K == kKeyEqual && tb < kWin);
+                head = p == s || final_class || K != ((fin[p - 1] >> 8) & 0x7ffu);
+                const uint32_t m = sm.mem[mb][s + (kk & 255u)];
+                sm.mem[mb ^ 1][p] = (uint16_t)m;
+                info[k] = (K << 16) | m;
+            }
+            const uint32_t word = __ballot_sync(kFull, head);
+            if ((tid & 31) == 0 && word) sm.hw[p >> 5] |= word;
+        }
+        __syncthreads();
+        // new group bounds; members alone in their group are placed for good; the others name their next pivot
+        uint32_t regather = 0;
+#pragma unroll
+        for (int k = 0; k < kLocalItems; ++k) {
+            const int p = k * kLocalThreads + tid;
+            uint32_t cand = 0, slot = 0;
+            if (info[k] != ~0u) {
+                const uint32_t m = info[k] & 0xffffu, K = info[k] >> 16;
+                const uint32_t lo = sm.hw[p >> 5], hi = sm.hw[(p >> 5) + 1];
+                uint64_t loc = sm.loc[m];
+                if (((((uint64_t)hi << 32) | lo) >> (p & 31) & 3u) == 3u) {   // head bits of p and p + 1: alone, placed
+                    sm.sym[p] = loc_symbol(loc);
+                    sm.gs[p] = kNone;
                 } else {
-                    const int t = sm.ge[e];
-                    sm.gs[e] = (uint16_t)prev_head(sm.hw, e, s);
-                    sm.ge[e] = (uint16_t)next_head(sm.hw, e, t);
+                    const int s2 = prev_head(sm.hw, p, sm.gs[p]);
+                    const int t2 = next_head(sm.hw, p, sm.ge[p]);
+                    sm.gs[p] = (uint16_t)s2;
+                    sm.ge[p] = (uint16_t)t2;
+                    uint32_t take = loc_take(loc);
+                    if (K == kKeyEqual) {   // equal to the pivot through a full window: on to the next window of the read
+                        const uint32_t rem = sm.mrem[m] - kWin;
+                        sm.mrem[m] = rem;
+                        take = rem < kWin ? rem : kWin;
+                        loc = (loc & ~((0xffull << kLocTakeShift) | kLocBaseMask)) | ((uint64_t)take << kLocTakeShift) | ((loc & kLocBaseMask) + kWin) | kLocGather;
+                        sm.loc[m] = loc;
+                        regather = 1;
+                    }
+                    cand = (take << 10) | m;
+                    slot = (uint32_t)s2 >> 1;
                 }
             }
+            seg_max_publish(cand, sm.hw[p >> 5], sm.gpiv[pb ^ 1], slot);
+        }
+        if (__syncthreads_or(regather)) {
+            Window wd[kLocalItems];
+            uint32_t mm[kLocalItems];
+#pragma unroll
+            for (int k = 0; k < kLocalItems; ++k) {
+                const int p = k * kLocalThreads + tid;
+                mm[k] = ~0u;
+                uint64_t loc = 0;
+                if (sm.gs[p] != kNone) {
+                    const uint32_t m = sm.mem[mb ^ 1][p];
+                    loc = sm.loc[m];
+                    if (loc & kLocGather) mm[k] = m;
+                }
+                window_load(R.packed, loc & kLocBaseMask, loc_take(loc), mm[k] != ~0u, wd[k]);
+            }
+#pragma unroll
+            for (int k = 0; k < kLocalItems; ++k) {
+                if (mm[k] == ~0u) continue;
+                window_store(wd[k], sm, (int)mm[k]);
+                sm.loc[mm[k]] &= ~kLocGather;
+            }
+            __syncthreads();
         }
     }
 
@@ -615,13 +687,14 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
 #pragma unroll
     for (int k = 0; k < kLocalItems; ++k) {
         const int e = k * kLocalThreads + tid;
-        const uint64_t loc = sm.loc[e];
-        if (loc) out[base + e] = loc_symbol(loc);
+        if (((state >> (2 * k)) & 3u) == 2) out[base + e] = sm.sym[e];
     }
-    for (int i = tid; i < kLocalWords; i += kLocalThreads) {
-        if (w0 + i > n_words) continue;
-        const uint32_t add = FIRST ? (i < kLocalElems / 32 ? sm.hw[i] : 0u) : (sm.hw[i] & ~sm.hw0[i]);
-        if (add) atomicOr(&heads[w0 + i], add);
+    if (!FIRST) {   // FIRST: the warp kernel has published every position of a group of at most cap members as placed
+        for (int i = tid; i < kLocalWords; i += kLocalThreads) {
+            if (w0 + i > n_words) continue;
+            const uint32_t add = sm.hw[i] & ~sm.hw0[i];
+            if (add) atomicOr(&heads[w0 + i], add);
+        }
     }
     // one statistics update per block (hundreds of thousands of atomics on one address would serialise in L2)
     __shared__ uint32_t s_done, s_cmp;
@@ -635,7 +708,555 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
     __syncthreads();
     if (tid == 0 && s_done) {
         atomicAdd(elems_done, (unsigned long long)s_done);
-        atomicAdd(elems_done + 2, (unsigned long long)s_cmp);   // 128-bit key comparisons done (the ALU work of this kernel)
+        atomicAdd(elems_done + 2, (unsigned long long)s_cmp);
+        atomicAdd(elems_done + 3, (unsigned long long)n_rounds);   // refinement rounds (diagnostic)
+    }
+}
+
+// Persistent blocks over the tiles.  FIRST: only tiles in which the warp kernel met a group of 33..cap members (big_tiles bit).
+template <typename KeyT, typename IdT, bool FIRST, bool PACKED>
+__global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_kernel(Reads R, const KeyT* __restrict__ keys1, uint32_t w1, uint32_t len_mask,
+                                                                    const uint32_t* __restrict__ heads_in, uint32_t* __restrict__ heads,
+                                                                    const IdT* __restrict__ ids, uint64_t n, uint32_t depth0, uint32_t min_group,
+                                                                    uint32_t cap, const uint32_t* __restrict__ big_tiles, uint8_t* __restrict__ out,
+                                                                    unsigned long long* elems_done) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    LocalSmem& sm = *reinterpret_cast<LocalSmem*>(smem_raw);
+    const uint64_t n_tiles = (n + kLocalTile - 1) / kLocalTile;
+    for (uint64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        if (FIRST && !((__ldg(big_tiles + (tile >> 5)) >> (tile & 31)) & 1u)) continue;
+        finish_tile<KeyT, IdT, FIRST, PACKED>(sm, tile, R, keys1, w1, len_mask, heads_in, heads, ids, n, depth0, min_group, cap, out, elems_done);
+        __syncthreads();   // the next tile reuses the shared memory
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a7 + a8 for the common case, one WARP per chunk of sorted positions: tie groups of at most 32 S suffixes (coverage-sized
+// groups of short-read collections; S = 2 slots per lane) never leave the registers of a warp.
+//
+// A warp walks its chunk in windows of 32 S positions that start at a group head; position p of the window lives in
+// slot p / 32 of lane p % 32.  Groups that end inside the window are finished at once, the one cut by the window's end
+// starts the next window.  Per window:
+//   head flags from adjacent first-round keys (one shuffle); every position decodes its suffix id and gathers the base
+//   before the suffix and -- members of a group of two or more -- its window of the next 96 bases, ONCE, as six 32-bit
+//   words (bases past the end of the read are whatever follows in the packed text: they are never looked at);
+//   the group's pivot is its member with the most bases (segmented max scan); its window reaches the others by shuffles;
+//   one XOR + count-leading-zeros against the pivot gives where a member first differs from it, a second one where it
+//   differs next (a pivot with a sequencing error sends its whole group to the same first divergence; the second level
+//   orders them without another round): key = [group's first position : 6][level 1 : 10][level 2 : 10][index in group : 6];
+//   a bitonic sort of the window's keys ranks every group stably and keeps groups in place;
+//   classes that share a key and did not END there go round again (their data follows them by shuffles).
+// Singletons and finished members are emitted as coalesced byte stores.
+// Groups of more than 32 S and at most cap suffixes are left to the block kernel (their tile is flagged); larger ones to
+// the global path (only their head bit is published, their ids handed over, and they are counted).
+// ---------------------------------------------------------------------------------------------
+constexpr int kWarpChunk = 2048;    // sorted positions per warp: a chunk owns the groups that START in it
+constexpr int kWarpThreads = 256;
+constexpr int kWarpSlots = 2;
+
+// Event codes (the two levels of the rank key), order-preserving; 0 = no event:
+//   1 + 5 d + s         below the pivot at base d: s = 0 my end-marker (FINAL: identical strings), 1..4 my base A..T
+//   1 + kCodeEqual      equal to the pivot, which ends inside the window (FINAL);  + 1: equal through a full window, both go on
+//   1 + kCodeAbove + 4 (95 - d) + b   above the pivot at base d, my base b = 0..3 there
+constexpr uint32_t kCodeEqual = kWin * 5, kCodeAbove = kCodeEqual + 2;
+// what a code says about the class of members that share it: 0 no event, 1 FINAL, 2 next window needed, 3 a base mismatch
+__device__ __forceinline__ uint32_t code_type(uint32_t c) {
+    const uint32_t k = c - 1;
+    const uint32_t r = k - 5u * ((k * 13108u) >> 16);            // k % 5 for k < 2^13
+    const bool fin = k == kCodeEqual || (k < kCodeEqual && r == 0);
+    return c == 0 ? 0u : fin ? 1u : k == kCodeEqual + 1 ? 2u : 3u;
+}
+
+struct Win6 {
+    uint32_t w[6];   // 16 bases per word, first base in the most significant bits
+};
+// Where window a (ta bases) differs from the pivot's window b (tb >= ta bases: the pivot is its group's longest member):
+// the first two events (see the codes above).  Bases at or past ta are never looked at.
+// (Every array index below is a compile-time constant: a data-dependent one would move the windows to local memory.)
+__device__ __forceinline__ void diverge2(const Win6& a, const Win6& b, uint32_t ta, uint32_t tb, uint32_t& c1, uint32_t& c2) {
+    uint32_t x[6];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) x[i] = a.w[i] ^ b.w[i];
+    // first base at which the windows differ (kWin: none), the XOR word it is in and my word there
+    uint32_t d = kWin, xw = 0, aw = 0;
+#pragma unroll
+    for (int i = 5; i >= 0; --i) {
+        const bool hit = x[i] != 0;
+        d = hit ? 16u * i + ((uint32_t)__clz(x[i]) >> 1) : d;
+        xw = hit ? x[i] : xw;
+        aw = hit ? a.w[i] : aw;
+    }
+    c2 = 0;
+    if (d >= ta) {   // no base of mine differs: my end-marker against a base of the pivot ($ is the smallest symbol), or equal
+        c1 = 1 + (ta < tb ? 5 * ta : (tb < kWin ? kCodeEqual : kCodeEqual + 1));
+        return;
+    }
+    {
+        const uint32_t sh = 30 - 2 * (d & 15);
+        const uint32_t sa = (aw >> sh) & 3u, sb = sa ^ ((xw >> sh) & 3u);
+        c1 = 1 + (sa < sb ? 5 * d + sa + 1 : kCodeAbove + 4 * (kWin - 1 - d) + sa);
+        xw &= ~(3u << sh);   // forget this base: where do we differ next?
+    }
+    uint32_t d2 = kWin, xw2 = 0, aw2 = 0;
+#pragma unroll
+    for (int i = 5; i >= 0; --i) {
+        const bool hit = x[i] != 0 && 16u * i > (d | 15u);   // words after the one of the first difference
+        d2 = hit ? 16u * i + ((uint32_t)__clz(x[i]) >> 1) : d2;
+        xw2 = hit ? x[i] : xw2;
+        aw2 = hit ? a.w[i] : aw2;
+    }
+    if (xw) d2 = (d & ~15u) + ((uint32_t)__clz(xw) >> 1), xw2 = xw, aw2 = aw;   // the same word again
+    if (d2 >= ta) {
+        c2 = 1 + (ta < tb ? 5 * ta : (tb < kWin ? kCodeEqual : kCodeEqual + 1));
+    } else {
+        const uint32_t sh = 30 - 2 * (d2 & 15);
+        const uint32_t sa = (aw2 >> sh) & 3u, sb = sa ^ ((xw2 >> sh) & 3u);
+        c2 = 1 + (sa < sb ? 5 * d2 + sa + 1 : kCodeAbove + 4 * (kWin - 1 - d2) + sa);
+    }
+}
+
+template <typename KeyT, bool PACKED>
+__device__ __forceinline__ uint64_t load_keyword(const KeyT* __restrict__ keys1, uint64_t j) {
+    if constexpr (PACKED) return __ldg(reinterpret_cast<const uint64_t*>(keys1) + j);   // key << 32 | id
+    else return (uint64_t)__ldg(keys1 + j);
+}
+template <bool PACKED>
+__device__ __forceinline__ uint64_t key_of(uint64_t word) { return PACKED ? word >> 32 : word; }
+
+// first head at or after position p >= 1 (position n counts as one): a head starts a tie group
+template <typename KeyT, bool PACKED>
+__device__ __forceinline__ uint64_t scan_to_head(const KeyT* __restrict__ keys1, uint64_t p, uint64_t n, uint32_t w1, uint32_t len_mask) {
+    const uint32_t lane = lane_id();
+    uint64_t carry = key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, p - 1));
+    while (true) {
+        const uint64_t j = p + lane;
+        const uint64_t k = j < n ? key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j)) : 0ull;
+        uint64_t kp = __shfl_up_sync(kFull, k, 1);
+        if (lane == 0) kp = carry;
+        const bool head = j >= n || k != kp || ((uint32_t)k & len_mask) < w1;
+        const uint32_t m = __ballot_sync(kFull, head);
+        if (m) return p + (uint32_t)__ffs(m) - 1;
+        carry = __shfl_sync(kFull, k, 31);
+        p += 32;
+    }
+}
+
+// OR `bits` (bit i = position a + i) into the head bitmask; whole-warp call, two lanes write
+__device__ __forceinline__ void publish_heads(uint32_t* __restrict__ heads, uint64_t a, uint32_t bits) {
+    const uint32_t sh = (uint32_t)(a & 31);
+    const uint32_t lane = lane_id();
+    if (lane == 0 && (bits << sh)) atomicOr(heads + (a >> 5), bits << sh);
+    if (lane == 1 && sh && (bits >> (32 - sh))) atomicOr(heads + (a >> 5) + 1, bits >> (32 - sh));
+}
+
+// value of `v` at window position q (slot q / 32 of lane q % 32), for every lane its own q
+template <int S, typename T>
+__device__ __forceinline__ T fetch_at(const T (&v)[S], uint32_t q) {
+    static_assert(S == 1 || S == 2, "written out per slot count: a loop over slots ends up in local memory");
+    if constexpr (S == 1) {
+        return __shfl_sync(kFull, v[0], q & 31);
+    } else {
+        const T lo = __shfl_sync(kFull, v[0], q & 31), hi = __shfl_sync(kFull, v[1], q & 31);
+        return (q & 32u) ? hi : lo;
+    }
+}
+
+// the packed bases from index b on, as six 32-bit words (16 bases each); loads only the words that `take` bases touch
+__device__ __forceinline__ void window_words(const uint64_t* __restrict__ packed, uint64_t b, uint32_t take, bool want, Win6& out) {
+    const uint32_t shift = (uint32_t)(b & 31) * 2;
+    const uint32_t n_w = want && take ? (shift + 2 * take + 63) >> 6 : 0u;   // 64-bit words the window touches (<= 4)
+    const uint64_t* p = packed + (b >> 5);
+    uint32_t X[8];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint64_t v = i < (int)n_w ? __ldg(p + i) : 0ull;
+        X[2 * i] = (uint32_t)(v >> 32);
+        X[2 * i + 1] = (uint32_t)v;
+    }
+    const bool odd = shift >= 32;
+    const uint32_t sh = shift & 31;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+        const uint32_t hi = odd ? X[i + 1] : X[i], lo = odd ? X[i + 2] : X[i + 1];
+        out.w[i] = __funnelshift_l(lo, hi, sh);
+    }
+}
+
+// PUBLISH = false: refine and emit.  PUBLISH = true (run only when groups larger than cap exist, before the global path):
+// nothing is gathered or emitted; the head bitmask the global path works on is written -- every position of a group of at
+// most cap suffixes counts as a group of one (placed), a larger group shows only its first position.
+template <typename KeyT, typename IdT, bool PACKED, int S, bool PUBLISH>
+__global__ void __launch_bounds__(kWarpThreads, 3) finish_warp_kernel(Reads R, const KeyT* __restrict__ keys1, const IdT* __restrict__ ids_in,
+                                                                   IdT* __restrict__ ids_out, uint32_t w1, uint32_t len_mask, uint64_t n,
+                                                                   uint32_t depth0, uint32_t cap, uint32_t* __restrict__ heads,
+                                                                   uint32_t* __restrict__ big_tiles, uint8_t* __restrict__ out,
+                                                                   unsigned long long* counters) {
+    constexpr uint32_t kSpan = 32 * S;                  // positions per window
+    constexpr uint32_t kPosBits = S == 1 ? 5 : 6;       // bits of a window position
+    static_assert(S == 1 || S == 2, "the rank key holds window positions of at most 6 bits");
+    const uint32_t lane = lane_id();
+    const uint64_t c0 = ((uint64_t)blockIdx.x * (kWarpThreads / 32) + (threadIdx.x >> 5)) * kWarpChunk;
+    const uint64_t c1 = c0 + kWarpChunk < n ? c0 + kWarpChunk : n;
+    const uint32_t cap_a = cap < kSpan ? cap : kSpan;   // largest group finished here
+    const uint64_t pos_mask = (1ull << R.pos_bits) - 1;
+    uint32_t n_members = 0, n_sorts = 0, n_over = 0;     // lane 0's tallies
+    uint64_t a = c0;
+    if (PUBLISH && c0 < n && c1 == n) publish_heads(heads, n, kFull);   // positions past the end count as heads (the bitmask's padding)
+    if (c0 < n && c0 > 0) a = scan_to_head<KeyT, PACKED>(keys1, c0, n, w1, len_mask);   // groups that began before the chunk are the previous warp's
+    while (a < c1) {
+        // ---- the window [a, a + 32 S): a is a head --------------------------------------------------------------
+        uint64_t word[S];
+        uint32_t hw[S + 1];                                  // bit i of hw[s]: position a + 32 s + i is a head
+        {
+            uint64_t k[S];
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                const uint64_t j = a + 32 * s + lane;
+                word[s] = j < n ? load_keyword<KeyT, PACKED>(keys1, j) : 0ull;
+                k[s] = key_of<PACKED>(word[s]);
+            }
+            uint32_t carry_in = 1;                           // head bit of the slot's first position
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                const uint64_t j = a + 32 * s + lane;
+                uint64_t kn = __shfl_down_sync(kFull, k[s], 1);   // key of the next position
+                const bool valid_next = j + 1 < n;
+                if (s + 1 < S) {
+                    const uint64_t first_of_next_slot = __shfl_sync(kFull, k[s + 1 < S ? s + 1 : s], 0);
+                    if (lane == 31) kn = first_of_next_slot;
+                } else if (lane == 31) {
+                    kn = valid_next ? key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j + 1)) : 0ull;
+                }
+                const bool head_next = !valid_next || kn != k[s] || ((uint32_t)kn & len_mask) < w1;
+                const uint32_t HN = __ballot_sync(kFull, head_next);
+                hw[s] = (HN << 1) | carry_in;
+                carry_in = HN >> 31;
+            }
+            hw[S] = carry_in;
+        }
+        // complete groups: everything before the last head, or the whole window if position a + 32 S is a head; groups that
+        // start at or after the end of the chunk are the next warp's
+        uint32_t n_comp = kSpan;
+        if (!hw[S]) {
+            n_comp = 0;
+#pragma unroll
+            for (int s = 0; s < S; ++s)
+                if (hw[s]) n_comp = 32 * s + 31 - (uint32_t)__clz(hw[s]);
+        }
+        if (a + n_comp > c1) {                               // c1 - a is 1 .. 32 S - 1 here
+            const uint32_t cut = (uint32_t)(c1 - a);
+            uint32_t first_later = n_comp;
+#pragma unroll
+            for (int s = S - 1; s >= 0; --s) {
+                const uint32_t from = cut > 32u * s ? cut - 32u * s : 0u;
+                const uint32_t later = from >= 32 ? 0u : hw[s] & ~((1u << from) - 1);
+                if (later) first_later = 32 * s + (uint32_t)__ffs(later) - 1;
+            }
+            n_comp = min(n_comp, first_later);
+        }
+        if (n_comp == 0) {
+            // one group fills the window and goes on: more than 32 S members
+            const uint64_t e = scan_to_head<KeyT, PACKED>(keys1, a + kSpan, n, w1, len_mask);
+            const uint64_t g = e - a;
+            if (g <= cap) {          // the block kernel's: flag the tile it starts in; its positions count as placed
+                if (!PUBLISH && lane == 0) atomicOr(big_tiles + (a / kLocalTile >> 5), 1u << (a / kLocalTile & 31));
+                if (PUBLISH)
+                    for (uint64_t q = a; q < e; q += 32) publish_heads(heads, q, e - q >= 32 ? kFull : (1u << (uint32_t)(e - q)) - 1);
+            } else if (PUBLISH) {    // the global path's: only its head bit
+                publish_heads(heads, a, 1u);
+            } else {                 // hand its ids over, count it
+                if constexpr (PACKED) {
+                    for (uint64_t q = a + lane; q < e; q += 32) ids_out[q] = (IdT)(uint32_t)load_keyword<KeyT, PACKED>(keys1, q);
+                }
+                n_over += 1;
+            }
+            a = e;
+            continue;
+        }
+        // a head closes the complete part
+#pragma unroll
+        for (int s = 0; s <= S; ++s) {
+            const int lim = (int)n_comp - 32 * s;       // positions of this slot before the closing head
+            const uint32_t keep = lim >= 32 ? kFull : lim <= 0 ? 0u : (1u << lim) - 1;
+            const uint32_t close = lim >= 0 && lim < 32 ? 1u << lim : 0u;
+            hw[s] = (hw[s] & keep) | close;
+        }
+        // ---- my groups inside the window; locators, the base before every suffix, the members' windows: one batch of gathers -----
+        uint32_t gs[S], ge[S], code[S], take[S], mrem[S];
+        uint64_t wbase[S];
+        Win6 win[S];
+        bool mine[S], member[S];
+        IdT idv[S];
+        uint32_t open = 0;
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            const uint32_t p = 32 * s + lane;
+            const uint64_t j = a + p;
+            const bool active = p < n_comp && j < n;
+            // first position of my group: the last head at or below p; one past its last: the next head above p
+            uint32_t lo_bits = hw[s] & (0xffffffffu >> (31 - lane));
+            gs[s] = 32 * s + 31 - (uint32_t)__clz(lo_bits);
+#pragma unroll
+            for (int t = s - 1; t >= 0; --t)
+                if (!lo_bits && hw[t]) lo_bits = 1, gs[s] = 32 * t + 31 - (uint32_t)__clz(hw[t]);
+            uint32_t hi_bits = lane == 31 ? 0u : hw[s] >> (lane + 1);
+            ge[s] = p + (uint32_t)__ffs(hi_bits);
+#pragma unroll
+            for (int t = s + 1; t <= S; ++t)
+                if (!hi_bits && hw[t]) hi_bits = 1, ge[s] = 32 * t + (uint32_t)__ffs(hw[t]) - 1;
+            if (!active) gs[s] = p, ge[s] = p + 1;
+            const uint32_t size = ge[s] - gs[s];
+            mine[s] = active && size <= cap_a;              // (a complete group larger than cap_a exists only when cap < 32 S)
+            member[s] = !PUBLISH && mine[s] && size >= 2;
+            idv[s] = 0;
+            if (active && !PUBLISH) {
+                if constexpr (PACKED) idv[s] = (IdT)(uint32_t)word[s];
+                else idv[s] = __ldg(ids_in + j);
+            }
+        }
+        uint64_t before[S], first_base[S];
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            uint64_t left;
+            const uint64_t read = (uint64_t)idv[s] >> R.pos_bits, pos = (uint64_t)idv[s] & pos_mask;
+            if (R.uniform) {
+                first_base[s] = read * R.uniform_len + pos;
+                left = R.uniform_len - pos;
+            } else {
+                const uint64_t* q = R.offsets + (mine[s] && !PUBLISH ? read : 0ull);
+                const uint64_t lo = __ldg(q), hi = __ldg(q + 1);
+                first_base[s] = lo + pos;
+                left = hi - lo - pos;
+            }
+            const bool has_prev = !PUBLISH && mine[s] && pos;
+            before[s] = has_prev ? __ldg(R.packed + ((first_base[s] - 1) >> 5)) : 0ull;   // no load for a read's first suffix
+            wbase[s] = first_base[s] + depth0;                // index of the window's first base
+            mrem[s] = member[s] ? (uint32_t)(left - depth0) : 0u;   // a member of an open group has >= depth0 bases
+            take[s] = mrem[s] < kWin ? mrem[s] : kWin;
+            code[s] = has_prev ? 2u : 1u;                     // 1 = $: the suffix starts its read
+        }
+#pragma unroll
+        for (int s = 0; s < S; ++s) window_words(R.packed, wbase[s], take[s], member[s], win[s]);
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            if (code[s] == 2u) code[s] = 2 + (uint32_t)((before[s] >> (62 - 2 * ((first_base[s] - 1) & 31))) & 3u);
+            const uint32_t mb = __ballot_sync(kFull, member[s]);
+            open |= mb;
+            if (lane == 0) n_members += (uint32_t)__popc(mb);
+        }
+        // ---- rounds over the groups of the window that are still open ---------------------------------------------------------
+        while (open) {
+            // pivot of every group: its member with the most bases in its window (segmented max scan, read at the group's last position)
+            uint32_t best[S];
+#pragma unroll
+            for (int s = 0; s < S; ++s) best[s] = member[s] ? (take[s] << kPosBits) | (32 * s + lane) : 0u;
+#pragma unroll
+            for (uint32_t o = 1; o < 32; o <<= 1) {
+#pragma unroll
+                for (int s = 0; s < S; ++s) {
+                    const uint32_t v = __shfl_up_sync(kFull, best[s], o);
+                    if (lane >= o && 32 * s + lane >= gs[s] + o && v > best[s]) best[s] = v;
+                }
+            }
+#pragma unroll
+            for (int s = 1; s < S; ++s) {                    // a group that began in the slot before
+                const uint32_t carry = __shfl_sync(kFull, best[s - 1], 31);
+                if (gs[s] < 32u * s && carry > best[s]) best[s] = carry;
+            }
+            uint32_t key[S];
+            uint32_t c1v[S], tbv[S];
+            Win6 piv[S];
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                const uint32_t tot = fetch_at<S>(best, ge[s] - 1);
+                const uint32_t pp = tot & (kSpan - 1);
+                tbv[s] = tot >> kPosBits;
+#pragma unroll
+                for (int i = 0; i < 6; ++i) {
+                    uint32_t col[S];
+#pragma unroll
+                    for (int t = 0; t < S; ++t) col[t] = win[t].w[i];
+                    piv[s].w[i] = fetch_at<S>(col, pp);
+                }
+            }
+            uint32_t c2v[S];
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                c1v[s] = 0, c2v[s] = 0;
+                if (member[s]) diverge2(win[s], piv[s], take[s], tbv[s], c1v[s], c2v[s]);
+            }
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                const uint32_t p = 32 * s + lane;
+                key[s] = member[s] ? (gs[s] << (32 - kPosBits)) | (c1v[s] << (kPosBits + 10)) | (c2v[s] << kPosBits) | (p - gs[s])
+                                   : p << (32 - kPosBits);   // a position outside every open group keeps its place
+            }
+            // bitonic sort of the window: groups stay in place (their first position leads the key), members are ranked inside
+#pragma unroll
+            for (uint32_t kk = 2; kk <= kSpan; kk <<= 1) {
+#pragma unroll
+                for (uint32_t jj = kk >> 1; jj > 0; jj >>= 1) {
+                    if (jj >= 32) {                         // partner in the other slot of the same lane
+#pragma unroll
+                        for (int s = 0; s < S; ++s) {
+                            const int t = s ^ (int)(jj >> 5);
+                            if (t > s) {
+                                const uint32_t lo = key[s] < key[t] ? key[s] : key[t], hi = key[s] < key[t] ? key[t] : key[s];
+                                const bool up = ((32u * s) & kk) == 0;
+                                key[s] = up ? lo : hi;
+                                key[t] = up ? hi : lo;
+                            }
+                        }
+                    } else {
+#pragma unroll
+                        for (int s = 0; s < S; ++s) {
+                            const uint32_t p = 32 * s + lane;
+                            const uint32_t other = __shfl_xor_sync(kFull, key[s], jj);
+                            const bool keep_min = ((p & kk) == 0) == ((p & jj) == 0);
+                            key[s] = keep_min ? (key[s] < other ? key[s] : other) : (key[s] > other ? key[s] : other);
+                        }
+                    }
+                }
+            }
+            if (lane == 0) n_sorts += 1;
+            // the member that ranked at each position; classes = runs of equal (level 1, level 2)
+            uint32_t src[S], cls[S];
+            bool head[S], was[S], nextwin[S];
+            uint32_t hb[S + 1];
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                src[s] = (key[s] >> (32 - kPosBits)) + (key[s] & (kSpan - 1));
+                cls[s] = (key[s] >> kPosBits) & 0xfffffu;
+            }
+#pragma unroll
+            for (int s = 0; s < S; ++s) was[s] = cls[s] != 0;   // a member's level-1 code is never 0
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                const uint32_t p = 32 * s + lane;
+                uint32_t prev = __shfl_up_sync(kFull, cls[s], 1);
+                if (s > 0) {
+                    const uint32_t last = __shfl_sync(kFull, cls[s > 0 ? s - 1 : 0], 31);
+                    if (lane == 0) prev = last;
+                }
+                const uint32_t t1 = code_type(cls[s] >> 10);
+                const uint32_t ty = t1 == 3 ? code_type(cls[s] & 0x3ffu) : t1;   // the class's last event decides
+                nextwin[s] = ty == 2;
+                head[s] = !was[s] || p == (key[s] >> (32 - kPosBits)) || ty == 1 || cls[s] != prev;
+                hb[s] = __ballot_sync(kFull, head[s]);
+            }
+            hb[S] = 1;
+            open = 0;
+            bool still[S];
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                const uint32_t hn = lane == 31 ? hb[s + 1] & 1u : (hb[s] >> (lane + 1)) & 1u;
+                still[s] = was[s] && !(head[s] && hn);      // not alone in my class yet
+                open |= __ballot_sync(kFull, still[s]);
+            }
+            // my data follows me
+            {
+                uint32_t t32[S];
+#pragma unroll
+                for (int s = 0; s < S; ++s) t32[s] = code[s];
+                uint32_t r[S];
+#pragma unroll
+                for (int s = 0; s < S; ++s) r[s] = fetch_at<S>(t32, src[s]);
+#pragma unroll
+                for (int s = 0; s < S; ++s) code[s] = r[s];
+            }
+            if (!open) break;
+            {
+                uint32_t col[S], r[S];
+#pragma unroll
+                for (int i = 0; i < 6; ++i) {
+#pragma unroll
+                    for (int s = 0; s < S; ++s) col[s] = win[s].w[i];
+#pragma unroll
+                    for (int s = 0; s < S; ++s) r[s] = fetch_at<S>(col, src[s]);
+#pragma unroll
+                    for (int s = 0; s < S; ++s) win[s].w[i] = r[s];
+                }
+#pragma unroll
+                for (int s = 0; s < S; ++s) col[s] = mrem[s];
+#pragma unroll
+                for (int s = 0; s < S; ++s) r[s] = fetch_at<S>(col, src[s]);
+#pragma unroll
+                for (int s = 0; s < S; ++s) mrem[s] = r[s], take[s] = r[s] < kWin ? r[s] : kWin;
+                uint64_t r64[S];
+#pragma unroll
+                for (int s = 0; s < S; ++s) r64[s] = fetch_at<S>(wbase, src[s]);
+#pragma unroll
+                for (int s = 0; s < S; ++s) wbase[s] = r64[s];
+            }
+            bool any_next = false;
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                const uint32_t p = 32 * s + lane;
+                member[s] = still[s];
+                uint32_t lo_bits = hb[s] & (0xffffffffu >> (31 - lane));
+                gs[s] = 32 * s + 31 - (uint32_t)__clz(lo_bits);
+#pragma unroll
+                for (int t = s - 1; t >= 0; --t)
+                    if (!lo_bits && hb[t]) lo_bits = 1, gs[s] = 32 * t + 31 - (uint32_t)__clz(hb[t]);
+                uint32_t hi_bits = lane == 31 ? 0u : hb[s] >> (lane + 1);
+                ge[s] = p + (uint32_t)__ffs(hi_bits);
+#pragma unroll
+                for (int t = s + 1; t <= S; ++t)
+                    if (!hi_bits && hb[t]) hi_bits = 1, ge[s] = 32 * t + (uint32_t)__ffs(hb[t]) - 1;
+                any_next |= __any_sync(kFull, member[s] && nextwin[s]);
+            }
+            if (any_next) {                                 // equal to the pivot through a full window: the next window of the read
+#pragma unroll
+                for (int s = 0; s < S; ++s) {
+                    const bool g = member[s] && nextwin[s];
+                    if (g) {
+                        wbase[s] += kWin;
+                        mrem[s] -= kWin;
+                        take[s] = mrem[s] < kWin ? mrem[s] : kWin;
+                    }
+                    Win6 nw;
+                    window_words(R.packed, wbase[s], take[s], g, nw);
+                    if (g) win[s] = nw;
+                }
+            }
+        }
+        // ---- emit; publish head bits (everything finished here counts as a group of one from now on) -----------------------
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            const uint32_t p = 32 * s + lane;
+            const uint64_t j = a + p;
+            if (!PUBLISH && mine[s]) out[j] = (uint8_t)(0x544743412400ull >> (8 * code[s]));
+            const bool active = p < n_comp && j < n;
+            const bool over = active && !mine[s];             // a complete group of more than cap members (cap < 32 S only)
+            const bool over_head = over && ((hw[s] >> lane) & 1u);
+            if (PUBLISH) {
+                const uint32_t bits = __ballot_sync(kFull, mine[s] || over_head);
+                publish_heads(heads, a + 32 * s, bits);
+            } else if (__any_sync(kFull, over)) {
+                if constexpr (PACKED) {
+                    if (over) ids_out[j] = idv[s];
+                }
+                const uint32_t over_heads = __ballot_sync(kFull, over_head);
+                if (lane == 0) n_over += (uint32_t)__popc(over_heads);
+            }
+        }
+        a += n_comp;
+    }
+    // ---- tallies: one update per block ------------------------------------------------------------------------------------------
+    __shared__ uint32_t s_tally[3];
+    if (threadIdx.x < 3) s_tally[threadIdx.x] = 0;
+    __syncthreads();
+    if (lane == 0) {
+        if (n_members) atomicAdd(&s_tally[0], n_members);
+        if (n_sorts) atomicAdd(&s_tally[1], n_sorts);
+        if (n_over) atomicAdd(&s_tally[2], n_over);
+    }
+    __syncthreads();
+    if (!PUBLISH && threadIdx.x == 0) {
+        if (s_tally[0]) atomicAdd(counters, (unsigned long long)s_tally[0]);                       // suffixes refined here
+        if (s_tally[1]) atomicAdd(counters + 2, (unsigned long long)s_tally[1] * (S == 1 ? 80 : 192));   // rank-key comparisons of the sorts
+        if (s_tally[1]) atomicAdd(counters + 3, (unsigned long long)s_tally[1]);                  // refinement rounds (warp windows)
+        if (s_tally[2]) atomicAdd(counters + 4, (unsigned long long)s_tally[2]);                  // groups left to the global path
     }
 }
 
@@ -681,31 +1302,67 @@ cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, cons
 
 template <typename KeyT, typename IdT>
 cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t depth0, uint32_t* heads_out, IdT* ids, uint64_t n,
-                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, bool packed, cudaStream_t s) {
+                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, uint32_t* big_tiles, int n_sms, bool packed,
+                                Launch* prof, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
     constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
     if (packed && !kCanPack) return cudaErrorInvalidValue;
-    auto kernel = packed ? finish_tile_kernel<KeyT, IdT, true, kCanPack> : finish_tile_kernel<KeyT, IdT, true, false>;
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem<IdT>));
-    if (e != cudaSuccess) return e;
     if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
-    uint64_t blocks = (n + kLocalTile - 1) / kLocalTile;
-    kernel<<<(unsigned)blocks, kLocalThreads, sizeof(LocalSmem<IdT>), s>>>(R, keys1, w1, (1u << key_len_bits(w1)) - 1, nullptr, heads_out, ids, n,
-                                                                          depth0, group_cap, out, elems_done);
+    const uint32_t len_mask = (1u << key_len_bits(w1)) - 1;
+    const uint64_t tiles = (n + kLocalTile - 1) / kLocalTile;
+    cudaError_t e = cudaMemsetAsync(big_tiles, 0, ((tiles + 31) / 32 + 1) * sizeof(uint32_t), s);
+    if (e != cudaSuccess) return e;
+    {   // singletons and groups of at most 32: one warp per chunk, registers only
+        ScopedLaunch sl(prof, CX_K_FINISH, n * (sizeof(KeyT) + sizeof(IdT) + 1) + n / 8, s);
+        const uint64_t warps = (n + kWarpChunk - 1) / kWarpChunk;
+        const unsigned grid = (unsigned)((warps + kWarpThreads / 32 - 1) / (kWarpThreads / 32));
+        if (packed)
+            finish_warp_kernel<KeyT, IdT, kCanPack, kWarpSlots, false><<<grid, kWarpThreads, 0, s>>>(R, keys1, ids, ids, w1, len_mask, n, depth0, group_cap, heads_out, big_tiles, out, elems_done);
+        else
+            finish_warp_kernel<KeyT, IdT, false, kWarpSlots, false><<<grid, kWarpThreads, 0, s>>>(R, keys1, ids, ids, w1, len_mask, n, depth0, group_cap, heads_out, big_tiles, out, elems_done);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    if (group_cap <= 32 * kWarpSlots) return cudaSuccess;
+    // larger groups, up to cap: persistent blocks over the flagged tiles
+    auto kernel = packed ? finish_tile_kernel<KeyT, IdT, true, kCanPack> : finish_tile_kernel<KeyT, IdT, true, false>;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem));
+    if (e != cudaSuccess) return e;
+    const uint64_t resident = (uint64_t)n_sms * kLocalBlocksPerSM;
+    ScopedLaunch sl(prof, CX_K_FINISH_BLOCK, 0, s);
+    kernel<<<(unsigned)(tiles < resident ? tiles : resident), kLocalThreads, sizeof(LocalSmem), s>>>(R, keys1, w1, len_mask, nullptr, nullptr, ids, n, depth0, 32u * kWarpSlots + 1,
+                                                                                                   group_cap, big_tiles, out, elems_done);
+    return cudaGetLastError();
+}
+
+template <typename KeyT, typename IdT>
+cudaError_t launch_publish_heads(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t* heads_out, uint64_t n, uint32_t group_cap, bool packed,
+                                 cudaStream_t s) {
+    if (n == 0) return cudaSuccess;
+    constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
+    if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
+    const uint32_t len_mask = (1u << key_len_bits(w1)) - 1;
+    const uint64_t warps = (n + kWarpChunk - 1) / kWarpChunk;
+    const unsigned grid = (unsigned)((warps + kWarpThreads / 32 - 1) / (kWarpThreads / 32));
+    if (packed)
+        finish_warp_kernel<KeyT, IdT, kCanPack, kWarpSlots, true><<<grid, kWarpThreads, 0, s>>>(R, keys1, nullptr, nullptr, w1, len_mask, n, 0, group_cap, heads_out, nullptr, nullptr, nullptr);
+    else
+        finish_warp_kernel<KeyT, IdT, false, kWarpSlots, true><<<grid, kWarpThreads, 0, s>>>(R, keys1, nullptr, nullptr, w1, len_mask, n, 0, group_cap, heads_out, nullptr, nullptr, nullptr);
     return cudaGetLastError();
 }
 
 template <typename IdT>
 cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32_t* heads_out, const IdT* ids, uint64_t n, uint32_t depth,
-                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, cudaStream_t s) {
+                                uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, int n_sms, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
     auto kernel = finish_tile_kernel<uint64_t, IdT, false, false>;
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem<IdT>));
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem));
     if (e != cudaSuccess) return e;
     if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
-    uint64_t blocks = (n + kLocalTile - 1) / kLocalTile;
-    kernel<<<(unsigned)blocks, kLocalThreads, sizeof(LocalSmem<IdT>), s>>>(R, nullptr, 0, 0, heads_in, heads_out, const_cast<IdT*>(ids), n, depth, group_cap, out,
-                                                                          elems_done);
+    const uint64_t tiles = (n + kLocalTile - 1) / kLocalTile;
+    const uint64_t resident = (uint64_t)n_sms * kLocalBlocksPerSM;
+    kernel<<<(unsigned)(tiles < resident ? tiles : resident), kLocalThreads, sizeof(LocalSmem), s>>>(R, nullptr, 0, 0, heads_in, heads_out, ids, n, depth, 2u, group_cap,
+                                                                                                   nullptr, out, elems_done);
     return cudaGetLastError();
 }
 
@@ -715,11 +1372,13 @@ cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32
     template cudaError_t launch_refine_writeback<IdT>(const Reads&, const uint64_t*, const IdT*, const uint32_t*, uint64_t,         \
                                                       uint32_t, IdT*, uint32_t*, uint8_t*, cudaStream_t);                            \
     template cudaError_t launch_finish_first<uint32_t, IdT>(const Reads&, const uint32_t*, uint32_t, uint32_t, uint32_t*, IdT*, uint64_t, \
-                                                            uint32_t, uint8_t*, unsigned long long*, bool, cudaStream_t);            \
+                                                            uint32_t, uint8_t*, unsigned long long*, uint32_t*, int, bool, Launch*, cudaStream_t); \
     template cudaError_t launch_finish_first<uint64_t, IdT>(const Reads&, const uint64_t*, uint32_t, uint32_t, uint32_t*, IdT*, uint64_t, \
-                                                            uint32_t, uint8_t*, unsigned long long*, bool, cudaStream_t);            \
+                                                            uint32_t, uint8_t*, unsigned long long*, uint32_t*, int, bool, Launch*, cudaStream_t); \
+    template cudaError_t launch_publish_heads<uint32_t, IdT>(const Reads&, const uint32_t*, uint32_t, uint32_t*, uint64_t, uint32_t, bool, cudaStream_t); \
+    template cudaError_t launch_publish_heads<uint64_t, IdT>(const Reads&, const uint64_t*, uint32_t, uint32_t*, uint64_t, uint32_t, bool, cudaStream_t); \
     template cudaError_t launch_finish_later<IdT>(const Reads&, const uint32_t*, uint32_t*, const IdT*, uint64_t, uint32_t,         \
-                                                  uint32_t, uint8_t*, unsigned long long*, cudaStream_t);
+                                                  uint32_t, uint8_t*, unsigned long long*, int, cudaStream_t);
 CX_INSTANTIATE(uint32_t)
 CX_INSTANTIATE(uint64_t)
 

@@ -132,3 +132,26 @@ class ReadRecipe:
             codes = substitute(codes, H(self.seed, 4, idx[rid] * 256 + k), self.err_num, self.err_den)
         lut = torch.tensor(list(b"ACGT"), dtype=torch.uint8, device=dev)
         return lut[codes.to(torch.int64)]
+
+
+def read_chunks(recipe: ReadRecipe, chunk_reads: int):
+    """The recipe's reads in chunks of at most `chunk_reads`: yields (a, b, lens int64[b - a], ascii uint8) on the recipe's
+    device.  The whole ASCII form never exists at once (configs[4] is 100 GB of it)."""
+    n = recipe.n_reads
+    for a in range(0, n, chunk_reads):
+        b = min(n, a + chunk_reads)
+        lens = recipe.lengths(a, b)
+        yield a, b, lens, recipe.reads_ascii(a, b, lens)
+
+
+def offsets_of(recipe: ReadRecipe, step: int = 1 << 26) -> torch.Tensor:
+    """read_offsets (int64[n_reads + 1]) of the recipe on its device."""
+    n = recipe.n_reads
+    off = torch.zeros(n + 1, dtype=torch.int64, device=recipe.device)
+    run = 0
+    for a in range(0, n, step):
+        b = min(n, a + step)
+        torch.cumsum(recipe.lengths(a, b), 0, out=off[a + 1:b + 1])
+        off[a + 1:b + 1] += run
+        run = int(off[b])
+    return off
