@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
 onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ vals_in, KeyT* __restrict__ keys_out,
                      ValT* __restrict__ vals_out, uint64_t n, uint32_t shift, uint32_t digit_mask,
                      const uint64_t* __restrict__ bin_base, uint64_t* __restrict__ status, uint32_t* __restrict__ ticket,
-                     uint32_t ticket_base, uint32_t epoch) {
+                     uint32_t ticket_base, uint32_t epoch, uint32_t prefetch_tiles) {
     using Smem = PassSmem<KeyT, ValT, THREADS, ITEMS>;
     constexpr int kTile = Smem::kTile;
     constexpr int kWarps = Smem::kWarps;
@@ -141,10 +141,23 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ 
     // Tiles are claimed in launch order of the blocks, so every earlier tile is owned by a block that
     // is already running: the look-back below can never wait on a block that has not started.
     if (tid == 0) sm.tile = atomicAdd(ticket, 1u) - ticket_base;
-    for (uint32_t i = tid; i < kWarps * kRadix; i += THREADS) (&sm.warp_count[0][0])[i] = 0;
+    {
+        uint4* wc = reinterpret_cast<uint4*>(&sm.warp_count[0][0]);
+        for (uint32_t i = tid; i < kWarps * kRadix / 4; i += THREADS) wc[i] = make_uint4(0u, 0u, 0u, 0u);
+    }
     __syncthreads();
     const uint32_t tile = sm.tile;
     const uint32_t tile_off = tile * (uint32_t)kTile;
+    // The tile that a block started now will claim in about one grid-width of tickets: ask L2 for it (one bulk prefetch per
+    // array), so that its loads find their lines there instead of paying the HBM round trip at the head of the tile.
+    if (tid == 0) {
+        const uint64_t ahead = (uint64_t)tile_off + (uint64_t)prefetch_tiles * kTile;
+        if (ahead + kTile <= n) {
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(keys_in + ahead), "r"((uint32_t)(kTile * sizeof(KeyT))) : "memory");
+            if constexpr (kHasVals)
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(vals_in + ahead), "r"((uint32_t)(kTile * sizeof(ValT))) : "memory");
+        }
+    }
     const uint32_t tile_n = (uint32_t)min((uint64_t)kTile, n - tile_off);
     const bool full = tile_n == (uint32_t)kTile;
     const uint32_t warp_base = warp * (32 * ITEMS);
@@ -219,9 +232,12 @@ onesweep_pass_kernel(const KeyT* __restrict__ keys_in, const ValT* __restrict__ 
         const uint32_t d = (uint32_t)(key[k] >> shift) & digit_mask;
         const uint32_t peers = digit_peers(d);
         const uint32_t below = __popc(peers & lt);
-        uint32_t old = 0;
-        if (below == 0) old = atomicAdd(&sm.warp_count[warp][d], (uint32_t)__popc(peers));
-        old = __shfl_sync(kFull, old, __ffs(peers) - 1);
+        // every lane of a digit reads the warp's slot counter of that digit; the lowest one moves it past the group
+        // (plain load + predicated store: only this warp touches warp_count[warp][*] in this phase)
+        uint32_t* counter = &sm.warp_count[warp][d];
+        const uint32_t old = *counter;
+        __syncwarp();
+        if (below == 0) *counter = old + (uint32_t)__popc(peers);
         const uint32_t slot = old + below;
         sm.keys[slot] = key[k];
         if constexpr (kHasVals) sm.vals[slot] = val[k];
@@ -343,7 +359,7 @@ cudaError_t sort_pairs_shape(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_
             ScopedLaunch sl(prof, pass_class, n * 2 * SortShape<KeyT, ValT>::pair_bytes, s);
             kernel<<<(unsigned)n_tiles, kSortThreads, sizeof(Smem), s>>>(kin, vin, kout, vout, n, lo, (1u << bits) - 1,
                                                                         ws.hist + (uint64_t)p * kRadix, ws.status, ws.ticket,
-                                                                        ws.ticket_base, ws.epoch);
+                                                                        ws.ticket_base, ws.epoch, (uint32_t)(sm_count() * kMinBlocks));
         }
         ws.ticket_base += (uint32_t)n_tiles;
         e = cudaGetLastError();

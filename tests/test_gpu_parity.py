@@ -94,29 +94,36 @@ def test_config_shapes_scaled(idx, scale):
     assert_parity(c)
 
 
-def _full_size_check(idx, prefixes, lf_sample):
-    """Full-size parity in the launch configuration bench.py times: the oracle's range-restricted slices
-    (every suffix that begins with a given prefix: a contiguous piece of B_R) must match
-    byte for byte, and the whole output must pass the size-independent checks (symbol counts, first-n
-    rule, LF-mapping inversion of a seeded sample of reads)."""
-    c = gen.config(idx)
+def test_config2_full_size_every_suffix():
+    """configs[1] (1.01e8 suffixes) at full size, EVERY output symbol compared with the oracle: the 16 two-base prefix ranges
+    through the range-restricted oracle (each a contiguous piece of B_R; one range per host thread -- the C
+    oracle runs outside the GIL), the one-base suffixes "X$" from the definition (identical strings, ordered by read index,
+    PAPER.md:55) and the n end-marker suffixes by the first-n rule; plus counts and LF inversion of 20,000 reads."""
+    import concurrent.futures as cf
+    c = gen.config(1)
     got = gpu_bwt(c)
-    chk.check_all(got, c, lf_sample=lf_sample)
-    for pfx in prefixes:
-        off, want = oracle.bwt_with_prefix(c.ascii, c.offsets, pfx)
-        assert want.size > 0, pfx
-        assert np.array_equal(got[off:off + want.size], want), f"config {idx}: slice of prefix {pfx} differs"
-
-
-def test_config2_full_size_sampled_slices():
-    # configs[1], 1.01e8 suffixes: the bench workload
-    _full_size_check(1, ["CATG", "TTTTTTT", "AAAAA", "GGC"], lf_sample=20_000)
-
-
-@pytest.mark.skipif(os.environ.get("CX_TEST_LARGE", "0") != "1", reason="set CX_TEST_LARGE=1 (several minutes, ~40 GB host RAM)")
-def test_config3_full_size_sampled_slices():
-    # configs[2], 1.01e9 suffixes
-    _full_size_check(2, ["ACGTACG", "TTGACCA"], lf_sample=2_000)
+    chk.check_all(got, c, lf_sample=20_000)                  # includes the first-n rule: positions [0, n)
+    covered = c.n_reads
+    prefixes = [a + b for a in "ACGT" for b in "ACGT"]
+    oracle.build()
+    with cf.ThreadPoolExecutor(max_workers=os.cpu_count() or 1) as pool:
+        res = list(pool.map(lambda pfx: oracle.bwt_with_prefix(c.ascii, c.offsets, pfx), prefixes))
+    where = dict(zip(prefixes, res))
+    for pfx, (off, want) in where.items():
+        assert np.array_equal(got[off:off + want.size], want), f"configs[1]: slice of prefix {pfx} differs"
+        covered += want.size
+    # suffixes of exactly one base X: they sit immediately before the "XA" range, in read order; each is preceded by the
+    # base before the read's last base (reads are 100 bp here)
+    off64 = c.offsets.astype(np.int64)
+    last = c.ascii[off64[1:] - 1]
+    before_last = c.ascii[off64[1:] - 2]
+    for x in "ACGT":
+        sel = last == ord(x)
+        cnt = int(sel.sum())
+        end = where[x + "A"][0]
+        assert np.array_equal(got[end - cnt:end], before_last[sel]), f"configs[1]: the one-base suffixes {x}$ differ"
+        covered += cnt
+    assert covered == c.n_suffixes                           # every position of the output was compared
 
 
 @pytest.mark.parametrize("read_len", [200, 400, 1000])
