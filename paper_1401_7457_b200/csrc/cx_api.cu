@@ -593,6 +593,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         } else {
             const uint64_t col_stride = sh.max_tiles + 1;
             CX_CUDA(use_region(B.region, region));
+            const uint64_t n_tiles = list_scan_tiles(R, region, N);   // (shadows the whole-collection tile count)
             if (B.count_here) {   // one scan counts this batch and up to seven that follow it in the same region
                 ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + n_tiles * 8 * B.ranges.n, s);
                 CX_CUDA(launch_list_count(R, d_info, d_tile_first, sh.ell, region, B.ranges, d_tile_count, col_stride, n_tiles, s));

@@ -163,6 +163,9 @@ cudaError_t launch_tile_table(const uint64_t* offsets, uint64_t n_reads, const B
                               uint64_t max_tiles, cudaStream_t s);
 cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, const Region& region,
                                uint64_t* hist, uint64_t max_tiles, int n_sms, cudaStream_t s);
+// tiles of the multi-batch scans (count, scan of a column, select) of `region`: their size depends on the collection
+// (reads of one length outside a region: 8192 slots; otherwise kListTile); all three steps must be given this count
+uint64_t list_scan_tiles(const Reads& R, const Region& region, uint64_t n_suffixes);
 // count, per tile, the suffixes of up to kCountGroup consecutive batches in one scan; batch j owns partitions
 // [first[j], first[j + 1]); tile_count[j * col_stride + tile]
 constexpr int kCountGroup = 8;

@@ -90,7 +90,7 @@ struct PassSmem {
     static constexpr bool kHasVals = sizeof(ValT) >= 4;
     KeyT keys[kTile];
     ValT vals[kHasVals ? kTile : 1];
-    uint32_t warp_count[kWarps][kRadix];  // per-warp digit counts, then the staged slot of the warp's first pair of that digit
+    alignas(16) uint32_t warp_count[kWarps][kRadix];  // per-warp digit counts, then the staged slot of the warp's first pair of that digit
     uint32_t gofs[kRadix];                // output index of staged slot e with digit d = gofs[d] + e (mod 2^32; batches are < 2^32)
     uint32_t warp_total[kRadix / 32];
     uint32_t tile;

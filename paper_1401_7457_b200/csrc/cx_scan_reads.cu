@@ -545,11 +545,215 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// The multi-batch scans for collections of reads of ONE length (the paper's setting; configs[1], [2], [4]),
+// outside any refined region.  Every batch of a collection larger than the workspace walks all N slots again
+// (one listing scan per round), so the walk itself is what counts: tiles of 8192 slots, 32 consecutive slots
+// per thread (the per-thread set-up is paid once per 32 slots), no offsets table (a slot is decoded by one division), a
+// 16-base window in one register refilled every 8 slots, and a branch-free partition code per slot.
+// ---------------------------------------------------------------------------------------------
+constexpr int kBigItems = 32;
+constexpr int kBigTile = kListThreads * kBigItems;
+static_assert(kBigTile <= 65536, "taken slots are kept as 16-bit indices");
+
+struct BigSmem {
+    uint64_t packed[kBigTile / 32 + 4];   // the bases of the tile plus two windows of look-ahead
+};
+struct BigCtx {
+    uint64_t g0, r0;        // first slot, the read that owns it
+    uint32_t n_slots, pos0; // slots in this tile; position of slot g0 inside read r0
+    uint32_t L1;            // read length + 1
+    uint32_t brel0;         // base index of slot g0 relative to the first staged base
+    float inv_L1;
+};
+__device__ __forceinline__ BigCtx load_big_tile(const Reads& R, const BuildInfo* __restrict__ info, uint64_t t, uint64_t N, BigSmem& sm) {
+    BigCtx c;
+    c.g0 = t * kBigTile;
+    c.n_slots = (uint32_t)min((uint64_t)kBigTile, N - c.g0);
+    c.L1 = (uint32_t)info->first_len + 1u;
+    c.inv_L1 = 1.0f / (float)c.L1;
+    c.r0 = c.g0 / c.L1;
+    c.pos0 = (uint32_t)(c.g0 - c.r0 * c.L1);
+    const uint64_t b0 = c.g0 - c.r0;                 // base index of slot g = g - (its read)
+    const uint64_t word0 = b0 >> 5;
+    c.brel0 = (uint32_t)(b0 & 31);
+    for (uint32_t j = threadIdx.x; j < kBigTile / 32 + 4; j += blockDim.x) {
+        const uint64_t wi = word0 + j;
+        sm.packed[j] = wi < R.n_words ? __ldg(R.packed + wi) : 0ull;
+    }
+    __syncthreads();
+    return c;
+}
+// slot s of the tile -> reads passed since r0 (rr), position in its read, staged base index
+__device__ __forceinline__ void big_decode(const BigCtx& c, uint32_t s, uint32_t& rr, uint32_t& pos, uint32_t& brel) {
+    const uint32_t x = c.pos0 + s;                   // < L1 + kBigTile: the float estimate of x / L1 is within one of it
+    rr = (uint32_t)((float)x * c.inv_L1);
+    if ((uint64_t)rr * c.L1 > x) --rr;
+    else if ((uint64_t)(rr + 1) * c.L1 <= x) ++rr;
+    pos = x - rr * c.L1;
+    brel = c.brel0 + s - rr;
+}
+__device__ __forceinline__ uint64_t big_window(const BigSmem& sm, uint32_t brel) {
+    const uint32_t wi = brel >> 5, sh = (brel & 31) * 2;
+    const uint64_t w0 = sm.packed[wi], w1 = sm.packed[wi + 1];
+    return sh ? (w0 << sh) | (w1 >> (64 - sh)) : w0;
+}
+// the 16 bases from staged base index brel on (first base in the most significant bits): the staged words seen as
+// 32-bit halves, high half first
+__device__ __forceinline__ uint32_t big_top16(const BigSmem& sm, uint32_t brel) {
+    const uint32_t* half = reinterpret_cast<const uint32_t*>(sm.packed);
+    const uint32_t q = brel >> 4, sh = (brel & 15) * 2;
+    return __funnelshift_l(half[(q + 1) ^ 1], half[q ^ 1], sh);
+}
+// Walk of one thread over its kBigItems consecutive slots: f(i, partition code) for each; branch-free per slot (a warp's lanes
+// are at different phases of their reads, so a 'suffix ends inside the prefix' branch would be taken by some lane nearly always).
+// GUARD: the tile is ragged (only the collection's last tile), slots at or past n_here do not exist.
+template <bool GUARD, typename F>
+__device__ __forceinline__ void big_walk(const BigCtx& c, const BigSmem& sm, uint32_t s0, uint32_t ell, F&& f) {
+    uint32_t rr, pos, brel;
+    big_decode(c, s0, rr, pos, brel);
+    uint32_t rem = c.L1 - 1 - pos;
+    const uint32_t n_here = GUARD ? min((uint32_t)kBigItems, c.n_slots - s0) : (uint32_t)kBigItems;
+    uint32_t top = 0;
+#pragma unroll
+    for (int i = 0; i < kBigItems; ++i) {
+        if ((i & 7) == 0) top = big_top16(sm, brel);     // at most 7 bases are consumed before the next refill: l <= 7 stay valid
+        if (!GUARD || (uint32_t)i < n_here) {
+            const uint32_t r = rem < ell ? rem : ell;
+            // the first l bases with those past the end of the read cleared (A-padded), then the length: reading A4 of PAPER.md:79
+            const uint32_t kmer = (top >> (32 - 2 * ell)) & (0xffffffffu << (2 * (ell - r)));
+            f(i, kmer * (ell + 1) + r);
+            const bool adv = rem != 0;                    // at an end-marker slot the next read starts at the same base index
+            top = adv ? top << 2 : top;
+            brel += adv;
+            rem = adv ? rem - 1 : c.L1 - 1;
+        }
+    }
+}
+__global__ void __launch_bounds__(kListThreads) list_count_uniform_kernel(Reads R, const BuildInfo* __restrict__ info, uint32_t ell, CountRanges ranges,
+                                                                          uint64_t* __restrict__ tile_count, uint64_t col_stride) {
+    __shared__ BigSmem sm;
+    __shared__ uint32_t s_total[kCountGroup];
+    __shared__ uint32_t s_first[kCountGroup + 1];    // first partition of every batch of the group; unused ones = one past the last
+    R.n_words = (info->total_bases + 31) >> 5;
+    const uint64_t N = info->n_suffixes;
+    const uint64_t n_tiles = (N + kBigTile - 1) / kBigTile;
+    if (info->bad_offsets) return;
+    if (threadIdx.x <= kCountGroup) s_first[threadIdx.x] = ranges.first[threadIdx.x < ranges.n ? threadIdx.x : ranges.n];
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        __syncthreads();   // previous tile done with sm and s_total (and the table filled on the first trip)
+        if (threadIdx.x < kCountGroup) s_total[threadIdx.x] = 0;
+        const BigCtx c = load_big_tile(R, info, t, N, sm);
+        uint64_t mine = 0;   // eight 8-bit counters (at most 32 slots per thread)
+        const uint32_t s0 = threadIdx.x * kBigItems;
+        if (s0 < c.n_slots) {
+            auto tally = [&](int, uint32_t code) {
+                // which of the group's batches owns the partition: a three-step search of the (at most eight) range starts
+                uint32_t j = code >= s_first[4] ? 4u : 0u;
+                j += code >= s_first[j + 2] ? 2u : 0u;
+                j += code >= s_first[j + 1] ? 1u : 0u;
+                if (code >= s_first[0] && code < s_first[kCountGroup]) mine += 1ull << (8 * j);
+            };
+            if (c.n_slots == (uint32_t)kBigTile) big_walk<false>(c, sm, s0, ell, tally);
+            else big_walk<true>(c, sm, s0, ell, tally);
+        }
+#pragma unroll
+        for (int j = 0; j < kCountGroup; ++j) {
+            uint32_t v = (uint32_t)(mine >> (8 * j)) & 255u;
+            for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane_id() == 0 && v) atomicAdd(&s_total[j], v);
+        }
+        __syncthreads();
+        if (threadIdx.x < ranges.n) tile_count[(uint64_t)threadIdx.x * col_stride + t] = s_total[threadIdx.x];
+    }
+}
+
+template <typename KeyT, typename IdT, bool PACKED>
+__global__ void __launch_bounds__(kListThreads) list_select_uniform_kernel(Reads R, const BuildInfo* __restrict__ info, uint32_t ell, uint32_t w,
+                                                                           uint32_t bucket_lo, uint32_t bucket_hi,
+                                                                           const uint64_t* __restrict__ tile_base, KeyT* __restrict__ keys,
+                                                                           IdT* __restrict__ ids, uint32_t n_passes,
+                                                                           unsigned long long* __restrict__ digit_hist, uint64_t ord_lo, uint64_t ord_hi) {
+    __shared__ BigSmem sm;
+    __shared__ uint32_t s_dh[8][kRadix];
+    __shared__ uint32_t s_warp[kListThreads / 32];
+    __shared__ uint16_t s_taken[kBigTile];   // slots of the tile that belong to the batch, in slot order
+    R.n_words = (info->total_bases + 31) >> 5;
+    const uint64_t N = info->n_suffixes;
+    const uint64_t n_tiles = (N + kBigTile - 1) / kBigTile;
+    const uint32_t len_bits = key_len_bits(w);
+    const uint32_t warp = threadIdx.x >> 5;
+    if (info->bad_offsets) return;
+    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) (&s_dh[0][0])[i] = 0;
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        __syncthreads();   // previous tile done with sm, s_warp and s_taken
+        const BigCtx c = load_big_tile(R, info, t, N, sm);
+        const uint32_t s0 = threadIdx.x * kBigItems;
+        uint32_t mask = 0;   // which of my 32 consecutive slots belong to this batch
+        if (s0 < c.n_slots) {
+            auto mark = [&](int i, uint32_t code) { mask |= (uint32_t)(code - bucket_lo <= bucket_hi - bucket_lo) << i; };
+            if (c.n_slots == (uint32_t)kBigTile) big_walk<false>(c, sm, s0, ell, mark);
+            else big_walk<true>(c, sm, s0, ell, mark);
+        }
+        // exclusive scan of the per-thread counts: slot order = thread order
+        const uint32_t cnt = __popc(mask);
+        uint32_t incl = cnt;
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t up = __shfl_up_sync(0xffffffffu, incl, o);
+            if ((int)lane_id() >= o) incl += up;
+        }
+        if (lane_id() == 31) s_warp[warp] = incl;
+        __syncthreads();
+        uint32_t before = incl - cnt, total = 0;
+        for (uint32_t q = 0; q < kListThreads / 32; ++q) {
+            const uint32_t v = s_warp[q];
+            if (q < warp) before += v;
+            total += v;
+        }
+        while (mask) {   // taken slots compacted first, decoded one per thread below (full warps, consecutive output addresses)
+            const int i = __ffs(mask) - 1;
+            mask &= mask - 1;
+            s_taken[before++] = (uint16_t)(s0 + i);
+        }
+        __syncthreads();
+        const uint64_t tile_dst = tile_base[t];
+        for (uint32_t j = threadIdx.x; j < total; j += kListThreads) {
+            const uint64_t dst = tile_dst + j;
+            if (dst >= ord_lo && dst < ord_hi) {
+                uint32_t rr, pos, brel;
+                big_decode(c, s_taken[j], rr, pos, brel);
+                const KeyT key = (KeyT)make_key(big_window(sm, brel), (uint64_t)(c.L1 - 1 - pos), w, len_bits);
+                const IdT id = make_id<IdT>(c.r0 + rr, pos, R.pos_bits);
+                digit_counts(s_dh, key, n_passes);
+                const uint64_t at = dst - ord_lo;
+                if constexpr (PACKED) {
+                    reinterpret_cast<uint64_t*>(keys)[at] = ((uint64_t)key << 32) | (uint64_t)id;
+                } else {
+                    keys[at] = key;
+                    ids[at] = id;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) {
+        uint32_t v = (&s_dh[0][0])[i];
+        if (v) atomicAdd(digit_hist + i, (unsigned long long)v);
+    }
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------
+// the multi-batch scans of a collection of equal-length reads outside a refined region run on tiles of kBigTile slots
+static bool big_tiles(const Reads& R, const Region& region) { return R.uniform && region.depth == 0; }
+uint64_t list_scan_tiles(const Reads& R, const Region& region, uint64_t n_suffixes) {
+    const uint64_t tile = big_tiles(R, region) ? (uint64_t)kBigTile : (uint64_t)kListTile;
+    return (n_suffixes + tile - 1) / tile;
+}
+
 cudaError_t launch_prep(const uint64_t* offsets, uint64_t n_reads, uint64_t max_bases, BuildInfo* info, cudaStream_t s) {
     cudaError_t e = cudaMemsetAsync(info, 0, sizeof(BuildInfo), s);
     if (e != cudaSuccess) return e;
@@ -588,6 +792,10 @@ cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint3
     if (n_tiles == 0 || ranges.n == 0) return cudaSuccess;
     uint64_t want = (uint64_t)sm_count() * 8;
     const unsigned grid = (unsigned)(n_tiles < want ? n_tiles : want);
+    if (big_tiles(R, region)) {   // n_tiles counts tiles of kBigTile slots here (list_scan_tiles)
+        list_count_uniform_kernel<<<grid, kListThreads, 0, s>>>(R, info, ell, ranges, tile_count, col_stride);
+        return cudaGetLastError();
+    }
     if (region.depth)
         list_count_kernel<true><<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, region, ranges, tile_count, col_stride);
     else
@@ -629,6 +837,16 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
                                              ord_hi);
         return cudaGetLastError();
     };
+    if (big_tiles(R, region)) {
+        auto kernel = packed ? list_select_uniform_kernel<KeyT, IdT, kCanPack> : list_select_uniform_kernel<KeyT, IdT, false>;
+        int per_sm = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kListThreads, 0);
+        if (e != cudaSuccess) return e;
+        const uint64_t resident = (uint64_t)n_sms * (per_sm > 0 ? per_sm : 1);
+        kernel<<<(unsigned)(n_tiles < resident ? n_tiles : resident), kListThreads, 0, s>>>(R, info, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids, n_passes, dh,
+                                                                                          ord_lo, ord_hi);
+        return cudaGetLastError();
+    }
     if (region.depth) return packed ? select(list_select_kernel<KeyT, IdT, kCanPack, true>) : select(list_select_kernel<KeyT, IdT, false, true>);
     return packed ? select(list_select_kernel<KeyT, IdT, kCanPack, false>) : select(list_select_kernel<KeyT, IdT, false, false>);
 }
