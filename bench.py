@@ -52,7 +52,9 @@ REF_SAMPLE_SCALE = {0: 1.0, 1: 0.25, 2: 0.04, 3: 0.004, 4: 0.0004}  # --impl ref
 KERNEL_NAMES = {"pack": "pack_kernel (a1)", "prep": "prep_kernel + tile_table_kernel", "hist": "bucket_hist_kernel (a2)",
                 "list": "list_write_kernel / list_count + list_select (a4+a5)", "sort_hist": "digit_hist_kernel (a6)",
                 "sort_scan": "bin_scan_kernel (a6)", "sort_pass": "onesweep_pass_kernel (a6, one radix pass of the first sort)",
-                "finish": "finish_tile_kernel (a7+a8)", "refine_scan": "active_count + scan (a7, global path)",
+                "finish": "finish_warp_kernel (a7+a8: head flags, tie groups of <= 64 refined in registers, emit)",
+                "finish_block": "finish_tile_kernel (a7+a8: tie groups of 65..256 refined in shared memory)",
+                "refine_scan": "publish heads + active_count + scan (a7, global path)",
                 "refine_key": "refine_rekey_kernel (a7, global path)", "refine_write": "refine_writeback_kernel (a7+a8, global path)",
                 "refine_sort": "onesweep_pass_kernel (a7, global path re-sort)", "fasta": "fasta_* kernels (NEXT-4 ingest)"}
 
@@ -520,17 +522,43 @@ def run_cx(args) -> None:
 
     # ---- end to end: pinned host in, pinned host out ----------------------------------------------------
     e2e_steps = max(3, min(args.steps, 10))
-    for _ in range(2):
-        step_e2e(plan)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        step_e2e(plan)
-    torch.cuda.synchronize()
-    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
-    barrier()
+
+    def time_e2e(step):
+        for _ in range(2):
+            step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            step()
+        torch.cuda.synchronize()
+        ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+        barrier()
+        return ms
+
+    e2e_variants = {"sequential": time_e2e(lambda: step_e2e(plan))}     # H2D, build into device memory, D2H: one after the other
     plan.free()
     del plan
+    if not sharded and not one_shard and not args.fasta and args.out_bits == 8 and N >= 4_000_000:
+        # the library's own pinned-host output path (a9): four batches, each batch's D2H copy on a side stream while the next
+        # batch computes; and the same with the packed output (NEXT-4: half the bytes back over PCIe)
+        for name, extra, nbytes in (("streamed", {}, N), ("streamed_packed", {"out_bits": 4}, (N + 1) // 2)):
+            so = dict(plan_opts, out_is_host_pinned=1, max_batch_suffixes=N // 4 + N // 64, **extra)
+            sp = cx.Plan(n_reads, total, profile=0, **so)
+            h_res = h_out[:nbytes]
+
+            def step_streamed(sp=sp, h_res=h_res):
+                cx.pack_reads_from_host(h_ascii, d_ascii, d_packed, stream=stream)
+                d_off.copy_(h_off, non_blocking=True)
+                sp.build(d_packed, d_off, n_reads, h_res)       # returns when the last batch has been copied to the host
+            e2e_variants[name] = time_e2e(step_streamed)
+            if name == "streamed":                               # the streamed result must be the same bytes
+                got = torch.bincount(h_res.to(dev).to(torch.int64), minlength=256)
+                if not torch.equal(got, want_counts):
+                    raise SystemExit("bench.py: streamed output symbol counts differ from the input's")
+            sp.free()
+            del sp
+    e2e_name = min((k for k in e2e_variants if k != "streamed_packed"), key=lambda k: e2e_variants[k])
+    e2e_ms = e2e_variants[e2e_name]
 
     # ---- per-class table: a separate pass with CUDA events around every launch (cx_bwt_kernel_time) --------------
     prof_steps = 3
@@ -608,8 +636,12 @@ def run_cx(args) -> None:
                    "refine_rounds": stats["refine_rounds"], "refine_elements": stats["refine_elements"],
                    "small_group_elems": stats["small_group_elems"]},
         "gbases_per_hour": units * total / (dev_ms * 1e-3) * 3600 / 1e9,
-        "e2e": {"value": units * N / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
-                "h2d_bytes_per_step": int(h_text.numel()) if args.fasta else int(h_ascii.numel() + h_off.numel() * 8), "d2h_bytes_per_step": int(h_out.numel())},
+        "e2e": {"value": units * N / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps, "path": e2e_name,
+                "h2d_bytes_per_step": int(h_text.numel()) if args.fasta else int(h_ascii.numel() + h_off.numel() * 8), "d2h_bytes_per_step": int(h_out.numel()),
+                "variants_ms_per_step": {k: round(v, 3) for k, v in e2e_variants.items()},
+                "variants": "sequential: copy in, cx_bwt_build into device memory, copy out; streamed: cx_bwt_build with out_is_host_pinned in four "
+                            "batches, each batch's copy overlapping the next batch's compute; streamed_packed: the same with out_bits = 4 "
+                            "(half the bytes out; reported only here, e2e is the better of the two ASCII-output paths)"},
         "gpu_launches": int(launches),
         "clocks": clocks,
         # the kernel class with the largest share of the step, against the HBM roofline of its algorithmic bytes

@@ -57,6 +57,13 @@ typedef struct cx_bwt_opts_s {
     uint32_t small_group_max;    /* tie refinement: groups up to this many suffixes are finished inside one
                                     thread block; 0 = default (256); 1 = use only the global re-key + sort   */
     uint32_t profile;            /* 1: bracket every kernel with CUDA events (see cx_bwt_kernel_time)         */
+    uint32_t finish_slots;       /* tie refinement in registers: positions per warp window / 32.  0 = chosen per batch from a
+                                    sample of its tie-group sizes; 2 = windows of 64 (groups up to 64, two-level keys);
+                                    4 = windows of 128 (groups up to 128)                                       */
+    uint32_t out_bits;           /* 0 or 8: out_bwt holds one ASCII byte per suffix.  4: NEXT-4, packed output,
+                                    two symbols per byte, first symbol in the high nibble, codes $ A C G T = 0 1 2 3 4;
+                                    out_bwt then has ceil(N / 2) bytes (the low nibble of the last byte is 0 if N is odd).
+                                    Halves the device->host stream of an out-of-core build.  Not with shard_count > 1  */
     uint32_t shard_index;        /* with shard_count > 1: which contiguous range of partitions this plan sorts     */
     uint32_t shard_count;        /* 0 or 1: the whole collection.  W > 1: the paper's distributed scheme (PAPER.md:103,
                                     Section 3.3): every worker holds all reads and computes the same partition sizes;
@@ -163,7 +170,8 @@ int cx_fasta_parse(const uint8_t *text_dev, uint64_t n_bytes, uint8_t *bases_out
  *   packed_reads: DEVICE, ceil(total_bases/32) words in the cx_pack_reads layout
  *   read_offsets: DEVICE, n_reads+1 base offsets, [0] = 0, non-decreasing; total_bases = [n_reads]
  *   out_bwt     : N = total_bases + n_reads bytes over "$ACGT" (ASCII), equal to B_R of
- *                 PAPER.md:55.  DEVICE, or pinned HOST if the plan was made with out_is_host_pinned.
+ *                 PAPER.md:55 (ceil(N / 2) bytes of 4-bit codes with opts.out_bits = 4).  DEVICE, or pinned HOST if the
+ *                 plan was made with out_is_host_pinned.
  * With opts.shard_count = W > 1 only the bytes [stats.shard_offset, + stats.shard_suffixes) of out_bwt are
  * written (the piece of worker opts.shard_index); out_bwt is still addressed from position 0.
  * Reads may have different lengths, including 0 (one suffix, preceded by '$').  n_reads = 0 is a

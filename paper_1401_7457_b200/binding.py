@@ -28,7 +28,7 @@ class CxError(RuntimeError):
 class cx_bwt_opts_t(ctypes.Structure):
     _fields_ = [("prefix_len", ctypes.c_uint32), ("key_bases", ctypes.c_uint32), ("max_batch_suffixes", ctypes.c_uint64),
                 ("max_read_len", ctypes.c_uint32), ("out_is_host_pinned", ctypes.c_int32), ("small_group_max", ctypes.c_uint32),
-                ("profile", ctypes.c_uint32), ("shard_index", ctypes.c_uint32), ("shard_count", ctypes.c_uint32)]
+                ("profile", ctypes.c_uint32), ("finish_slots", ctypes.c_uint32), ("out_bits", ctypes.c_uint32), ("shard_index", ctypes.c_uint32), ("shard_count", ctypes.c_uint32)]
 
 
 class cx_bwt_stats_t(ctypes.Structure):

@@ -58,7 +58,7 @@ constexpr uint32_t kMaxRegionDepth = 1u << 20;   // bases; deeper refinement is 
 // Byte offsets of every region of the workspace for a given m1.
 struct Layout {
     uint64_t info, hist, tile_first, tile_count, tile_sums, scalars, prefix;
-    uint64_t keys[2], ids[3], pos, heads[2], big_tiles, word_counts, word_sums, sort, stage[2];
+    uint64_t keys[2], ids[3], pos, heads[2], big_tiles, word_counts, word_sums, sort, stage[2], pstage[2];
     uint64_t total;
 };
 
@@ -66,7 +66,7 @@ struct Shape {
     uint64_t max_reads, max_bases, max_suffixes, max_tiles;
     uint32_t ell, w, cap, id_bytes, pos_bits, prefix_words;
     uint64_t n_buckets;
-    bool host_out;
+    bool host_out, pack_out;   // pack_out: NEXT-4, 4-bit output codes
     uint32_t shard_index, shard_count;   // NEXT-2: this plan sorts one of shard_count contiguous partition ranges
     bool sharded() const { return shard_count > 1; }
 };
@@ -96,7 +96,10 @@ Layout make_layout(const Shape& sh, uint64_t m1) {
     L.word_counts = take(words * 8);
     L.word_sums = take((scan_block_count(words) + 1) * 8);
     L.sort = take(sort_workspace_bytes(m1));
-    for (int i = 0; i < 2; ++i) L.stage[i] = take(sh.host_out ? m1 : 0);
+    // batches are emitted into a staging buffer when the output is pinned host memory (a9) or packed (NEXT-4: the pack
+    // step reads it); a packed host output goes through a second, packed staging buffer
+    for (int i = 0; i < 2; ++i) L.stage[i] = take(sh.host_out ? m1 : (sh.pack_out && i == 0 ? m1 : 0));
+    for (int i = 0; i < 2; ++i) L.pstage[i] = take(sh.host_out && sh.pack_out ? m1 / 2 + 16 : 0);
     L.total = at;
     return L;
 }
@@ -109,6 +112,7 @@ int make_shape(uint64_t max_reads, uint64_t max_bases, const cx_bwt_opts_t* o, S
     sh.w = o->key_bases;   // 0 = chosen in cx_bwt_plan from m1
     sh.cap = o->small_group_max ? o->small_group_max : (uint32_t)kLocalGroupCap;
     if (sh.ell < 1 || sh.ell > 7 || sh.w > 29 || (sh.w && sh.w < sh.ell)) return CX_ERR_ARG;
+    if (o->finish_slots != 0 && o->finish_slots != 2 && o->finish_slots != 4) return CX_ERR_ARG;
     if (sh.cap > (uint32_t)kLocalGroupCap) sh.cap = kLocalGroupCap;
     if (max_reads >= 0xFFFFFFFFull) return CX_ERR_ARG;   // read indices travel as 32 bits in the tile table
     sh.max_reads = max_reads;
@@ -124,9 +128,12 @@ int make_shape(uint64_t max_reads, uint64_t max_bases, const cx_bwt_opts_t* o, S
     sh.id_bytes = sh.pos_bits + read_bits <= 32 ? 4 : 8;
     sh.n_buckets = (1ull << (2 * sh.ell)) * (sh.ell + 1);
     sh.host_out = o->out_is_host_pinned != 0;
+    if (o->out_bits != 0 && o->out_bits != 8 && o->out_bits != 4) return CX_ERR_ARG;
+    sh.pack_out = o->out_bits == 4;
     sh.shard_count = o->shard_count ? o->shard_count : 1;
     sh.shard_index = o->shard_index;
     if (sh.shard_count > 65536 || sh.shard_index >= sh.shard_count) return CX_ERR_ARG;
+    if (sh.pack_out && sh.shard_count > 1) return CX_ERR_ARG;   // pieces of a packed output would share bytes at their ends
     return CX_OK;
 }
 
@@ -618,25 +625,33 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         const int cur = in_alt;
         IdT* ids = pack_kv ? d_ids[0] : d_ids[cur];
         // a9: with pinned-host output the batch is emitted into a staging buffer of the workspace
-        const int st = (int)(bi & 1);
-        uint8_t* dst = sh.host_out ? ws + L.stage[st] : out + B.out_offset;
+        const int st = sh.host_out ? (int)(bi & 1) : 0;
+        uint8_t* dst = sh.host_out || sh.pack_out ? ws + L.stage[st] : out + B.out_offset;
         if (sh.host_out && p->stage_busy[st]) CX_CUDA(cudaStreamWaitEvent(s, p->stage_free[st], 0));
         // ---- steps 3(c)ii-iii fused: head flags, in-block tie refinement, emit ----------------------
         const uint64_t n_words = (nb + 31) >> 5;
         int hc = 0;
         unsigned long long* d_done = reinterpret_cast<unsigned long long*>(d_scalars + 1);
+        // window width of the register refinement: from a sample of this batch's tie-group sizes unless the plan fixes it
+        uint32_t slots = p->opts.finish_slots;
+        if (slots == 0) {
+            uint64_t sampled = 0;
+            const uint64_t big_before = p->h_scalars[6];
+            CX_CUDA((launch_group_probe<KeyT, IdT>(d_keys1[cur], w, nb, pack_kv, reinterpret_cast<unsigned long long*>(d_scalars + 6), &sampled, s)));
+            if (sampled) {
+                CX_CUDA(cudaMemcpyAsync(p->h_scalars + 6, d_scalars + 6, 8, cudaMemcpyDeviceToHost, s));
+                CX_CUDA(cudaStreamSynchronize(s));
+            }
+            slots = sampled && (p->h_scalars[6] - big_before) * 4 > sampled ? 4u : 2u;   // more than a quarter in groups above 64
+        }
+        CX_CUDA(cudaMemsetAsync(d_heads[0], 0xff, (n_words + 1) * 4, s));   // every position a group of one until the warp kernel says otherwise
         CX_CUDA((launch_finish_first<KeyT, IdT>(R, d_keys1[cur], w, depth_base + w, d_heads[0], ids, nb, cap, dst, d_done, d_big_tiles, p->n_sms, pack_kv,
-                                                prof, s)));
+                                                slots, prof, s)));
         // groups of more than cap suffixes (counted by the warp kernel) go through global rounds; usually there are none
         const uint64_t over_before = p->h_scalars[5], local_before = p->h_scalars[1];
         CX_CUDA(cudaMemcpyAsync(p->h_scalars, d_scalars, 48, cudaMemcpyDeviceToHost, s));
         CX_CUDA(cudaStreamSynchronize(s));
         const bool any_oversize = p->h_scalars[5] != over_before;
-        if (any_oversize) {   // the head bitmask of what is left: groups of more than cap suffixes
-            CX_CUDA(cudaMemsetAsync(d_heads[0], 0, (n_words + 1) * 4, s));
-            ScopedLaunch sl(prof, CX_K_REFINE_SCAN, nb * sizeof(KeyT) + nb / 8, s);
-            CX_CUDA((launch_publish_heads<KeyT, IdT>(R, d_keys1[cur], w, d_heads[0], nb, cap, pack_kv, s)));
-        }
         // ---- what is still tied goes through global rounds: re-key, sort, write back ------------------
         uint32_t depth = depth_base + w, rounds = 0;
         while (any_oversize) {
@@ -687,11 +702,23 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         p->stats.refine_elements += p->h_scalars[1] - local_before;
         if (rounds > p->stats.refine_rounds) p->stats.refine_rounds = rounds;
 
+        // NEXT-4: two symbols per byte.  Batches come in output order, so a byte shared by two batches is completed by the
+        // later one (its high nibble is the earlier batch's last symbol, kept in a device word).
+        const uint8_t* copy_src = dst;
+        uint64_t copy_at = B.out_offset, copy_bytes = nb;
+        if (sh.pack_out) {
+            uint32_t* d_carry = reinterpret_cast<uint32_t*>(d_scalars + 7);
+            uint8_t* packed = sh.host_out ? ws + L.pstage[st] : out + B.out_offset / 2;
+            ScopedLaunch sl(prof, CX_K_PACK, nb + nb / 2, s);
+            CX_CUDA(launch_pack_symbols(dst, nb, B.out_offset, packed, d_carry, s));
+            prof->launches[CX_K_PACK] += 1;
+            copy_src = packed, copy_at = B.out_offset / 2, copy_bytes = (nb + (B.out_offset & 1) + 1) / 2;
+        }
         if (sh.host_out) {
             // a9: copy the staged batch on the side stream while the next batch computes
             CX_CUDA(cudaEventRecord(p->emit_done, s));
             CX_CUDA(cudaStreamWaitEvent(p->copy_stream, p->emit_done, 0));
-            CX_CUDA(cudaMemcpyAsync(out + B.out_offset, dst, nb, cudaMemcpyDeviceToHost, p->copy_stream));
+            CX_CUDA(cudaMemcpyAsync(out + copy_at, copy_src, copy_bytes, cudaMemcpyDeviceToHost, p->copy_stream));
             CX_CUDA(cudaEventRecord(p->stage_free[st], p->copy_stream));
             p->stage_busy[st] = true;
         }
@@ -715,7 +742,7 @@ extern "C" int cx_bwt_build(cx_bwt_plan_t* p, const uint64_t* packed_reads, cons
     if (!p) return CX_ERR_ARG;
     p->prof.reset();
     memset(&p->stats, 0, sizeof(p->stats));
-    p->h_scalars[0] = p->h_scalars[1] = p->h_scalars[3] = p->h_scalars[4] = p->h_scalars[5] = 0;
+    p->h_scalars[0] = p->h_scalars[1] = p->h_scalars[3] = p->h_scalars[4] = p->h_scalars[5] = p->h_scalars[6] = 0;
     if (n_reads == 0) return CX_OK;
     if (!read_offsets || !out_bwt || n_reads > p->sh.max_reads) return CX_ERR_ARG;
     if (!packed_reads && p->sh.max_bases) return CX_ERR_ARG;

@@ -156,6 +156,9 @@ cudaError_t launch_fasta_parse(const uint8_t* text, uint64_t n, uint8_t* bases_o
                                unsigned char* ws, cudaStream_t s);
 cudaError_t launch_pack(const uint8_t* ascii, uint64_t total_bases, uint64_t* packed, uint32_t* status, cudaStream_t s);
 uint32_t* pack_fallback_status();
+// NEXT-4: n symbols of BWT positions [out_offset, out_offset + n) -> 4-bit codes; packed[0] = byte out_offset / 2 of the output;
+// *carry holds the code of the symbol before the piece (and, afterwards, of the piece's last symbol)
+cudaError_t launch_pack_symbols(const uint8_t* sym, uint64_t n, uint64_t out_offset, uint8_t* packed, uint32_t* carry, cudaStream_t s);
 
 // cx_scan_reads.cu
 cudaError_t launch_prep(const uint64_t* offsets, uint64_t n_reads, uint64_t max_bases, BuildInfo* info, cudaStream_t s);
@@ -217,18 +220,19 @@ template <typename IdT>
 cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, const IdT* ids_c, const uint32_t* pos_c, uint64_t n_c,
                                     uint32_t w, IdT* ids, uint32_t* heads, uint8_t* out, cudaStream_t s);
 // a7 + a8 over the freshly sorted first-round keys: the warp kernel finishes singletons and tie groups of at most 32
-// suffixes and counts the groups it leaves to the global path (elems_done[4]; their head bitmask is launch_publish_heads'); the block kernel then finishes the groups of 33..group_cap in the tiles the warp
+// suffixes, counts the groups it leaves to the global path (elems_done[4]) and clears all but their first bit in heads_out
+// (the head bitmask of that path; filled with ones by the caller: every other position counts as a group of one); the block kernel then finishes the groups of 33..group_cap in the tiles the warp
 // kernel flagged in big_tiles (n / kLocalTile / 32 + 2 words).  depth0: symbols the first-round sort has settled.
 // packed: keys1 holds 64-bit words (32-bit key << 32 | 32-bit id); `ids` then receives the ids of the groups left to the
 // global path (nothing else will need the others).
 template <typename KeyT, typename IdT>
 cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t depth0, uint32_t* heads_out, IdT* ids, uint64_t n,
                                 uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, uint32_t* big_tiles, int n_sms, bool packed,
-                                Launch* prof, cudaStream_t s);
-// the head bitmask of the global path (zero-filled by the caller): run only when launch_finish_first counted oversize groups
+                                uint32_t slots, Launch* prof, cudaStream_t s);
+// a sample of the sorted first-round keys: *counter += sampled positions in tie groups of more than 64 suffixes, *sampled (HOST) =
+// positions looked at (0: batch too small to sample).  slots of launch_finish_first: 4 if those are a large share, else 2
 template <typename KeyT, typename IdT>
-cudaError_t launch_publish_heads(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t* heads_out, uint64_t n, uint32_t group_cap, bool packed,
-                                 cudaStream_t s);
+cudaError_t launch_group_probe(const KeyT* keys1, uint32_t w1, uint64_t n, bool packed, unsigned long long* counter, uint64_t* sampled, cudaStream_t s);
 // in-block refinement + emit of the groups a global round has split to at most group_cap members; heads_out = copy of heads_in
 template <typename IdT>
 cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32_t* heads_out, const IdT* ids, uint64_t n, uint32_t depth,

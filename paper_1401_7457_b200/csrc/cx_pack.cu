@@ -53,6 +53,29 @@ __global__ void __launch_bounds__(256) pack_kernel(const uint8_t* __restrict__ a
 
 __device__ uint32_t g_pack_status;   // used when the caller passes no status word
 
+// NEXT-4, packed output: n ASCII symbols over "$ACGT" that belong at positions [off, off + n) of the BWT -> 4-bit codes
+// ($ A C G T = 0 1 2 3 4), two per byte, first symbol of a byte in its high nibble.  packed[0] is the byte that holds
+// position off (byte off / 2 of the whole output).  If off is odd that byte's high nibble is the symbol before this
+// piece: *carry (its code, written by the previous call on this stream).  Four output bytes per thread.
+__device__ __forceinline__ uint32_t nibble_of(uint8_t c) { return (c & 0x40u) ? 1u + (((c >> 1) ^ (c >> 2)) & 3u) : 0u; }
+__global__ void __launch_bounds__(256) pack_symbols_kernel(const uint8_t* __restrict__ sym, uint64_t n, uint32_t odd, uint8_t* __restrict__ packed,
+                                                           uint32_t* __restrict__ carry) {
+    const uint64_t n_bytes = (n + odd + 1) >> 1;
+    const uint64_t b0 = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const uint64_t b = b0 + k;
+        if (b >= n_bytes) break;
+        const int64_t i = (int64_t)(2 * b) - (int64_t)odd;        // local index of the byte's first symbol
+        const uint32_t hi = i >= 0 ? nibble_of(__ldg(sym + i)) : *carry;
+        const uint32_t lo = (uint64_t)(i + 1) < n ? nibble_of(__ldg(sym + i + 1)) : 0u;
+        packed[b] = (uint8_t)((hi << 4) | lo);
+    }
+}
+__global__ void last_symbol_kernel(const uint8_t* __restrict__ sym, uint64_t n, uint32_t* __restrict__ carry) {
+    if (n) *carry = nibble_of(sym[n - 1]);
+}
+
 }  // namespace
 
 cudaError_t launch_pack(const uint8_t* ascii, uint64_t total_bases, uint64_t* packed, uint32_t* status, cudaStream_t s) {
@@ -65,6 +88,15 @@ cudaError_t launch_pack(const uint8_t* ascii, uint64_t total_bases, uint64_t* pa
         pack_kernel<true><<<grid, 256, 0, s>>>(ascii, total_bases, packed, status);
     else
         pack_kernel<false><<<grid, 256, 0, s>>>(ascii, total_bases, packed, status);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_pack_symbols(const uint8_t* sym, uint64_t n, uint64_t out_offset, uint8_t* packed, uint32_t* carry, cudaStream_t s) {
+    if (n == 0) return cudaSuccess;
+    const uint32_t odd = (uint32_t)(out_offset & 1);
+    const uint64_t n_bytes = (n + odd + 1) >> 1;
+    pack_symbols_kernel<<<(unsigned)((n_bytes + 1023) / 1024), 256, 0, s>>>(sym, n, odd, packed, carry);
+    last_symbol_kernel<<<1, 1, 0, s>>>(sym, n, carry);   // after the pack: it read the previous piece's last symbol
     return cudaGetLastError();
 }
 

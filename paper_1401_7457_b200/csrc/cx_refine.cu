@@ -752,7 +752,9 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
 // ---------------------------------------------------------------------------------------------
 constexpr int kWarpChunk = 2048;    // sorted positions per warp: a chunk owns the groups that START in it
 constexpr int kWarpThreads = 256;
-constexpr int kWarpSlots = 2;
+// slots per lane: 2 (windows of 64 positions, two-level keys) unless the batch's tie groups are mostly larger, then 4
+// (windows of 128 positions; the rank key has room for one level only)
+constexpr int kWarpSlotsSmall = 2, kWarpSlotsLarge = 4;
 
 // Event codes (the two levels of the rank key), order-preserving; 0 = no event:
 //   1 + 5 d + s         below the pivot at base d: s = 0 my end-marker (FINAL: identical strings), 1..4 my base A..T
@@ -841,23 +843,35 @@ __device__ __forceinline__ uint64_t scan_to_head(const KeyT* __restrict__ keys1,
     }
 }
 
-// OR `bits` (bit i = position a + i) into the head bitmask; whole-warp call, two lanes write
-__device__ __forceinline__ void publish_heads(uint32_t* __restrict__ heads, uint64_t a, uint32_t bits) {
-    const uint32_t sh = (uint32_t)(a & 31);
-    const uint32_t lane = lane_id();
-    if (lane == 0 && (bits << sh)) atomicOr(heads + (a >> 5), bits << sh);
-    if (lane == 1 && sh && (bits >> (32 - sh))) atomicOr(heads + (a >> 5) + 1, bits >> (32 - sh));
+// The head bitmask of the global path starts as all ones (every position a group of one: placed); a group left to that
+// path keeps only its first position's bit.  Clear the bits of positions [lo, hi); whole-warp call.
+__device__ __forceinline__ void clear_heads(uint32_t* __restrict__ heads, uint64_t lo, uint64_t hi) {
+    if (lo >= hi) return;
+    const uint64_t w_lo = lo >> 5, w_hi = (hi - 1) >> 5;
+    for (uint64_t w = w_lo + lane_id(); w <= w_hi; w += 32) {
+        uint32_t m = kFull;
+        if (w == w_lo) m &= kFull << (lo & 31);
+        if (w == w_hi) m &= kFull >> (31 - ((hi - 1) & 31));
+        if (m == kFull) heads[w] = 0u;          // a word inside one group has no other writer
+        else atomicAnd(heads + w, ~m);
+    }
 }
 
 // value of `v` at window position q (slot q / 32 of lane q % 32), for every lane its own q
+// (written out per slot count: a loop over slots with a data-dependent pick ends up in local memory)
 template <int S, typename T>
 __device__ __forceinline__ T fetch_at(const T (&v)[S], uint32_t q) {
-    static_assert(S == 1 || S == 2, "written out per slot count: a loop over slots ends up in local memory");
+    static_assert(S == 1 || S == 2 || S == 4, "slots per lane");
     if constexpr (S == 1) {
         return __shfl_sync(kFull, v[0], q & 31);
-    } else {
+    } else if constexpr (S == 2) {
         const T lo = __shfl_sync(kFull, v[0], q & 31), hi = __shfl_sync(kFull, v[1], q & 31);
         return (q & 32u) ? hi : lo;
+    } else {
+        const T a0 = __shfl_sync(kFull, v[0], q & 31), a1 = __shfl_sync(kFull, v[1], q & 31);
+        const T a2 = __shfl_sync(kFull, v[2], q & 31), a3 = __shfl_sync(kFull, v[3], q & 31);
+        const T lo = (q & 32u) ? a1 : a0, hi = (q & 32u) ? a3 : a2;
+        return (q & 64u) ? hi : lo;
     }
 }
 
@@ -882,18 +896,17 @@ __device__ __forceinline__ void window_words(const uint64_t* __restrict__ packed
     }
 }
 
-// PUBLISH = false: refine and emit.  PUBLISH = true (run only when groups larger than cap exist, before the global path):
-// nothing is gathered or emitted; the head bitmask the global path works on is written -- every position of a group of at
-// most cap suffixes counts as a group of one (placed), a larger group shows only its first position.
-template <typename KeyT, typename IdT, bool PACKED, int S, bool PUBLISH>
-__global__ void __launch_bounds__(kWarpThreads, 3) finish_warp_kernel(Reads R, const KeyT* __restrict__ keys1, const IdT* __restrict__ ids_in,
+template <typename KeyT, typename IdT, bool PACKED, int S>
+__global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : 3) finish_warp_kernel(Reads R, const KeyT* __restrict__ keys1, const IdT* __restrict__ ids_in,
                                                                    IdT* __restrict__ ids_out, uint32_t w1, uint32_t len_mask, uint64_t n,
                                                                    uint32_t depth0, uint32_t cap, uint32_t* __restrict__ heads,
                                                                    uint32_t* __restrict__ big_tiles, uint8_t* __restrict__ out,
                                                                    unsigned long long* counters) {
     constexpr uint32_t kSpan = 32 * S;                  // positions per window
-    constexpr uint32_t kPosBits = S == 1 ? 5 : 6;       // bits of a window position
-    static_assert(S == 1 || S == 2, "the rank key holds window positions of at most 6 bits");
+    constexpr uint32_t kPosBits = S == 1 ? 5 : S == 2 ? 6 : 7;   // bits of a window position
+    constexpr bool kTwoLevels = 2 * kPosBits + 20 <= 32;         // room for the second event in the 32-bit rank key
+    constexpr uint32_t kClsBits = kTwoLevels ? 20 : 10;
+    static_assert(S == 1 || S == 2 || S == 4, "slots per lane");
     const uint32_t lane = lane_id();
     const uint64_t c0 = ((uint64_t)blockIdx.x * (kWarpThreads / 32) + (threadIdx.x >> 5)) * kWarpChunk;
     const uint64_t c1 = c0 + kWarpChunk < n ? c0 + kWarpChunk : n;
@@ -901,7 +914,6 @@ __global__ void __launch_bounds__(kWarpThreads, 3) finish_warp_kernel(Reads R, c
     const uint64_t pos_mask = (1ull << R.pos_bits) - 1;
     uint32_t n_members = 0, n_sorts = 0, n_over = 0;     // lane 0's tallies
     uint64_t a = c0;
-    if (PUBLISH && c0 < n && c1 == n) publish_heads(heads, n, kFull);   // positions past the end count as heads (the bitmask's padding)
     if (c0 < n && c0 > 0) a = scan_to_head<KeyT, PACKED>(keys1, c0, n, w1, len_mask);   // groups that began before the chunk are the previous warp's
     while (a < c1) {
         // ---- the window [a, a + 32 S): a is a head --------------------------------------------------------------
@@ -958,13 +970,10 @@ __global__ void __launch_bounds__(kWarpThreads, 3) finish_warp_kernel(Reads R, c
             // one group fills the window and goes on: more than 32 S members
             const uint64_t e = scan_to_head<KeyT, PACKED>(keys1, a + kSpan, n, w1, len_mask);
             const uint64_t g = e - a;
-            if (g <= cap) {          // the block kernel's: flag the tile it starts in; its positions count as placed
-                if (!PUBLISH && lane == 0) atomicOr(big_tiles + (a / kLocalTile >> 5), 1u << (a / kLocalTile & 31));
-                if (PUBLISH)
-                    for (uint64_t q = a; q < e; q += 32) publish_heads(heads, q, e - q >= 32 ? kFull : (1u << (uint32_t)(e - q)) - 1);
-            } else if (PUBLISH) {    // the global path's: only its head bit
-                publish_heads(heads, a, 1u);
-            } else {                 // hand its ids over, count it
+            if (g <= cap) {          // the block kernel's: flag the tile it starts in
+                if (lane == 0) atomicOr(big_tiles + (a / kLocalTile >> 5), 1u << (a / kLocalTile & 31));
+            } else {                 // the global path's: only its first position stays a head; hand its ids over, count it
+                clear_heads(heads, a + 1, e);
                 if constexpr (PACKED) {
                     for (uint64_t q = a + lane; q < e; q += 32) ids_out[q] = (IdT)(uint32_t)load_keyword<KeyT, PACKED>(keys1, q);
                 }
@@ -1007,9 +1016,9 @@ __global__ void __launch_bounds__(kWarpThreads, 3) finish_warp_kernel(Reads R, c
             if (!active) gs[s] = p, ge[s] = p + 1;
             const uint32_t size = ge[s] - gs[s];
             mine[s] = active && size <= cap_a;              // (a complete group larger than cap_a exists only when cap < 32 S)
-            member[s] = !PUBLISH && mine[s] && size >= 2;
+            member[s] = mine[s] && size >= 2;
             idv[s] = 0;
-            if (active && !PUBLISH) {
+            if (active) {
                 if constexpr (PACKED) idv[s] = (IdT)(uint32_t)word[s];
                 else idv[s] = __ldg(ids_in + j);
             }
@@ -1023,12 +1032,12 @@ __global__ void __launch_bounds__(kWarpThreads, 3) finish_warp_kernel(Reads R, c
                 first_base[s] = read * R.uniform_len + pos;
                 left = R.uniform_len - pos;
             } else {
-                const uint64_t* q = R.offsets + (mine[s] && !PUBLISH ? read : 0ull);
+                const uint64_t* q = R.offsets + (mine[s] ? read : 0ull);
                 const uint64_t lo = __ldg(q), hi = __ldg(q + 1);
                 first_base[s] = lo + pos;
                 left = hi - lo - pos;
             }
-            const bool has_prev = !PUBLISH && mine[s] && pos;
+            const bool has_prev = mine[s] && pos;
             before[s] = has_prev ? __ldg(R.packed + ((first_base[s] - 1) >> 5)) : 0ull;   // no load for a read's first suffix
             wbase[s] = first_base[s] + depth0;                // index of the window's first base
             mrem[s] = member[s] ? (uint32_t)(left - depth0) : 0u;   // a member of an open group has >= depth0 bases
@@ -1088,7 +1097,7 @@ __global__ void __launch_bounds__(kWarpThreads, 3) finish_warp_kernel(Reads R, c
 #pragma unroll
             for (int s = 0; s < S; ++s) {
                 const uint32_t p = 32 * s + lane;
-                key[s] = member[s] ? (gs[s] << (32 - kPosBits)) | (c1v[s] << (kPosBits + 10)) | (c2v[s] << kPosBits) | (p - gs[s])
+                key[s] = member[s] ? (gs[s] << (32 - kPosBits)) | (c1v[s] << (kPosBits + kClsBits - 10)) | (kTwoLevels ? c2v[s] << kPosBits : 0u) | (p - gs[s])
                                    : p << (32 - kPosBits);   // a position outside every open group keeps its place
             }
             // bitonic sort of the window: groups stay in place (their first position leads the key), members are ranked inside
@@ -1126,7 +1135,7 @@ __global__ void __launch_bounds__(kWarpThreads, 3) finish_warp_kernel(Reads R, c
 #pragma unroll
             for (int s = 0; s < S; ++s) {
                 src[s] = (key[s] >> (32 - kPosBits)) + (key[s] & (kSpan - 1));
-                cls[s] = (key[s] >> kPosBits) & 0xfffffu;
+                cls[s] = (key[s] >> kPosBits) & ((1u << kClsBits) - 1);
             }
 #pragma unroll
             for (int s = 0; s < S; ++s) was[s] = cls[s] != 0;   // a member's level-1 code is never 0
@@ -1138,8 +1147,9 @@ __global__ void __launch_bounds__(kWarpThreads, 3) finish_warp_kernel(Reads R, c
                     const uint32_t last = __shfl_sync(kFull, cls[s > 0 ? s - 1 : 0], 31);
                     if (lane == 0) prev = last;
                 }
-                const uint32_t t1 = code_type(cls[s] >> 10);
-                const uint32_t ty = t1 == 3 ? code_type(cls[s] & 0x3ffu) : t1;   // the class's last event decides
+                const uint32_t t1 = code_type(kTwoLevels ? cls[s] >> 10 : cls[s]);
+                // the class's last event decides (with one level a base mismatch simply goes round again)
+                const uint32_t ty = kTwoLevels && t1 == 3 && (cls[s] & 0x3ffu) ? code_type(cls[s] & 0x3ffu) : t1;
                 nextwin[s] = ty == 2;
                 head[s] = !was[s] || p == (key[s] >> (32 - kPosBits)) || ty == 1 || cls[s] != prev;
                 hb[s] = __ballot_sync(kFull, head[s]);
@@ -1225,18 +1235,19 @@ __global__ void __launch_bounds__(kWarpThreads, 3) finish_warp_kernel(Reads R, c
         for (int s = 0; s < S; ++s) {
             const uint32_t p = 32 * s + lane;
             const uint64_t j = a + p;
-            if (!PUBLISH && mine[s]) out[j] = (uint8_t)(0x544743412400ull >> (8 * code[s]));
+            if (mine[s]) out[j] = (uint8_t)(0x544743412400ull >> (8 * code[s]));
             const bool active = p < n_comp && j < n;
             const bool over = active && !mine[s];             // a complete group of more than cap members (cap < 32 S only)
-            const bool over_head = over && ((hw[s] >> lane) & 1u);
-            if (PUBLISH) {
-                const uint32_t bits = __ballot_sync(kFull, mine[s] || over_head);
-                publish_heads(heads, a + 32 * s, bits);
-            } else if (__any_sync(kFull, over)) {
+            if (__any_sync(kFull, over)) {                    // the global path's: clear all but its first position's head bit
+                const bool over_head = over && ((hw[s] >> lane) & 1u);
                 if constexpr (PACKED) {
                     if (over) ids_out[j] = idv[s];
                 }
-                const uint32_t over_heads = __ballot_sync(kFull, over_head);
+                const uint32_t clear = __ballot_sync(kFull, over && !over_head), over_heads = __ballot_sync(kFull, over_head);
+                const uint64_t at = a + 32 * s;
+                const uint32_t sh = (uint32_t)(at & 31);
+                if (lane == 0 && (clear << sh)) atomicAnd(heads + (at >> 5), ~(clear << sh));
+                if (lane == 1 && sh && (clear >> (32 - sh))) atomicAnd(heads + (at >> 5) + 1, ~(clear >> (32 - sh)));
                 if (lane == 0) n_over += (uint32_t)__popc(over_heads);
             }
         }
@@ -1252,12 +1263,51 @@ __global__ void __launch_bounds__(kWarpThreads, 3) finish_warp_kernel(Reads R, c
         if (n_over) atomicAdd(&s_tally[2], n_over);
     }
     __syncthreads();
-    if (!PUBLISH && threadIdx.x == 0) {
+    if (threadIdx.x == 0) {
         if (s_tally[0]) atomicAdd(counters, (unsigned long long)s_tally[0]);                       // suffixes refined here
         if (s_tally[1]) atomicAdd(counters + 2, (unsigned long long)s_tally[1] * (S == 1 ? 80 : 192));   // rank-key comparisons of the sorts
         if (s_tally[1]) atomicAdd(counters + 3, (unsigned long long)s_tally[1]);                  // refinement rounds (warp windows)
         if (s_tally[2]) atomicAdd(counters + 4, (unsigned long long)s_tally[2]);                  // groups left to the global path
     }
+}
+
+// How large are the tie groups of this batch?  A sample of windows of 2048 sorted positions: positions that sit in a run of
+// more than `limit` equal first-round keys (runs are cut at the window's ends, so this underestimates).  Decides the window
+// width of the warp kernel.  counter[0] += such positions.
+constexpr int kProbeSpan = 2048, kProbeBlocks = 128;
+template <typename KeyT, bool PACKED>
+__global__ void __launch_bounds__(256) group_probe_kernel(const KeyT* __restrict__ keys1, uint64_t n, uint32_t w1, uint32_t len_mask, uint32_t limit,
+                                                          unsigned long long* counter) {
+    __shared__ uint32_t s_heads[kProbeSpan / 32 + 1];
+    __shared__ uint32_t s_big;
+    const uint64_t stride = n / gridDim.x;
+    const uint64_t a = (uint64_t)blockIdx.x * stride;
+    if (threadIdx.x == 0) s_big = 0, s_heads[kProbeSpan / 32] = 1u;
+#pragma unroll
+    for (int k = 0; k < kProbeSpan / 256; ++k) {
+        const uint32_t e = k * 256 + threadIdx.x;
+        const uint64_t j = a + e;
+        bool head = true;
+        if (j < n && e > 0) {
+            const uint64_t kc = key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j)), kp = key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j - 1));
+            head = kc != kp || ((uint32_t)kc & len_mask) < w1;
+        }
+        const uint32_t word = __ballot_sync(kFull, head);
+        if ((threadIdx.x & 31) == 0) s_heads[e >> 5] = word;
+    }
+    __syncthreads();
+    uint32_t big = 0;
+#pragma unroll
+    for (int k = 0; k < kProbeSpan / 256; ++k) {
+        const int e = k * 256 + (int)threadIdx.x;
+        if (a + e >= n) continue;
+        const int ps = prev_head(s_heads, e, 0), ne = next_head(s_heads, e, kProbeSpan);
+        big += (uint32_t)((ne < 0 ? kProbeSpan : ne) - ps > (int)limit);
+    }
+    for (int o = 16; o; o >>= 1) big += __shfl_xor_sync(kFull, big, o);
+    if ((threadIdx.x & 31) == 0 && big) atomicAdd(&s_big, big);
+    __syncthreads();
+    if (threadIdx.x == 0 && s_big) atomicAdd(counter, (unsigned long long)s_big);
 }
 
 }  // namespace
@@ -1303,10 +1353,11 @@ cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, cons
 template <typename KeyT, typename IdT>
 cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t depth0, uint32_t* heads_out, IdT* ids, uint64_t n,
                                 uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, uint32_t* big_tiles, int n_sms, bool packed,
-                                Launch* prof, cudaStream_t s) {
+                                uint32_t slots, Launch* prof, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
     constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
     if (packed && !kCanPack) return cudaErrorInvalidValue;
+    if (slots != (uint32_t)kWarpSlotsSmall && slots != (uint32_t)kWarpSlotsLarge) return cudaErrorInvalidValue;
     if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
     const uint32_t len_mask = (1u << key_len_bits(w1)) - 1;
     const uint64_t tiles = (n + kLocalTile - 1) / kLocalTile;
@@ -1316,38 +1367,39 @@ cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, 
         ScopedLaunch sl(prof, CX_K_FINISH, n * (sizeof(KeyT) + sizeof(IdT) + 1) + n / 8, s);
         const uint64_t warps = (n + kWarpChunk - 1) / kWarpChunk;
         const unsigned grid = (unsigned)((warps + kWarpThreads / 32 - 1) / (kWarpThreads / 32));
-        if (packed)
-            finish_warp_kernel<KeyT, IdT, kCanPack, kWarpSlots, false><<<grid, kWarpThreads, 0, s>>>(R, keys1, ids, ids, w1, len_mask, n, depth0, group_cap, heads_out, big_tiles, out, elems_done);
-        else
-            finish_warp_kernel<KeyT, IdT, false, kWarpSlots, false><<<grid, kWarpThreads, 0, s>>>(R, keys1, ids, ids, w1, len_mask, n, depth0, group_cap, heads_out, big_tiles, out, elems_done);
+        auto launch = [&](auto kernel) { kernel<<<grid, kWarpThreads, 0, s>>>(R, keys1, ids, ids, w1, len_mask, n, depth0, group_cap, heads_out, big_tiles, out, elems_done); };
+        if (slots == (uint32_t)kWarpSlotsLarge) {
+            if (packed) launch(finish_warp_kernel<KeyT, IdT, kCanPack, kWarpSlotsLarge>);
+            else launch(finish_warp_kernel<KeyT, IdT, false, kWarpSlotsLarge>);
+        } else {
+            if (packed) launch(finish_warp_kernel<KeyT, IdT, kCanPack, kWarpSlotsSmall>);
+            else launch(finish_warp_kernel<KeyT, IdT, false, kWarpSlotsSmall>);
+        }
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
-    if (group_cap <= 32 * kWarpSlots) return cudaSuccess;
+    if (group_cap <= 32 * slots) return cudaSuccess;
     // larger groups, up to cap: persistent blocks over the flagged tiles
     auto kernel = packed ? finish_tile_kernel<KeyT, IdT, true, kCanPack> : finish_tile_kernel<KeyT, IdT, true, false>;
     e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(LocalSmem));
     if (e != cudaSuccess) return e;
     const uint64_t resident = (uint64_t)n_sms * kLocalBlocksPerSM;
     ScopedLaunch sl(prof, CX_K_FINISH_BLOCK, 0, s);
-    kernel<<<(unsigned)(tiles < resident ? tiles : resident), kLocalThreads, sizeof(LocalSmem), s>>>(R, keys1, w1, len_mask, nullptr, nullptr, ids, n, depth0, 32u * kWarpSlots + 1,
+    kernel<<<(unsigned)(tiles < resident ? tiles : resident), kLocalThreads, sizeof(LocalSmem), s>>>(R, keys1, w1, len_mask, nullptr, nullptr, ids, n, depth0, 32u * slots + 1,
                                                                                                    group_cap, big_tiles, out, elems_done);
     return cudaGetLastError();
 }
 
 template <typename KeyT, typename IdT>
-cudaError_t launch_publish_heads(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t* heads_out, uint64_t n, uint32_t group_cap, bool packed,
-                                 cudaStream_t s) {
-    if (n == 0) return cudaSuccess;
+cudaError_t launch_group_probe(const KeyT* keys1, uint32_t w1, uint64_t n, bool packed, unsigned long long* counter, uint64_t* sampled, cudaStream_t s) {
     constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
-    if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
+    *sampled = 0;
+    if (n < (uint64_t)kProbeSpan * 2) return cudaSuccess;
+    const unsigned blocks = (unsigned)(n / kProbeSpan < (uint64_t)kProbeBlocks ? n / kProbeSpan : (uint64_t)kProbeBlocks);
+    *sampled = (uint64_t)blocks * kProbeSpan;
     const uint32_t len_mask = (1u << key_len_bits(w1)) - 1;
-    const uint64_t warps = (n + kWarpChunk - 1) / kWarpChunk;
-    const unsigned grid = (unsigned)((warps + kWarpThreads / 32 - 1) / (kWarpThreads / 32));
-    if (packed)
-        finish_warp_kernel<KeyT, IdT, kCanPack, kWarpSlots, true><<<grid, kWarpThreads, 0, s>>>(R, keys1, nullptr, nullptr, w1, len_mask, n, 0, group_cap, heads_out, nullptr, nullptr, nullptr);
-    else
-        finish_warp_kernel<KeyT, IdT, false, kWarpSlots, true><<<grid, kWarpThreads, 0, s>>>(R, keys1, nullptr, nullptr, w1, len_mask, n, 0, group_cap, heads_out, nullptr, nullptr, nullptr);
+    if (packed) group_probe_kernel<KeyT, kCanPack><<<blocks, 256, 0, s>>>(keys1, n, w1, len_mask, 32u * kWarpSlotsSmall, counter);
+    else group_probe_kernel<KeyT, false><<<blocks, 256, 0, s>>>(keys1, n, w1, len_mask, 32u * kWarpSlotsSmall, counter);
     return cudaGetLastError();
 }
 
@@ -1372,11 +1424,11 @@ cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32
     template cudaError_t launch_refine_writeback<IdT>(const Reads&, const uint64_t*, const IdT*, const uint32_t*, uint64_t,         \
                                                       uint32_t, IdT*, uint32_t*, uint8_t*, cudaStream_t);                            \
     template cudaError_t launch_finish_first<uint32_t, IdT>(const Reads&, const uint32_t*, uint32_t, uint32_t, uint32_t*, IdT*, uint64_t, \
-                                                            uint32_t, uint8_t*, unsigned long long*, uint32_t*, int, bool, Launch*, cudaStream_t); \
+                                                            uint32_t, uint8_t*, unsigned long long*, uint32_t*, int, bool, uint32_t, Launch*, cudaStream_t); \
     template cudaError_t launch_finish_first<uint64_t, IdT>(const Reads&, const uint64_t*, uint32_t, uint32_t, uint32_t*, IdT*, uint64_t, \
-                                                            uint32_t, uint8_t*, unsigned long long*, uint32_t*, int, bool, Launch*, cudaStream_t); \
-    template cudaError_t launch_publish_heads<uint32_t, IdT>(const Reads&, const uint32_t*, uint32_t, uint32_t*, uint64_t, uint32_t, bool, cudaStream_t); \
-    template cudaError_t launch_publish_heads<uint64_t, IdT>(const Reads&, const uint64_t*, uint32_t, uint32_t*, uint64_t, uint32_t, bool, cudaStream_t); \
+                                                            uint32_t, uint8_t*, unsigned long long*, uint32_t*, int, bool, uint32_t, Launch*, cudaStream_t); \
+    template cudaError_t launch_group_probe<uint32_t, IdT>(const uint32_t*, uint32_t, uint64_t, bool, unsigned long long*, uint64_t*, cudaStream_t); \
+    template cudaError_t launch_group_probe<uint64_t, IdT>(const uint64_t*, uint32_t, uint64_t, bool, unsigned long long*, uint64_t*, cudaStream_t); \
     template cudaError_t launch_finish_later<IdT>(const Reads&, const uint32_t*, uint32_t*, const IdT*, uint64_t, uint32_t,         \
                                                   uint32_t, uint8_t*, unsigned long long*, int, cudaStream_t);
 CX_INSTANTIATE(uint32_t)

@@ -67,6 +67,7 @@ def test_random_ragged_collections(seed):
     assert_parity(c)
     assert_parity(c, small_group_max=1)                 # global re-key path only
     assert_parity(c, key_bases=7 + seed % 20, prefix_len=1 + seed % 7)
+    assert_parity(c, finish_slots=[2, 4][seed % 2], key_bases=[0, 9][seed % 3 == 0])      # window width of the register refinement fixed
 
 
 def test_homopolymer_reads_one_giant_group():
@@ -92,6 +93,8 @@ def test_config1_full():
 def test_config_shapes_scaled(idx, scale):
     c = gen.config(idx, scale)
     assert_parity(c)
+    assert_parity(c, finish_slots=4)
+    assert_parity(c, finish_slots=2)
 
 
 def test_config2_full_size_every_suffix():
@@ -374,3 +377,34 @@ def test_read_longer_than_2_pow_21_in_tie_groups():
     long_read = "".join(np.frombuffer(b"ACGT", np.uint8)[rng.integers(0, 4, 2_200_000)].tobytes().decode())
     reads = [long_read, long_read[100:160], long_read[100:160], long_read[5000:5100], long_read[2_199_900:], ""]
     assert_parity(gen.from_strings(reads))
+
+
+# ---- NEXT-4: packed output, two symbols per byte (include/cx_bwt.h, opts.out_bits = 4) -----------------------------------
+
+def _unpack4(packed: np.ndarray, n: int) -> np.ndarray:
+    codes = np.stack([packed >> 4, packed & 15], 1).reshape(-1)[:n]
+    assert codes.max(initial=0) <= 4
+    return np.frombuffer(b"$ACGT", np.uint8)[codes]
+
+
+@pytest.mark.parametrize("opts", [dict(), dict(max_batch_suffixes=70_001, prefix_len=5), dict(max_batch_suffixes=33_333, small_group_max=1),
+                                  dict(max_batch_suffixes=150_001, out_is_host_pinned=1), dict(out_is_host_pinned=1)])
+def test_packed_output_four_bits_per_symbol(opts):
+    import paper_1401_7457_b200 as cx
+    for c in (gen.config(2, 0.001), gen.from_strings(["ACGT", "TAGT", "GGAA"]), gen.random_collection(9, 301, 77)):   # N even, 15, odd
+        want = oracle.bwt(c.ascii, c.offsets)
+        N = c.n_suffixes
+        p = cx.Plan(c.n_reads, c.total_bases, max_read_len=max(c.max_read_len, 1), out_bits=4, **opts)
+        out = torch.full(((N + 1) // 2,), 0xEE, dtype=torch.uint8)
+        out = out.pin_memory() if opts.get("out_is_host_pinned") else out.cuda()
+        a = torch.from_numpy(c.ascii).cuda()
+        p.build(cx.cx_pack_reads(a), torch.from_numpy(c.offsets.astype(np.int64)).cuda(), c.n_reads, out)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy()
+        assert np.array_equal(_unpack4(got, N), want), (c.name, opts)
+        if N & 1:
+            assert got[-1] & 15 == 0                      # the unused low nibble of the last byte
+    with pytest.raises(cx.CxError):
+        cx.Plan(100, 1000, out_bits=4, shard_index=0, shard_count=2)
+    with pytest.raises(cx.CxError):
+        cx.Plan(100, 1000, out_bits=3)
