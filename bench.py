@@ -401,6 +401,8 @@ def run_cx(args) -> None:
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
+        if args.shard:
+            os.environ.setdefault("NCCL_DEBUG", "INFO")      # the communicator lines (ranks, transport) go to stderr beside the record
         dist.init_process_group("nccl", device_id=dev)
     cx.lib()
     if args.config >= 3 and not args.table4 and args.scale == 1.0:
@@ -541,22 +543,24 @@ def run_cx(args) -> None:
     if not sharded and not one_shard and not args.fasta and args.out_bits == 8 and N >= 4_000_000:
         # the library's own pinned-host output path (a9): four batches, each batch's D2H copy on a side stream while the next
         # batch computes; and the same with the packed output (NEXT-4: half the bytes back over PCIe)
-        for name, extra, nbytes in (("streamed", {}, N), ("streamed_packed", {"out_bits": 4}, (N + 1) // 2)):
+        def streamed(extra: dict, nbytes: int, check: bool) -> float:
             so = dict(plan_opts, out_is_host_pinned=1, max_batch_suffixes=N // 4 + N // 64, **extra)
             sp = cx.Plan(n_reads, total, profile=0, **so)
             h_res = h_out[:nbytes]
 
-            def step_streamed(sp=sp, h_res=h_res):
+            def step():
                 cx.pack_reads_from_host(h_ascii, d_ascii, d_packed, stream=stream)
                 d_off.copy_(h_off, non_blocking=True)
                 sp.build(d_packed, d_off, n_reads, h_res)       # returns when the last batch has been copied to the host
-            e2e_variants[name] = time_e2e(step_streamed)
-            if name == "streamed":                               # the streamed result must be the same bytes
+            ms = time_e2e(step)
+            if check:                                            # the streamed result must be the same bytes
                 got = torch.bincount(h_res.to(dev).to(torch.int64), minlength=256)
                 if not torch.equal(got, want_counts):
                     raise SystemExit("bench.py: streamed output symbol counts differ from the input's")
             sp.free()
-            del sp
+            return ms
+        e2e_variants["streamed"] = streamed({}, N, True)
+        e2e_variants["streamed_packed"] = streamed({"out_bits": 4}, (N + 1) // 2, False)
     e2e_name = min((k for k in e2e_variants if k != "streamed_packed"), key=lambda k: e2e_variants[k])
     e2e_ms = e2e_variants[e2e_name]
 
@@ -657,7 +661,11 @@ def run_cx(args) -> None:
                          "(abstract: 'BRC ... 12 hours'); other hardware, context only",
     }
     # release everything of the main workload before the larger configurations
-    del d_ascii, d_off, d_packed, d_out, h_ascii, h_off, h_out, flush
+    del d_ascii, d_off, d_packed, d_out, h_ascii, h_off, h_out, flush, want_counts
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+    line["config"]["hbm_free_gb_before_other_configs"] = round(torch.cuda.mem_get_info(dev)[0] / (1 << 30), 1)
     if world == 1 and not args.no_other_configs and args.scale == 1.0 and not args.table4 and not one_shard:
         others = []
         for idx in ([0, 1] if args.all_configs else []) + [3, 4]:

@@ -5,7 +5,7 @@ reads, gets "a contiguous range of partitions" of about equal total size, sorts 
 pieces can be sent back to the master node" where they are "simply concatenated".  Here every
 rank computes the same partition sizes redundantly (one scan, cheaper than a broadcast round trip), a plan made with
 shard_index / shard_count sorts only its range and writes it at its final position of the output, and the single
-exchange step is an all-gather-v of the pieces over torch.distributed (NCCL on GPUs, gloo on CPU tensors in
+exchange step is an all-gather of the (padded) pieces over torch.distributed (NCCL on GPUs, gloo on CPU tensors in
 the tests).  Argument marshalling and the collective only: all arithmetic of the method stays in libcxbwt.so.
 """
 from __future__ import annotations
@@ -38,16 +38,27 @@ def exchange_pieces(out: torch.Tensor, offset: int, count: int, group=None) -> l
     """All-gather-v of the BWT pieces, in place: on return every rank holds the whole of `out`.
 
     out[offset : offset + count] is this rank's piece (cx_bwt_stats_t.shard_offset / shard_suffixes).  Pieces have
-    different lengths, so each one travels as a broadcast from its owner into the same slice of every rank's buffer
-    (bandwidth-trivial next to the sort: N bytes in total)."""
+    different lengths (partition ranges are equal only roughly), so every rank sends its piece padded to the
+    longest one in ONE all_gather_into_tensor and copies the others' pieces from the gathered rows to their places --
+    N bytes in total (plus padding), bandwidth-trivial next to the sort."""
     if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size(group) == 1:
         check_pieces([(offset, count)], out.numel())
         return [(offset, count)]
+    world = dist.get_world_size(group)
+    me = dist.get_rank(group)
     pieces = piece_table(offset, count, out.device, group)
     check_pieces(pieces, out.numel())
+    longest = max(c for _, c in pieces)
+    if longest == 0:
+        return pieces
+    send = torch.zeros(longest, dtype=out.dtype, device=out.device)
+    if count:
+        send[:count] = out[offset:offset + count]
+    rows = torch.empty(world * longest, dtype=out.dtype, device=out.device)
+    dist.all_gather_into_tensor(rows, send, group=group)
     for r, (o, c) in enumerate(pieces):
-        if c:
-            dist.broadcast(out[o:o + c], src=dist.get_global_rank(group, r) if group is not None else r, group=group)
+        if c and r != me:
+            out[o:o + c] = rows[r * longest: r * longest + c]
     return pieces
 
 

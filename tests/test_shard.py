@@ -126,6 +126,38 @@ def test_exchange_pieces_two_gloo_ranks():
         assert ok and refused and pieces == [(0, 377), (377, 623)]
 
 
+def _worker3(rank, world, port, q):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import sys
+    sys.path.insert(0, ROOT)
+    from paper_1401_7457_b200 import shard
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    full = (torch.arange(5003, dtype=torch.int64) * 13 % 241).to(torch.uint8)
+    cuts = [0, 4000, 4000, 5003]                            # a long piece, an EMPTY one, a short one: padding and skipping
+    out = torch.full((5003,), 255, dtype=torch.uint8)
+    lo, hi = cuts[rank], cuts[rank + 1]
+    out[lo:hi] = full[lo:hi]
+    pieces = shard.exchange_pieces(out, lo, hi - lo)
+    dist.barrier()
+    dist.destroy_process_group()
+    q.put((rank, bool(torch.equal(out, full)), pieces))
+
+
+def test_exchange_pieces_three_gloo_ranks_one_empty_piece():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 35500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_worker3, args=(r, 3, port, q)) for r in range(3)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    for rank, ok, pieces in res:
+        assert ok and pieces == [(0, 4000), (4000, 0), (4000, 1003)]
+
+
 def test_check_pieces():
     from paper_1401_7457_b200 import shard
     shard.check_pieces([(0, 5), (5, 0), (5, 7)], 12)
