@@ -45,9 +45,12 @@ enum {
 /* Parameters of Figure 2 plus the knobs of this implementation.  Zero = default. */
 typedef struct cx_bwt_opts_s {
     uint32_t prefix_len;         /* l: partition prefix length in bases, 1..7; default 6        */
-    uint32_t key_bases;          /* w: bases in the first-round sort key, l..29 ("stringword").  w <= 14
-                                    packs into a 32-bit key (4 radix passes), larger w into a 64-bit key.
-                                    0 = 14 up to 2^30 suffixes in the collection, else ceil(log4 N) + 1       */
+    uint32_t key_bases;          /* w: bases in the first-round sort key, l..29 ("stringword").  The key is
+                                    the rank of the window's symbols among all strings of at most w bases plus one
+                                    bit, about 2 w + 1.5 bits: w <= 15 packs into a 32-bit key (4 radix passes), larger
+                                    w into a 64-bit key.  0 = 15 up to 2^30 suffixes in the collection, else what the
+                                    radix passes that ceil(log4 N) bases need can carry (19 bases, 5 passes, at
+                                    6e9 .. 1e11 suffixes)                                                       */
     uint64_t max_batch_suffixes; /* m1: most suffixes sorted in one GPU batch;
                                     0 = as many as the workspace allows                                       */
     uint32_t max_read_len;       /* longest read the plan must accept; 0 = unknown (forces 64-bit suffix ids

@@ -202,16 +202,18 @@ extern "C" int cx_bwt_plan(cx_bwt_plan_t** plan_out, uint64_t max_reads, uint64_
     CX_CUDA(cudaDeviceGetAttribute(&n_sms, cudaDevAttrMultiProcessorCount, dev));
 
     // First-round window ("stringword"): wide enough that 4^w exceeds the number of suffixes of the
-    // whole collection, so that random collisions are rare and tie groups are the genuinely shared substrings.
-    // 14 bases + a 4-bit length is the most a 32-bit key holds: half the bytes per radix pass and 4 passes; it
-    // still wins at 1e9 suffixes (C3: 86 ms against 115 ms with w = 29).  Beyond 2^30 suffixes the key is
-    // 64-bit with w = ceil(log4 N) + 1 bases (6 passes at 6e9 .. 1e11 suffixes instead of 8).
+    // whole collection, so that random collisions are rare and tie groups are the genuinely shared substrings.  The key
+    // (first_key: rank of the window's symbols + a "has w bases" bit) takes 32 bits at w = 15 -- half the bytes per
+    // radix pass and 4 passes -- which is used up to 2^30 suffixes.  Beyond that the key is 64-bit with as many bases
+    // as the passes that ceil(log4 N) bases need anyway can carry (19 bases in 40 bits, 5 passes, at 6e9 .. 1e11 suffixes).
     if (sh.w == 0) {
         if (sh.max_suffixes <= (1ull << 30)) {
-            sh.w = 14;
+            sh.w = 15;
         } else {
-            uint32_t log4 = (bit_width64(sh.max_suffixes - 1) + 1) / 2;
-            sh.w = log4 + 1 > 29 ? 29 : log4 + 1;
+            const uint32_t log4 = (bit_width64(sh.max_suffixes - 1) + 1) / 2;
+            const uint32_t passes = (first_key_bits(log4) + kRadixBits - 1) / kRadixBits;
+            sh.w = log4;
+            while (sh.w < 29 && (first_key_bits(sh.w + 1) + kRadixBits - 1) / kRadixBits == passes) ++sh.w;
         }
     }
     if (sh.w < sh.ell) sh.w = sh.ell;
@@ -507,7 +509,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     // scan then counts them on the way (one read of the collection instead of two).
     const bool fused_scan = sh.max_suffixes <= p->m1 && !sh.sharded();
     const uint32_t w = sh.w;
-    const uint32_t key_bits = 2 * w + key_len_bits(w);
+    const uint32_t key_bits = first_key_bits(w);
     const uint32_t n_passes = (key_bits + kRadixBits - 1) / kRadixBits;
     KeyT* d_keys1[2] = {reinterpret_cast<KeyT*>(d_keys[0]), reinterpret_cast<KeyT*>(d_keys[1])};   // first-round keys
     // 32-bit key and 32-bit id: one 64-bit word per suffix (key << 32 | id), sorted keys-only over its upper half
@@ -746,7 +748,7 @@ extern "C" int cx_bwt_build(cx_bwt_plan_t* p, const uint64_t* packed_reads, cons
     if (n_reads == 0) return CX_OK;
     if (!read_offsets || !out_bwt || n_reads > p->sh.max_reads) return CX_ERR_ARG;
     if (!packed_reads && p->sh.max_bases) return CX_ERR_ARG;
-    const bool key32 = 2 * p->sh.w + key_len_bits(p->sh.w) <= 32;
+    const bool key32 = first_key_bits(p->sh.w) <= 32;
     if (p->sh.id_bytes == 4)
         return key32 ? build_impl<uint32_t, uint32_t>(p, packed_reads, read_offsets, n_reads, out_bwt, stream)
                      : build_impl<uint64_t, uint32_t>(p, packed_reads, read_offsets, n_reads, out_bwt, stream);

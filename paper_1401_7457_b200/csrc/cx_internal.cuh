@@ -102,10 +102,44 @@ __device__ __forceinline__ uint64_t load_window(const uint64_t* __restrict__ pac
     return (w0 << sh) | (w1 >> (64 - sh));
 }
 
-// Order-preserving key of a window (reading A3 of PAPER.md:99):
-// the first min(rem, w) bases, A-padded to w bases, then min(rem, w) in the low len_bits bits
-// (len_bits = bit width of w: 5 for w = 29, 4 for w = 14).  A value < w in the length field means
-// the end-marker falls inside this window.
+// Order-preserving keys of a window of w bases (reading A3 of PAPER.md:99).
+//
+// first_key (the first sort of a batch): the RANK of the suffix's first min(rem, w) symbols, end-marker included if it falls
+// inside the window, among all strings of at most w bases over $ < A < C < G < T -- then one bit: 1 = the suffix has at least
+// w bases.  With T(k) = (4^(w-k+1) - 1) / 3 strings below a node at depth k of that trie, the rank of c_0 .. c_(r-1) is
+// sum_i (1 + c_i T(i+1)) = r + (4 B - S) / 3, B = the bases as a 2w-bit number (A-padded), S = the sum of their codes
+// (4^k = 1 mod 3 makes the division exact).  Different strings get different keys in their true order; equal keys with the
+// bit clear are IDENTICAL strings (final at once), equal keys with the bit set share their first w bases.
+// The rank is below 4^(w+1) / 3: 15 bases and the bit fill a 32-bit key, 19 bases a 40-bit one (five 8-bit radix passes).
+//
+// make_key (the global path's re-keying): the bases, A-padded, then min(rem, w) in the low len_bits bits; a value < w in that
+// field means the end-marker falls inside this window, and equal keys then mean identical strings.
+__host__ __device__ __forceinline__ uint32_t first_key_bits(uint32_t w) {
+    uint32_t bits = 0;
+    for (uint64_t top = ((1ull << (2 * w + 2)) - 4) / 3; top; top >>= 1) ++bits;   // the largest rank, (4^(w+1) - 4) / 3
+    return bits + 1;
+}
+__device__ __forceinline__ uint64_t first_key(uint64_t window, uint64_t rem, uint32_t w) {
+    const uint32_t r = rem < (uint64_t)w ? (uint32_t)rem : w;
+    const uint64_t B = r ? ((window >> (64 - 2 * r)) << (2 * (w - r))) : 0ull;
+    const uint64_t S = (uint64_t)__popcll((long long)(B & 0x5555555555555555ull)) + 2ull * (uint64_t)__popcll((long long)(B & 0xAAAAAAAAAAAAAAAAull));
+    const uint64_t rank = r + (4 * B - S) * 0xAAAAAAAAAAAAAAABull;   // exact division by 3 (the multiplier is 3^-1 mod 2^64)
+    return (rank << 1) | (uint64_t)(r == w);
+}
+// the same for w <= 15 in 32-bit arithmetic (the listing scans are bound by instruction issue); window = the next 32 bases
+__device__ __forceinline__ uint32_t first_key32(uint64_t window, uint32_t rem, uint32_t w) {
+    const uint32_t r = rem < w ? rem : w;
+    const uint32_t top = (uint32_t)(window >> 34);                       // the first 15 bases, right-aligned
+    const uint32_t B = r ? (top >> (30 - 2 * r)) << (2 * (w - r)) : 0u;
+    const uint32_t S = (uint32_t)__popc(B & 0x55555555u) + 2u * (uint32_t)__popc(B & 0xAAAAAAAAu);
+    const uint32_t rank = r + (4u * B - S) * 0xAAAAAAABu;                // exact division by 3 (3^-1 mod 2^32); 4 B < 2^32 for w <= 15
+    return (rank << 1) | (uint32_t)(r == w);
+}
+template <typename KeyT>
+__device__ __forceinline__ KeyT first_key_as(uint64_t window, uint64_t rem, uint32_t w) {
+    if constexpr (sizeof(KeyT) == 4) return first_key32(window, (uint32_t)(rem < 64 ? rem : 64), w);
+    else return first_key(window, rem, w);
+}
 __host__ __device__ __forceinline__ uint32_t key_len_bits(uint32_t w) { return w >= 16 ? 5u : w >= 8 ? 4u : w >= 4 ? 3u : w >= 2 ? 2u : 1u; }
 __device__ __forceinline__ uint64_t make_key(uint64_t window, uint64_t rem, uint32_t w, uint32_t len_bits = 5) {
     uint32_t r = rem < (uint64_t)w ? (uint32_t)rem : w;

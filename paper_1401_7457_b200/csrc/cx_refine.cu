@@ -376,11 +376,11 @@ __device__ __forceinline__ void finish_tile(LocalSmem& sm, uint64_t tile, const 
                     const uint64_t* pairs = reinterpret_cast<const uint64_t*>(keys1);
                     const uint64_t pc = __ldcs(pairs + j);
                     const uint32_t kc = (uint32_t)(pc >> 32);
-                    head = j == 0 || kc != (uint32_t)(__ldg(pairs + j - 1) >> 32) || (kc & len_mask) < w1;
+                    head = j == 0 || kc != (uint32_t)(__ldg(pairs + j - 1) >> 32) || !(kc & 1u);
                     sm.loc[e] = (uint32_t)pc;
                 } else {
                     const KeyT kc = __ldcs(keys1 + j);
-                    head = j == 0 || kc != __ldg(keys1 + j - 1) || ((uint32_t)kc & len_mask) < w1;
+                    head = j == 0 || kc != __ldg(keys1 + j - 1) || !((uint32_t)kc & 1u);
                     sm.loc[e] = (uint64_t)__ldcs(ids + j);
                 }
             }
@@ -835,7 +835,7 @@ __device__ __forceinline__ uint64_t scan_to_head(const KeyT* __restrict__ keys1,
         const uint64_t k = j < n ? key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j)) : 0ull;
         uint64_t kp = __shfl_up_sync(kFull, k, 1);
         if (lane == 0) kp = carry;
-        const bool head = j >= n || k != kp || ((uint32_t)k & len_mask) < w1;
+        const bool head = j >= n || k != kp || !((uint32_t)k & 1u);
         const uint32_t m = __ballot_sync(kFull, head);
         if (m) return p + (uint32_t)__ffs(m) - 1;
         carry = __shfl_sync(kFull, k, 31);
@@ -939,7 +939,7 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : 3) finish_warp_kern
                 } else if (lane == 31) {
                     kn = valid_next ? key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j + 1)) : 0ull;
                 }
-                const bool head_next = !valid_next || kn != k[s] || ((uint32_t)kn & len_mask) < w1;
+                const bool head_next = !valid_next || kn != k[s] || !((uint32_t)kn & 1u);
                 const uint32_t HN = __ballot_sync(kFull, head_next);
                 hw[s] = (HN << 1) | carry_in;
                 carry_in = HN >> 31;
@@ -1290,7 +1290,7 @@ __global__ void __launch_bounds__(256) group_probe_kernel(const KeyT* __restrict
         bool head = true;
         if (j < n && e > 0) {
             const uint64_t kc = key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j)), kp = key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j - 1));
-            head = kc != kp || ((uint32_t)kc & len_mask) < w1;
+            head = kc != kp || !((uint32_t)kc & 1u);
         }
         const uint32_t word = __ballot_sync(kFull, head);
         if ((threadIdx.x & 31) == 0) s_heads[e >> 5] = word;
@@ -1359,7 +1359,7 @@ cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, 
     if (packed && !kCanPack) return cudaErrorInvalidValue;
     if (slots != (uint32_t)kWarpSlotsSmall && slots != (uint32_t)kWarpSlotsLarge) return cudaErrorInvalidValue;
     if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
-    const uint32_t len_mask = (1u << key_len_bits(w1)) - 1;
+    const uint32_t len_mask = 0;   // (unused: a first-round key says in its lowest bit whether its suffix has w1 bases)
     const uint64_t tiles = (n + kLocalTile - 1) / kLocalTile;
     cudaError_t e = cudaMemsetAsync(big_tiles, 0, ((tiles + 31) / 32 + 1) * sizeof(uint32_t), s);
     if (e != cudaSuccess) return e;
@@ -1397,7 +1397,7 @@ cudaError_t launch_group_probe(const KeyT* keys1, uint32_t w1, uint64_t n, bool 
     if (n < (uint64_t)kProbeSpan * 2) return cudaSuccess;
     const unsigned blocks = (unsigned)(n / kProbeSpan < (uint64_t)kProbeBlocks ? n / kProbeSpan : (uint64_t)kProbeBlocks);
     *sampled = (uint64_t)blocks * kProbeSpan;
-    const uint32_t len_mask = (1u << key_len_bits(w1)) - 1;
+    const uint32_t len_mask = 0;   // (unused: a first-round key says in its lowest bit whether its suffix has w1 bases)
     if (packed) group_probe_kernel<KeyT, kCanPack><<<blocks, 256, 0, s>>>(keys1, n, w1, len_mask, 32u * kWarpSlotsSmall, counter);
     else group_probe_kernel<KeyT, false><<<blocks, 256, 0, s>>>(keys1, n, w1, len_mask, 32u * kWarpSlotsSmall, counter);
     return cudaGetLastError();

@@ -393,7 +393,6 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
     R.n_words = (info->total_bases + 31) >> 5;
     const uint64_t N = info->n_suffixes;
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
-    const uint32_t len_bits = key_len_bits(w);
     const uint32_t warp = threadIdx.x >> 5;
     if (info->bad_offsets) return;
     for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) (&s_dh[0][0])[i] = 0;
@@ -453,7 +452,7 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
                     sl.window = load_window(R.packed, R.n_words, sl.b + region.depth);
                     sl.rem -= region.depth;
                 }
-                const KeyT key = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
+                const KeyT key = first_key_as<KeyT>(sl.window, sl.rem, w);
                 const IdT id = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
                 digit_counts(s_dh, key, n_passes);
                 const uint64_t at = dst - ord_lo;
@@ -497,7 +496,6 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
     const uint64_t N = info->n_suffixes;
     if (N > max_n || info->bad_offsets) return;   // the host reports both after reading `info`
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
-    const uint32_t len_bits = key_len_bits(w);
     for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) (&s_dh[0][0])[i] = 0;
 
     for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
@@ -514,7 +512,7 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
                 if (r == ell) atomicAdd(&s_bh[kmer], 1u);
                 else atomicAdd(&s_bh[n_kmers + (((1u << (2 * r)) - 1) / 3) + (kmer >> (2 * (ell - r)))], 1u);
             }
-            const KeyT key = (KeyT)make_key(sl.window, sl.rem, w, len_bits);
+            const KeyT key = first_key_as<KeyT>(sl.window, sl.rem, w);
             const IdT id = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
             digit_counts(s_dh, key, n_passes);
             if constexpr (PACKED) {
@@ -681,7 +679,6 @@ __global__ void __launch_bounds__(kListThreads) list_select_uniform_kernel(Reads
     R.n_words = (info->total_bases + 31) >> 5;
     const uint64_t N = info->n_suffixes;
     const uint64_t n_tiles = (N + kBigTile - 1) / kBigTile;
-    const uint32_t len_bits = key_len_bits(w);
     const uint32_t warp = threadIdx.x >> 5;
     if (info->bad_offsets) return;
     for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) (&s_dh[0][0])[i] = 0;
@@ -722,7 +719,7 @@ __global__ void __launch_bounds__(kListThreads) list_select_uniform_kernel(Reads
             if (dst >= ord_lo && dst < ord_hi) {
                 uint32_t rr, pos, brel;
                 big_decode(c, s_taken[j], rr, pos, brel);
-                const KeyT key = (KeyT)make_key(big_window(sm, brel), (uint64_t)(c.L1 - 1 - pos), w, len_bits);
+                const KeyT key = first_key_as<KeyT>(big_window(sm, brel), (uint64_t)(c.L1 - 1 - pos), w);
                 const IdT id = make_id<IdT>(c.r0 + rr, pos, R.pos_bits);
                 digit_counts(s_dh, key, n_passes);
                 const uint64_t at = dst - ord_lo;
