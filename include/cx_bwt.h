@@ -220,6 +220,24 @@ int cx_sort_pairs(uint64_t *keys, void *vals, uint64_t *keys_alt, void *vals_alt
                   uint32_t val_bytes, uint32_t begin_bit, uint32_t end_bit, void *workspace_dev,
                   uint64_t workspace_bytes, int *result_in_alt, cx_stream_t stream);
 
+/*
+ * cx_sort_pairs for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the same stable LSD radix sort (step a6), but its scratch (digit histograms, look-back tile states, ticket)
+ * lives in a file-scope `static __device__` array of the library instead of a caller-supplied workspace.  The call makes no
+ * cudaMalloc / cudaFree and uses no allocating library routine; the caller still passes inputs and outputs.
+ *   n <= CX_SORT_STATIC_MAX_PAIRS (1,048,576 pairs; the array is cx_sort_pairs_workspace_bytes of that: about 0.86 MB, held
+ *   by every GPU that loads the library until the process exits); larger n returns CX_ERR_ARG (text via cx_strerror_static).
+ *   The array is resolved once per device on the first call there (cudaGetSymbolAddress with that device current), cleared
+ *   on `stream` at the start of every call (it keeps the last call's contents) and SHARED by all calls: two calls whose GPU
+ *   work overlaps (different streams, threads or processes on one context) race -- serialise them.
+ * Other arguments and results as cx_sort_pairs.
+ */
+#define CX_SORT_STATIC_MAX_PAIRS 1048576ull
+int cx_sort_pairs_static(uint64_t *keys, void *vals, uint64_t *keys_alt, void *vals_alt, uint64_t n, uint32_t val_bytes,
+                         uint32_t begin_bit, uint32_t end_bit, int *result_in_alt, cx_stream_t stream);
+/* Text of the last error cx_sort_pairs_static returned on this thread (which limit was exceeded, or the CUDA error). */
+const char *cx_strerror_static(void);
+
 /* Text for an error code; for CX_ERR_CUDA the text of the last CUDA error seen by this thread. */
 const char *cx_strerror(int code);
 

@@ -64,6 +64,10 @@ def lib() -> ctypes.CDLL:
         L.cx_sort_pairs.argtypes = [vp, vp, vp, vp, u64, u32, u32, u32, vp, u64, ctypes.POINTER(i32), vp]
         L.cx_fasta_workspace_bytes.argtypes = [u64, ctypes.POINTER(u64)]
         L.cx_fasta_parse.argtypes = [vp, u64, vp, vp, u64, vp, vp, u64, vp]
+        L.cx_sort_pairs_static.argtypes = [vp, vp, vp, vp, u64, u32, u32, u32, ctypes.POINTER(i32), vp]
+        L.cx_sort_pairs_static.restype = i32
+        L.cx_strerror_static.argtypes = []
+        L.cx_strerror_static.restype = ctypes.c_char_p
         L.cx_strerror.argtypes = [i32]
         L.cx_strerror.restype = ctypes.c_char_p
         for name in ("cx_bwt_workspace_bytes", "cx_bwt_plan", "cx_pack_reads", "cx_bwt_build", "cx_bwt_free", "cx_bwt_get_stats",
@@ -233,6 +237,25 @@ def cx_sort_pairs(keys: torch.Tensor, vals: torch.Tensor, begin_bit: int = 0, en
     _check(lib().cx_sort_pairs(k0.data_ptr(), v0.data_ptr(), k1.data_ptr(), v1.data_ptr(), n, vals.element_size(), begin_bit,
                                end_bit, ws.data_ptr(), int(wsb.value), ctypes.byref(alt), _stream_ptr(stream)))
     return (k1, v1) if alt.value else (k0, v0)
+
+
+CX_SORT_STATIC_MAX_PAIRS = 1 << 20
+
+
+def cx_sort_pairs_static(keys: torch.Tensor, vals: torch.Tensor, keys_alt: torch.Tensor, vals_alt: torch.Tensor, begin_bit: int = 0,
+                         end_bit: int = 64, stream=None):
+    """cx_sort_pairs_static: sorts in place over the caller's double buffers (keys/vals are overwritten); the library's static
+    device scratch serves as workspace, so nothing is allocated here or in the library.  Returns the pair of tensors that holds
+    the result.  n <= CX_SORT_STATIC_MAX_PAIRS, else CxError(CX_ERR_ARG)."""
+    assert keys.is_cuda and keys.dtype == torch.int64 and vals.dtype in (torch.int32, torch.int64)
+    assert keys_alt.shape == keys.shape and vals_alt.shape == vals.shape and keys_alt.dtype == keys.dtype and vals_alt.dtype == vals.dtype
+    alt = ctypes.c_int(0)
+    with torch.cuda.device(keys.device):
+        rc = lib().cx_sort_pairs_static(keys.data_ptr(), vals.data_ptr(), keys_alt.data_ptr(), vals_alt.data_ptr(), keys.numel(), vals.element_size(),
+                                        begin_bit, end_bit, ctypes.byref(alt), _stream_ptr(stream))
+    if rc != CX_OK:
+        raise CxError(rc, lib().cx_strerror_static().decode())
+    return (keys_alt, vals_alt) if alt.value else (keys, vals)
 
 
 def cx_fasta_parse(text_dev: torch.Tensor, max_reads: int | None = None, stream=None):

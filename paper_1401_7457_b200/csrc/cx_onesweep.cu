@@ -9,6 +9,8 @@
 // pairs are staged in shared memory in digit order and leave as runs of consecutive addresses.
 //
 // Algorithmic traffic per pass: 2 * (8 + sizeof(id)) bytes per pair; histogram kernel: 8 bytes per pair.
+#include <stdio.h>
+
 #include "cx_internal.cuh"
 #include "cx_launch.h"
 
@@ -384,6 +386,89 @@ cudaError_t sort_pairs(KeyT* keys, ValT* vals, KeyT* keys_alt, ValT* vals_alt, u
         return sort_pairs_shape<KeyT, ValT, 384, 16, 3>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready, pass_class);
     return sort_pairs_shape<KeyT, ValT, kSortThreads, ITEMS, 4>(keys, vals, keys_alt, vals_alt, n, begin_bit, end_bit, ws, result_in_alt, prof, s, hist_ready, pass_class);
 }
+
+// ---------------------------------------------------------------------------------------------
+// cx_sort_pairs_static: the sorter with its scratch in a file-scope device array (no allocation anywhere on the call)
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+constexpr uint64_t kStaticMaxPairs = CX_SORT_STATIC_MAX_PAIRS;
+constexpr size_t kStaticTiles = (size_t)((kStaticMaxPairs + kSortTileMin - 1) / kSortTileMin + 1);
+constexpr size_t kStaticBytes = 8 * kRadix * sizeof(uint64_t) + kStaticTiles * kRadix * sizeof(uint64_t) + 256;   // = sort_workspace_bytes(max)
+
+// Digit histograms, tile states and the ticket of one sort of up to kStaticMaxPairs pairs.  In HOST code this name is a
+// host-side stand-in, not a device address: the address comes from cudaGetSymbolAddress (static_scratch below).
+static __device__ __align__(256) unsigned char g_sort_scratch[kStaticBytes];
+
+constexpr int kMaxDevices = 64;
+void* g_scratch_of_device[kMaxDevices] = {};   // resolved once per device, with that device current
+thread_local char g_static_msg[192] = "no error";
+
+// device address of the array on the CURRENT device (nullptr + message on failure)
+void* static_scratch() {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess || dev < 0 || dev >= kMaxDevices) {
+        snprintf(g_static_msg, sizeof(g_static_msg), "cx_sort_pairs_static: no current CUDA device (%s)", e != cudaSuccess ? cudaGetErrorString(e) : "index out of range");
+        return nullptr;
+    }
+    void* p = __atomic_load_n(&g_scratch_of_device[dev], __ATOMIC_ACQUIRE);
+    if (p) return p;
+    e = cudaGetSymbolAddress(&p, g_sort_scratch);
+    if (e != cudaSuccess || !p) {
+        snprintf(g_static_msg, sizeof(g_static_msg), "cx_sort_pairs_static: cudaGetSymbolAddress failed on device %d: %s", dev, cudaGetErrorString(e));
+        cudaGetLastError();
+        return nullptr;
+    }
+    __atomic_store_n(&g_scratch_of_device[dev], p, __ATOMIC_RELEASE);   // (two threads may both resolve it: same value)
+    return p;
+}
+
+}  // namespace
+}  // namespace cx
+
+extern "C" const char* cx_strerror_static(void) { return cx::g_static_msg; }
+
+extern "C" int cx_sort_pairs_static(uint64_t* keys, void* vals, uint64_t* keys_alt, void* vals_alt, uint64_t n, uint32_t val_bytes,
+                                    uint32_t begin_bit, uint32_t end_bit, int* result_in_alt, cx_stream_t stream) {
+    using namespace cx;
+    if (!result_in_alt || (val_bytes != 4 && val_bytes != 8) || begin_bit > end_bit || end_bit > 64) {
+        snprintf(g_static_msg, sizeof(g_static_msg), "cx_sort_pairs_static: bad argument (result_in_alt, val_bytes 4 or 8, begin_bit <= end_bit <= 64)");
+        return CX_ERR_ARG;
+    }
+    *result_in_alt = 0;
+    if (n > kStaticMaxPairs) {
+        snprintf(g_static_msg, sizeof(g_static_msg), "cx_sort_pairs_static: n = %llu exceeds CX_SORT_STATIC_MAX_PAIRS = %llu (the static scratch is sized for that; use cx_sort_pairs)",
+                 (unsigned long long)n, (unsigned long long)kStaticMaxPairs);
+        return CX_ERR_ARG;
+    }
+    if (n == 0) return CX_OK;
+    if (!keys || !vals || !keys_alt || !vals_alt) {
+        snprintf(g_static_msg, sizeof(g_static_msg), "cx_sort_pairs_static: null buffer");
+        return CX_ERR_ARG;
+    }
+    void* scratch = static_scratch();
+    if (!scratch) return CX_ERR_CUDA;
+    // the array keeps the last call's contents: tile states and the ticket must start from zero
+    const size_t bytes = sort_workspace_bytes(n);   // <= kStaticBytes
+    cudaError_t e = cudaMemsetAsync(scratch, 0, bytes, stream);
+    SortWorkspace ws;
+    sort_workspace_carve(ws, scratch, n);
+    if (e == cudaSuccess) {
+        if (val_bytes == 4)
+            e = sort_pairs<uint64_t, uint32_t>(keys, (uint32_t*)vals, keys_alt, (uint32_t*)vals_alt, n, begin_bit, end_bit, ws, result_in_alt, nullptr, stream);
+        else
+            e = sort_pairs<uint64_t, uint64_t>(keys, (uint64_t*)vals, keys_alt, (uint64_t*)vals_alt, n, begin_bit, end_bit, ws, result_in_alt, nullptr, stream);
+    }
+    if (e != cudaSuccess) {
+        snprintf(g_static_msg, sizeof(g_static_msg), "cx_sort_pairs_static: CUDA error %d: %s", (int)e, cudaGetErrorString(e));
+        cudaGetLastError();
+        return CX_ERR_CUDA;
+    }
+    return CX_OK;
+}
+
+namespace cx {
 
 #define CX_SORT_INST(K, V)                                                                                               \
     template cudaError_t sort_pairs<K, V>(K*, V*, K*, V*, uint64_t, uint32_t, uint32_t, SortWorkspace&, int*, Launch*, cudaStream_t, bool, int);
