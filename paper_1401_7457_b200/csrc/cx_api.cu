@@ -654,6 +654,8 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         CX_CUDA(cudaMemcpyAsync(p->h_scalars, d_scalars, 48, cudaMemcpyDeviceToHost, s));
         CX_CUDA(cudaStreamSynchronize(s));
         const bool any_oversize = p->h_scalars[5] != over_before;
+        // every suffix refined here also costs its id read, an 8-byte window gathered and its id written
+        prof->bytes[CX_K_FINISH] += (p->h_scalars[1] - local_before) * (2 * sizeof(IdT) + 8);
         // ---- what is still tied goes through global rounds: re-key, sort, write back ------------------
         uint32_t depth = depth_base + w, rounds = 0;
         while (any_oversize) {

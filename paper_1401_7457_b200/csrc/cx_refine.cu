@@ -354,7 +354,7 @@ __device__ __forceinline__ int merge_levels(int s, int t) {
 }
 
 template <typename KeyT, typename IdT, bool FIRST, bool PACKED>
-__device__ __forceinline__ void finish_tile(LocalSmem& sm, uint64_t tile, const Reads& R, const KeyT* __restrict__ keys1, uint32_t w1, uint32_t len_mask,
+__device__ __forceinline__ void finish_tile(LocalSmem& sm, uint64_t tile, const Reads& R, const KeyT* __restrict__ keys1,
                                             const uint32_t* __restrict__ heads_in, uint32_t* __restrict__ heads, const IdT* __restrict__ ids,
                                             uint64_t n, uint32_t depth0, uint32_t min_group, uint32_t cap, uint8_t* __restrict__ out,
                                             unsigned long long* elems_done) {
@@ -715,7 +715,7 @@ __device__ __forceinline__ void finish_tile(LocalSmem& sm, uint64_t tile, const 
 
 // Persistent blocks over the tiles.  FIRST: only tiles in which the warp kernel met a group of 33..cap members (big_tiles bit).
 template <typename KeyT, typename IdT, bool FIRST, bool PACKED>
-__global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_kernel(Reads R, const KeyT* __restrict__ keys1, uint32_t w1, uint32_t len_mask,
+__global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_kernel(Reads R, const KeyT* __restrict__ keys1,
                                                                     const uint32_t* __restrict__ heads_in, uint32_t* __restrict__ heads,
                                                                     const IdT* __restrict__ ids, uint64_t n, uint32_t depth0, uint32_t min_group,
                                                                     uint32_t cap, const uint32_t* __restrict__ big_tiles, uint8_t* __restrict__ out,
@@ -725,7 +725,7 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
     const uint64_t n_tiles = (n + kLocalTile - 1) / kLocalTile;
     for (uint64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         if (FIRST && !((__ldg(big_tiles + (tile >> 5)) >> (tile & 31)) & 1u)) continue;
-        finish_tile<KeyT, IdT, FIRST, PACKED>(sm, tile, R, keys1, w1, len_mask, heads_in, heads, ids, n, depth0, min_group, cap, out, elems_done);
+        finish_tile<KeyT, IdT, FIRST, PACKED>(sm, tile, R, keys1, heads_in, heads, ids, n, depth0, min_group, cap, out, elems_done);
         __syncthreads();   // the next tile reuses the shared memory
     }
 }
@@ -827,7 +827,7 @@ __device__ __forceinline__ uint64_t key_of(uint64_t word) { return PACKED ? word
 
 // first head at or after position p >= 1 (position n counts as one): a head starts a tie group
 template <typename KeyT, bool PACKED>
-__device__ __forceinline__ uint64_t scan_to_head(const KeyT* __restrict__ keys1, uint64_t p, uint64_t n, uint32_t w1, uint32_t len_mask) {
+__device__ __forceinline__ uint64_t scan_to_head(const KeyT* __restrict__ keys1, uint64_t p, uint64_t n) {
     const uint32_t lane = lane_id();
     uint64_t carry = key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, p - 1));
     while (true) {
@@ -898,8 +898,7 @@ __device__ __forceinline__ void window_words(const uint64_t* __restrict__ packed
 
 template <typename KeyT, typename IdT, bool PACKED, int S>
 __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : 3) finish_warp_kernel(Reads R, const KeyT* __restrict__ keys1, const IdT* __restrict__ ids_in,
-                                                                   IdT* __restrict__ ids_out, uint32_t w1, uint32_t len_mask, uint64_t n,
-                                                                   uint32_t depth0, uint32_t cap, uint32_t* __restrict__ heads,
+                                                                   IdT* __restrict__ ids_out, uint64_t n, uint32_t depth0, uint32_t cap, uint32_t* __restrict__ heads,
                                                                    uint32_t* __restrict__ big_tiles, uint8_t* __restrict__ out,
                                                                    unsigned long long* counters) {
     constexpr uint32_t kSpan = 32 * S;                  // positions per window
@@ -914,7 +913,7 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : 3) finish_warp_kern
     const uint64_t pos_mask = (1ull << R.pos_bits) - 1;
     uint32_t n_members = 0, n_sorts = 0, n_over = 0;     // lane 0's tallies
     uint64_t a = c0;
-    if (c0 < n && c0 > 0) a = scan_to_head<KeyT, PACKED>(keys1, c0, n, w1, len_mask);   // groups that began before the chunk are the previous warp's
+    if (c0 < n && c0 > 0) a = scan_to_head<KeyT, PACKED>(keys1, c0, n);   // groups that began before the chunk are the previous warp's
     while (a < c1) {
         // ---- the window [a, a + 32 S): a is a head --------------------------------------------------------------
         uint64_t word[S];
@@ -968,7 +967,7 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : 3) finish_warp_kern
         }
         if (n_comp == 0) {
             // one group fills the window and goes on: more than 32 S members
-            const uint64_t e = scan_to_head<KeyT, PACKED>(keys1, a + kSpan, n, w1, len_mask);
+            const uint64_t e = scan_to_head<KeyT, PACKED>(keys1, a + kSpan, n);
             const uint64_t g = e - a;
             if (g <= cap) {          // the block kernel's: flag the tile it starts in
                 if (lane == 0) atomicOr(big_tiles + (a / kLocalTile >> 5), 1u << (a / kLocalTile & 31));
@@ -1276,7 +1275,7 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : 3) finish_warp_kern
 // width of the warp kernel.  counter[0] += such positions.
 constexpr int kProbeSpan = 2048, kProbeBlocks = 128;
 template <typename KeyT, bool PACKED>
-__global__ void __launch_bounds__(256) group_probe_kernel(const KeyT* __restrict__ keys1, uint64_t n, uint32_t w1, uint32_t len_mask, uint32_t limit,
+__global__ void __launch_bounds__(256) group_probe_kernel(const KeyT* __restrict__ keys1, uint64_t n, uint32_t limit,
                                                           unsigned long long* counter) {
     __shared__ uint32_t s_heads[kProbeSpan / 32 + 1];
     __shared__ uint32_t s_big;
@@ -1358,16 +1357,17 @@ cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, 
     constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
     if (packed && !kCanPack) return cudaErrorInvalidValue;
     if (slots != (uint32_t)kWarpSlotsSmall && slots != (uint32_t)kWarpSlotsLarge) return cudaErrorInvalidValue;
+    (void)w1;   // (a first-round key says in its lowest bit whether its suffix has w1 bases)
     if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
-    const uint32_t len_mask = 0;   // (unused: a first-round key says in its lowest bit whether its suffix has w1 bases)
     const uint64_t tiles = (n + kLocalTile - 1) / kLocalTile;
     cudaError_t e = cudaMemsetAsync(big_tiles, 0, ((tiles + 31) / 32 + 1) * sizeof(uint32_t), s);
     if (e != cudaSuccess) return e;
     {   // singletons and groups of at most 32: one warp per chunk, registers only
-        ScopedLaunch sl(prof, CX_K_FINISH, n * (sizeof(KeyT) + sizeof(IdT) + 1) + n / 8, s);
+        // a7 flagging (key + 1) and a8 emit (id + base + byte) per suffix; the refined suffixes' term is added by the caller
+        ScopedLaunch sl(prof, CX_K_FINISH, n * (sizeof(KeyT) + 1 + sizeof(IdT) + 2), s);
         const uint64_t warps = (n + kWarpChunk - 1) / kWarpChunk;
         const unsigned grid = (unsigned)((warps + kWarpThreads / 32 - 1) / (kWarpThreads / 32));
-        auto launch = [&](auto kernel) { kernel<<<grid, kWarpThreads, 0, s>>>(R, keys1, ids, ids, w1, len_mask, n, depth0, group_cap, heads_out, big_tiles, out, elems_done); };
+        auto launch = [&](auto kernel) { kernel<<<grid, kWarpThreads, 0, s>>>(R, keys1, ids, ids, n, depth0, group_cap, heads_out, big_tiles, out, elems_done); };
         if (slots == (uint32_t)kWarpSlotsLarge) {
             if (packed) launch(finish_warp_kernel<KeyT, IdT, kCanPack, kWarpSlotsLarge>);
             else launch(finish_warp_kernel<KeyT, IdT, false, kWarpSlotsLarge>);
@@ -1385,7 +1385,7 @@ cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, 
     if (e != cudaSuccess) return e;
     const uint64_t resident = (uint64_t)n_sms * kLocalBlocksPerSM;
     ScopedLaunch sl(prof, CX_K_FINISH_BLOCK, 0, s);
-    kernel<<<(unsigned)(tiles < resident ? tiles : resident), kLocalThreads, sizeof(LocalSmem), s>>>(R, keys1, w1, len_mask, nullptr, nullptr, ids, n, depth0, 32u * slots + 1,
+    kernel<<<(unsigned)(tiles < resident ? tiles : resident), kLocalThreads, sizeof(LocalSmem), s>>>(R, keys1, nullptr, nullptr, ids, n, depth0, 32u * slots + 1,
                                                                                                    group_cap, big_tiles, out, elems_done);
     return cudaGetLastError();
 }
@@ -1397,9 +1397,9 @@ cudaError_t launch_group_probe(const KeyT* keys1, uint32_t w1, uint64_t n, bool 
     if (n < (uint64_t)kProbeSpan * 2) return cudaSuccess;
     const unsigned blocks = (unsigned)(n / kProbeSpan < (uint64_t)kProbeBlocks ? n / kProbeSpan : (uint64_t)kProbeBlocks);
     *sampled = (uint64_t)blocks * kProbeSpan;
-    const uint32_t len_mask = 0;   // (unused: a first-round key says in its lowest bit whether its suffix has w1 bases)
-    if (packed) group_probe_kernel<KeyT, kCanPack><<<blocks, 256, 0, s>>>(keys1, n, w1, len_mask, 32u * kWarpSlotsSmall, counter);
-    else group_probe_kernel<KeyT, false><<<blocks, 256, 0, s>>>(keys1, n, w1, len_mask, 32u * kWarpSlotsSmall, counter);
+    (void)w1;
+    if (packed) group_probe_kernel<KeyT, kCanPack><<<blocks, 256, 0, s>>>(keys1, n, 32u * kWarpSlotsSmall, counter);
+    else group_probe_kernel<KeyT, false><<<blocks, 256, 0, s>>>(keys1, n, 32u * kWarpSlotsSmall, counter);
     return cudaGetLastError();
 }
 
@@ -1413,7 +1413,7 @@ cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32
     if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
     const uint64_t tiles = (n + kLocalTile - 1) / kLocalTile;
     const uint64_t resident = (uint64_t)n_sms * kLocalBlocksPerSM;
-    kernel<<<(unsigned)(tiles < resident ? tiles : resident), kLocalThreads, sizeof(LocalSmem), s>>>(R, nullptr, 0, 0, heads_in, heads_out, ids, n, depth, 2u, group_cap,
+    kernel<<<(unsigned)(tiles < resident ? tiles : resident), kLocalThreads, sizeof(LocalSmem), s>>>(R, nullptr, heads_in, heads_out, ids, n, depth, 2u, group_cap,
                                                                                                    nullptr, out, elems_done);
     return cudaGetLastError();
 }
