@@ -44,7 +44,8 @@ WORKLOADS = {
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed `ncu --set full` captures of THIS round at the
 # benched configuration (profiles/r02_ncu_full.md); keyed by (config, kernel class).  None until a capture exists.
-NCU_TRAFFIC: dict = {}
+NCU_TRAFFIC: dict = {(2, "finish"): 103_076_731_000, (2, "sort_pass"): 16_442_550_500, (2, "list"): 8_278_552_000, (2, "pack"): 1_195_503_000,
+                     (2, "finish_block"): 315_000}
 NCU_TRAFFIC_FILE = "profiles/r02_ncu_full.md"
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 CPU_SAMPLE_SCALE = {0: 1.0, 1: 0.5, 2: 0.1, 3: 0.01, 4: 0.001}      # cpu_baseline: the recipe at this scale (coverage preserved), all cores
@@ -633,7 +634,7 @@ def run_cx(args) -> None:
                                    else "replicas only" if world > 1 else
                                    f"1 gpu, shard {args.shard_index} of {args.shard_of} only (its piece: {N} suffixes)" if one_shard else "1 gpu"),
                    "l2": "256 MiB L2-flush write between timed steps; working set >> L2", "prefix_len": 6,
-                   "key_bases": "auto (14 bases in a 32-bit key up to 2^30 suffixes, else ceil(log4 N)+1 bases in a 64-bit key)",
+                   "key_bases": "auto (15 bases in a 32-bit key up to 2^30 suffixes, else 19 bases in a 40-bit key)",
                    "timing": "value/ms_per_step: CUDA events around each step, library built with profile=0; kernels{}/roofline{}: a "
                              "separate pass of the same steps with CUDA events around every launch (profile=1)",
                    "id_bytes": stats["id_bytes"], "n_batches": stats["n_batches"], "sort_passes": stats["sort_passes"],
