@@ -750,7 +750,13 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
 // Groups of more than 32 S and at most cap suffixes are left to the block kernel (their tile is flagged); larger ones to
 // the global path (only their head bit is published, their ids handed over, and they are counted).
 // ---------------------------------------------------------------------------------------------
-constexpr int kWarpChunk = 2048;    // sorted positions per warp: a chunk owns the groups that START in it
+#ifndef CX_WARP_CHUNK
+#define CX_WARP_CHUNK 2048
+#endif
+#ifndef CX_WARP_MINB
+#define CX_WARP_MINB 3
+#endif
+constexpr int kWarpChunk = CX_WARP_CHUNK;    // sorted positions per warp: a chunk owns the groups that START in it
 constexpr int kWarpThreads = 256;
 // slots per lane: 2 (windows of 64 positions, two-level keys) unless the batch's tie groups are mostly larger, then 4
 // (windows of 128 positions; the rank key has room for one level only)
@@ -897,7 +903,7 @@ __device__ __forceinline__ void window_words(const uint64_t* __restrict__ packed
 }
 
 template <typename KeyT, typename IdT, bool PACKED, int S>
-__global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : 3) finish_warp_kernel(Reads R, const KeyT* __restrict__ keys1, const IdT* __restrict__ ids_in,
+__global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finish_warp_kernel(Reads R, const KeyT* __restrict__ keys1, const IdT* __restrict__ ids_in,
                                                                    IdT* __restrict__ ids_out, uint64_t n, uint32_t depth0, uint32_t cap, uint32_t* __restrict__ heads,
                                                                    uint32_t* __restrict__ big_tiles, uint8_t* __restrict__ out,
                                                                    unsigned long long* counters) {

@@ -261,7 +261,7 @@ __device__ __forceinline__ void digit_counts(uint32_t (*s_dh)[kRadix], KeyT key,
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kListThreads) bucket_hist_kernel(Reads R, const BuildInfo* __restrict__ info,
                                                                    const uint32_t* __restrict__ tile_first_read, uint32_t ell, Region region,
-                                                                   unsigned long long* __restrict__ hist) {
+                                                                   unsigned long long* __restrict__ hist, uint32_t skip_if_uniform) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem& sm = *reinterpret_cast<TileSmem*>(smem_raw);
     uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem_raw + sizeof(TileSmem));
@@ -271,6 +271,7 @@ __global__ void __launch_bounds__(kListThreads) bucket_hist_kernel(Reads R, cons
     const uint32_t n_short = (n_kmers - 1) / 3;
     for (uint32_t k = threadIdx.x; k < n_kmers + n_short; k += blockDim.x) s_hist[k] = 0;
     if (info->bad_offsets) return;   // reported by the host after it reads `info`
+    if (skip_if_uniform && !info->nonuniform) return;   // bucket_hist_uniform_kernel has it
     R.n_words = (info->total_bases + 31) >> 5;
     const uint64_t N = info->n_suffixes;
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
@@ -603,7 +604,7 @@ __device__ __forceinline__ uint32_t big_top16(const BigSmem& sm, uint32_t brel) 
     const uint32_t q = brel >> 4, sh = (brel & 15) * 2;
     return __funnelshift_l(half[(q + 1) ^ 1], half[q ^ 1], sh);
 }
-// Walk of one thread over its kBigItems consecutive slots: f(i, partition code) for each; branch-free per slot (a warp's lanes
+// Walk of one thread over its kBigItems consecutive slots: f(i, l-mer A-padded, min(rem, l)) for each; branch-free per slot (a warp's lanes
 // are at different phases of their reads, so a 'suffix ends inside the prefix' branch would be taken by some lane nearly always).
 // GUARD: the tile is ragged (only the collection's last tile), slots at or past n_here do not exist.
 template <bool GUARD, typename F>
@@ -620,7 +621,7 @@ __device__ __forceinline__ void big_walk(const BigCtx& c, const BigSmem& sm, uin
             const uint32_t r = rem < ell ? rem : ell;
             // the first l bases with those past the end of the read cleared (A-padded), then the length: reading A4 of PAPER.md:79
             const uint32_t kmer = (top >> (32 - 2 * ell)) & (0xffffffffu << (2 * (ell - r)));
-            f(i, kmer * (ell + 1) + r);
+            f(i, kmer, r);   // partition code = kmer * (ell + 1) + r
             const bool adv = rem != 0;                    // at an end-marker slot the next read starts at the same base index
             top = adv ? top << 2 : top;
             brel += adv;
@@ -645,7 +646,8 @@ __global__ void __launch_bounds__(kListThreads) list_count_uniform_kernel(Reads 
         uint64_t mine = 0;   // eight 8-bit counters (at most 32 slots per thread)
         const uint32_t s0 = threadIdx.x * kBigItems;
         if (s0 < c.n_slots) {
-            auto tally = [&](int, uint32_t code) {
+            auto tally = [&](int, uint32_t kmer, uint32_t r) {
+                const uint32_t code = kmer * (ell + 1) + r;
                 // which of the group's batches owns the partition: a three-step search of the (at most eight) range starts
                 uint32_t j = code >= s_first[4] ? 4u : 0u;
                 j += code >= s_first[j + 2] ? 2u : 0u;
@@ -663,6 +665,45 @@ __global__ void __launch_bounds__(kListThreads) list_count_uniform_kernel(Reads 
         }
         __syncthreads();
         if (threadIdx.x < ranges.n) tile_count[(uint64_t)threadIdx.x * col_stride + t] = s_total[threadIdx.x];
+    }
+}
+
+// a2 on the same walk: partition sizes of a collection of equal-length reads (the whole collection, no region).  Counters as in
+// bucket_hist_kernel: full-length partitions by l-mer, the short ones behind them.
+__global__ void __launch_bounds__(kListThreads) bucket_hist_uniform_kernel(Reads R, const BuildInfo* __restrict__ info, uint32_t ell,
+                                                                           unsigned long long* __restrict__ hist) {
+    __shared__ BigSmem sm;
+    extern __shared__ uint32_t s_hist_u[];
+    const uint32_t n_kmers = 1u << (2 * ell), n_short = (n_kmers - 1) / 3;
+    for (uint32_t k = threadIdx.x; k < n_kmers + n_short; k += blockDim.x) s_hist_u[k] = 0;
+    if (info->bad_offsets || info->nonuniform) return;   // (reads of different lengths: bucket_hist_kernel has it)
+    R.n_words = (info->total_bases + 31) >> 5;
+    const uint64_t N = info->n_suffixes;
+    const uint64_t n_tiles = (N + kBigTile - 1) / kBigTile;
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        __syncthreads();   // previous tile done with sm (and the counters zeroed on the first trip)
+        const BigCtx c = load_big_tile(R, info, t, N, sm);
+        const uint32_t s0 = threadIdx.x * kBigItems;
+        if (s0 < c.n_slots) {
+            auto count = [&](int, uint32_t kmer, uint32_t r) {
+                const uint32_t at = r == ell ? kmer : n_kmers + (((1u << (2 * r)) - 1) / 3) + (kmer >> (2 * (ell - r)));
+                atomicAdd(&s_hist_u[at], 1u);
+            };
+            if (c.n_slots == (uint32_t)kBigTile) big_walk<false>(c, sm, s0, ell, count);
+            else big_walk<true>(c, sm, s0, ell, count);
+        }
+    }
+    __syncthreads();
+    for (uint32_t k = threadIdx.x; k < n_kmers; k += blockDim.x) {
+        const uint32_t v = s_hist_u[k];
+        if (v) atomicAdd(hist + (uint64_t)k * (ell + 1) + ell, (unsigned long long)v);
+    }
+    for (uint32_t r = 0; r < ell; ++r) {
+        const uint32_t first = n_kmers + ((1u << (2 * r)) - 1) / 3, count = 1u << (2 * r);
+        for (uint32_t k = threadIdx.x; k < count; k += blockDim.x) {
+            const uint32_t v = s_hist_u[first + k];
+            if (v) atomicAdd(hist + ((uint64_t)k << (2 * (ell - r))) * (ell + 1) + r, (unsigned long long)v);
+        }
     }
 }
 
@@ -688,7 +729,7 @@ __global__ void __launch_bounds__(kListThreads) list_select_uniform_kernel(Reads
         const uint32_t s0 = threadIdx.x * kBigItems;
         uint32_t mask = 0;   // which of my 32 consecutive slots belong to this batch
         if (s0 < c.n_slots) {
-            auto mark = [&](int i, uint32_t code) { mask |= (uint32_t)(code - bucket_lo <= bucket_hi - bucket_lo) << i; };
+            auto mark = [&](int i, uint32_t kmer, uint32_t r) { mask |= (uint32_t)(kmer * (ell + 1) + r - bucket_lo <= bucket_hi - bucket_lo) << i; };
             if (c.n_slots == (uint32_t)kBigTile) big_walk<false>(c, sm, s0, ell, mark);
             else big_walk<true>(c, sm, s0, ell, mark);
         }
@@ -780,7 +821,19 @@ cudaError_t launch_bucket_hist(const Reads& R, const BuildInfo* info, const uint
     int per_sm = ell <= 6 ? 4 : 2;
     uint64_t want = (uint64_t)n_sms * per_sm;
     unsigned grid = (unsigned)(max_tiles < want ? max_tiles : want);
-    bucket_hist_kernel<<<grid, kListThreads, smem, s>>>(R, info, tile_first_read, ell, region, (unsigned long long*)hist);
+    // Reads of one length outside a region (the DEVICE knows; the host may not have read BuildInfo yet) are counted on the
+    // 8192-slot walk, anything else by the general kernel: both are launched, the one that does not apply returns at once.
+    const uint32_t skip_uniform = region.depth == 0;
+    if (skip_uniform) {
+        const size_t smem_u = smem - sizeof(TileSmem);
+        e = cudaFuncSetAttribute(bucket_hist_uniform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bucket_hist_smem(7) - sizeof(TileSmem)));
+        if (e != cudaSuccess) return e;
+        const uint64_t big = (max_tiles * kListTile + kBigTile - 1) / kBigTile;
+        bucket_hist_uniform_kernel<<<(unsigned)(big < want ? big : want), kListThreads, smem_u, s>>>(R, info, ell, (unsigned long long*)hist);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    bucket_hist_kernel<<<grid, kListThreads, smem, s>>>(R, info, tile_first_read, ell, region, (unsigned long long*)hist, skip_uniform);
     return cudaGetLastError();
 }
 
