@@ -780,6 +780,221 @@ __global__ void __launch_bounds__(kListThreads) list_select_uniform_kernel(Reads
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// The multi-batch scans for reads of ONE length L <= 127 (the paper's 100 bp reads; configs[1], [2], [4]), outside any region:
+// ONE READ PER THREAD.  Position p of the read has the same `bases left` in every lane, so the walk has no divergence, no
+// per-slot decode and no end-marker bookkeeping: per slot a shift, the partition code and the range test.  A tile is 256
+// consecutive reads (256 (L + 1) slots); a thread's slots are consecutive in listing order, so thread order = slot order
+// (PAPER.md:99).  Every batch of a collection larger than the workspace walks all slots again, so this walk is
+// what the out-of-core build spends its listing time on.
+// ---------------------------------------------------------------------------------------------
+constexpr int kReadMaxLen = 127;                      // L + 1 <= 128 slots per read: four 32-bit masks per thread
+constexpr int kReadMinLen = 16;                       // (below, the tile tables sized per 2048 slots would be too small)
+constexpr int kReadTileWords = kListThreads * kReadMaxLen / 32 + 6;
+constexpr int kTakenCap = 8192;                       // taken slots decoded per round
+
+struct ReadTileCtx {
+    uint64_t r0;        // first read of the tile
+    uint32_t n;         // reads in the tile
+    uint32_t L;         // read length
+    uint32_t brel0;     // index of read r0's first base among the staged bases
+};
+__device__ __forceinline__ ReadTileCtx load_read_tile(const Reads& R, const BuildInfo* __restrict__ info, uint64_t t, uint64_t* packed_sm) {
+    ReadTileCtx c;
+    c.r0 = t * kListThreads;
+    c.n = (uint32_t)min((uint64_t)kListThreads, R.n_reads - c.r0);
+    c.L = (uint32_t)info->first_len;
+    const uint64_t b0 = c.r0 * c.L;
+    const uint64_t word0 = b0 >> 5;
+    c.brel0 = (uint32_t)(b0 & 31);
+    const uint32_t words = (c.brel0 + c.n * c.L + 31) / 32 + 3;   // + the look-ahead of the last read's last windows
+    for (uint32_t j = threadIdx.x; j < words; j += blockDim.x) {
+        const uint64_t wi = word0 + j;
+        packed_sm[j] = wi < R.n_words ? __ldg(R.packed + wi) : 0ull;
+    }
+    __syncthreads();
+    return c;
+}
+__device__ __forceinline__ uint32_t top16_at(const uint64_t* packed_sm, uint32_t brel) {
+    const uint32_t* half = reinterpret_cast<const uint32_t*>(packed_sm);   // 32-bit halves, high half first
+    const uint32_t q = brel >> 4, sh = (brel & 15) * 2;
+    return __funnelshift_l(half[(q + 1) ^ 1], half[q ^ 1], sh);
+}
+__device__ __forceinline__ uint64_t window_at(const uint64_t* packed_sm, uint32_t brel) {
+    const uint32_t wi = brel >> 5, sh = (brel & 31) * 2;
+    const uint64_t w0 = packed_sm[wi], w1 = packed_sm[wi + 1];
+    return sh ? (w0 << sh) | (w1 >> (64 - sh)) : w0;
+}
+// f(p, partition code) for every position p = 0 .. L of the thread's read (p = L: the end-marker suffix)
+template <typename F>
+__device__ __forceinline__ void read_walk(const uint64_t* packed_sm, uint32_t brel, uint32_t L, uint32_t ell, F&& f) {
+    uint32_t top = 0;
+#pragma unroll
+    for (int p = 0; p <= kReadMaxLen; ++p) {
+        if ((uint32_t)p <= L) {                           // the same in every lane
+            if ((p & 7) == 0) top = top16_at(packed_sm, brel + p);   // at most 7 bases are consumed before the next refill: l <= 7 stay valid
+            const uint32_t left = L - (uint32_t)p, r = left < ell ? left : ell;
+            // the first l bases with those past the end of the read cleared (A-padded), then the length: reading A4 of PAPER.md:79
+            const uint32_t kmer = (top >> (32 - 2 * ell)) & (0xffffffffu << (2 * (ell - r)));
+            f(p, kmer * (ell + 1) + r);
+            top <<= 2;
+        }
+    }
+}
+
+// The same walk for the select scan: which positions of the read belong to the partition range [lo, hi]?  Bit p of (mhi:mlo).
+// Positions with at least l bases left (all but the last l of a read) are taken in blocks of eight with a range test on the raw
+// l-mer: code = kmer (l + 1) + l in [lo, hi]  <=>  kmer - klo <= kspan; only the blocks that reach the read's end pay for the
+// length arithmetic.  Every branch depends on p, L and l only: the same in every lane.
+__device__ __forceinline__ void read_select_walk(const uint64_t* packed_sm, uint32_t brel, uint32_t L, uint32_t ell, uint32_t lo, uint32_t hi,
+                                                 uint64_t& mlo, uint64_t& mhi) {
+    const uint32_t e1 = ell + 1, sh = 32 - 2 * ell;
+    uint32_t klo = lo / e1, kspan = 0;
+    if (hi >= ell && (hi - ell) / e1 >= klo) kspan = (hi - ell) / e1 - klo;
+    else klo = 0xffffffffu;                           // no full-length partition in the range: kmer - klo <= 0 never holds
+    const uint32_t n_full = L + 1 - ell;              // positions 0 .. n_full - 1 have at least l bases left (L >= kReadMinLen > l)
+    mlo = 0, mhi = 0;
+    uint32_t p = 0;
+    for (; p + 8 <= n_full; p += 8) {
+        uint32_t top = top16_at(packed_sm, brel + p);
+        uint32_t acc = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            acc |= (uint32_t)((top >> sh) - klo <= kspan) << i;
+            top <<= 2;
+        }
+        if (p < 64) mlo |= (uint64_t)acc << p;
+        else mhi |= (uint64_t)acc << (p - 64);
+    }
+    for (; p <= L; p += 8) {                          // the rest: up to 7 full-length positions and the l + 1 that end inside the prefix
+        uint32_t top = top16_at(packed_sm, brel + p);
+        uint32_t acc = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const uint32_t q = p + i;
+            if (q <= L) {
+                const uint32_t left = L - q, r = left < ell ? left : ell;
+                const uint32_t kmer = (top >> sh) & (0xffffffffu << (2 * (ell - r)));   // bases past the end of the read cleared (A4)
+                acc |= (uint32_t)(kmer * e1 + r - lo <= hi - lo) << i;
+            }
+            top <<= 2;
+        }
+        if (p < 64) mlo |= (uint64_t)acc << p;
+        else mhi |= (uint64_t)acc << (p - 64);
+    }
+}
+
+__global__ void __launch_bounds__(kListThreads) list_count_reads_kernel(Reads R, const BuildInfo* __restrict__ info, uint32_t ell, CountRanges ranges,
+                                                                        uint64_t* __restrict__ tile_count, uint64_t col_stride) {
+    __shared__ uint64_t s_packed[kReadTileWords];
+    __shared__ uint32_t s_total[kCountGroup];
+    __shared__ uint32_t s_first[kCountGroup + 1];    // first partition of every batch of the group; unused ones = one past the last
+    R.n_words = (info->total_bases + 31) >> 5;
+    if (info->bad_offsets) return;
+    const uint64_t n_tiles = (R.n_reads + kListThreads - 1) / kListThreads;
+    if (threadIdx.x <= kCountGroup) s_first[threadIdx.x] = ranges.first[threadIdx.x < ranges.n ? threadIdx.x : ranges.n];
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        __syncthreads();   // previous tile done with s_packed and s_total
+        if (threadIdx.x < kCountGroup) s_total[threadIdx.x] = 0;
+        const ReadTileCtx c = load_read_tile(R, info, t, s_packed);
+        uint64_t mine = 0;   // eight 8-bit counters (at most 128 slots per thread)
+        if (threadIdx.x < c.n) {
+            read_walk(s_packed, c.brel0 + threadIdx.x * c.L, c.L, ell, [&](int, uint32_t code) {
+                uint32_t j = code >= s_first[4] ? 4u : 0u;   // which of the group's batches owns the partition
+                j += code >= s_first[j + 2] ? 2u : 0u;
+                j += code >= s_first[j + 1] ? 1u : 0u;
+                if (code >= s_first[0] && code < s_first[kCountGroup]) mine += 1ull << (8 * j);
+            });
+        }
+#pragma unroll
+        for (int j = 0; j < kCountGroup; ++j) {
+            uint32_t v = (uint32_t)(mine >> (8 * j)) & 255u;
+            for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane_id() == 0 && v) atomicAdd(&s_total[j], v);
+        }
+        __syncthreads();
+        if (threadIdx.x < ranges.n) tile_count[(uint64_t)threadIdx.x * col_stride + t] = s_total[threadIdx.x];
+    }
+}
+
+template <typename KeyT, typename IdT, bool PACKED>
+__global__ void __launch_bounds__(kListThreads) list_select_reads_kernel(Reads R, const BuildInfo* __restrict__ info, uint32_t ell, uint32_t w,
+                                                                         uint32_t bucket_lo, uint32_t bucket_hi,
+                                                                         const uint64_t* __restrict__ tile_base, KeyT* __restrict__ keys,
+                                                                         IdT* __restrict__ ids, uint32_t n_passes,
+                                                                         unsigned long long* __restrict__ digit_hist, uint64_t ord_lo, uint64_t ord_hi) {
+    __shared__ uint64_t s_packed[kReadTileWords];
+    __shared__ uint32_t s_dh[8][kRadix];
+    __shared__ uint32_t s_warp[kListThreads / 32];
+    __shared__ uint16_t s_taken[kTakenCap];   // slots of the tile that belong to the batch, in slot order, one round's worth
+    R.n_words = (info->total_bases + 31) >> 5;
+    if (info->bad_offsets) return;
+    const uint64_t n_tiles = (R.n_reads + kListThreads - 1) / kListThreads;
+    const uint32_t warp = threadIdx.x >> 5;
+    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) (&s_dh[0][0])[i] = 0;
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        __syncthreads();   // previous tile done with s_packed, s_warp and s_taken
+        const ReadTileCtx c = load_read_tile(R, info, t, s_packed);
+        uint64_t mlo = 0, mhi = 0;   // which of my read's slots belong to this batch (position p -> bit p)
+        if (threadIdx.x < c.n) read_select_walk(s_packed, c.brel0 + threadIdx.x * c.L, c.L, ell, bucket_lo, bucket_hi, mlo, mhi);
+        // exclusive scan of the per-thread counts: slot order = thread order
+        const uint32_t cnt = (uint32_t)__popcll(mlo) + (uint32_t)__popcll(mhi);
+        uint32_t incl = cnt;
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t up = __shfl_up_sync(0xffffffffu, incl, o);
+            if ((int)lane_id() >= o) incl += up;
+        }
+        if (lane_id() == 31) s_warp[warp] = incl;
+        __syncthreads();
+        uint32_t before = incl - cnt, total = 0;
+        for (uint32_t q = 0; q < kListThreads / 32; ++q) {
+            const uint32_t v = s_warp[q];
+            if (q < warp) before += v;
+            total += v;
+        }
+        const uint64_t tile_dst = tile_base[t];
+        // taken slots are compacted (slot order) and then decoded one per thread: full warps, consecutive output addresses;
+        // kTakenCap of them per round (one round unless the batch takes a large share of the collection)
+        for (uint32_t round0 = 0; round0 < total; round0 += kTakenCap) {
+            if (round0) __syncthreads();   // the previous round's decode is done with s_taken
+            uint32_t at = before;
+            auto put = [&](uint64_t m, uint32_t p0) {
+                while (m) {
+                    const uint32_t i = (uint32_t)__ffsll((long long)m) - 1;
+                    m &= m - 1;
+                    if (at - round0 < (uint32_t)kTakenCap) s_taken[at - round0] = (uint16_t)((threadIdx.x << 7) | (p0 + i));   // (unsigned: below round0 wraps high)
+                    ++at;
+                }
+            };
+            put(mlo, 0), put(mhi, 64);
+            __syncthreads();
+            const uint32_t here = min((uint32_t)kTakenCap, total - round0);
+            for (uint32_t j = threadIdx.x; j < here; j += kListThreads) {
+                const uint64_t dst = tile_dst + round0 + j;
+                if (dst >= ord_lo && dst < ord_hi) {
+                    const uint32_t sl = s_taken[j];
+                    const uint32_t rr = sl >> 7, pos = sl & 127u;   // (thread = read of the tile, position)
+                    const KeyT key = first_key_as<KeyT>(window_at(s_packed, c.brel0 + rr * c.L + pos), (uint64_t)(c.L - pos), w);
+                    const IdT id = make_id<IdT>(c.r0 + rr, pos, R.pos_bits);
+                    digit_counts(s_dh, key, n_passes);
+                    const uint64_t o = dst - ord_lo;
+                    if constexpr (PACKED) {
+                        reinterpret_cast<uint64_t*>(keys)[o] = ((uint64_t)key << 32) | (uint64_t)id;
+                    } else {
+                        keys[o] = key;
+                        ids[o] = id;
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) {
+        uint32_t v = (&s_dh[0][0])[i];
+        if (v) atomicAdd(digit_hist + i, (unsigned long long)v);
+    }
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------
@@ -787,7 +1002,12 @@ __global__ void __launch_bounds__(kListThreads) list_select_uniform_kernel(Reads
 // ---------------------------------------------------------------------------------------------
 // the multi-batch scans of a collection of equal-length reads outside a refined region run on tiles of kBigTile slots
 static bool big_tiles(const Reads& R, const Region& region) { return R.uniform && region.depth == 0; }
+// ... and one read per thread when that length is 16 .. 127 bases (tiles of 256 reads)
+static bool read_tiles(const Reads& R, const Region& region) {
+    return big_tiles(R, region) && R.uniform_len >= (uint64_t)kReadMinLen && R.uniform_len <= (uint64_t)kReadMaxLen;
+}
 uint64_t list_scan_tiles(const Reads& R, const Region& region, uint64_t n_suffixes) {
+    if (read_tiles(R, region)) return (R.n_reads + kListThreads - 1) / kListThreads;
     const uint64_t tile = big_tiles(R, region) ? (uint64_t)kBigTile : (uint64_t)kListTile;
     return (n_suffixes + tile - 1) / tile;
 }
@@ -842,6 +1062,10 @@ cudaError_t launch_list_count(const Reads& R, const BuildInfo* info, const uint3
     if (n_tiles == 0 || ranges.n == 0) return cudaSuccess;
     uint64_t want = (uint64_t)sm_count() * 8;
     const unsigned grid = (unsigned)(n_tiles < want ? n_tiles : want);
+    if (read_tiles(R, region)) {  // n_tiles counts tiles of 256 reads here (list_scan_tiles)
+        list_count_reads_kernel<<<grid, kListThreads, 0, s>>>(R, info, ell, ranges, tile_count, col_stride);
+        return cudaGetLastError();
+    }
     if (big_tiles(R, region)) {   // n_tiles counts tiles of kBigTile slots here (list_scan_tiles)
         list_count_uniform_kernel<<<grid, kListThreads, 0, s>>>(R, info, ell, ranges, tile_count, col_stride);
         return cudaGetLastError();
@@ -887,6 +1111,16 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
                                              ord_hi);
         return cudaGetLastError();
     };
+    if (read_tiles(R, region)) {
+        auto kernel = packed ? list_select_reads_kernel<KeyT, IdT, kCanPack> : list_select_reads_kernel<KeyT, IdT, false>;
+        int per_sm = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kListThreads, 0);
+        if (e != cudaSuccess) return e;
+        const uint64_t resident = (uint64_t)n_sms * (per_sm > 0 ? per_sm : 1);
+        kernel<<<(unsigned)(n_tiles < resident ? n_tiles : resident), kListThreads, 0, s>>>(R, info, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids, n_passes, dh,
+                                                                                          ord_lo, ord_hi);
+        return cudaGetLastError();
+    }
     if (big_tiles(R, region)) {
         auto kernel = packed ? list_select_uniform_kernel<KeyT, IdT, kCanPack> : list_select_uniform_kernel<KeyT, IdT, false>;
         int per_sm = 0;
