@@ -14,6 +14,10 @@ constexpr int kListThreads = 256;
 constexpr int kListItems = 8;
 constexpr int kListTile = kListThreads * kListItems;   // suffix slots per listing / histogram tile
 
+// scans with one read per thread (collections of equal-length reads): read lengths they take
+constexpr int kReadMaxLen = 127;   // L + 1 <= 128 slots per read: a 128-bit mask per thread
+constexpr int kReadMinLen = 16;    // (below, the tile tables sized per 2048 slots would be too small)
+
 constexpr int kRadixBits = 8;
 constexpr int kRadix = 1 << kRadixBits;
 

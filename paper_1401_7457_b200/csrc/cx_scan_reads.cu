@@ -486,7 +486,7 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
                                                                   const uint32_t* __restrict__ tile_first_read, uint32_t ell, uint32_t w,
                                                                   KeyT* __restrict__ keys, IdT* __restrict__ ids, uint32_t n_passes,
                                                                   unsigned long long* __restrict__ digit_hist,
-                                                                  unsigned long long* __restrict__ bucket_hist, uint64_t max_n) {
+                                                                  unsigned long long* __restrict__ bucket_hist, uint64_t max_n, uint32_t skip_if_reads) {
     __shared__ TileSmem sm;
     __shared__ uint32_t s_dh[8][kRadix];   // digit counts of every radix pass of the sort that follows (a6's upfront histogram)
     extern __shared__ uint32_t s_bh[];     // partition counters, laid out as in bucket_hist_kernel
@@ -496,6 +496,7 @@ __global__ void __launch_bounds__(kListThreads) list_write_kernel(Reads R, const
     R.n_words = (info->total_bases + 31) >> 5;
     const uint64_t N = info->n_suffixes;
     if (N > max_n || info->bad_offsets) return;   // the host reports both after reading `info`
+    if (skip_if_reads && !info->nonuniform && info->first_len >= (uint64_t)kReadMinLen && info->first_len <= (uint64_t)kReadMaxLen) return;   // list_write_reads_kernel has it
     const uint64_t n_tiles = (N + kListTile - 1) / kListTile;
     for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) (&s_dh[0][0])[i] = 0;
 
@@ -788,8 +789,6 @@ __global__ void __launch_bounds__(kListThreads) list_select_uniform_kernel(Reads
 // (PAPER.md:99).  Every batch of a collection larger than the workspace walks all slots again, so this walk is
 // what the out-of-core build spends its listing time on.
 // ---------------------------------------------------------------------------------------------
-constexpr int kReadMaxLen = 127;                      // L + 1 <= 128 slots per read: four 32-bit masks per thread
-constexpr int kReadMinLen = 16;                       // (below, the tile tables sized per 2048 slots would be too small)
 constexpr int kReadTileWords = kListThreads * kReadMaxLen / 32 + 6;
 constexpr int kTakenCap = 8192;                       // taken slots decoded per round
 
@@ -995,6 +994,107 @@ __global__ void __launch_bounds__(kListThreads) list_select_reads_kernel(Reads R
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// a4 + a5 (+ a2) for a collection of equal-length reads (16..127 bases) that is sorted as ONE batch (configs[0..2]):
+// list_write_kernel's work with one read per thread.  Everything that depends on the position p is the same in every lane:
+// positions with at least w bases left take a key without masking, those with at least l a partition counter without length
+// arithmetic.  A thread's (key, id) words are consecutive in the output, so they are staged in shared memory eight positions
+// at a time (rows padded to nine words: conflict-free) and leave as runs of 64 bytes.
+// ---------------------------------------------------------------------------------------------
+constexpr int kStageCols = 8, kStagePitch = kStageCols + 1;
+template <typename KeyT, typename IdT, bool PACKED>
+__global__ void __launch_bounds__(kListThreads) list_write_reads_kernel(Reads R, const BuildInfo* __restrict__ info, uint32_t ell, uint32_t w,
+                                                                        KeyT* __restrict__ keys, IdT* __restrict__ ids, uint32_t n_passes,
+                                                                        unsigned long long* __restrict__ digit_hist,
+                                                                        unsigned long long* __restrict__ bucket_hist, uint64_t max_n) {
+    __shared__ uint64_t s_packed[kReadTileWords];
+    __shared__ uint32_t s_dh[8][kRadix];   // digit counts of every radix pass of the sort that follows (a6's upfront histogram)
+    __shared__ uint64_t s_stage[kListThreads * kStagePitch];   // PACKED: key << 32 | id; else keys, and ids in s_stage_id
+    extern __shared__ __align__(8) unsigned char s_dyn[];      // [!PACKED: id staging rows][partition counters, laid out as in bucket_hist_kernel]
+    uint64_t* s_stage_id = reinterpret_cast<uint64_t*>(s_dyn);
+    uint32_t* s_bh = reinterpret_cast<uint32_t*>(s_dyn + (PACKED ? 0 : sizeof(uint64_t) * kListThreads * kStagePitch));
+    const uint32_t n_kmers = 1u << (2 * ell), n_short = (n_kmers - 1) / 3;
+    if (bucket_hist)
+        for (uint32_t k = threadIdx.x; k < n_kmers + n_short; k += blockDim.x) s_bh[k] = 0;
+    R.n_words = (info->total_bases + 31) >> 5;
+    const uint64_t N = info->n_suffixes;
+    const uint64_t L64 = info->first_len;
+    if (N > max_n || info->bad_offsets || info->nonuniform || L64 < (uint64_t)kReadMinLen || L64 > (uint64_t)kReadMaxLen) return;   // list_write_kernel has it
+    const uint64_t n_tiles = (R.n_reads + kListThreads - 1) / kListThreads;
+    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) (&s_dh[0][0])[i] = 0;
+    const uint32_t tid = threadIdx.x;
+    for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        __syncthreads();   // previous tile done with s_packed and the staging rows (and the counters zeroed on the first trip)
+        const ReadTileCtx c = load_read_tile(R, info, t, s_packed);
+        const uint32_t L = c.L, L1 = L + 1;
+        const bool have = tid < c.n;
+        const uint32_t brel = c.brel0 + tid * L;
+        const uint64_t id_hi = (c.r0 + tid) << R.pos_bits;
+        uint64_t win = 0;
+        for (uint32_t p0 = 0; p0 <= L; p0 += kStageCols) {
+            if ((p0 & 15) == 0 && have) win = window_at(s_packed, brel + p0);   // 32 bases; 16 are consumed before the next refill: w <= 16 stay valid
+#pragma unroll
+            for (int i = 0; i < kStageCols; ++i) {
+                const uint32_t p = p0 + i;
+                if (p <= L && have) {                         // (p <= L: the same in every lane)
+                    const uint32_t left = L - p;
+                    if (bucket_hist) {
+                        if (left >= ell) {
+                            atomicAdd(&s_bh[(uint32_t)(win >> (64 - 2 * ell))], 1u);
+                        } else {
+                            const uint32_t kmer = (uint32_t)(win >> (64 - 2 * ell)) & (0xffffffffu << (2 * (ell - left)));
+                            atomicAdd(&s_bh[n_kmers + (((1u << (2 * left)) - 1) / 3) + (kmer >> (2 * (ell - left)))], 1u);
+                        }
+                    }
+                    const KeyT key = first_key_as<KeyT>(win, (uint64_t)left, w);
+                    digit_counts(s_dh, key, n_passes);
+                    if constexpr (PACKED) {
+                        s_stage[tid * kStagePitch + i] = ((uint64_t)key << 32) | id_hi | p;
+                    } else {
+                        s_stage[tid * kStagePitch + i] = (uint64_t)key;
+                        s_stage_id[tid * kStagePitch + i] = id_hi | p;
+                    }
+                    win <<= 2;
+                }
+            }
+            __syncthreads();
+            // the block's rows of eight words leave in slot order: word q of the block = (read q / 8, position p0 + q % 8)
+            const uint32_t cols = min((uint32_t)kStageCols, L1 - p0);
+            for (uint32_t q = tid; q < c.n * kStageCols; q += kListThreads) {
+                const uint32_t rr = q / kStageCols, k = q % kStageCols;
+                if (k < cols) {
+                    const uint64_t at = (c.r0 + rr) * L1 + p0 + k;
+                    if constexpr (PACKED) {
+                        reinterpret_cast<uint64_t*>(keys)[at] = s_stage[rr * kStagePitch + k];
+                    } else {
+                        keys[at] = (KeyT)s_stage[rr * kStagePitch + k];
+                        ids[at] = (IdT)s_stage_id[rr * kStagePitch + k];
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    }
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) {
+        uint32_t v = (&s_dh[0][0])[i];
+        if (v) atomicAdd(digit_hist + i, (unsigned long long)v);
+    }
+    if (bucket_hist) {
+        for (uint32_t k = threadIdx.x; k < n_kmers; k += blockDim.x) {
+            uint32_t v = s_bh[k];
+            if (v) atomicAdd(bucket_hist + (uint64_t)k * (ell + 1) + ell, (unsigned long long)v);
+        }
+        for (uint32_t r = 0; r < ell; ++r) {
+            const uint32_t first = n_kmers + ((1u << (2 * r)) - 1) / 3, count = 1u << (2 * r);
+            for (uint32_t k = threadIdx.x; k < count; k += blockDim.x) {
+                uint32_t v = s_bh[first + k];
+                if (v) atomicAdd(bucket_hist + ((uint64_t)k << (2 * (ell - r))) * (ell + 1) + r, (unsigned long long)v);
+            }
+        }
+    }
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------
@@ -1090,15 +1190,36 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
     constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
     if ((packed && !kCanPack) || (bucket_hist && tile_base)) return cudaErrorInvalidValue;
     const size_t smem = bucket_hist ? bucket_hist_smem(ell) - sizeof(TileSmem) : 0;
+    const uint32_t skip_reads = tile_base == nullptr && w <= 16 && !region.depth && R.n_reads > 0;   // (a register pair holds the 16 bases a key may need)
     auto launch = [&](auto kernel) {
         if (smem) {
             cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bucket_hist_smem(7) - sizeof(TileSmem)));
             if (e != cudaSuccess) return e;
         }
-        kernel<<<grid, kListThreads, smem, s>>>(R, info, tile_first_read, ell, w, keys, ids, n_passes, dh, bh, max_n);
+        kernel<<<grid, kListThreads, smem, s>>>(R, info, tile_first_read, ell, w, keys, ids, n_passes, dh, bh, max_n, skip_reads);
         return cudaGetLastError();
     };
-    if (tile_base == nullptr) return packed ? launch(list_write_kernel<KeyT, IdT, kCanPack>) : launch(list_write_kernel<KeyT, IdT, false>);
+    if (tile_base == nullptr) {
+        // Reads of one length of 16..127 bases (the paper's setting; the DEVICE knows, the host may not have read BuildInfo yet) are
+        // listed one read per thread, any other collection by the general kernel: both are launched, the one that does not apply
+        // returns at once.
+        if (skip_reads) {
+            auto kernel = packed ? list_write_reads_kernel<KeyT, IdT, kCanPack> : list_write_reads_kernel<KeyT, IdT, false>;
+            const size_t stage_id = packed ? 0 : sizeof(uint64_t) * kListThreads * kStagePitch;
+            const size_t smem_r = smem + stage_id;
+            cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bucket_hist_smem(7) - sizeof(TileSmem) + stage_id));
+            if (e != cudaSuccess) return e;
+            int per_sm = 0;
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kListThreads, smem_r);
+            if (e != cudaSuccess) return e;
+            const uint64_t resident = (uint64_t)n_sms * (per_sm > 0 ? per_sm : 1);
+            const uint64_t tiles = (R.n_reads + kListThreads - 1) / kListThreads;
+            kernel<<<(unsigned)(tiles < resident ? tiles : resident), kListThreads, smem_r, s>>>(R, info, ell, w, keys, ids, n_passes, dh, bh, max_n);
+            e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+        }
+        return packed ? launch(list_write_kernel<KeyT, IdT, kCanPack>) : launch(list_write_kernel<KeyT, IdT, false>);
+    }
     auto select = [&](auto kernel) {
         // persistent blocks: exactly as many as are resident at once (48 registers: five per SM); a sixth per SM would
         // run as a second wave on an almost empty machine
