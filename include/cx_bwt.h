@@ -181,7 +181,8 @@ int cx_fasta_parse(const uint8_t *text_dev, uint64_t n_bytes, uint8_t *bases_out
  * successful no-op.  Work is enqueued on `stream` (and joined side streams); the call synchronises
  * `stream` to read the partition sizes and once per refinement round, and returns after the last
  * batch has been enqueued and -- for pinned-host output -- copied.
- * Errors: CX_ERR_ARG (also for sizes above the plan's), CX_ERR_BUCKET_TOO_LARGE, CX_ERR_CUDA.
+ * Errors: CX_ERR_ARG (also for sizes above the plan's, a read of 2^32 bases or more, or 2^40 bases or more in total:
+ * the tie refinement keeps 32-bit lengths and 40-bit base indices), CX_ERR_BUCKET_TOO_LARGE, CX_ERR_CUDA.
  * The result is unique, so two runs on the same input are byte-identical.
  */
 int cx_bwt_build(cx_bwt_plan_t *plan, const uint64_t *packed_reads, const uint64_t *read_offsets,
