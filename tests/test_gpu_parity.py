@@ -408,3 +408,36 @@ def test_packed_output_four_bits_per_symbol(opts):
         cx.Plan(100, 1000, out_bits=4, shard_index=0, shard_count=2)
     with pytest.raises(cx.CxError):
         cx.Plan(100, 1000, out_bits=3)
+
+
+@pytest.mark.parametrize("L", [15, 16, 17, 31, 32, 33, 63, 64, 65, 95, 96, 97, 126, 127, 128, 200])
+def test_equal_length_reads_at_the_kernel_dispatch_boundaries(L):
+    """Collections of equal-length reads take their own scan kernels: one read per thread for 16 <= L <= 127 (a 128-bit mask per
+    thread: positions 31/32, 63/64, 95/96 cross its words; L = 127 fills it), the 8192-slot walk otherwise.  Single batch (fused
+    listing), several batches (count + select), 64-bit ids and two shards; 700 reads = two full tiles of 256 and a ragged one.
+    Reads are copies from a short genome: deep ties, duplicates."""
+    rng = np.random.default_rng(1000 + L)
+    genome = np.frombuffer(b"ACGT", np.uint8)[rng.integers(0, 4, 3 * L + 40)]
+    starts = rng.integers(0, genome.size - L + 1, 700)
+    reads = ["".join(map(chr, genome[s:s + L])) for s in starts]
+    c = gen.from_strings(reads)
+    assert_parity(c)
+    assert_parity(c, max_batch_suffixes=c.n_suffixes // 5 + 1, prefix_len=3)
+    assert_parity(c, max_batch_suffixes=c.n_suffixes // 3 + 1, max_read_len=0)      # unknown read length: 64-bit ids
+    import paper_1401_7457_b200 as cx
+    want = oracle.bwt(c.ascii, c.offsets)
+    a = torch.from_numpy(c.ascii).cuda()
+    off = torch.from_numpy(c.offsets.astype(np.int64)).cuda()
+    packed = cx.cx_pack_reads(a)
+    out = torch.zeros(c.n_suffixes, dtype=torch.uint8, device="cuda")
+    for k in range(2):
+        p = cx.Plan(c.n_reads, c.total_bases, max_read_len=L, shard_index=k, shard_count=2)
+        p.build(packed, off, c.n_reads, out)
+        p.free()
+    assert np.array_equal(out.cpu().numpy(), want)
+
+
+def test_bad_finish_slots_option_is_rejected():
+    import paper_1401_7457_b200 as cx
+    with pytest.raises(cx.CxError):
+        cx.Plan(100, 1000, finish_slots=3)
