@@ -1008,11 +1008,14 @@ __global__ void __launch_bounds__(kListThreads) list_write_reads_kernel(Reads R,
                                                                         unsigned long long* __restrict__ digit_hist,
                                                                         unsigned long long* __restrict__ bucket_hist, uint64_t max_n) {
     __shared__ uint64_t s_packed[kReadTileWords];
-    __shared__ uint32_t s_dh[8][kRadix];   // digit counts of every radix pass of the sort that follows (a6's upfront histogram)
+    // digit counts of every radix pass of the sort that follows (a6's upfront histogram), one 16-bit counter per (pass, digit,
+    // lane): lanes 2k and 2k + 1 share a word, every lane pair has a bank of its own -- at most a 2-way bank conflict where
+    // counters indexed by the digit alone see 3.4 lanes per bank with random digits.  Flushed before a counter can overflow.
     __shared__ uint64_t s_stage[kListThreads * kStagePitch];   // PACKED: key << 32 | id; else keys, and ids in s_stage_id
     extern __shared__ __align__(8) unsigned char s_dyn[];      // [!PACKED: id staging rows][partition counters, laid out as in bucket_hist_kernel]
     uint64_t* s_stage_id = reinterpret_cast<uint64_t*>(s_dyn);
-    uint32_t* s_bh = reinterpret_cast<uint32_t*>(s_dyn + (PACKED ? 0 : sizeof(uint64_t) * kListThreads * kStagePitch));
+    uint32_t* s_dl = reinterpret_cast<uint32_t*>(s_dyn + (PACKED ? 0 : sizeof(uint64_t) * kListThreads * kStagePitch));   // [pass][digit][16]
+    uint32_t* s_bh = s_dl + n_passes * kRadix * 16;
     const uint32_t n_kmers = 1u << (2 * ell), n_short = (n_kmers - 1) / 3;
     if (bucket_hist)
         for (uint32_t k = threadIdx.x; k < n_kmers + n_short; k += blockDim.x) s_bh[k] = 0;
@@ -1021,9 +1024,27 @@ __global__ void __launch_bounds__(kListThreads) list_write_reads_kernel(Reads R,
     const uint64_t L64 = info->first_len;
     if (N > max_n || info->bad_offsets || info->nonuniform || L64 < (uint64_t)kReadMinLen || L64 > (uint64_t)kReadMaxLen) return;   // list_write_kernel has it
     const uint64_t n_tiles = (R.n_reads + kListThreads - 1) / kListThreads;
-    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) (&s_dh[0][0])[i] = 0;
+    for (uint32_t i = threadIdx.x; i < n_passes * kRadix * 16; i += kListThreads) s_dl[i] = 0;
     const uint32_t tid = threadIdx.x;
+    const uint32_t my_word = (tid & 31) >> 1, my_inc = (tid & 1) ? 0x10000u : 1u;
+    auto flush_digits = [&]() {   // all threads; the counters are zero afterwards
+        __syncthreads();
+        for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) {
+            uint32_t sum = 0;
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                const uint32_t v = s_dl[i * 16 + q];
+                sum += (v & 0xffffu) + (v >> 16);
+                s_dl[i * 16 + q] = 0;
+            }
+            if (sum) atomicAdd(digit_hist + i, (unsigned long long)sum);
+        }
+        __syncthreads();
+    };
+    uint32_t tiles_since_flush = 0;
     for (uint64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        // a counter takes at most 8 warps x 128 positions per tile: flush before 65535
+        if (++tiles_since_flush > 60) flush_digits(), tiles_since_flush = 1;
         __syncthreads();   // previous tile done with s_packed and the staging rows (and the counters zeroed on the first trip)
         const ReadTileCtx c = load_read_tile(R, info, t, s_packed);
         const uint32_t L = c.L, L1 = L + 1;
@@ -1047,7 +1068,9 @@ __global__ void __launch_bounds__(kListThreads) list_write_reads_kernel(Reads R,
                         }
                     }
                     const KeyT key = first_key_as<KeyT>(win, (uint64_t)left, w);
-                    digit_counts(s_dh, key, n_passes);
+#pragma unroll
+                    for (uint32_t q = 0; q < sizeof(KeyT); ++q)
+                        if (q < n_passes) atomicAdd(&s_dl[((q * kRadix + ((uint32_t)(key >> (q * kRadixBits)) & (kRadix - 1))) << 4) + my_word], my_inc);
                     if constexpr (PACKED) {
                         s_stage[tid * kStagePitch + i] = ((uint64_t)key << 32) | id_hi | p;
                     } else {
@@ -1075,11 +1098,7 @@ __global__ void __launch_bounds__(kListThreads) list_write_reads_kernel(Reads R,
             __syncthreads();
         }
     }
-    __syncthreads();
-    for (uint32_t i = threadIdx.x; i < n_passes * kRadix; i += kListThreads) {
-        uint32_t v = (&s_dh[0][0])[i];
-        if (v) atomicAdd(digit_hist + i, (unsigned long long)v);
-    }
+    flush_digits();
     if (bucket_hist) {
         for (uint32_t k = threadIdx.x; k < n_kmers; k += blockDim.x) {
             uint32_t v = s_bh[k];
@@ -1205,9 +1224,9 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
         // returns at once.
         if (skip_reads) {
             auto kernel = packed ? list_write_reads_kernel<KeyT, IdT, kCanPack> : list_write_reads_kernel<KeyT, IdT, false>;
-            const size_t stage_id = packed ? 0 : sizeof(uint64_t) * kListThreads * kStagePitch;
+            const size_t stage_id = (packed ? 0 : sizeof(uint64_t) * kListThreads * kStagePitch) + (size_t)n_passes * kRadix * 16 * sizeof(uint32_t);
             const size_t smem_r = smem + stage_id;
-            cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bucket_hist_smem(7) - sizeof(TileSmem) + stage_id));
+            cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_r);
             if (e != cudaSuccess) return e;
             int per_sm = 0;
             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kListThreads, smem_r);
