@@ -824,18 +824,33 @@ __device__ __forceinline__ uint64_t window_at(const uint64_t* packed_sm, uint32_
     const uint64_t w0 = packed_sm[wi], w1 = packed_sm[wi + 1];
     return sh ? (w0 << sh) | (w1 >> (64 - sh)) : w0;
 }
-// f(p, partition code) for every position p = 0 .. L of the thread's read (p = L: the end-marker suffix)
+// f(partition code) for every position p = 0 .. L of the thread's read (p = L: the end-marker suffix).  Positions with at least
+// l bases left (all but the last l of a read) go in blocks of eight without length arithmetic; every branch depends on p, L and
+// l only: the same in every lane.
 template <typename F>
 __device__ __forceinline__ void read_walk(const uint64_t* packed_sm, uint32_t brel, uint32_t L, uint32_t ell, F&& f) {
-    uint32_t top = 0;
+    const uint32_t e1 = ell + 1, sh = 32 - 2 * ell;
+    const uint32_t n_full = L + 1 - ell;              // positions 0 .. n_full - 1 have at least l bases left (L >= kReadMinLen > l)
+    uint32_t p = 0;
+    for (; p + 8 <= n_full; p += 8) {
+        uint32_t top = top16_at(packed_sm, brel + p);   // 16 bases; 8 are consumed: l <= 7 stay valid
 #pragma unroll
-    for (int p = 0; p <= kReadMaxLen; ++p) {
-        if ((uint32_t)p <= L) {                           // the same in every lane
-            if ((p & 7) == 0) top = top16_at(packed_sm, brel + p);   // at most 7 bases are consumed before the next refill: l <= 7 stay valid
-            const uint32_t left = L - (uint32_t)p, r = left < ell ? left : ell;
-            // the first l bases with those past the end of the read cleared (A-padded), then the length: reading A4 of PAPER.md:79
-            const uint32_t kmer = (top >> (32 - 2 * ell)) & (0xffffffffu << (2 * (ell - r)));
-            f(p, kmer * (ell + 1) + r);
+        for (int i = 0; i < 8; ++i) {
+            f((top >> sh) * e1 + ell);
+            top <<= 2;
+        }
+    }
+    for (; p <= L; p += 8) {
+        uint32_t top = top16_at(packed_sm, brel + p);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const uint32_t q = p + i;
+            if (q <= L) {
+                const uint32_t left = L - q, r = left < ell ? left : ell;
+                // the first l bases with those past the end of the read cleared (A-padded), then the length: reading A4 of PAPER.md:79
+                const uint32_t kmer = (top >> sh) & (0xffffffffu << (2 * (ell - r)));
+                f(kmer * e1 + r);
+            }
             top <<= 2;
         }
     }
@@ -898,7 +913,7 @@ __global__ void __launch_bounds__(kListThreads) list_count_reads_kernel(Reads R,
         const ReadTileCtx c = load_read_tile(R, info, t, s_packed);
         uint64_t mine = 0;   // eight 8-bit counters (at most 128 slots per thread)
         if (threadIdx.x < c.n) {
-            read_walk(s_packed, c.brel0 + threadIdx.x * c.L, c.L, ell, [&](int, uint32_t code) {
+            read_walk(s_packed, c.brel0 + threadIdx.x * c.L, c.L, ell, [&](uint32_t code) {
                 uint32_t j = code >= s_first[4] ? 4u : 0u;   // which of the group's batches owns the partition
                 j += code >= s_first[j + 2] ? 2u : 0u;
                 j += code >= s_first[j + 1] ? 1u : 0u;
