@@ -55,7 +55,7 @@ KERNEL_NAMES = {"pack": "pack_kernel (a1)", "prep": "prep_kernel + tile_table_ke
                 "sort_scan": "bin_scan_kernel (a6)", "sort_pass": "onesweep_pass_kernel (a6, one radix pass of the first sort)",
                 "finish": "finish_warp_kernel (a7+a8: head flags, tie groups of <= 64 refined in registers, emit)",
                 "finish_block": "finish_tile_kernel (a7+a8: tie groups of 65..256 refined in shared memory)",
-                "refine_scan": "publish heads + active_count + scan (a7, global path)",
+                "refine_scan": "active_count + scan (a7, global path)",
                 "refine_key": "refine_rekey_kernel (a7, global path)", "refine_write": "refine_writeback_kernel (a7+a8, global path)",
                 "refine_sort": "onesweep_pass_kernel (a7, global path re-sort)", "fasta": "fasta_* kernels (NEXT-4 ingest)"}
 
