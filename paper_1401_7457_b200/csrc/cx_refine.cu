@@ -751,12 +751,15 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
 // the global path (only their head bit is published, their ids handed over, and they are counted).
 // ---------------------------------------------------------------------------------------------
 #ifndef CX_WARP_CHUNK
-#define CX_WARP_CHUNK 2048
+#define CX_WARP_CHUNK 4096
 #endif
 #ifndef CX_WARP_MINB
 #define CX_WARP_MINB 3
 #endif
 constexpr int kWarpChunk = CX_WARP_CHUNK;    // sorted positions per warp: a chunk owns the groups that START in it
+#ifndef CX_WARP_QUEUE
+#define CX_WARP_QUEUE 1
+#endif
 constexpr int kWarpThreads = 256;
 // slots per lane: 2 (windows of 64 positions, two-level keys) unless the batch's tie groups are mostly larger, then 4
 // (windows of 128 positions; the rank key has room for one level only)
@@ -902,6 +905,37 @@ __device__ __forceinline__ void window_words(const uint64_t* __restrict__ packed
     }
 }
 
+// Group bounds of every window position from head bits (bit i of hb[s]: position 32 s + i starts a group; bit 0 of hb[S], the
+// position after the window, is set): gs = the last head at or below the position, ge = the next head above it.
+template <int S>
+__device__ __forceinline__ void bounds_from_heads(const uint32_t (&hb)[S + 1], uint32_t lane, uint32_t (&gs)[S], uint32_t (&ge)[S]) {
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+        const uint32_t p = 32 * s + lane;
+        uint32_t lo_bits = hb[s] & (0xffffffffu >> (31 - lane));
+        gs[s] = 32 * s + 31 - (uint32_t)__clz(lo_bits);
+#pragma unroll
+        for (int t = s - 1; t >= 0; --t)
+            if (!lo_bits && hb[t]) lo_bits = 1, gs[s] = 32 * t + 31 - (uint32_t)__clz(hb[t]);
+        uint32_t hi_bits = lane == 31 ? 0u : hb[s] >> (lane + 1);
+        ge[s] = p + (uint32_t)__ffs(hi_bits);
+#pragma unroll
+        for (int t = s + 1; t <= S; ++t)
+            if (!hi_bits && hb[t]) hi_bits = 1, ge[s] = 32 * t + (uint32_t)__ffs(hb[t]) - 1;
+    }
+}
+
+// Members whose class is still open after the first round of their window wait here, one queue per warp, and are refined
+// again in dense windows of whole classes (a second round over the sparse leftovers of one window costs as much as a full
+// one).  A ring of kQueueCap entries, structure of arrays; an entry is a member's state between two rounds.
+constexpr uint32_t kQueueCap = 128, kQueueTake = 64;
+struct WarpQueue {
+    uint32_t win[6][kQueueCap];
+    uint64_t wbase[kQueueCap];
+    uint32_t mrem[kQueueCap];
+    uint32_t meta[kQueueCap];   // symbol code | first of its class << 3 | (sorted position - start of the warp's chunk) << 4
+};
+
 template <typename KeyT, typename IdT, bool PACKED, int S>
 __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finish_warp_kernel(Reads R, const KeyT* __restrict__ keys1, const IdT* __restrict__ ids_in,
                                                                    IdT* __restrict__ ids_out, uint64_t n, uint32_t depth0, uint32_t cap, uint32_t* __restrict__ heads,
@@ -911,7 +945,12 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
     constexpr uint32_t kPosBits = S == 1 ? 5 : S == 2 ? 6 : 7;   // bits of a window position
     constexpr bool kTwoLevels = 2 * kPosBits + 20 <= 32;         // room for the second event in the 32-bit rank key
     constexpr uint32_t kClsBits = kTwoLevels ? 20 : 10;
+    constexpr bool kQueue = CX_WARP_QUEUE && kSpan == kQueueTake;   // leftovers of a window's first round are queued
+    constexpr bool kQueueAll = kQueue && CX_WARP_QUEUE >= 2;      // ... or every member, before its first round
     static_assert(S == 1 || S == 2 || S == 4, "slots per lane");
+    static_assert(kWarpChunk + kSpan < (1 << 28), "a queued position is kept in 28 bits");
+    __shared__ WarpQueue s_queue[kQueue ? kWarpThreads / 32 : 1];
+    WarpQueue& Q = s_queue[kQueue ? threadIdx.x >> 5 : 0];
     const uint32_t lane = lane_id();
     const uint64_t c0 = ((uint64_t)blockIdx.x * (kWarpThreads / 32) + (threadIdx.x >> 5)) * kWarpChunk;
     const uint64_t c1 = c0 + kWarpChunk < n ? c0 + kWarpChunk : n;
@@ -920,146 +959,216 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
     uint32_t n_members = 0, n_sorts = 0, n_over = 0;     // lane 0's tallies
     uint64_t a = c0;
     if (c0 < n && c0 > 0) a = scan_to_head<KeyT, PACKED>(keys1, c0, n);   // groups that began before the chunk are the previous warp's
-    while (a < c1) {
-        // ---- the window [a, a + 32 S): a is a head --------------------------------------------------------------
-        uint64_t word[S];
-        uint32_t hw[S + 1];                                  // bit i of hw[s]: position a + 32 s + i is a head
-        {
-            uint64_t k[S];
+    // ---- the work item: a window of the sorted order [a, a + n_comp), or a window of queued members ---------------------------
+    uint32_t hw[S + 1];                                  // bit i of hw[s]: position a + 32 s + i is a head
+    uint32_t n_comp = 0;
+    uint32_t gs[S], ge[S], code[S], take[S], mrem[S];
+    uint64_t wbase[S];
+    Win6 win[S];
+    bool mine[S], member[S];
+    IdT idv[S];
+    uint32_t open = 0;                                   // lanes with a member of a group that is not finished
+    bool queued = false;                                 // the item came from the queue
+    uint32_t q_head = 0, q_count = 0, q_take = 0;
 #pragma unroll
-            for (int s = 0; s < S; ++s) {
-                const uint64_t j = a + 32 * s + lane;
-                word[s] = j < n ? load_keyword<KeyT, PACKED>(keys1, j) : 0ull;
-                k[s] = key_of<PACKED>(word[s]);
-            }
-            uint32_t carry_in = 1;                           // head bit of the slot's first position
-#pragma unroll
-            for (int s = 0; s < S; ++s) {
-                const uint64_t j = a + 32 * s + lane;
-                uint64_t kn = __shfl_down_sync(kFull, k[s], 1);   // key of the next position
-                const bool valid_next = j + 1 < n;
-                if (s + 1 < S) {
-                    const uint64_t first_of_next_slot = __shfl_sync(kFull, k[s + 1 < S ? s + 1 : s], 0);
-                    if (lane == 31) kn = first_of_next_slot;
-                } else if (lane == 31) {
-                    kn = valid_next ? key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j + 1)) : 0ull;
-                }
-                const bool head_next = !valid_next || kn != k[s] || !((uint32_t)kn & 1u);
-                const uint32_t HN = __ballot_sync(kFull, head_next);
-                hw[s] = (HN << 1) | carry_in;
-                carry_in = HN >> 31;
-            }
-            hw[S] = carry_in;
-        }
-        // complete groups: everything before the last head, or the whole window if position a + 32 S is a head; groups that
-        // start at or after the end of the chunk are the next warp's
-        uint32_t n_comp = kSpan;
-        if (!hw[S]) {
-            n_comp = 0;
-#pragma unroll
-            for (int s = 0; s < S; ++s)
-                if (hw[s]) n_comp = 32 * s + 31 - (uint32_t)__clz(hw[s]);
-        }
-        if (a + n_comp > c1) {                               // c1 - a is 1 .. 32 S - 1 here
-            const uint32_t cut = (uint32_t)(c1 - a);
-            uint32_t first_later = n_comp;
-#pragma unroll
-            for (int s = S - 1; s >= 0; --s) {
-                const uint32_t from = cut > 32u * s ? cut - 32u * s : 0u;
-                const uint32_t later = from >= 32 ? 0u : hw[s] & ~((1u << from) - 1);
-                if (later) first_later = 32 * s + (uint32_t)__ffs(later) - 1;
-            }
-            n_comp = min(n_comp, first_later);
-        }
-        if (n_comp == 0) {
-            // one group fills the window and goes on: more than 32 S members
-            const uint64_t e = scan_to_head<KeyT, PACKED>(keys1, a + kSpan, n);
-            const uint64_t g = e - a;
-            if (g <= cap) {          // the block kernel's: flag the tile it starts in
-                if (lane == 0) atomicOr(big_tiles + (a / kLocalTile >> 5), 1u << (a / kLocalTile & 31));
-            } else {                 // the global path's: only its first position stays a head; hand its ids over, count it
-                clear_heads(heads, a + 1, e);
-                if constexpr (PACKED) {
-                    for (uint64_t q = a + lane; q < e; q += 32) ids_out[q] = (IdT)(uint32_t)load_keyword<KeyT, PACKED>(keys1, q);
-                }
-                n_over += 1;
-            }
-            a = e;
-            continue;
-        }
-        // a head closes the complete part
-#pragma unroll
-        for (int s = 0; s <= S; ++s) {
-            const int lim = (int)n_comp - 32 * s;       // positions of this slot before the closing head
-            const uint32_t keep = lim >= 32 ? kFull : lim <= 0 ? 0u : (1u << lim) - 1;
-            const uint32_t close = lim >= 0 && lim < 32 ? 1u << lim : 0u;
-            hw[s] = (hw[s] & keep) | close;
-        }
-        // ---- my groups inside the window; locators, the base before every suffix, the members' windows: one batch of gathers -----
-        uint32_t gs[S], ge[S], code[S], take[S], mrem[S];
-        uint64_t wbase[S];
-        Win6 win[S];
-        bool mine[S], member[S];
-        IdT idv[S];
-        uint32_t open = 0;
+    for (int s = 0; s < S; ++s) mine[s] = false, member[s] = false, idv[s] = 0, code[s] = 0;
+
+    // emit the finished positions of a sorted-order window; publish head bits (everything finished here counts as a group of
+    // one from now on)
+    auto emit_window = [&]() {
 #pragma unroll
         for (int s = 0; s < S; ++s) {
             const uint32_t p = 32 * s + lane;
             const uint64_t j = a + p;
+            if (mine[s] && !member[s]) out[j] = (uint8_t)(0x544743412400ull >> (8 * code[s]));
             const bool active = p < n_comp && j < n;
-            // first position of my group: the last head at or below p; one past its last: the next head above p
-            uint32_t lo_bits = hw[s] & (0xffffffffu >> (31 - lane));
-            gs[s] = 32 * s + 31 - (uint32_t)__clz(lo_bits);
-#pragma unroll
-            for (int t = s - 1; t >= 0; --t)
-                if (!lo_bits && hw[t]) lo_bits = 1, gs[s] = 32 * t + 31 - (uint32_t)__clz(hw[t]);
-            uint32_t hi_bits = lane == 31 ? 0u : hw[s] >> (lane + 1);
-            ge[s] = p + (uint32_t)__ffs(hi_bits);
-#pragma unroll
-            for (int t = s + 1; t <= S; ++t)
-                if (!hi_bits && hw[t]) hi_bits = 1, ge[s] = 32 * t + (uint32_t)__ffs(hw[t]) - 1;
-            if (!active) gs[s] = p, ge[s] = p + 1;
-            const uint32_t size = ge[s] - gs[s];
-            mine[s] = active && size <= cap_a;              // (a complete group larger than cap_a exists only when cap < 32 S)
-            member[s] = mine[s] && size >= 2;
-            idv[s] = 0;
-            if (active) {
-                if constexpr (PACKED) idv[s] = (IdT)(uint32_t)word[s];
-                else idv[s] = __ldg(ids_in + j);
+            const bool over = active && !mine[s];             // a complete group of more than cap members (cap < 32 S only)
+            if (__any_sync(kFull, over)) {                    // the global path's: clear all but its first position's head bit
+                const bool over_head = over && ((hw[s] >> lane) & 1u);
+                if constexpr (PACKED) {
+                    if (over) ids_out[j] = idv[s];
+                }
+                const uint32_t clear = __ballot_sync(kFull, over && !over_head), over_heads = __ballot_sync(kFull, over_head);
+                const uint64_t at = a + 32 * s;
+                const uint32_t sh = (uint32_t)(at & 31);
+                if (lane == 0 && (clear << sh)) atomicAnd(heads + (at >> 5), ~(clear << sh));
+                if (lane == 1 && sh && (clear >> (32 - sh))) atomicAnd(heads + (at >> 5) + 1, ~(clear >> (32 - sh)));
+                if (lane == 0) n_over += (uint32_t)__popc(over_heads);
             }
         }
-        uint64_t before[S], first_base[S];
+    };
+
+    while (true) {
+        if (!open) {
+            if (kQueue && (q_count >= kQueueTake || (a >= c1 && q_count))) {
+                // ---- a window of queued members: whole classes, at most 32 S of them ----------------------------------------
+                uint32_t meta[S];
 #pragma unroll
-        for (int s = 0; s < S; ++s) {
-            uint64_t left;
-            const uint64_t read = (uint64_t)idv[s] >> R.pos_bits, pos = (uint64_t)idv[s] & pos_mask;
-            if (R.uniform) {
-                first_base[s] = read * R.uniform_len + pos;
-                left = R.uniform_len - pos;
+                for (int s = 0; s < S; ++s) {
+                    const uint32_t i = 32 * s + lane;
+                    meta[s] = i < q_count ? Q.meta[(q_head + i) & (kQueueCap - 1)] : 8u;
+                }
+                q_take = q_count;
+                if (q_count > kSpan) {
+                    q_take = kSpan;
+                    if (!((Q.meta[(q_head + kSpan) & (kQueueCap - 1)] >> 3) & 1u)) {   // a class would be cut: stop at its head
+#pragma unroll
+                        for (int s = 0; s < S; ++s) {
+                            const uint32_t hd = __ballot_sync(kFull, (meta[s] >> 3) & 1u);
+                            if (hd) q_take = 32 * s + 31 - (uint32_t)__clz(hd);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int s = 0; s < S; ++s) {
+                    const uint32_t i = 32 * s + lane;
+                    const uint32_t slot = (q_head + i) & (kQueueCap - 1);
+                    const bool in = i < q_take;
+                    member[s] = in;
+                    mine[s] = false;
+                    code[s] = meta[s] & 7u;
+                    hw[s] = __ballot_sync(kFull, !in || ((meta[s] >> 3) & 1u));
+                    mrem[s] = in ? Q.mrem[slot] : 0u;
+                    take[s] = mrem[s] < kWin ? mrem[s] : kWin;
+                    wbase[s] = Q.wbase[slot];
+#pragma unroll
+                    for (int w = 0; w < 6; ++w) win[s].w[w] = Q.win[w][slot];
+                }
+                hw[S] = 1;
+                bounds_from_heads<S>(hw, lane, gs, ge);
+                queued = true;
+                open = 1;
+            } else if (a < c1) {
+                // ---- the window [a, a + 32 S): a is a head --------------------------------------------------------------
+                uint64_t word[S];
+                {
+                    uint64_t k[S];
+#pragma unroll
+                    for (int s = 0; s < S; ++s) {
+                        const uint64_t j = a + 32 * s + lane;
+                        word[s] = j < n ? load_keyword<KeyT, PACKED>(keys1, j) : 0ull;
+                        k[s] = key_of<PACKED>(word[s]);
+                    }
+                    uint32_t carry_in = 1;                           // head bit of the slot's first position
+#pragma unroll
+                    for (int s = 0; s < S; ++s) {
+                        const uint64_t j = a + 32 * s + lane;
+                        uint64_t kn = __shfl_down_sync(kFull, k[s], 1);   // key of the next position
+                        const bool valid_next = j + 1 < n;
+                        if (s + 1 < S) {
+                            const uint64_t first_of_next_slot = __shfl_sync(kFull, k[s + 1 < S ? s + 1 : s], 0);
+                            if (lane == 31) kn = first_of_next_slot;
+                        } else if (lane == 31) {
+                            kn = valid_next ? key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j + 1)) : 0ull;
+                        }
+                        const bool head_next = !valid_next || kn != k[s] || !((uint32_t)kn & 1u);
+                        const uint32_t HN = __ballot_sync(kFull, head_next);
+                        hw[s] = (HN << 1) | carry_in;
+                        carry_in = HN >> 31;
+                    }
+                    hw[S] = carry_in;
+                }
+                // complete groups: everything before the last head, or the whole window if position a + 32 S is a head; groups that
+                // start at or after the end of the chunk are the next warp's
+                n_comp = kSpan;
+                if (!hw[S]) {
+                    n_comp = 0;
+#pragma unroll
+                    for (int s = 0; s < S; ++s)
+                        if (hw[s]) n_comp = 32 * s + 31 - (uint32_t)__clz(hw[s]);
+                }
+                if (a + n_comp > c1) {                               // c1 - a is 1 .. 32 S - 1 here
+                    const uint32_t cut = (uint32_t)(c1 - a);
+                    uint32_t first_later = n_comp;
+#pragma unroll
+                    for (int s = S - 1; s >= 0; --s) {
+                        const uint32_t from = cut > 32u * s ? cut - 32u * s : 0u;
+                        const uint32_t later = from >= 32 ? 0u : hw[s] & ~((1u << from) - 1);
+                        if (later) first_later = 32 * s + (uint32_t)__ffs(later) - 1;
+                    }
+                    n_comp = min(n_comp, first_later);
+                }
+                if (n_comp == 0) {
+                    // one group fills the window and goes on: more than 32 S members
+                    const uint64_t e = scan_to_head<KeyT, PACKED>(keys1, a + kSpan, n);
+                    const uint64_t g = e - a;
+                    if (g <= cap) {          // the block kernel's: flag the tile it starts in
+                        if (lane == 0) atomicOr(big_tiles + (a / kLocalTile >> 5), 1u << (a / kLocalTile & 31));
+                    } else {                 // the global path's: only its first position stays a head; hand its ids over, count it
+                        clear_heads(heads, a + 1, e);
+                        if constexpr (PACKED) {
+                            for (uint64_t q = a + lane; q < e; q += 32) ids_out[q] = (IdT)(uint32_t)load_keyword<KeyT, PACKED>(keys1, q);
+                        }
+                        n_over += 1;
+                    }
+                    a = e;
+                    continue;
+                }
+                // a head closes the complete part
+#pragma unroll
+                for (int s = 0; s <= S; ++s) {
+                    const int lim = (int)n_comp - 32 * s;       // positions of this slot before the closing head
+                    const uint32_t keep = lim >= 32 ? kFull : lim <= 0 ? 0u : (1u << lim) - 1;
+                    const uint32_t close = lim >= 0 && lim < 32 ? 1u << lim : 0u;
+                    hw[s] = (hw[s] & keep) | close;
+                }
+                // ---- my groups inside the window; locators, the base before every suffix, the members' windows: one batch of gathers -----
+                bounds_from_heads<S>(hw, lane, gs, ge);
+#pragma unroll
+                for (int s = 0; s < S; ++s) {
+                    const uint32_t p = 32 * s + lane;
+                    const uint64_t j = a + p;
+                    const bool active = p < n_comp && j < n;
+                    if (!active) gs[s] = p, ge[s] = p + 1;
+                    const uint32_t size = ge[s] - gs[s];
+                    mine[s] = active && size <= cap_a;              // (a complete group larger than cap_a exists only when cap < 32 S)
+                    member[s] = mine[s] && size >= 2;
+                    idv[s] = 0;
+                    if (active) {
+                        if constexpr (PACKED) idv[s] = (IdT)(uint32_t)word[s];
+                        else idv[s] = __ldg(ids_in + j);
+                    }
+                }
+                uint64_t before[S], first_base[S];
+#pragma unroll
+                for (int s = 0; s < S; ++s) {
+                    uint64_t left;
+                    const uint64_t read = (uint64_t)idv[s] >> R.pos_bits, pos = (uint64_t)idv[s] & pos_mask;
+                    if (R.uniform) {
+                        first_base[s] = read * R.uniform_len + pos;
+                        left = R.uniform_len - pos;
+                    } else {
+                        const uint64_t* q = R.offsets + (mine[s] ? read : 0ull);
+                        const uint64_t lo = __ldg(q), hi = __ldg(q + 1);
+                        first_base[s] = lo + pos;
+                        left = hi - lo - pos;
+                    }
+                    const bool has_prev = mine[s] && pos;
+                    before[s] = has_prev ? __ldg(R.packed + ((first_base[s] - 1) >> 5)) : 0ull;   // no load for a read's first suffix
+                    wbase[s] = first_base[s] + depth0;                // index of the window's first base
+                    mrem[s] = member[s] ? (uint32_t)(left - depth0) : 0u;   // a member of an open group has >= depth0 bases
+                    take[s] = mrem[s] < kWin ? mrem[s] : kWin;
+                    code[s] = has_prev ? 2u : 1u;                     // 1 = $: the suffix starts its read
+                }
+#pragma unroll
+                for (int s = 0; s < S; ++s) window_words(R.packed, wbase[s], take[s], member[s], win[s]);
+#pragma unroll
+                for (int s = 0; s < S; ++s) {
+                    if (code[s] == 2u) code[s] = 2 + (uint32_t)((before[s] >> (62 - 2 * ((first_base[s] - 1) & 31))) & 3u);
+                    const uint32_t mb = __ballot_sync(kFull, member[s]);
+                    open |= mb;
+                    if (lane == 0) n_members += (uint32_t)__popc(mb);
+                }
+                queued = false;
             } else {
-                const uint64_t* q = R.offsets + (mine[s] ? read : 0ull);
-                const uint64_t lo = __ldg(q), hi = __ldg(q + 1);
-                first_base[s] = lo + pos;
-                left = hi - lo - pos;
+                break;
             }
-            const bool has_prev = mine[s] && pos;
-            before[s] = has_prev ? __ldg(R.packed + ((first_base[s] - 1) >> 5)) : 0ull;   // no load for a read's first suffix
-            wbase[s] = first_base[s] + depth0;                // index of the window's first base
-            mrem[s] = member[s] ? (uint32_t)(left - depth0) : 0u;   // a member of an open group has >= depth0 bases
-            take[s] = mrem[s] < kWin ? mrem[s] : kWin;
-            code[s] = has_prev ? 2u : 1u;                     // 1 = $: the suffix starts its read
         }
+        // ---- one round over the item's open groups -----------------------------------------------------------------------------
+        uint32_t hb[S + 1];
 #pragma unroll
-        for (int s = 0; s < S; ++s) window_words(R.packed, wbase[s], take[s], member[s], win[s]);
-#pragma unroll
-        for (int s = 0; s < S; ++s) {
-            if (code[s] == 2u) code[s] = 2 + (uint32_t)((before[s] >> (62 - 2 * ((first_base[s] - 1) & 31))) & 3u);
-            const uint32_t mb = __ballot_sync(kFull, member[s]);
-            open |= mb;
-            if (lane == 0) n_members += (uint32_t)__popc(mb);
-        }
-        // ---- rounds over the groups of the window that are still open ---------------------------------------------------------
-        while (open) {
+        for (int s = 0; s <= S; ++s) hb[s] = hw[s];
+        if (open && (queued || !kQueueAll)) {
             // pivot of every group: its member with the most bases in its window (segmented max scan, read at the group's last position)
             uint32_t best[S];
 #pragma unroll
@@ -1136,7 +1245,6 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
             // the member that ranked at each position; classes = runs of equal (level 1, level 2)
             uint32_t src[S], cls[S];
             bool head[S], was[S], nextwin[S];
-            uint32_t hb[S + 1];
 #pragma unroll
             for (int s = 0; s < S; ++s) {
                 src[s] = (key[s] >> (32 - kPosBits)) + (key[s] & (kSpan - 1));
@@ -1179,8 +1287,7 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
 #pragma unroll
                 for (int s = 0; s < S; ++s) code[s] = r[s];
             }
-            if (!open) break;
-            {
+            if (open) {
                 uint32_t col[S], r[S];
 #pragma unroll
                 for (int i = 0; i < 6; ++i) {
@@ -1203,23 +1310,13 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
 #pragma unroll
                 for (int s = 0; s < S; ++s) wbase[s] = r64[s];
             }
+#pragma unroll
+            for (int s = 0; s < S; ++s) member[s] = still[s];
+            if (open) {
             bool any_next = false;
+            bounds_from_heads<S>(hb, lane, gs, ge);
 #pragma unroll
-            for (int s = 0; s < S; ++s) {
-                const uint32_t p = 32 * s + lane;
-                member[s] = still[s];
-                uint32_t lo_bits = hb[s] & (0xffffffffu >> (31 - lane));
-                gs[s] = 32 * s + 31 - (uint32_t)__clz(lo_bits);
-#pragma unroll
-                for (int t = s - 1; t >= 0; --t)
-                    if (!lo_bits && hb[t]) lo_bits = 1, gs[s] = 32 * t + 31 - (uint32_t)__clz(hb[t]);
-                uint32_t hi_bits = lane == 31 ? 0u : hb[s] >> (lane + 1);
-                ge[s] = p + (uint32_t)__ffs(hi_bits);
-#pragma unroll
-                for (int t = s + 1; t <= S; ++t)
-                    if (!hi_bits && hb[t]) hi_bits = 1, ge[s] = 32 * t + (uint32_t)__ffs(hb[t]) - 1;
-                any_next |= __any_sync(kFull, member[s] && nextwin[s]);
-            }
+            for (int s = 0; s < S; ++s) any_next |= __any_sync(kFull, member[s] && nextwin[s]);
             if (any_next) {                                 // equal to the pivot through a full window: the next window of the read
 #pragma unroll
                 for (int s = 0; s < S; ++s) {
@@ -1234,29 +1331,47 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
                     if (g) win[s] = nw;
                 }
             }
-        }
-        // ---- emit; publish head bits (everything finished here counts as a group of one from now on) -----------------------
-#pragma unroll
-        for (int s = 0; s < S; ++s) {
-            const uint32_t p = 32 * s + lane;
-            const uint64_t j = a + p;
-            if (mine[s]) out[j] = (uint8_t)(0x544743412400ull >> (8 * code[s]));
-            const bool active = p < n_comp && j < n;
-            const bool over = active && !mine[s];             // a complete group of more than cap members (cap < 32 S only)
-            if (__any_sync(kFull, over)) {                    // the global path's: clear all but its first position's head bit
-                const bool over_head = over && ((hw[s] >> lane) & 1u);
-                if constexpr (PACKED) {
-                    if (over) ids_out[j] = idv[s];
-                }
-                const uint32_t clear = __ballot_sync(kFull, over && !over_head), over_heads = __ballot_sync(kFull, over_head);
-                const uint64_t at = a + 32 * s;
-                const uint32_t sh = (uint32_t)(at & 31);
-                if (lane == 0 && (clear << sh)) atomicAnd(heads + (at >> 5), ~(clear << sh));
-                if (lane == 1 && sh && (clear >> (32 - sh))) atomicAnd(heads + (at >> 5) + 1, ~(clear >> (32 - sh)));
-                if (lane == 0) n_over += (uint32_t)__popc(over_heads);
             }
         }
-        a += n_comp;
+        if (!queued) {
+            if (kQueue) {
+                // the window's finished positions are emitted now; the members of its open classes wait in the queue
+                emit_window();
+                if (open) {
+                    uint32_t at = q_head + q_count;
+#pragma unroll
+                    for (int s = 0; s < S; ++s) {
+                        const uint32_t mb = __ballot_sync(kFull, member[s]);
+                        if (member[s]) {
+                            const uint32_t slot = (at + (uint32_t)__popc(mb & ((1u << lane) - 1))) & (kQueueCap - 1);
+#pragma unroll
+                            for (int w = 0; w < 6; ++w) Q.win[w][slot] = win[s].w[w];
+                            Q.wbase[slot] = wbase[s];
+                            Q.mrem[slot] = mrem[s];
+                            Q.meta[slot] = code[s] | (((hb[s] >> lane) & 1u) << 3) | ((uint32_t)(a + 32 * s + lane - c0) << 4);
+                        }
+                        at += (uint32_t)__popc(mb);
+                    }
+                    q_count = at - q_head;
+                    __syncwarp();
+                    open = 0;
+                }
+                a += n_comp;
+            } else if (!open) {
+                emit_window();
+                a += n_comp;
+            }
+        } else if (!open) {
+            // the queued window is finished: its symbols go to the positions its members were queued from
+#pragma unroll
+            for (int s = 0; s < S; ++s) {
+                const uint32_t i = 32 * s + lane;
+                if (i < q_take) out[c0 + (Q.meta[(q_head + i) & (kQueueCap - 1)] >> 4)] = (uint8_t)(0x544743412400ull >> (8 * code[s]));
+            }
+            __syncwarp();
+            q_head += q_take;
+            q_count -= q_take;
+        }
     }
     // ---- tallies: one update per block ------------------------------------------------------------------------------------------
     __shared__ uint32_t s_tally[3];
