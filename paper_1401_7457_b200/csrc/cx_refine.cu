@@ -750,13 +750,12 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
 // Groups of more than 32 S and at most cap suffixes are left to the block kernel (their tile is flagged); larger ones to
 // the global path (only their head bit is published, their ids handed over, and they are counted).
 // ---------------------------------------------------------------------------------------------
-#ifndef CX_WARP_CHUNK
-#define CX_WARP_CHUNK 4096
-#endif
 #ifndef CX_WARP_MINB
 #define CX_WARP_MINB 3
 #endif
-constexpr int kWarpChunk = CX_WARP_CHUNK;    // sorted positions per warp: a chunk owns the groups that START in it
+// sorted positions per warp (a chunk owns the groups that START in it): the larger one when the batch still fills the GPU
+// several times over (fewer partly filled queue windows at the ends of chunks)
+constexpr uint32_t kWarpChunkSmall = 2048, kWarpChunkLarge = 4096, kWarpChunkWaves = 8;
 #ifndef CX_WARP_QUEUE
 #define CX_WARP_QUEUE 1
 #endif
@@ -940,7 +939,7 @@ template <typename KeyT, typename IdT, bool PACKED, int S>
 __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finish_warp_kernel(Reads R, const KeyT* __restrict__ keys1, const IdT* __restrict__ ids_in,
                                                                    IdT* __restrict__ ids_out, uint64_t n, uint32_t depth0, uint32_t cap, uint32_t* __restrict__ heads,
                                                                    uint32_t* __restrict__ big_tiles, uint8_t* __restrict__ out,
-                                                                   unsigned long long* counters) {
+                                                                   unsigned long long* counters, uint32_t chunk) {
     constexpr uint32_t kSpan = 32 * S;                  // positions per window
     constexpr uint32_t kPosBits = S == 1 ? 5 : S == 2 ? 6 : 7;   // bits of a window position
     constexpr bool kTwoLevels = 2 * kPosBits + 20 <= 32;         // room for the second event in the 32-bit rank key
@@ -948,12 +947,12 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
     constexpr bool kQueue = CX_WARP_QUEUE && kSpan == kQueueTake;   // leftovers of a window's first round are queued
     constexpr bool kQueueAll = kQueue && CX_WARP_QUEUE >= 2;      // ... or every member, before its first round
     static_assert(S == 1 || S == 2 || S == 4, "slots per lane");
-    static_assert(kWarpChunk + kSpan < (1 << 28), "a queued position is kept in 28 bits");
+    static_assert(kWarpChunkLarge + kSpan < (1 << 28), "a queued position is kept in 28 bits");
     __shared__ WarpQueue s_queue[kQueue ? kWarpThreads / 32 : 1];
     WarpQueue& Q = s_queue[kQueue ? threadIdx.x >> 5 : 0];
     const uint32_t lane = lane_id();
-    const uint64_t c0 = ((uint64_t)blockIdx.x * (kWarpThreads / 32) + (threadIdx.x >> 5)) * kWarpChunk;
-    const uint64_t c1 = c0 + kWarpChunk < n ? c0 + kWarpChunk : n;
+    const uint64_t c0 = ((uint64_t)blockIdx.x * (kWarpThreads / 32) + (threadIdx.x >> 5)) * chunk;
+    const uint64_t c1 = c0 + chunk < n ? c0 + chunk : n;
     const uint32_t cap_a = cap < kSpan ? cap : kSpan;   // largest group finished here
     const uint64_t pos_mask = (1ull << R.pos_bits) - 1;
     uint32_t n_members = 0, n_sorts = 0, n_over = 0;     // lane 0's tallies
@@ -1486,9 +1485,11 @@ cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, 
     {   // singletons and groups of at most 32: one warp per chunk, registers only
         // a7 flagging (key + 1) and a8 emit (id + base + byte) per suffix; the refined suffixes' term is added by the caller
         ScopedLaunch sl(prof, CX_K_FINISH, n * (sizeof(KeyT) + 1 + sizeof(IdT) + 2), s);
-        const uint64_t warps = (n + kWarpChunk - 1) / kWarpChunk;
+        const uint64_t resident_warps = (uint64_t)n_sms * (slots == (uint32_t)kWarpSlotsLarge ? 2 : CX_WARP_MINB) * (kWarpThreads / 32);
+        const uint32_t chunk = n >= resident_warps * kWarpChunkWaves * kWarpChunkLarge ? kWarpChunkLarge : kWarpChunkSmall;
+        const uint64_t warps = (n + chunk - 1) / chunk;
         const unsigned grid = (unsigned)((warps + kWarpThreads / 32 - 1) / (kWarpThreads / 32));
-        auto launch = [&](auto kernel) { kernel<<<grid, kWarpThreads, 0, s>>>(R, keys1, ids, ids, n, depth0, group_cap, heads_out, big_tiles, out, elems_done); };
+        auto launch = [&](auto kernel) { kernel<<<grid, kWarpThreads, 0, s>>>(R, keys1, ids, ids, n, depth0, group_cap, heads_out, big_tiles, out, elems_done, chunk); };
         if (slots == (uint32_t)kWarpSlotsLarge) {
             if (packed) launch(finish_warp_kernel<KeyT, IdT, kCanPack, kWarpSlotsLarge>);
             else launch(finish_warp_kernel<KeyT, IdT, false, kWarpSlotsLarge>);

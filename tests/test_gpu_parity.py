@@ -437,6 +437,23 @@ def test_equal_length_reads_at_the_kernel_dispatch_boundaries(L):
     assert np.array_equal(out.cpu().numpy(), want)
 
 
+@pytest.mark.parametrize("L", [16, 24, 37, 100, 127])
+def test_equal_length_reads_in_many_small_batches(L):
+    """A batch that is a short range of partitions: the select scan finds the positions whose first two bases fit the range
+    with word-wide bit operations (24 positions per 32-base window: L = 24, 37 end a window early) and tests only those
+    exactly; a wider range takes the plain walk.  Random reads (every l-mer about equally often) and copies from a short
+    genome (few, heavy partitions); prefix lengths 2 (the two bases are the whole partition code), 6 and 7."""
+    rng = np.random.default_rng(4000 + L)
+    random_reads = ["".join(rng.choice(list("ACGT"), L)) for _ in range(600)]
+    genome = np.frombuffer(b"ACGT", np.uint8)[rng.integers(0, 4, 2 * L + 30)]
+    copies = ["".join(map(chr, genome[s:s + L])) for s in rng.integers(0, genome.size - L + 1, 300)]
+    for reads in (random_reads, random_reads[:257] + copies):
+        c = gen.from_strings(reads)
+        assert_parity(c, max_batch_suffixes=c.n_suffixes // 40 + 1)
+        assert_parity(c, max_batch_suffixes=c.n_suffixes // 150 + 1, prefix_len=7)
+        assert_parity(c, max_batch_suffixes=c.n_suffixes // 9 + 1, prefix_len=2)
+
+
 def test_bad_finish_slots_option_is_rejected():
     import paper_1401_7457_b200 as cx
     with pytest.raises(cx.CxError):
