@@ -44,8 +44,8 @@ WORKLOADS = {
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed `ncu --set full` captures of THIS round at the
 # benched configuration (profiles/r02_ncu_full.md); keyed by (config, kernel class).  None until a capture exists.
-NCU_TRAFFIC: dict = {(2, "finish"): 103_077_998_000, (2, "sort_pass"): 16_442_251_500, (2, "list"): 10_580_514_000, (2, "pack"): 1_196_039_000,
-                     (2, "finish_block"): 316_000}
+NCU_TRAFFIC: dict = {(2, "finish"): 103_799_879_000, (2, "sort_pass"): 16_442_149_750, (2, "list"): 9_380_498_000, (2, "pack"): 1_195_254_000,
+                     (2, "finish_block"): 315_000}
 NCU_TRAFFIC_FILE = "profiles/r02_ncu_full.md"
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 CPU_SAMPLE_SCALE = {0: 1.0, 1: 0.5, 2: 0.1, 3: 0.01, 4: 0.001}      # cpu_baseline: the recipe at this scale (coverage preserved), all cores
@@ -53,7 +53,7 @@ REF_SAMPLE_SCALE = {0: 1.0, 1: 0.25, 2: 0.04, 3: 0.004, 4: 0.0004}  # --impl ref
 KERNEL_NAMES = {"pack": "pack_kernel (a1)", "prep": "prep_kernel + tile_table_kernel", "hist": "bucket_hist_kernel (a2)",
                 "list": "list_write_reads_kernel / list_write_kernel, or list_count + list_select per batch (a4+a5)", "sort_hist": "digit_hist_kernel (a6)",
                 "sort_scan": "bin_scan_kernel (a6)", "sort_pass": "onesweep_pass_kernel (a6, one radix pass of the first sort)",
-                "finish": "finish_warp_kernel (a7+a8: head flags, tie groups of <= 64 refined in registers, emit)",
+                "finish": "finish_warp_kernel (a7+a8: head flags, tie groups of <= 64 refined in registers, leftovers in dense queued windows, emit)",
                 "finish_block": "finish_tile_kernel (a7+a8: tie groups of 65..256 refined in shared memory)",
                 "refine_scan": "active_count + scan (a7, global path)",
                 "refine_key": "refine_rekey_kernel (a7, global path)", "refine_write": "refine_writeback_kernel (a7+a8, global path)",
