@@ -22,6 +22,7 @@ the `cpu_baseline` leg.
 from __future__ import annotations
 
 import argparse
+import itertools
 import json
 import os
 import statistics
@@ -44,8 +45,8 @@ WORKLOADS = {
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed `ncu --set full` captures of THIS round at the
 # benched configuration (profiles/r02_ncu_full.md); keyed by (config, kernel class).  None until a capture exists.
-NCU_TRAFFIC: dict = {(2, "finish"): 103_799_879_000, (2, "sort_pass"): 16_442_149_750, (2, "list"): 9_380_498_000, (2, "pack"): 1_195_254_000,
-                     (2, "finish_block"): 315_000}
+NCU_TRAFFIC: dict = {(2, "finish"): 103_789_166_000, (2, "sort_pass"): 16_442_852_000, (2, "list"): 9_384_456_000, (2, "pack"): 1_195_324_000,
+                     (2, "finish_block"): 316_000}
 NCU_TRAFFIC_FILE = "profiles/r02_ncu_full.md"
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 CPU_SAMPLE_SCALE = {0: 1.0, 1: 0.5, 2: 0.1, 3: 0.01, 4: 0.001}      # cpu_baseline: the recipe at this scale (coverage preserved), all cores
@@ -562,6 +563,27 @@ def run_cx(args) -> None:
             return ms
         e2e_variants["streamed"] = streamed({}, N, True)
         e2e_variants["streamed_packed"] = streamed({"out_bits": 4}, (N + 1) // 2, False)
+
+        def pipelined() -> float:
+            """THROUGHPUT of back-to-back builds through cx.HostPipeline (two sets of buffers, three streams): while step i computes,
+            step i + 1's reads are copied in and packed and step i - 1's output is copied out.  Every step's H2D and D2H is
+            inside the timed region; ms per step = elapsed / steps.  Not the latency of one step: that is `sequential`."""
+            pp = cx.Plan(n_reads, total, profile=0, **plan_opts)
+            pipe = cx.HostPipeline(pp, n_reads, total)
+            results = pipe.run(itertools.repeat((h_ascii, h_off, n_reads)))
+            seen = []
+
+            def step():
+                seen.append(next(results))              # the result of the step before this one, complete in pinned host memory
+            ms = time_e2e(step)
+            for hout in seen[-2:]:                      # the last two results: one from each set of buffers
+                got = torch.bincount(hout.to(dev).to(torch.int64), minlength=256)
+                if not torch.equal(got, want_counts):
+                    raise SystemExit("bench.py: pipelined output symbol counts differ from the input's")
+            del results, pipe
+            pp.free()
+            return ms
+        e2e_variants["pipelined"] = pipelined()
     e2e_name = min((k for k in e2e_variants if k != "streamed_packed"), key=lambda k: e2e_variants[k])
     e2e_ms = e2e_variants[e2e_name]
 
@@ -644,8 +666,13 @@ def run_cx(args) -> None:
         "e2e": {"value": units * N / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps, "path": e2e_name,
                 "h2d_bytes_per_step": int(h_text.numel()) if args.fasta else int(h_ascii.numel() + h_off.numel() * 8), "d2h_bytes_per_step": int(h_out.numel()),
                 "variants_ms_per_step": {k: round(v, 3) for k, v in e2e_variants.items()},
+                "selected": f"the fastest of the {sum(1 for k in e2e_variants if k != 'streamed_packed')} ASCII-output variants tried (all listed in variants_ms_per_step)",
+                "kind": {"sequential": "latency of one step", "streamed": "latency of one step", "streamed_packed": "latency of one step",
+                         "pipelined": "throughput of overlapped back-to-back steps (elapsed / steps)"}[e2e_name],
                 "variants": "sequential: copy in, cx_bwt_build into device memory, copy out; streamed: cx_bwt_build with out_is_host_pinned in four "
-                            "batches, each batch's copy overlapping the next batch's compute; streamed_packed: the same with out_bits = 4 "
+                            "batches, each batch's copy overlapping the next batch's compute; pipelined: back-to-back builds, step i + 1's copy-in "
+                            "and pack and step i - 1's copy-out on side streams while step i computes (two sets of buffers; every step's H2D and "
+                            "D2H inside the timed region); streamed_packed: the same as streamed with out_bits = 4 "
                             "(half the bytes out; reported only here, e2e is the better of the two ASCII-output paths)"},
         "gpu_launches": int(launches),
         "clocks": clocks,

@@ -157,6 +157,74 @@ def pack_reads_from_host(ascii_host: torch.Tensor, ascii_dev: torch.Tensor, pack
     return packed_out
 
 
+class HostPipeline:
+    """Back-to-back builds from pinned HOST memory with the copies of neighbouring builds overlapped (copies and calls
+    only): while collection i is built, collection i + 1 is copied in and packed on a second stream and the output of
+    collection i - 1 is copied to pinned host memory on a third.  Two sets of device buffers, one plan.
+
+    `run(collections)` takes an iterable of (ascii_host, offsets_host, n_reads) -- pinned uint8 / int64 tensors -- and
+    yields one pinned uint8 tensor per collection, in order.  A yielded tensor is overwritten two collections later:
+    use it (or copy it) before asking for the result after the next.  This is a THROUGHPUT arrangement: the time from
+    a collection's first byte in to its last byte out is longer than with a single build, not shorter."""
+
+    def __init__(self, plan: "Plan", max_reads: int, max_total_bases: int):
+        dev = plan.device
+        self.plan, self.device = plan, dev
+        self.s_in, self.s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+        n_out = max_total_bases + max_reads
+        self.sets = [dict(ascii=torch.empty(max(1, max_total_bases), dtype=torch.uint8, device=dev),
+                          packed=torch.empty((max_total_bases + 31) // 32 + 1, dtype=torch.int64, device=dev),
+                          off=torch.empty(max_reads + 1, dtype=torch.int64, device=dev),
+                          out=torch.empty(max(1, n_out), dtype=torch.uint8, device=dev),
+                          host=torch.empty(max(1, n_out), dtype=torch.uint8).pin_memory(),
+                          in_ready=None, built=None, copied=None) for _ in range(2)]
+
+    def _load(self, b: int, item) -> None:
+        ascii_host, offsets_host, n_reads = item
+        st = self.sets[b]
+        assert offsets_host.dtype == torch.int64 and offsets_host.is_pinned() and offsets_host.numel() == n_reads + 1
+        if st["built"] is not None:
+            self.s_in.wait_event(st["built"])            # the build that read this set is done
+        with torch.cuda.stream(self.s_in):
+            pack_reads_from_host(ascii_host, st["ascii"], st["packed"], stream=self.s_in)
+            st["off"][:n_reads + 1].copy_(offsets_host, non_blocking=True)
+        st["in_ready"] = torch.cuda.Event()
+        st["in_ready"].record(self.s_in)
+
+    def run(self, collections):
+        main = torch.cuda.current_stream(self.device)
+        it = iter(collections)
+        nxt = next(it, None)
+        if nxt is not None:
+            self._load(0, nxt)
+        i, pending = 0, None
+        while nxt is not None:
+            cur, st = nxt, self.sets[i & 1]
+            nxt = next(it, None)
+            main.wait_event(st["in_ready"])
+            if nxt is not None:
+                self._load((i & 1) ^ 1, nxt)             # the next collection arrives while this one is built
+            if st["copied"] is not None:
+                main.wait_event(st["copied"])            # this set's previous output has left the device
+            n_reads, n_out = cur[2], cur[0].numel() + cur[2]
+            self.plan.build(st["packed"], st["off"], n_reads, st["out"], stream=main)
+            st["built"] = torch.cuda.Event()
+            st["built"].record(main)
+            self.s_out.wait_event(st["built"])
+            with torch.cuda.stream(self.s_out):
+                st["host"][:n_out].copy_(st["out"][:n_out], non_blocking=True)
+            st["copied"] = torch.cuda.Event()
+            st["copied"].record(self.s_out)
+            if pending is not None:
+                pending[1].synchronize()
+                yield pending[0]
+            pending = (st["host"][:n_out], st["copied"])
+            i += 1
+        if pending is not None:
+            pending[1].synchronize()
+            yield pending[0]
+
+
 _status_words: dict = {}
 
 

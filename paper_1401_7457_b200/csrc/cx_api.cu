@@ -149,6 +149,7 @@ struct cx_bwt_plan_s {
     SortWorkspace sort;
     // pinned host mirror: BuildInfo | scalars[8] | hist
     unsigned char* h_pinned;
+    unsigned char* h_pinned_dev;   // the same memory as kernels address it
     BuildInfo* h_info;
     uint64_t* h_scalars;
     uint64_t* h_hist;
@@ -231,11 +232,13 @@ extern "C" int cx_bwt_plan(cx_bwt_plan_t** plan_out, uint64_t max_reads, uint64_
     p->built = false;
     p->stage_busy[0] = p->stage_busy[1] = false;
     p->h_pinned = nullptr;
+    p->h_pinned_dev = nullptr;
     p->copy_stream = nullptr;
     p->emit_done = p->stage_free[0] = p->stage_free[1] = nullptr;
 
     size_t host_bytes = sizeof(BuildInfo) + 64 + 2 * sh.n_buckets * 8;
-    cudaError_t e = cudaMallocHost((void**)&p->h_pinned, host_bytes);
+    cudaError_t e = cudaHostAlloc((void**)&p->h_pinned, host_bytes, cudaHostAllocMapped);
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&p->h_pinned_dev, p->h_pinned, 0);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->emit_done, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->stage_free[0], cudaEventDisableTiming);
@@ -467,6 +470,26 @@ struct Planner {
     }
 };
 
+// Small results (sizes, counters, the partition histogram) come back through pinned host memory that a kernel writes itself.
+// A cudaMemcpyAsync of a few bytes would queue behind whatever large copy the caller has in flight on the same copy engine
+// (a pipelined caller's previous output on its way to the host) and stall the build for as long as that copy takes.
+__global__ void readback_kernel(const uint64_t* __restrict__ src, uint64_t* __restrict__ dst_host, uint32_t n_words) {
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_words; i += gridDim.x * blockDim.x) dst_host[i] = src[i];
+}
+static_assert(sizeof(BuildInfo) % 8 == 0, "read back in 8-byte words");
+// dst_host: an address inside the plan's pinned block (whole 8-byte words); visible to the host after the stream is synchronised
+cudaError_t readback(cx_bwt_plan_t* p, void* dst_host, const void* src_dev, size_t bytes, cudaStream_t s) {
+#if defined(CX_READBACK_MEMCPY) && CX_READBACK_MEMCPY   // the alternative it replaced, kept for the A/B in DESIGN.md section 16
+    return cudaMemcpyAsync(dst_host, src_dev, bytes, cudaMemcpyDeviceToHost, s);
+#endif
+    const uint32_t n = (uint32_t)((bytes + 7) / 8);
+    const uint32_t blocks = (n + 255) / 256;
+    unsigned char* dst = p->h_pinned_dev + (static_cast<unsigned char*>(dst_host) - p->h_pinned);
+    readback_kernel<<<blocks < 64 ? blocks : 64, 256, 0, s>>>(static_cast<const uint64_t*>(src_dev), reinterpret_cast<uint64_t*>(dst), n);
+    p->prof.launches[CX_K_PREP] += 1;
+    return cudaGetLastError();
+}
+
 template <typename KeyT, typename IdT>
 int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets, uint64_t n_reads, uint8_t* out, cudaStream_t s) {
     const Shape& sh = p->sh;
@@ -523,8 +546,8 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         ScopedLaunch sl(prof, CX_K_HIST, 0, s);
         CX_CUDA(launch_bucket_hist(R, d_info, d_tile_first, sh.ell, Region{}, d_hist, sh.max_tiles, p->n_sms, s));
     }
-    CX_CUDA(cudaMemcpyAsync(p->h_info, d_info, sizeof(BuildInfo), cudaMemcpyDeviceToHost, s));
-    CX_CUDA(cudaMemcpyAsync(p->h_hist, d_hist, sh.n_buckets * 8, cudaMemcpyDeviceToHost, s));
+    CX_CUDA(readback(p, p->h_info, d_info, sizeof(BuildInfo), s));
+    CX_CUDA(readback(p, p->h_hist, d_hist, sh.n_buckets * 8, s));
     CX_CUDA(cudaStreamSynchronize(s));
     const BuildInfo info = *p->h_info;
     if (info.bad_offsets || info.total_bases > sh.max_bases || (info.max_len >> sh.pos_bits) != 0) return CX_ERR_ARG;
@@ -567,7 +590,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             ScopedLaunch sl(prof, CX_K_HIST, info.total_bases / 4 + (n_reads + 1) * 8, s);
             CX_CUDA(launch_bucket_hist(R, d_info, d_tile_first, sh.ell, dev, d_hist, sh.max_tiles, p->n_sms, s));
         }
-        CX_CUDA(cudaMemcpyAsync(p->h_hist2, d_hist, sh.n_buckets * 8, cudaMemcpyDeviceToHost, s));
+        CX_CUDA(readback(p, p->h_hist2, d_hist, sh.n_buckets * 8, s));
         CX_CUDA(cudaStreamSynchronize(s));
         memcpy(hist_out, p->h_hist2, sh.n_buckets * 8);
         return CX_OK;
@@ -641,7 +664,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             const uint64_t big_before = p->h_scalars[6];
             CX_CUDA((launch_group_probe<KeyT, IdT>(d_keys1[cur], w, nb, pack_kv, reinterpret_cast<unsigned long long*>(d_scalars + 6), &sampled, s)));
             if (sampled) {
-                CX_CUDA(cudaMemcpyAsync(p->h_scalars + 6, d_scalars + 6, 8, cudaMemcpyDeviceToHost, s));
+                CX_CUDA(readback(p, p->h_scalars + 6, d_scalars + 6, 8, s));
                 CX_CUDA(cudaStreamSynchronize(s));
             }
             slots = sampled && (p->h_scalars[6] - big_before) * 4 > sampled ? 4u : 2u;   // more than a quarter in groups above 64
@@ -651,7 +674,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
                                                 slots, prof, s)));
         // groups of more than cap suffixes (counted by the warp kernel) go through global rounds; usually there are none
         const uint64_t over_before = p->h_scalars[5], local_before = p->h_scalars[1];
-        CX_CUDA(cudaMemcpyAsync(p->h_scalars, d_scalars, 48, cudaMemcpyDeviceToHost, s));
+        CX_CUDA(readback(p, p->h_scalars, d_scalars, 48, s));
         CX_CUDA(cudaStreamSynchronize(s));
         const bool any_oversize = p->h_scalars[5] != over_before;
         // every suffix refined here also costs its id read, an 8-byte window gathered and its id written
@@ -668,7 +691,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
                 CX_CUDA(launch_scan_u64(d_word_counts, n_words, d_word_sums, d_scalars, s));
             }
             prof->launches[CX_K_REFINE_SCAN] += 2;
-            CX_CUDA(cudaMemcpyAsync(p->h_scalars, d_scalars, 48, cudaMemcpyDeviceToHost, s));
+            CX_CUDA(readback(p, p->h_scalars, d_scalars, 48, s));
             CX_CUDA(cudaStreamSynchronize(s));
             const uint64_t n_act = p->h_scalars[0] & 0xffffffffull;
             const uint64_t n_groups = p->h_scalars[0] >> 32;

@@ -454,6 +454,28 @@ def test_equal_length_reads_in_many_small_batches(L):
         assert_parity(c, max_batch_suffixes=c.n_suffixes // 9 + 1, prefix_len=2)
 
 
+def test_host_pipeline_overlapped_builds_match_the_oracle():
+    """HostPipeline: five DIFFERENT collections (sizes differ, one is a single read, two are tie-heavy) through two sets of
+    buffers with the copies of neighbouring builds overlapped; every output compared with the oracle at every position.  A
+    stale buffer, a missed event or a result taken before its copy finished shows up as another collection's bytes."""
+    import paper_1401_7457_b200 as cx
+    rng = np.random.default_rng(77)
+    colls = [gen.random_collection(1, 300, 90), gen.from_strings(["ACGTACGTACGTAACC"]),
+             gen.from_strings(["".join(rng.choice(list("AC"), 60)) for _ in range(400)]),
+             gen.config(0, 0.1), gen.from_strings(["GATTACA" * 9] * 70 + ["GATTACA" * 5])]
+    max_reads, max_bases = max(c.n_reads for c in colls), max(c.total_bases for c in colls)
+    plan = cx.Plan(max_reads, max_bases)
+    pipe = cx.HostPipeline(plan, max_reads, max_bases)
+    items = [(torch.from_numpy(c.ascii.copy()).pin_memory(), torch.from_numpy(c.offsets.astype(np.int64)).pin_memory(), c.n_reads) for c in colls]
+    n = 0
+    for c, got in zip(colls, pipe.run(items)):
+        assert np.array_equal(got.numpy().copy(), oracle.bwt(c.ascii, c.offsets)), f"collection {n}"
+        n += 1
+    assert n == len(colls)
+    assert list(pipe.run([])) == []
+    plan.free()
+
+
 def test_bad_finish_slots_option_is_rejected():
     import paper_1401_7457_b200 as cx
     with pytest.raises(cx.CxError):
