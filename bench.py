@@ -322,7 +322,7 @@ def one_step_record(index: int, dev, peak: float) -> dict:
     torch.cuda.empty_cache()
     free_gb = torch.cuda.mem_get_info(dev)[0] / (1 << 30)
     host_out = index == 4
-    need_gpu, need_host = {0: 1, 1: 8, 2: 60, 3: 150, 4: 165}[index], {4: 115}.get(index, 4)
+    need_gpu, need_host = {0: 1, 1: 8, 2: 60, 3: 150, 4: 170}[index], {4: 115}.get(index, 4)
     if free_gb < need_gpu or host_ram_gb() < need_host:
         return {"workload": WORKLOADS[index], "skipped": f"needs {need_gpu} GB of HBM and {need_host} GB of host RAM; free: {free_gb:.0f} GB, {host_ram_gb():.0f} GB"}
     t0 = time.time()
@@ -332,7 +332,7 @@ def one_step_record(index: int, dev, peak: float) -> dict:
     torch.cuda.synchronize()
     gen_s = time.time() - t0
     torch.cuda.empty_cache()
-    ws = {3: 130 << 30, 4: 118 << 30}.get(index)
+    ws = {3: 130 << 30, 4: 136 << 30}.get(index)
     plan = cx.Plan(n, total, workspace_bytes=ws, max_read_len=max_len, out_is_host_pinned=1 if host_out else 0, profile=1, device=dev)
     out = torch.empty(N, dtype=torch.uint8, pin_memory=True) if host_out else torch.empty(N, dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream()

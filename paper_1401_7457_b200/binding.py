@@ -169,6 +169,9 @@ class HostPipeline:
 
     def __init__(self, plan: "Plan", max_reads: int, max_total_bases: int):
         dev = plan.device
+        # the pipeline copies whole 8-bit outputs itself; a plan that streams to the host or packs its output is used on its own
+        if plan.opts.out_is_host_pinned or plan.opts.out_bits not in (0, 8) or plan.opts.shard_count > 1:
+            raise CxError(CX_ERR_ARG, "HostPipeline needs a plan with device output, 8-bit symbols and no sharding")
         self.plan, self.device = plan, dev
         self.s_in, self.s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
         n_out = max_total_bases + max_reads

@@ -474,6 +474,11 @@ def test_host_pipeline_overlapped_builds_match_the_oracle():
     assert n == len(colls)
     assert list(pipe.run([])) == []
     plan.free()
+    for bad in (dict(out_is_host_pinned=1), dict(out_bits=4)):
+        p2 = cx.Plan(10, 100, **bad)
+        with pytest.raises(cx.CxError):
+            cx.HostPipeline(p2, 10, 100)
+        p2.free()
 
 
 def test_bad_finish_slots_option_is_rejected():
