@@ -58,7 +58,7 @@ constexpr uint32_t kMaxRegionDepth = 1u << 20;   // bases; deeper refinement is 
 // Byte offsets of every region of the workspace for a given m1.
 struct Layout {
     uint64_t info, hist, tile_first, tile_count, tile_sums, scalars, prefix;
-    uint64_t keys[2], ids[3], pos, heads[2], big_tiles, word_counts, word_sums, sort, stage[2], pstage[2];
+    uint64_t keys[2], ids[2], pos, heads[2], big_tiles, word_counts, word_sums, sort, stage[2], pstage[2];
     uint64_t total;
 };
 
@@ -88,8 +88,10 @@ Layout make_layout(const Shape& sh, uint64_t m1) {
     L.scalars = take(64);
     L.prefix = take((uint64_t)(sh.prefix_words) * 8);
     for (int i = 0; i < 2; ++i) L.keys[i] = take(m1 * 8);
-    for (int i = 0; i < 3; ++i) L.ids[i] = take(m1 * sh.id_bytes);
-    L.pos = take(m1 * 4);
+    for (int i = 0; i < 2; ++i) L.ids[i] = take(m1 * sh.id_bytes + 16);   // (+16: the second position array starts 16-byte aligned)
+    // the global path sorts (key, position) pairs: its two arrays of 32-bit positions share the spare id buffer when ids have
+    // 8 bytes; with 4-byte ids the second one lives here
+    L.pos = take(sh.id_bytes == 4 ? m1 * 4 : 0);
     uint64_t words = (m1 + 31) / 32 + 2;
     for (int i = 0; i < 2; ++i) L.heads[i] = take(words * 4);
     L.big_tiles = take(((m1 + kLocalTile - 1) / kLocalTile / 32 + 2) * 4);
@@ -503,7 +505,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     uint64_t* d_tile_sums = reinterpret_cast<uint64_t*>(ws + L.tile_sums);
     uint64_t* d_scalars = reinterpret_cast<uint64_t*>(ws + L.scalars);   // [0] scan total, [1] elements finished locally
     uint64_t* d_keys[2] = {reinterpret_cast<uint64_t*>(ws + L.keys[0]), reinterpret_cast<uint64_t*>(ws + L.keys[1])};
-    IdT* d_ids[3] = {reinterpret_cast<IdT*>(ws + L.ids[0]), reinterpret_cast<IdT*>(ws + L.ids[1]), reinterpret_cast<IdT*>(ws + L.ids[2])};
+    IdT* d_ids[2] = {reinterpret_cast<IdT*>(ws + L.ids[0]), reinterpret_cast<IdT*>(ws + L.ids[1])};
     uint32_t* d_pos = reinterpret_cast<uint32_t*>(ws + L.pos);
     uint32_t* d_heads[2] = {reinterpret_cast<uint32_t*>(ws + L.heads[0]), reinterpret_cast<uint32_t*>(ws + L.heads[1])};
     uint32_t* d_big_tiles = reinterpret_cast<uint32_t*>(ws + L.big_tiles);
@@ -700,19 +702,25 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             const uint32_t gbits = n_groups > 1 ? bit_width64(n_groups - 1) : 0;
             uint32_t w_r = (59 - gbits) / 2;
             if (w_r > 29) w_r = 29;
+            // free at this point: both key buffers and the spare id buffer.  The sort ping-pongs (key, position) pairs between
+            // them; whichever key buffer does not hold the sorted keys afterwards takes the gathered ids.
             uint64_t* kc = d_keys[1 - cur];
-            IdT* ic = pack_kv ? d_ids[1] : d_ids[1 - cur];
+            uint32_t* pc = reinterpret_cast<uint32_t*>(pack_kv ? d_ids[1] : d_ids[1 - cur]);
+            uint32_t* pc_alt = sizeof(IdT) == 8 ? pc + ((p->m1 + 3) & ~3ull) : d_pos;
             {
-                ScopedLaunch sl(prof, CX_K_REFINE_KEY, nb / 8 + n_act * (2 * sizeof(IdT) + 8 + 8 + 4), s);
-                CX_CUDA(launch_refine_rekey<IdT>(R, d_heads[hc], d_word_counts, ids, nb, depth, w_r, kc, ic, d_pos, s));
+                ScopedLaunch sl(prof, CX_K_REFINE_KEY, nb / 8 + n_act * (sizeof(IdT) + 8 + 8 + 4), s);
+                CX_CUDA(launch_refine_rekey<IdT>(R, d_heads[hc], d_word_counts, ids, nb, depth, w_r, kc, pc, s));
             }
             int alt = 0;
-            CX_CUDA((sort_pairs<uint64_t, IdT>(kc, ic, d_keys[cur], d_ids[2], n_act, 0, 2 * w_r + 5 + gbits, p->sort, &alt, prof, s, false, CX_K_REFINE_SORT)));
+            CX_CUDA((sort_pairs<uint64_t, uint32_t>(kc, pc, d_keys[cur], pc_alt, n_act, 0, 2 * w_r + 5 + gbits, p->sort, &alt, prof, s, false, CX_K_REFINE_SORT)));
+            CX_CUDA(cudaMemcpyAsync(d_heads[1 - hc], d_heads[hc], (n_words + 1) * 4, cudaMemcpyDeviceToDevice, s));
             {
-                ScopedLaunch sl(prof, CX_K_REFINE_WRITE, n_act * (8 + 2 * sizeof(IdT) + 4 + 1), s);
-                CX_CUDA(launch_refine_writeback<IdT>(R, alt ? d_keys[cur] : kc, alt ? d_ids[2] : ic, d_pos, n_act, w_r, ids, d_heads[hc],
-                                                     dst, s));
+                ScopedLaunch sl(prof, CX_K_REFINE_WRITE, nb / 8 + n_act * (8 + 4 + 4 * sizeof(IdT) + 1), s);
+                CX_CUDA(launch_refine_writeback<IdT>(R, alt ? d_keys[cur] : kc, alt ? pc_alt : pc, reinterpret_cast<IdT*>(alt ? kc : d_keys[cur]),
+                                                     d_heads[hc], d_word_counts, nb, n_act, w_r, ids, d_heads[1 - hc], dst, s));
+                prof->launches[CX_K_REFINE_WRITE] += 1;   // gather + write-back
             }
+            hc = 1 - hc;                                  // the head bits with this round's new groups
             p->stats.refine_elements += n_act;
             depth += w_r;
             ++rounds;

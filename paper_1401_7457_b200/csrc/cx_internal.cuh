@@ -250,13 +250,17 @@ cudaError_t launch_active_count(const uint32_t* heads, uint64_t n, uint64_t* wor
 // exclusive scan in place; total written to *total; block_sums needs scan_block_count(n) entries
 uint64_t scan_block_count(uint64_t n);
 cudaError_t launch_scan_u64(uint64_t* data, uint64_t n, uint64_t* block_sums, uint64_t* total, cudaStream_t s);
+// keys of the active elements (members of open groups, in position order) and, as the sort's values, their positions
 template <typename IdT>
 cudaError_t launch_refine_rekey(const Reads& R, const uint32_t* heads, const uint64_t* word_base, const IdT* ids, uint64_t n,
-                                uint32_t depth, uint32_t w, uint64_t* keys_c, IdT* ids_c, uint32_t* pos_c, cudaStream_t s);
-// writes ids back in place, sets new head bits, emits the BWT symbol of every suffix that became final
+                                uint32_t depth, uint32_t w, uint64_t* keys_c, uint32_t* pos_c, cudaStream_t s);
+// after the sort: fetches the sorted elements' ids through their old positions (into ids_tmp, n_c entries), writes them to
+// the active positions in order, sets new head bits in heads_out (the caller's copy of `heads`, which is only read) and emits
+// the BWT symbol of every suffix that became final
 template <typename IdT>
-cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, const IdT* ids_c, const uint32_t* pos_c, uint64_t n_c,
-                                    uint32_t w, IdT* ids, uint32_t* heads, uint8_t* out, cudaStream_t s);
+cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, const uint32_t* pos_sorted, IdT* ids_tmp, const uint32_t* heads,
+                                    const uint64_t* word_base, uint64_t n, uint64_t n_c, uint32_t w, IdT* ids, uint32_t* heads_out, uint8_t* out,
+                                    cudaStream_t s);
 // a7 + a8 over the freshly sorted first-round keys: the warp kernel finishes singletons and tie groups of at most 32
 // suffixes, counts the groups it leaves to the global path (elems_done[4]) and clears all but their first bit in heads_out
 // (the head bitmask of that path; filled with ones by the caller: every other position counts as a group of one); the block kernel then finishes the groups of 33..group_cap in the tiles the warp

@@ -161,12 +161,10 @@ __device__ __forceinline__ uint8_t preceding_symbol(const Reads& R, IdT id) {
 // global path: compact + re-key, write back
 // ---------------------------------------------------------------------------------------------
 // One thread per 32 sorted positions looks for members still tied; the warp then handles every such word together,
-// one lane per position (oversize groups are rare, so nearly all threads leave after one load).
-template <typename IdT>
-__global__ void __launch_bounds__(256) refine_rekey_kernel(Reads R, const uint32_t* __restrict__ heads,
-                                                           const uint64_t* __restrict__ word_base, const IdT* __restrict__ ids,
-                                                           uint64_t n, uint32_t depth, uint32_t w, uint64_t* __restrict__ keys_c,
-                                                           IdT* __restrict__ ids_c, uint32_t* __restrict__ pos_c) {
+// one lane per position (oversize groups are rare, so nearly all threads leave after one load).  f(j, c, g): position j is
+// the c-th active one and belongs to the g-th open group.
+template <typename F>
+__device__ __forceinline__ void for_each_active(const uint32_t* __restrict__ heads, const uint64_t* __restrict__ word_base, uint64_t n, F&& f) {
     const uint64_t n_words = (n + 31) >> 5;
     const uint64_t wi = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     uint32_t act = 0, ah = 0;
@@ -181,37 +179,56 @@ __global__ void __launch_bounds__(256) refine_rekey_kernel(Reads R, const uint32
         const uint64_t wbase = __shfl_sync(kFull, base, src);
         const uint64_t wwi = wi - bit + src;   // word index of lane `src` (lanes hold consecutive words)
         if ((wact >> bit) & 1u) {
-            const uint64_t j = (wwi << 5) + bit;
             const uint32_t below = (1u << bit) - 1;
-            const uint64_t c = (wbase & 0xffffffffull) + __popc(wact & below);
-            const uint64_t g = (wbase >> 32) + __popc(wah & (below | (1u << bit))) - 1;   // ordinal of this element's group
-            const IdT id = ids[j];
-            keys_c[c] = (g << (2 * w + 5)) | key_at_depth(R, id, depth, w);
-            ids_c[c] = id;
-            pos_c[c] = (uint32_t)j;
+            f((wwi << 5) + bit, (wbase & 0xffffffffull) + __popc(wact & below), (wbase >> 32) + __popc(wah & (below | (1u << bit))) - 1);
         }
     }
 }
 
+// The sort of a global round carries, as its value, the POSITION of the element in the batch (32 bits: the ids stay where
+// they are and are fetched through it afterwards), so it needs no buffer beyond the two key buffers and one id buffer that
+// are free at this point.
+template <typename IdT>
+__global__ void __launch_bounds__(256) refine_rekey_kernel(Reads R, const uint32_t* __restrict__ heads,
+                                                           const uint64_t* __restrict__ word_base, const IdT* __restrict__ ids,
+                                                           uint64_t n, uint32_t depth, uint32_t w, uint64_t* __restrict__ keys_c,
+                                                           uint32_t* __restrict__ pos_c) {
+    for_each_active(heads, word_base, n, [&](uint64_t j, uint64_t c, uint64_t g) {
+        keys_c[c] = (g << (2 * w + 5)) | key_at_depth(R, ids[j], depth, w);
+        pos_c[c] = (uint32_t)j;
+    });
+}
+
+// ids of the sorted elements, fetched through their old positions (into a buffer of their own: the write-back below moves
+// them to positions that other threads still read from)
+template <typename IdT>
+__global__ void __launch_bounds__(256) refine_gather_kernel(const uint32_t* __restrict__ pos_sorted, uint64_t n_c, const IdT* __restrict__ ids,
+                                                            IdT* __restrict__ ids_c) {
+    const uint64_t c = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c < n_c) ids_c[c] = ids[pos_sorted[c]];
+}
+
+// The c-th sorted element goes to the c-th active position.  `heads` is read (which positions are active), `heads_out` --
+// a copy of it made by the caller -- receives the new head bits.
 template <typename IdT>
 __global__ void __launch_bounds__(256) refine_writeback_kernel(Reads R, const uint64_t* __restrict__ keys_c, const IdT* __restrict__ ids_c,
-                                                               const uint32_t* __restrict__ pos_c, uint64_t n_c, uint32_t w,
-                                                               IdT* __restrict__ ids, uint32_t* __restrict__ heads, uint8_t* __restrict__ out) {
-    uint64_t c = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= n_c) return;
-    uint64_t k = keys_c[c];
-    uint32_t pos = pos_c[c];
-    IdT id = ids_c[c];
-    ids[pos] = id;
-    bool head = c == 0 || k != keys_c[c - 1] || (uint32_t)(k & 31) < w;
-    if (head) atomicOr(&heads[pos >> 5], 1u << (pos & 31));
-    // alone in its group now (or its end-marker was inside the window): final, emit its BWT symbol
-    bool next_is_head = true;
-    if (c + 1 < n_c) {
-        uint64_t kn = keys_c[c + 1];
-        next_is_head = kn != k || (uint32_t)(kn & 31) < w;
-    }
-    if (head && next_is_head) out[pos] = preceding_symbol(R, id);
+                                                               const uint32_t* __restrict__ heads, const uint64_t* __restrict__ word_base,
+                                                               uint64_t n, uint64_t n_c, uint32_t w, IdT* __restrict__ ids,
+                                                               uint32_t* __restrict__ heads_out, uint8_t* __restrict__ out) {
+    for_each_active(heads, word_base, n, [&](uint64_t pos, uint64_t c, uint64_t) {
+        const uint64_t k = keys_c[c];
+        const IdT id = ids_c[c];
+        ids[pos] = id;
+        const bool head = c == 0 || k != keys_c[c - 1] || (uint32_t)(k & 31) < w;
+        if (head) atomicOr(&heads_out[pos >> 5], 1u << (pos & 31));
+        // alone in its group now (or its end-marker was inside the window): final, emit its BWT symbol
+        bool next_is_head = true;
+        if (c + 1 < n_c) {
+            const uint64_t kn = keys_c[c + 1];
+            next_is_head = kn != k || (uint32_t)(kn & 31) < w;
+        }
+        if (head && next_is_head) out[pos] = preceding_symbol(R, id);
+    });
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1454,18 +1471,21 @@ cudaError_t launch_scan_u64(uint64_t* data, uint64_t n, uint64_t* block_sums, ui
 
 template <typename IdT>
 cudaError_t launch_refine_rekey(const Reads& R, const uint32_t* heads, const uint64_t* word_base, const IdT* ids, uint64_t n,
-                                uint32_t depth, uint32_t w, uint64_t* keys_c, IdT* ids_c, uint32_t* pos_c, cudaStream_t s) {
+                                uint32_t depth, uint32_t w, uint64_t* keys_c, uint32_t* pos_c, cudaStream_t s) {
     if (n == 0) return cudaSuccess;
     const uint64_t n_words = (n + 31) >> 5;
-    refine_rekey_kernel<IdT><<<(unsigned)((n_words + 255) / 256), 256, 0, s>>>(R, heads, word_base, ids, n, depth, w, keys_c, ids_c, pos_c);
+    refine_rekey_kernel<IdT><<<(unsigned)((n_words + 255) / 256), 256, 0, s>>>(R, heads, word_base, ids, n, depth, w, keys_c, pos_c);
     return cudaGetLastError();
 }
 
 template <typename IdT>
-cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, const IdT* ids_c, const uint32_t* pos_c, uint64_t n_c,
-                                    uint32_t w, IdT* ids, uint32_t* heads, uint8_t* out, cudaStream_t s) {
+cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, const uint32_t* pos_sorted, IdT* ids_tmp, const uint32_t* heads,
+                                    const uint64_t* word_base, uint64_t n, uint64_t n_c, uint32_t w, IdT* ids, uint32_t* heads_out, uint8_t* out,
+                                    cudaStream_t s) {
     if (n_c == 0) return cudaSuccess;
-    refine_writeback_kernel<IdT><<<(unsigned)((n_c + 255) / 256), 256, 0, s>>>(R, keys_c, ids_c, pos_c, n_c, w, ids, heads, out);
+    refine_gather_kernel<IdT><<<(unsigned)((n_c + 255) / 256), 256, 0, s>>>(pos_sorted, n_c, ids, ids_tmp);
+    const uint64_t n_words = (n + 31) >> 5;
+    refine_writeback_kernel<IdT><<<(unsigned)((n_words + 255) / 256), 256, 0, s>>>(R, keys_c, ids_tmp, heads, word_base, n, n_c, w, ids, heads_out, out);
     return cudaGetLastError();
 }
 
@@ -1542,9 +1562,10 @@ cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32
 
 #define CX_INSTANTIATE(IdT)                                                                                                          \
     template cudaError_t launch_refine_rekey<IdT>(const Reads&, const uint32_t*, const uint64_t*, const IdT*, uint64_t, uint32_t,   \
-                                                  uint32_t, uint64_t*, IdT*, uint32_t*, cudaStream_t);                               \
-    template cudaError_t launch_refine_writeback<IdT>(const Reads&, const uint64_t*, const IdT*, const uint32_t*, uint64_t,         \
-                                                      uint32_t, IdT*, uint32_t*, uint8_t*, cudaStream_t);                            \
+                                                  uint32_t, uint64_t*, uint32_t*, cudaStream_t);                                     \
+    template cudaError_t launch_refine_writeback<IdT>(const Reads&, const uint64_t*, const uint32_t*, IdT*, const uint32_t*,        \
+                                                      const uint64_t*, uint64_t, uint64_t, uint32_t, IdT*, uint32_t*, uint8_t*,      \
+                                                      cudaStream_t);                                                                 \
     template cudaError_t launch_finish_first<uint32_t, IdT>(const Reads&, const uint32_t*, uint32_t, uint32_t, uint32_t*, IdT*, uint64_t, \
                                                             uint32_t, uint8_t*, unsigned long long*, uint32_t*, int, bool, uint32_t, Launch*, cudaStream_t); \
     template cudaError_t launch_finish_first<uint64_t, IdT>(const Reads&, const uint64_t*, uint32_t, uint32_t, uint32_t*, IdT*, uint64_t, \
