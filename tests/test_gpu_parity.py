@@ -77,6 +77,24 @@ def test_homopolymer_reads_one_giant_group():
     assert_parity(c, small_group_max=16)
 
 
+@pytest.mark.parametrize("id64", [False, True])
+def test_global_path_shares_the_buffers_of_the_first_sort(id64):
+    """Tie groups above the block kernel's limit go through rounds of re-key, sort, write back.  That path owns no buffers:
+    its (key, position) pairs ping-pong between the two key buffers and the spare id buffer (two position arrays in it with
+    8-byte ids, the second in `pos` with 4-byte ids), and the gathered ids pass through whichever key buffer is free.  Batch
+    sizes that are odd, a multiple of 4 plus 1, 2, 3 (where the second position array starts) and one that makes nearly
+    every suffix active; several rounds (groups of 900 equal suffixes of 300 bases: the window of a round is 27 bases)."""
+    rng = np.random.default_rng(5)
+    unit = "".join(rng.choice(list("ACGT"), 300))
+    reads = [unit] * 900 + [unit[:170]] * 300 + ["".join(rng.choice(list("ACGT"), 80)) for _ in range(50)]
+    c = gen.from_strings(reads)
+    extra = dict(max_read_len=0) if id64 else {}
+    assert_parity(c, **extra)
+    for m1 in (c.n_suffixes, c.n_suffixes // 2 + 1, c.n_suffixes // 3 + 2, c.n_suffixes // 5 + 3):
+        assert_parity(c, max_batch_suffixes=m1, **extra)
+    assert_parity(c, small_group_max=1, max_batch_suffixes=c.n_suffixes // 2 + 3, **extra)
+
+
 def test_long_reads_and_tandem_repeats():
     c = gen.from_strings(["ACGT" * 200, "ACGT" * 150 + "T", "CGTA" * 180, "G" * 900, ""] * 7)
     assert_parity(c)
