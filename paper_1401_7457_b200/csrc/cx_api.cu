@@ -56,6 +56,10 @@ struct Batch {
 constexpr uint32_t kMaxRegionDepth = 1u << 20;   // bases; deeper refinement is reported as CX_ERR_BUCKET_TOO_LARGE
 
 // Byte offsets of every region of the workspace for a given m1.
+#ifndef CX_SPLIT_PAIRS
+#define CX_SPLIT_PAIRS 1   // 12-byte (key, id) pairs through the first sort of batches with 64-bit keys and ids
+#endif
+
 struct Layout {
     uint64_t info, hist, tile_first, tile_count, tile_sums, scalars, prefix;
     uint64_t keys[2], ids[2], pos, heads[2], big_tiles, word_counts, word_sums, sort, stage[2], pstage[2];
@@ -610,6 +614,16 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
     if (fused_scan && !single) return CX_ERR_CUDA;   // cannot happen: N <= max_suffixes <= m1
     p->stats.sort_passes = (key_bits + kRadixBits - 1) / kRadixBits;
 
+    // Batches of a plan with 64-bit keys and ids travel through the sort as 12-byte pairs: the key above the id's high part in
+    // the 64-bit word, the id's low word as a 32-bit value (cx_internal.cuh, launch_list_write).  0 = not used.
+    uint32_t split = 0;
+#if CX_SPLIT_PAIRS
+    if (sizeof(KeyT) == 8 && sizeof(IdT) == 8 && !single && !fused_scan && key_bits < 64) {
+        const uint32_t id_bits = R.pos_bits + (n_reads > 1 ? bit_width64(n_reads - 1) : 0u);
+        if (id_bits <= 32 + (64 - key_bits)) split = 64 - key_bits;
+    }
+#endif
+
     for (size_t bi = 0; bi < p->batches.size(); ++bi) {
         const Batch& B = p->batches[bi];
         const uint64_t nb = B.count;
@@ -638,19 +652,25 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
                 CX_CUDA(launch_scan_u64(d_col, n_tiles, d_tile_sums, d_scalars + 2, s));
                 prof->launches[CX_K_LIST] += 2;   // the scan is three kernels
             }
-            ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (sizeof(KeyT) + sizeof(IdT)), s);
+            ScopedLaunch sl(prof, CX_K_LIST, info.total_bases / 4 + (n_reads + 1) * 8 + nb * (split ? 12 : sizeof(KeyT) + sizeof(IdT)), s);
             CX_CUDA((launch_list_write<KeyT, IdT>(R, d_info, d_tile_first, sh.ell, w, B.bucket_lo, B.bucket_hi, d_col, d_keys1[0], d_ids[0],
                                                   n_tiles, n_passes, p->sort.hist, p->n_sms, pack_kv, nullptr, ~0ull, region, B.ord_lo, B.ord_hi,
-                                                  s)));
+                                                  s, split)));
         }
         // ---- step 3(c)ii: sort (first w symbols) ------------------------------------------------
         int in_alt = 0;
         if (pack_kv)
             CX_CUDA((sort_pairs<uint64_t, NoVal>(d_keys[0], nullptr, d_keys[1], nullptr, nb, 32, 32 + key_bits, p->sort, &in_alt, prof, s, true)));
+        else if (split)
+            CX_CUDA((sort_pairs<uint64_t, uint32_t>(d_keys[0], reinterpret_cast<uint32_t*>(d_ids[0]), d_keys[1], reinterpret_cast<uint32_t*>(d_ids[1]), nb, split,
+                                                    64, p->sort, &in_alt, prof, s, true)));
         else
             CX_CUDA((sort_pairs<KeyT, IdT>(d_keys1[0], d_ids[0], d_keys1[1], d_ids[1], nb, 0, key_bits, p->sort, &in_alt, prof, s, true)));
         const int cur = in_alt;
-        IdT* ids = pack_kv ? d_ids[0] : d_ids[cur];
+        // `ids`: where the global path finds (and rearranges) the batch's ids.  Separate arrays: the sorted ids themselves.  Packed
+        // or split pairs: a buffer that the warp kernel fills for the groups it leaves to that path.
+        IdT* ids = pack_kv ? d_ids[0] : split ? d_ids[1 - cur] : d_ids[cur];
+        IdT* spare_ids = pack_kv ? d_ids[1] : split ? d_ids[cur] : d_ids[1 - cur];   // free once the warp and block kernels are done
         // a9: with pinned-host output the batch is emitted into a staging buffer of the workspace
         const int st = sh.host_out ? (int)(bi & 1) : 0;
         uint8_t* dst = sh.host_out || sh.pack_out ? ws + L.stage[st] : out + B.out_offset;
@@ -664,7 +684,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
         if (slots == 0) {
             uint64_t sampled = 0;
             const uint64_t big_before = p->h_scalars[6];
-            CX_CUDA((launch_group_probe<KeyT, IdT>(d_keys1[cur], w, nb, pack_kv, reinterpret_cast<unsigned long long*>(d_scalars + 6), &sampled, s)));
+            CX_CUDA((launch_group_probe<KeyT, IdT>(d_keys1[cur], w, nb, pack_kv, reinterpret_cast<unsigned long long*>(d_scalars + 6), &sampled, s, split)));
             if (sampled) {
                 CX_CUDA(readback(p, p->h_scalars + 6, d_scalars + 6, 8, s));
                 CX_CUDA(cudaStreamSynchronize(s));
@@ -672,8 +692,8 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             slots = sampled && (p->h_scalars[6] - big_before) * 4 > sampled ? 4u : 2u;   // more than a quarter in groups above 64
         }
         CX_CUDA(cudaMemsetAsync(d_heads[0], 0xff, (n_words + 1) * 4, s));   // every position a group of one until the warp kernel says otherwise
-        CX_CUDA((launch_finish_first<KeyT, IdT>(R, d_keys1[cur], w, depth_base + w, d_heads[0], ids, nb, cap, dst, d_done, d_big_tiles, p->n_sms, pack_kv,
-                                                slots, prof, s)));
+        CX_CUDA((launch_finish_first<KeyT, IdT>(R, d_keys1[cur], w, depth_base + w, d_heads[0], split ? d_ids[cur] : ids, nb, cap, dst, d_done, d_big_tiles,
+                                                p->n_sms, pack_kv, slots, prof, s, split, split ? ids : nullptr)));
         // groups of more than cap suffixes (counted by the warp kernel) go through global rounds; usually there are none
         const uint64_t over_before = p->h_scalars[5], local_before = p->h_scalars[1];
         CX_CUDA(readback(p, p->h_scalars, d_scalars, 48, s));
@@ -705,7 +725,7 @@ int build_impl(cx_bwt_plan_t* p, const uint64_t* packed, const uint64_t* offsets
             // free at this point: both key buffers and the spare id buffer.  The sort ping-pongs (key, position) pairs between
             // them; whichever key buffer does not hold the sorted keys afterwards takes the gathered ids.
             uint64_t* kc = d_keys[1 - cur];
-            uint32_t* pc = reinterpret_cast<uint32_t*>(pack_kv ? d_ids[1] : d_ids[1 - cur]);
+            uint32_t* pc = reinterpret_cast<uint32_t*>(spare_ids);
             uint32_t* pc_alt = sizeof(IdT) == 8 ? pc + ((p->m1 + 3) & ~3ull) : d_pos;
             {
                 ScopedLaunch sl(prof, CX_K_REFINE_KEY, nb / 8 + n_act * (sizeof(IdT) + 8 + 8 + 4), s);

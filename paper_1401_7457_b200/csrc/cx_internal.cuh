@@ -223,7 +223,8 @@ template <typename KeyT, typename IdT>
 cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
                               uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, KeyT* keys, IdT* ids,
                               uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, bool packed, uint64_t* bucket_hist,
-                              uint64_t max_n, const Region& region, uint64_t ord_lo, uint64_t ord_hi, cudaStream_t s);
+                              uint64_t max_n, const Region& region, uint64_t ord_lo, uint64_t ord_hi, cudaStream_t s, uint32_t split = 0);
+// split != 0 (select scans with 64-bit keys and ids only): a pair is (key << split | id >> 32) in `keys` and (uint32_t)id in a uint32 array at `ids`
 
 // cx_onesweep.cu
 struct SortWorkspace {
@@ -270,11 +271,14 @@ cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, cons
 template <typename KeyT, typename IdT>
 cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t depth0, uint32_t* heads_out, IdT* ids, uint64_t n,
                                 uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, uint32_t* big_tiles, int n_sms, bool packed,
-                                uint32_t slots, Launch* prof, cudaStream_t s);
+                                uint32_t slots, Launch* prof, cudaStream_t s, uint32_t split = 0, IdT* ids_out = nullptr);
+// split != 0 (64-bit keys and ids): keys1 holds key << split | id >> 32 and `ids` is a uint32 array of the ids' low words (the
+// sort's 12-byte pairs); the ids of the groups left to the global path are then assembled into ids_out (another buffer)
 // a sample of the sorted first-round keys: *counter += sampled positions in tie groups of more than 64 suffixes, *sampled (HOST) =
 // positions looked at (0: batch too small to sample).  slots of launch_finish_first: 4 if those are a large share, else 2
 template <typename KeyT, typename IdT>
-cudaError_t launch_group_probe(const KeyT* keys1, uint32_t w1, uint64_t n, bool packed, unsigned long long* counter, uint64_t* sampled, cudaStream_t s);
+cudaError_t launch_group_probe(const KeyT* keys1, uint32_t w1, uint64_t n, bool packed, unsigned long long* counter, uint64_t* sampled, cudaStream_t s,
+                               uint32_t split = 0);
 // in-block refinement + emit of the groups a global round has split to at most group_cap members; heads_out = copy of heads_in
 template <typename IdT>
 cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32_t* heads_out, const IdT* ids, uint64_t n, uint32_t depth,

@@ -157,6 +157,15 @@ __device__ __forceinline__ uint8_t preceding_symbol(const Reads& R, IdT id) {
     return (uint8_t)((0x54474341u >> (8 * code)) & 0xFFu);
 }
 
+// split != 0 (64-bit keys and ids, batches of a multi-batch plan): the word is key << split | id >> 32 and the id's low 32
+// bits are a uint32 array where the ids would be
+template <bool PACKED>
+__device__ __forceinline__ uint64_t key_of(uint64_t word, uint32_t split) { return PACKED ? word >> 32 : word >> split; }
+template <typename IdT>
+__device__ __forceinline__ IdT split_id(uint64_t word, uint32_t split, const IdT* __restrict__ ids_lo, uint64_t j) {
+    return (IdT)(((word & ((1ull << split) - 1)) << 32) | (uint64_t)__ldg(reinterpret_cast<const uint32_t*>(ids_lo) + j));
+}
+
 // ---------------------------------------------------------------------------------------------
 // global path: compact + re-key, write back
 // ---------------------------------------------------------------------------------------------
@@ -374,7 +383,7 @@ template <typename KeyT, typename IdT, bool FIRST, bool PACKED>
 __device__ __forceinline__ void finish_tile(LocalSmem& sm, uint64_t tile, const Reads& R, const KeyT* __restrict__ keys1,
                                             const uint32_t* __restrict__ heads_in, uint32_t* __restrict__ heads, const IdT* __restrict__ ids,
                                             uint64_t n, uint32_t depth0, uint32_t min_group, uint32_t cap, uint8_t* __restrict__ out,
-                                            unsigned long long* elems_done) {
+                                            unsigned long long* elems_done, uint32_t split) {
     const uint64_t base = tile * kLocalTile;
     const uint64_t w0 = base >> 5;
     const uint64_t n_words = (n + 31) >> 5;   // heads[n_words] is the padding word ("the next position is a head")
@@ -396,9 +405,10 @@ __device__ __forceinline__ void finish_tile(LocalSmem& sm, uint64_t tile, const 
                     head = j == 0 || kc != (uint32_t)(__ldg(pairs + j - 1) >> 32) || !(kc & 1u);
                     sm.loc[e] = (uint32_t)pc;
                 } else {
-                    const KeyT kc = __ldcs(keys1 + j);
-                    head = j == 0 || kc != __ldg(keys1 + j - 1) || !((uint32_t)kc & 1u);
-                    sm.loc[e] = (uint64_t)__ldcs(ids + j);
+                    const uint64_t wc = (uint64_t)__ldcs(keys1 + j);
+                    const uint64_t kc = wc >> split;
+                    head = j == 0 || kc != ((uint64_t)__ldg(keys1 + j - 1) >> split) || !((uint32_t)kc & 1u);
+                    sm.loc[e] = split ? (uint64_t)split_id<IdT>(wc, split, ids, j) : (uint64_t)__ldcs(ids + j);
                 }
             }
             const uint32_t word = __ballot_sync(kFull, head);
@@ -736,13 +746,13 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
                                                                     const uint32_t* __restrict__ heads_in, uint32_t* __restrict__ heads,
                                                                     const IdT* __restrict__ ids, uint64_t n, uint32_t depth0, uint32_t min_group,
                                                                     uint32_t cap, const uint32_t* __restrict__ big_tiles, uint8_t* __restrict__ out,
-                                                                    unsigned long long* elems_done) {
+                                                                    unsigned long long* elems_done, uint32_t split) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     LocalSmem& sm = *reinterpret_cast<LocalSmem*>(smem_raw);
     const uint64_t n_tiles = (n + kLocalTile - 1) / kLocalTile;
     for (uint64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         if (FIRST && !((__ldg(big_tiles + (tile >> 5)) >> (tile & 31)) & 1u)) continue;
-        finish_tile<KeyT, IdT, FIRST, PACKED>(sm, tile, R, keys1, heads_in, heads, ids, n, depth0, min_group, cap, out, elems_done);
+        finish_tile<KeyT, IdT, FIRST, PACKED>(sm, tile, R, keys1, heads_in, heads, ids, n, depth0, min_group, cap, out, elems_done, split);
         __syncthreads();   // the next tile reuses the shared memory
     }
 }
@@ -847,17 +857,15 @@ __device__ __forceinline__ uint64_t load_keyword(const KeyT* __restrict__ keys1,
     if constexpr (PACKED) return __ldg(reinterpret_cast<const uint64_t*>(keys1) + j);   // key << 32 | id
     else return (uint64_t)__ldg(keys1 + j);
 }
-template <bool PACKED>
-__device__ __forceinline__ uint64_t key_of(uint64_t word) { return PACKED ? word >> 32 : word; }
 
 // first head at or after position p >= 1 (position n counts as one): a head starts a tie group
 template <typename KeyT, bool PACKED>
-__device__ __forceinline__ uint64_t scan_to_head(const KeyT* __restrict__ keys1, uint64_t p, uint64_t n) {
+__device__ __forceinline__ uint64_t scan_to_head(const KeyT* __restrict__ keys1, uint64_t p, uint64_t n, uint32_t split) {
     const uint32_t lane = lane_id();
-    uint64_t carry = key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, p - 1));
+    uint64_t carry = key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, p - 1), split);
     while (true) {
         const uint64_t j = p + lane;
-        const uint64_t k = j < n ? key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j)) : 0ull;
+        const uint64_t k = j < n ? key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j), split) : 0ull;
         uint64_t kp = __shfl_up_sync(kFull, k, 1);
         if (lane == 0) kp = carry;
         const bool head = j >= n || k != kp || !((uint32_t)k & 1u);
@@ -956,7 +964,7 @@ template <typename KeyT, typename IdT, bool PACKED, int S>
 __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finish_warp_kernel(Reads R, const KeyT* __restrict__ keys1, const IdT* __restrict__ ids_in,
                                                                    IdT* __restrict__ ids_out, uint64_t n, uint32_t depth0, uint32_t cap, uint32_t* __restrict__ heads,
                                                                    uint32_t* __restrict__ big_tiles, uint8_t* __restrict__ out,
-                                                                   unsigned long long* counters, uint32_t chunk) {
+                                                                   unsigned long long* counters, uint32_t chunk, uint32_t split) {
     constexpr uint32_t kSpan = 32 * S;                  // positions per window
     constexpr uint32_t kPosBits = S == 1 ? 5 : S == 2 ? 6 : 7;   // bits of a window position
     constexpr bool kTwoLevels = 2 * kPosBits + 20 <= 32;         // room for the second event in the 32-bit rank key
@@ -974,7 +982,7 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
     const uint64_t pos_mask = (1ull << R.pos_bits) - 1;
     uint32_t n_members = 0, n_sorts = 0, n_over = 0;     // lane 0's tallies
     uint64_t a = c0;
-    if (c0 < n && c0 > 0) a = scan_to_head<KeyT, PACKED>(keys1, c0, n);   // groups that began before the chunk are the previous warp's
+    if (c0 < n && c0 > 0) a = scan_to_head<KeyT, PACKED>(keys1, c0, n, split);   // groups that began before the chunk are the previous warp's
     // ---- the work item: a window of the sorted order [a, a + n_comp), or a window of queued members ---------------------------
     uint32_t hw[S + 1];                                  // bit i of hw[s]: position a + 32 s + i is a head
     uint32_t n_comp = 0;
@@ -1001,7 +1009,7 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
             const bool over = active && !mine[s];             // a complete group of more than cap members (cap < 32 S only)
             if (__any_sync(kFull, over)) {                    // the global path's: clear all but its first position's head bit
                 const bool over_head = over && ((hw[s] >> lane) & 1u);
-                if constexpr (PACKED) {
+                if (PACKED || split) {
                     if (over) ids_out[j] = idv[s];
                 }
                 const uint32_t clear = __ballot_sync(kFull, over && !over_head), over_heads = __ballot_sync(kFull, over_head);
@@ -1063,7 +1071,7 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
                     for (int s = 0; s < S; ++s) {
                         const uint64_t j = a + 32 * s + lane;
                         word[s] = j < n ? load_keyword<KeyT, PACKED>(keys1, j) : 0ull;
-                        k[s] = key_of<PACKED>(word[s]);
+                        k[s] = key_of<PACKED>(word[s], split);
                     }
                     uint32_t carry_in = 1;                           // head bit of the slot's first position
 #pragma unroll
@@ -1075,7 +1083,7 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
                             const uint64_t first_of_next_slot = __shfl_sync(kFull, k[s + 1 < S ? s + 1 : s], 0);
                             if (lane == 31) kn = first_of_next_slot;
                         } else if (lane == 31) {
-                            kn = valid_next ? key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j + 1)) : 0ull;
+                            kn = valid_next ? key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j + 1), split) : 0ull;
                         }
                         const bool head_next = !valid_next || kn != k[s] || !((uint32_t)kn & 1u);
                         const uint32_t HN = __ballot_sync(kFull, head_next);
@@ -1106,7 +1114,7 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
                 }
                 if (n_comp == 0) {
                     // one group fills the window and goes on: more than 32 S members
-                    const uint64_t e = scan_to_head<KeyT, PACKED>(keys1, a + kSpan, n);
+                    const uint64_t e = scan_to_head<KeyT, PACKED>(keys1, a + kSpan, n, split);
                     const uint64_t g = e - a;
                     if (g <= cap) {          // the block kernel's: flag the tile it starts in
                         if (lane == 0) atomicOr(big_tiles + (a / kLocalTile >> 5), 1u << (a / kLocalTile & 31));
@@ -1114,6 +1122,8 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
                         clear_heads(heads, a + 1, e);
                         if constexpr (PACKED) {
                             for (uint64_t q = a + lane; q < e; q += 32) ids_out[q] = (IdT)(uint32_t)load_keyword<KeyT, PACKED>(keys1, q);
+                        } else if (split) {
+                            for (uint64_t q = a + lane; q < e; q += 32) ids_out[q] = split_id<IdT>(load_keyword<KeyT, PACKED>(keys1, q), split, ids_in, q);
                         }
                         n_over += 1;
                     }
@@ -1142,7 +1152,7 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
                     idv[s] = 0;
                     if (active) {
                         if constexpr (PACKED) idv[s] = (IdT)(uint32_t)word[s];
-                        else idv[s] = __ldg(ids_in + j);
+                        else idv[s] = split ? split_id<IdT>(word[s], split, ids_in, j) : __ldg(ids_in + j);
                     }
                 }
                 uint64_t before[S], first_base[S];
@@ -1413,7 +1423,7 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
 constexpr int kProbeSpan = 2048, kProbeBlocks = 128;
 template <typename KeyT, bool PACKED>
 __global__ void __launch_bounds__(256) group_probe_kernel(const KeyT* __restrict__ keys1, uint64_t n, uint32_t limit,
-                                                          unsigned long long* counter) {
+                                                          unsigned long long* counter, uint32_t split) {
     __shared__ uint32_t s_heads[kProbeSpan / 32 + 1];
     __shared__ uint32_t s_big;
     const uint64_t stride = n / gridDim.x;
@@ -1425,7 +1435,7 @@ __global__ void __launch_bounds__(256) group_probe_kernel(const KeyT* __restrict
         const uint64_t j = a + e;
         bool head = true;
         if (j < n && e > 0) {
-            const uint64_t kc = key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j)), kp = key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j - 1));
+            const uint64_t kc = key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j), split), kp = key_of<PACKED>(load_keyword<KeyT, PACKED>(keys1, j - 1), split);
             head = kc != kp || !((uint32_t)kc & 1u);
         }
         const uint32_t word = __ballot_sync(kFull, head);
@@ -1492,10 +1502,12 @@ cudaError_t launch_refine_writeback(const Reads& R, const uint64_t* keys_c, cons
 template <typename KeyT, typename IdT>
 cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, uint32_t depth0, uint32_t* heads_out, IdT* ids, uint64_t n,
                                 uint32_t group_cap, uint8_t* out, unsigned long long* elems_done, uint32_t* big_tiles, int n_sms, bool packed,
-                                uint32_t slots, Launch* prof, cudaStream_t s) {
+                                uint32_t slots, Launch* prof, cudaStream_t s, uint32_t split, IdT* ids_out) {
     if (n == 0) return cudaSuccess;
     constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
     if (packed && !kCanPack) return cudaErrorInvalidValue;
+    if (split && (packed || sizeof(KeyT) != 8 || sizeof(IdT) != 8 || !ids_out || ids_out == ids)) return cudaErrorInvalidValue;
+    if (!split) ids_out = ids;   // (separate arrays: the ids stay where they are; packed: the oversize groups' ids go there)
     if (slots != (uint32_t)kWarpSlotsSmall && slots != (uint32_t)kWarpSlotsLarge) return cudaErrorInvalidValue;
     (void)w1;   // (a first-round key says in its lowest bit whether its suffix has w1 bases)
     if (group_cap > (uint32_t)kLocalGroupCap) group_cap = kLocalGroupCap;
@@ -1504,12 +1516,12 @@ cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, 
     if (e != cudaSuccess) return e;
     {   // singletons and groups of at most 32: one warp per chunk, registers only
         // a7 flagging (key + 1) and a8 emit (id + base + byte) per suffix; the refined suffixes' term is added by the caller
-        ScopedLaunch sl(prof, CX_K_FINISH, n * (sizeof(KeyT) + 1 + sizeof(IdT) + 2), s);
+        ScopedLaunch sl(prof, CX_K_FINISH, n * ((split ? 12 : sizeof(KeyT) + sizeof(IdT)) + 1 + 2), s);
         const uint64_t resident_warps = (uint64_t)n_sms * (slots == (uint32_t)kWarpSlotsLarge ? 2 : CX_WARP_MINB) * (kWarpThreads / 32);
         const uint32_t chunk = n >= resident_warps * kWarpChunkWaves * kWarpChunkLarge ? kWarpChunkLarge : kWarpChunkSmall;
         const uint64_t warps = (n + chunk - 1) / chunk;
         const unsigned grid = (unsigned)((warps + kWarpThreads / 32 - 1) / (kWarpThreads / 32));
-        auto launch = [&](auto kernel) { kernel<<<grid, kWarpThreads, 0, s>>>(R, keys1, ids, ids, n, depth0, group_cap, heads_out, big_tiles, out, elems_done, chunk); };
+        auto launch = [&](auto kernel) { kernel<<<grid, kWarpThreads, 0, s>>>(R, keys1, ids, ids_out, n, depth0, group_cap, heads_out, big_tiles, out, elems_done, chunk, split); };
         if (slots == (uint32_t)kWarpSlotsLarge) {
             if (packed) launch(finish_warp_kernel<KeyT, IdT, kCanPack, kWarpSlotsLarge>);
             else launch(finish_warp_kernel<KeyT, IdT, false, kWarpSlotsLarge>);
@@ -1528,20 +1540,21 @@ cudaError_t launch_finish_first(const Reads& R, const KeyT* keys1, uint32_t w1, 
     const uint64_t resident = (uint64_t)n_sms * kLocalBlocksPerSM;
     ScopedLaunch sl(prof, CX_K_FINISH_BLOCK, 0, s);
     kernel<<<(unsigned)(tiles < resident ? tiles : resident), kLocalThreads, sizeof(LocalSmem), s>>>(R, keys1, nullptr, nullptr, ids, n, depth0, 32u * slots + 1,
-                                                                                                   group_cap, big_tiles, out, elems_done);
+                                                                                                   group_cap, big_tiles, out, elems_done, split);
     return cudaGetLastError();
 }
 
 template <typename KeyT, typename IdT>
-cudaError_t launch_group_probe(const KeyT* keys1, uint32_t w1, uint64_t n, bool packed, unsigned long long* counter, uint64_t* sampled, cudaStream_t s) {
+cudaError_t launch_group_probe(const KeyT* keys1, uint32_t w1, uint64_t n, bool packed, unsigned long long* counter, uint64_t* sampled, cudaStream_t s,
+                               uint32_t split) {
     constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
     *sampled = 0;
     if (n < (uint64_t)kProbeSpan * 2) return cudaSuccess;
     const unsigned blocks = (unsigned)(n / kProbeSpan < (uint64_t)kProbeBlocks ? n / kProbeSpan : (uint64_t)kProbeBlocks);
     *sampled = (uint64_t)blocks * kProbeSpan;
     (void)w1;
-    if (packed) group_probe_kernel<KeyT, kCanPack><<<blocks, 256, 0, s>>>(keys1, n, 32u * kWarpSlotsSmall, counter);
-    else group_probe_kernel<KeyT, false><<<blocks, 256, 0, s>>>(keys1, n, 32u * kWarpSlotsSmall, counter);
+    if (packed) group_probe_kernel<KeyT, kCanPack><<<blocks, 256, 0, s>>>(keys1, n, 32u * kWarpSlotsSmall, counter, 0u);
+    else group_probe_kernel<KeyT, false><<<blocks, 256, 0, s>>>(keys1, n, 32u * kWarpSlotsSmall, counter, split);
     return cudaGetLastError();
 }
 
@@ -1556,7 +1569,7 @@ cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32
     const uint64_t tiles = (n + kLocalTile - 1) / kLocalTile;
     const uint64_t resident = (uint64_t)n_sms * kLocalBlocksPerSM;
     kernel<<<(unsigned)(tiles < resident ? tiles : resident), kLocalThreads, sizeof(LocalSmem), s>>>(R, nullptr, heads_in, heads_out, ids, n, depth, 2u, group_cap,
-                                                                                                   nullptr, out, elems_done);
+                                                                                                   nullptr, out, elems_done, 0u);
     return cudaGetLastError();
 }
 
@@ -1567,11 +1580,11 @@ cudaError_t launch_finish_later(const Reads& R, const uint32_t* heads_in, uint32
                                                       const uint64_t*, uint64_t, uint64_t, uint32_t, IdT*, uint32_t*, uint8_t*,      \
                                                       cudaStream_t);                                                                 \
     template cudaError_t launch_finish_first<uint32_t, IdT>(const Reads&, const uint32_t*, uint32_t, uint32_t, uint32_t*, IdT*, uint64_t, \
-                                                            uint32_t, uint8_t*, unsigned long long*, uint32_t*, int, bool, uint32_t, Launch*, cudaStream_t); \
+                                                            uint32_t, uint8_t*, unsigned long long*, uint32_t*, int, bool, uint32_t, Launch*, cudaStream_t, uint32_t, IdT*); \
     template cudaError_t launch_finish_first<uint64_t, IdT>(const Reads&, const uint64_t*, uint32_t, uint32_t, uint32_t*, IdT*, uint64_t, \
-                                                            uint32_t, uint8_t*, unsigned long long*, uint32_t*, int, bool, uint32_t, Launch*, cudaStream_t); \
-    template cudaError_t launch_group_probe<uint32_t, IdT>(const uint32_t*, uint32_t, uint64_t, bool, unsigned long long*, uint64_t*, cudaStream_t); \
-    template cudaError_t launch_group_probe<uint64_t, IdT>(const uint64_t*, uint32_t, uint64_t, bool, unsigned long long*, uint64_t*, cudaStream_t); \
+                                                            uint32_t, uint8_t*, unsigned long long*, uint32_t*, int, bool, uint32_t, Launch*, cudaStream_t, uint32_t, IdT*); \
+    template cudaError_t launch_group_probe<uint32_t, IdT>(const uint32_t*, uint32_t, uint64_t, bool, unsigned long long*, uint64_t*, cudaStream_t, uint32_t); \
+    template cudaError_t launch_group_probe<uint64_t, IdT>(const uint64_t*, uint32_t, uint64_t, bool, unsigned long long*, uint64_t*, cudaStream_t, uint32_t); \
     template cudaError_t launch_finish_later<IdT>(const Reads&, const uint32_t*, uint32_t*, const IdT*, uint64_t, uint32_t,         \
                                                   uint32_t, uint8_t*, unsigned long long*, int, cudaStream_t);
 CX_INSTANTIATE(uint32_t)

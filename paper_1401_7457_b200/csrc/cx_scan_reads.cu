@@ -376,6 +376,26 @@ __global__ void __launch_bounds__(kListThreads) list_count_kernel(Reads R, const
 // [bucket_lo, bucket_hi], in (read, pos) order, each with its first key.  Most slots belong to other
 // batches, so the scan walks the slots with next_slot() and decodes in full only what it takes.
 // ---------------------------------------------------------------------------------------------
+// One (first-round key, id) pair of a batch's listing.  Three layouts: packed 32 + 32 in one word; separate arrays; or -- split != 0,
+// 64-bit keys and ids only -- the key shifted up by `split` bits above the id's high part in the word, and the id's low 32 bits in
+// a uint32 array at `ids`: 12 bytes per pair through the sort instead of 16 (the sort then runs over bits split .. 64).
+template <typename KeyT, typename IdT, bool PACKED>
+__device__ __forceinline__ void store_pair(KeyT* __restrict__ keys, IdT* __restrict__ ids, uint64_t at, KeyT key, IdT id, uint32_t split) {
+    if constexpr (PACKED) {
+        reinterpret_cast<uint64_t*>(keys)[at] = ((uint64_t)key << 32) | (uint64_t)id;
+    } else {
+        if constexpr (sizeof(KeyT) == 8 && sizeof(IdT) == 8) {
+            if (split) {
+                keys[at] = (key << split) | (id >> 32);
+                reinterpret_cast<uint32_t*>(ids)[at] = (uint32_t)id;
+                return;
+            }
+        }
+        keys[at] = key;
+        ids[at] = id;
+    }
+}
+
 template <typename KeyT, typename IdT, bool PACKED, bool REGION>
 __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, const BuildInfo* __restrict__ info,
                                                                    const uint32_t* __restrict__ tile_first_read, uint32_t ell, uint32_t w,
@@ -383,7 +403,7 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
                                                                    const uint64_t* __restrict__ tile_base, KeyT* __restrict__ keys,
                                                                    IdT* __restrict__ ids, uint32_t n_passes,
                                                                    unsigned long long* __restrict__ digit_hist, Region region,
-                                                                   uint64_t ord_lo, uint64_t ord_hi) {
+                                                                   uint64_t ord_lo, uint64_t ord_hi, uint32_t split) {
     // region: the scan is confined to the suffixes of an oversize partition and keys start at its depth.
     // [ord_lo, ord_hi): of the selected suffixes, in listing order, only these ordinals are written (at ordinal - ord_lo):
     // a partition of IDENTICAL suffixes larger than a batch is cut this way, its order being the listing order anyway.
@@ -456,13 +476,7 @@ __global__ void __launch_bounds__(kListThreads) list_select_kernel(Reads R, cons
                 const KeyT key = first_key_as<KeyT>(sl.window, sl.rem, w);
                 const IdT id = make_id<IdT>(sl.read, sl.pos, R.pos_bits);
                 digit_counts(s_dh, key, n_passes);
-                const uint64_t at = dst - ord_lo;
-                if constexpr (PACKED) {
-                    reinterpret_cast<uint64_t*>(keys)[at] = ((uint64_t)key << 32) | (uint64_t)id;
-                } else {
-                    keys[at] = key;
-                    ids[at] = id;
-                }
+                store_pair<KeyT, IdT, PACKED>(keys, ids, dst - ord_lo, key, id, split);
             }
         }
     }
@@ -713,7 +727,7 @@ __global__ void __launch_bounds__(kListThreads) list_select_uniform_kernel(Reads
                                                                            uint32_t bucket_lo, uint32_t bucket_hi,
                                                                            const uint64_t* __restrict__ tile_base, KeyT* __restrict__ keys,
                                                                            IdT* __restrict__ ids, uint32_t n_passes,
-                                                                           unsigned long long* __restrict__ digit_hist, uint64_t ord_lo, uint64_t ord_hi) {
+                                                                           unsigned long long* __restrict__ digit_hist, uint64_t ord_lo, uint64_t ord_hi, uint32_t split) {
     __shared__ BigSmem sm;
     __shared__ uint32_t s_dh[8][kRadix];
     __shared__ uint32_t s_warp[kListThreads / 32];
@@ -764,13 +778,7 @@ __global__ void __launch_bounds__(kListThreads) list_select_uniform_kernel(Reads
                 const KeyT key = first_key_as<KeyT>(big_window(sm, brel), (uint64_t)(c.L1 - 1 - pos), w);
                 const IdT id = make_id<IdT>(c.r0 + rr, pos, R.pos_bits);
                 digit_counts(s_dh, key, n_passes);
-                const uint64_t at = dst - ord_lo;
-                if constexpr (PACKED) {
-                    reinterpret_cast<uint64_t*>(keys)[at] = ((uint64_t)key << 32) | (uint64_t)id;
-                } else {
-                    keys[at] = key;
-                    ids[at] = id;
-                }
+                store_pair<KeyT, IdT, PACKED>(keys, ids, dst - ord_lo, key, id, split);
             }
         }
     }
@@ -936,7 +944,7 @@ __global__ void __launch_bounds__(kListThreads) list_select_reads_kernel(Reads R
                                                                          uint32_t bucket_lo, uint32_t bucket_hi,
                                                                          const uint64_t* __restrict__ tile_base, KeyT* __restrict__ keys,
                                                                          IdT* __restrict__ ids, uint32_t n_passes,
-                                                                         unsigned long long* __restrict__ digit_hist, uint64_t ord_lo, uint64_t ord_hi) {
+                                                                         unsigned long long* __restrict__ digit_hist, uint64_t ord_lo, uint64_t ord_hi, uint32_t split) {
     __shared__ uint64_t s_packed[kReadTileWords];
     __shared__ uint32_t s_dh[8][kRadix];
     __shared__ uint32_t s_warp[kListThreads / 32];
@@ -991,13 +999,7 @@ __global__ void __launch_bounds__(kListThreads) list_select_reads_kernel(Reads R
                     const KeyT key = first_key_as<KeyT>(window_at(s_packed, c.brel0 + rr * c.L + pos), (uint64_t)(c.L - pos), w);
                     const IdT id = make_id<IdT>(c.r0 + rr, pos, R.pos_bits);
                     digit_counts(s_dh, key, n_passes);
-                    const uint64_t o = dst - ord_lo;
-                    if constexpr (PACKED) {
-                        reinterpret_cast<uint64_t*>(keys)[o] = ((uint64_t)key << 32) | (uint64_t)id;
-                    } else {
-                        keys[o] = key;
-                        ids[o] = id;
-                    }
+                    store_pair<KeyT, IdT, PACKED>(keys, ids, dst - ord_lo, key, id, split);
                 }
             }
         }
@@ -1215,7 +1217,7 @@ template <typename KeyT, typename IdT>
 cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint32_t* tile_first_read, uint32_t ell, uint32_t w,
                               uint32_t bucket_lo, uint32_t bucket_hi, const uint64_t* tile_base, KeyT* keys, IdT* ids,
                               uint64_t n_tiles, uint32_t n_passes, uint64_t* digit_hist, int n_sms, bool packed, uint64_t* bucket_hist,
-                              uint64_t max_n, const Region& region, uint64_t ord_lo, uint64_t ord_hi, cudaStream_t s) {
+                              uint64_t max_n, const Region& region, uint64_t ord_lo, uint64_t ord_hi, cudaStream_t s, uint32_t split) {
     if (n_tiles == 0) return cudaSuccess;
     uint64_t want = (uint64_t)n_sms * (bucket_hist ? 4 : 6);
     unsigned grid = (unsigned)(n_tiles < want ? n_tiles : want);
@@ -1223,6 +1225,7 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
     unsigned long long* bh = (unsigned long long*)bucket_hist;
     constexpr bool kCanPack = sizeof(KeyT) == 4 && sizeof(IdT) == 4;
     if ((packed && !kCanPack) || (bucket_hist && tile_base)) return cudaErrorInvalidValue;
+    if (split && (tile_base == nullptr || packed || sizeof(KeyT) != 8 || sizeof(IdT) != 8)) return cudaErrorInvalidValue;   // select scans only
     const size_t smem = bucket_hist ? bucket_hist_smem(ell) - sizeof(TileSmem) : 0;
     const uint32_t skip_reads = tile_base == nullptr && w <= 16 && !region.depth && R.n_reads > 0;   // (a register pair holds the 16 bases a key may need)
     auto launch = [&](auto kernel) {
@@ -1263,7 +1266,7 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
         const uint64_t resident = (uint64_t)n_sms * (per_sm > 0 ? per_sm : 1);
         const unsigned grid = (unsigned)(n_tiles < resident ? n_tiles : resident);
         kernel<<<grid, kListThreads, 0, s>>>(R, info, tile_first_read, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids, n_passes, dh, region, ord_lo,
-                                             ord_hi);
+                                             ord_hi, split);
         return cudaGetLastError();
     };
     if (read_tiles(R, region)) {
@@ -1273,7 +1276,7 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
         if (e != cudaSuccess) return e;
         const uint64_t resident = (uint64_t)n_sms * (per_sm > 0 ? per_sm : 1);
         kernel<<<(unsigned)(n_tiles < resident ? n_tiles : resident), kListThreads, 0, s>>>(R, info, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids, n_passes, dh,
-                                                                                          ord_lo, ord_hi);
+                                                                                          ord_lo, ord_hi, split);
         return cudaGetLastError();
     }
     if (big_tiles(R, region)) {
@@ -1283,7 +1286,7 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
         if (e != cudaSuccess) return e;
         const uint64_t resident = (uint64_t)n_sms * (per_sm > 0 ? per_sm : 1);
         kernel<<<(unsigned)(n_tiles < resident ? n_tiles : resident), kListThreads, 0, s>>>(R, info, ell, w, bucket_lo, bucket_hi, tile_base, keys, ids, n_passes, dh,
-                                                                                          ord_lo, ord_hi);
+                                                                                          ord_lo, ord_hi, split);
         return cudaGetLastError();
     }
     if (region.depth) return packed ? select(list_select_kernel<KeyT, IdT, kCanPack, true>) : select(list_select_kernel<KeyT, IdT, false, true>);
@@ -1293,7 +1296,7 @@ cudaError_t launch_list_write(const Reads& R, const BuildInfo* info, const uint3
 #define CX_LIST_INST(K, I)                                                                                                        \
     template cudaError_t launch_list_write<K, I>(const Reads&, const BuildInfo*, const uint32_t*, uint32_t, uint32_t, uint32_t,  \
                                                  uint32_t, const uint64_t*, K*, I*, uint64_t, uint32_t, uint64_t*, int, bool, uint64_t*, uint64_t, const Region&,     \
-                                                 uint64_t, uint64_t, cudaStream_t);
+                                                 uint64_t, uint64_t, cudaStream_t, uint32_t);
 CX_LIST_INST(uint32_t, uint32_t)
 CX_LIST_INST(uint32_t, uint64_t)
 CX_LIST_INST(uint64_t, uint32_t)

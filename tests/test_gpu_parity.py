@@ -95,6 +95,33 @@ def test_global_path_shares_the_buffers_of_the_first_sort(id64):
     assert_parity(c, small_group_max=1, max_batch_suffixes=c.n_suffixes // 2 + 3, **extra)
 
 
+@pytest.mark.parametrize("case", range(5))
+def test_split_pairs_of_64_bit_keys_and_ids(case):
+    """Batches of a multi-batch plan with 64-bit keys (19 bases) and 64-bit ids go through the sort as 12-byte pairs: the key
+    above the id's high part in the 64-bit word, the id's low word as the value; the listing writes them, the probe, the warp
+    and the block kernel read them, and groups left to the global path get their ids assembled into another buffer.
+    Collections with every group size (singletons, <= 64, 65..256, above 256), ragged reads, a scaled configs[3]."""
+    rng = np.random.default_rng(300 + case)
+    if case == 0:
+        c = gen.random_collection(11, 400, 120)
+    elif case == 1:
+        unit = "".join(rng.choice(list("ACGT"), 200))
+        c = gen.from_strings([unit] * 700 + [unit[40:]] * 100 + [unit[:90]] * 30 + ["".join(rng.choice(list("ACGT"), 60)) for _ in range(200)])
+    elif case == 2:
+        genome = np.frombuffer(b"ACGT", np.uint8)[rng.integers(0, 4, 900)]
+        c = gen.from_strings(["".join(map(chr, genome[s:s + 100])) for s in rng.integers(0, 800, 3000)])     # groups of 2..200
+    elif case == 3:
+        c = gen.config(3, 0.0003)
+    else:
+        c = gen.from_strings(["AC" * 70] * 150 + ["ACGT"] * 40 + [""] * 3 + ["T"])
+    N = c.n_suffixes
+    base = dict(key_bases=19, max_read_len=0)
+    assert_parity(c, max_batch_suffixes=N // 3 + 1, **base)
+    assert_parity(c, max_batch_suffixes=N // 7 + 2, finish_slots=4, **base)
+    assert_parity(c, max_batch_suffixes=N // 2 + 3, small_group_max=1, **base)
+    assert_parity(c, max_batch_suffixes=N // 4 + 1, small_group_max=100, key_bases=29, max_read_len=0)     # 60-bit keys: 4-bit split
+
+
 def test_long_reads_and_tandem_repeats():
     c = gen.from_strings(["ACGT" * 200, "ACGT" * 150 + "T", "CGTA" * 180, "G" * 900, ""] * 7)
     assert_parity(c)
