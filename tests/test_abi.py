@@ -29,8 +29,12 @@ def test_workspace_bytes_and_argument_errors():
     a = cx.cx_bwt_workspace_bytes(10_000, 1_000_000, max_read_len=100)
     b = cx.cx_bwt_workspace_bytes(1_000_000, 100_000_000, max_read_len=100)
     assert 0 < a < b
-    # 4-byte ids: about 2*8 + 3*4 + 4 bytes per suffix plus flags and tile state
-    assert 32 * 101_000_000 < b < 40 * 101_000_000
+    # 4-byte ids: 2*8 (keys) + 2*4 (ids) + 4 (the global path's second position array) bytes per suffix plus flags and tile
+    # state (until the global path gave up its own buffers it was 2*8 + 3*4 + 4)
+    assert 28 * 101_000_000 < b < 33 * 101_000_000
+    # 8-byte ids (read length unknown) with pinned-host output: 2*8 + 2*8 + 2 staging bytes, no position array
+    c = cx.cx_bwt_workspace_bytes(1_000_000, 100_000_000, max_read_len=0, out_is_host_pinned=1)
+    assert 34 * 101_000_000 < c < 38 * 101_000_000
     c = cx.cx_bwt_workspace_bytes(1_000_000, 100_000_000, max_read_len=100, max_batch_suffixes=10_000_000)
     assert c < b / 5
     d = cx.cx_bwt_workspace_bytes(40_000_000, 6_000_000_000, max_read_len=250)     # 8-byte ids
