@@ -783,6 +783,9 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
 // sorted positions per warp (a chunk owns the groups that START in it): the larger one when the batch still fills the GPU
 // several times over (fewer partly filled queue windows at the ends of chunks)
 constexpr uint32_t kWarpChunkSmall = 2048, kWarpChunkLarge = 4096, kWarpChunkWaves = 8;
+#ifndef CX_WARP_PREFETCH
+#define CX_WARP_PREFETCH 8   // lanes that prefetch a 128-byte line of the following windows' keys (0: none)
+#endif
 #ifndef CX_WARP_QUEUE
 #define CX_WARP_QUEUE 1
 #endif
@@ -1064,6 +1067,14 @@ __global__ void __launch_bounds__(kWarpThreads, S == 4 ? 2 : CX_WARP_MINB) finis
                 open = 1;
             } else if (a < c1) {
                 // ---- the window [a, a + 32 S): a is a head --------------------------------------------------------------
+#if CX_WARP_PREFETCH
+                {   // ask L2 for the keys of the windows after this one (eight lanes, one 128-byte line each): their loads are
+                    // the first link of the next window's chain of dependent loads
+                    constexpr uint32_t kWordBytes = PACKED ? 8 : sizeof(KeyT);
+                    const uint64_t pf = (a + kSpan) * kWordBytes + 128ull * lane;
+                    if (lane < CX_WARP_PREFETCH && pf < n * kWordBytes) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(keys1) + pf));
+                }
+#endif
                 uint64_t word[S];
                 {
                     uint64_t k[S];
