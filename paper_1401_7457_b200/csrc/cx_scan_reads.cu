@@ -12,6 +12,10 @@
 // listing order PAPER.md:99 requires for the stable sort to realise $_i < $_j.
 #include "cx_internal.cuh"
 
+#ifndef CX_READ_TILE_PREFETCH
+#define CX_READ_TILE_PREFETCH 1   // L2 prefetch of the read tile a grid-width ahead in the one-read-per-thread scans
+#endif
+
 namespace cx {
 namespace {
 
@@ -819,6 +823,13 @@ __device__ __forceinline__ ReadTileCtx load_read_tile(const Reads& R, const Buil
         const uint64_t wi = word0 + j;
         packed_sm[j] = wi < R.n_words ? __ldg(R.packed + wi) : 0ull;
     }
+#if CX_READ_TILE_PREFETCH
+    {   // the tile this block takes next (a grid-width on): ask L2 for its lines now
+        const uint64_t next0 = ((t + gridDim.x) * kListThreads * c.L) >> 5;
+        const uint64_t wi = next0 + 16ull * threadIdx.x;                    // one 128-byte line per thread
+        if (16u * threadIdx.x < words && wi < R.n_words) asm volatile("prefetch.global.L2 [%0];" ::"l"(R.packed + wi));
+    }
+#endif
     __syncthreads();
     return c;
 }
