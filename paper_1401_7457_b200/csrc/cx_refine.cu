@@ -750,10 +750,41 @@ __global__ void __launch_bounds__(kLocalThreads, kLocalBlocksPerSM) finish_tile_
     extern __shared__ __align__(16) unsigned char smem_raw[];
     LocalSmem& sm = *reinterpret_cast<LocalSmem*>(smem_raw);
     const uint64_t n_tiles = (n + kLocalTile - 1) / kLocalTile;
-    for (uint64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        if (FIRST && !((__ldg(big_tiles + (tile >> 5)) >> (tile & 31)) & 1u)) continue;
-        finish_tile<KeyT, IdT, FIRST, PACKED>(sm, tile, R, keys1, heads_in, heads, ids, n, depth0, min_group, cap, out, elems_done, split);
-        __syncthreads();   // the next tile reuses the shared memory
+    if constexpr (!FIRST) {
+        // After a global round nearly every tile has nothing left to do, and finding that out inside finish_tile costs the whole
+        // block a barrier per tile.  So the tiles go by in eights: each warp looks at the head words of one tile (the same test as
+        // finish_tile's: does a group of two or more start at one of its positions?), and only the tiles that pass get the block.
+        constexpr uint32_t kPer = kLocalThreads / 32;
+        __shared__ uint32_t s_todo;
+        const uint64_t n_words = (n + 31) >> 5;
+        const uint32_t warp = threadIdx.x >> 5, lane = lane_id();
+        for (uint64_t t0 = (uint64_t)blockIdx.x * kPer; t0 < n_tiles; t0 += (uint64_t)gridDim.x * kPer) {
+            if (threadIdx.x == 0) s_todo = 0;
+            __syncthreads();
+            const uint64_t tile = t0 + warp;
+            uint32_t incomplete = 0;
+            if (tile < n_tiles && lane <= (uint32_t)kLocalTile / 32) {
+                const uint64_t wi = tile * (kLocalTile / 32) + lane;
+                const uint32_t v = wi <= n_words ? heads_in[wi] : kFull;
+                const uint32_t care = lane == 0 ? ~1u : (lane == (uint32_t)kLocalTile / 32 ? 1u : kFull);
+                incomplete = (~v) & care;
+            }
+            if (__any_sync(kFull, incomplete != 0) && lane == 0) atomicOr(&s_todo, 1u << warp);
+            __syncthreads();
+            uint32_t todo = s_todo;
+            while (todo) {
+                const uint32_t w = (uint32_t)__ffs(todo) - 1;
+                todo &= todo - 1;
+                finish_tile<KeyT, IdT, FIRST, PACKED>(sm, t0 + w, R, keys1, heads_in, heads, ids, n, depth0, min_group, cap, out, elems_done, split);
+                __syncthreads();   // the next tile reuses the shared memory
+            }
+        }
+    } else {
+        for (uint64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            if (!((__ldg(big_tiles + (tile >> 5)) >> (tile & 31)) & 1u)) continue;   // only the tiles the warp kernel flagged
+            finish_tile<KeyT, IdT, FIRST, PACKED>(sm, tile, R, keys1, heads_in, heads, ids, n, depth0, min_group, cap, out, elems_done, split);
+            __syncthreads();   // the next tile reuses the shared memory
+        }
     }
 }
 
