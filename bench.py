@@ -45,7 +45,7 @@ WORKLOADS = {
 }
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, from the committed `ncu --set full` captures of THIS round at the
 # benched configuration (profiles/r02_ncu_full.md); keyed by (config, kernel class).  None until a capture exists.
-NCU_TRAFFIC: dict = {(2, "finish"): 105_638_698_000, (2, "sort_pass"): 16_442_634_750, (2, "list"): 9_418_668_000, (2, "pack"): 1_194_596_000,
+NCU_TRAFFIC: dict = {(2, "finish"): 105_640_423_000, (2, "sort_pass"): 16_442_371_750, (2, "list"): 9_418_393_000, (2, "pack"): 1_195_345_000,
                      (2, "finish_block"): 316_000}
 NCU_TRAFFIC_FILE = "profiles/r02_ncu_full.md"
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
